@@ -1,0 +1,300 @@
+"""Pins for the CPU oracle (oracle/tb_oracle.py): what the paper and the mathematics fix.
+
+None of these tests touches the CUDA path.  Each pin is chosen so that a plausible slip in the
+oracle (dropped term, wrong sign or index, transposed operand) fails at least one of them.
+Citations are PAPER.md line numbers; T-numbers are SURVEY.md §4 / DESIGN.md §5.
+"""
+import math
+import os
+from fractions import Fraction
+
+import numpy as np
+import pytest
+
+from oracle import tb_oracle as orc
+
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden")
+
+
+# ------------------------------------------------------------------ T1 / T3 / T11: index map
+def test_t1_tau_zero_is_identity():
+    n = 4096
+    for tmpl in [(60.0, 0.0, 1.0, 0.0, 0.0), (33.0, 0.0, 2.5, 0.3, 1.1)]:
+        idx = orc.resample_indices(n, 1e-3, tmpl)
+        assert np.array_equal(idx, np.arange(n))
+
+
+def test_t3_first_index_is_zero():
+    rng = np.random.default_rng(3)
+    for _ in range(20):
+        tmpl = (rng.uniform(5, 90), rng.uniform(0, 4), rng.uniform(0, 2 * np.pi),
+                rng.uniform(0, 0.5), rng.uniform(0, 2 * np.pi))
+        assert orc.resample_indices(1024, 1e-3, tmpl)[0] == 0
+        circ = (tmpl[0], tmpl[1], tmpl[2], 0.0, 0.0)
+        assert orc.resample_indices(1024, 1e-3, circ)[0] == 0
+
+
+def test_t11_monotone_and_out_of_range_bound():
+    rng = np.random.default_rng(11)
+    n, tsamp = 1 << 16, 64e-6
+    T = n * tsamp
+    for _ in range(8):
+        p = rng.uniform(0.1 * T, 0.35 * T)
+        tau = rng.uniform(0.01, 0.8) * p / (2 * np.pi)      # orbital speed v/c = tau*Omega in [0.01, 0.8]
+        e, om, a = rng.uniform(0, 0.1), rng.uniform(0, 2 * np.pi), rng.uniform(0, 2 * np.pi)
+        stretch = tau * 2 * np.pi / p * math.sqrt((1 + e) / (1 - e))
+        assert stretch < 1
+        idx = orc.resample_indices(n, tsamp, (p, tau, a, e, om))
+        assert np.all(np.diff(idx) >= 0), "gather map must be monotone when tau*Omega*sqrt((1+e)/(1-e)) < 1"
+        max_shift = np.max(np.abs(np.arange(n) - idx))
+        assert max_shift <= 2 * tau * (1 + e) / tsamp + 1          # |delta| <= 2 tau (1+e)/tsamp
+        oob = np.count_nonzero((idx < 0) | (idx >= n))
+        assert oob <= 2 * (max_shift + 1)
+
+
+def test_shift_sign_and_magnitude_closed_form():
+    """Circular quarter-orbit: delta(P/4) - delta(0) = tau (sin(pi/2+phi0) - sin(phi0)) / tsamp
+    (eq A1 at e=0, L666; eq 4).  phi0 = 0 -> +tau/tsamp: source index j - tau/tsamp."""
+    tsamp, p, tau = 1e-3, 4.096, 0.25
+    idx = orc.resample_indices(2048, tsamp, (p, tau, 0.0, 0.0, 0.0))
+    j = 1024                                   # t = P/4
+    assert idx[j] == j - 250
+    j = 2047                                   # just before t = P/2: delta -> ~0+
+    assert abs((j - idx[j])) <= 1
+
+
+# ------------------------------------------------------------------ T2: e = 0 reduces to circular
+def test_t2_kepler_path_at_e0_is_the_circular_closed_form():
+    n, tsamp = 1 << 15, 1e-3
+    tmpl = (47.0, 0.8, 1.3, 0.0, 0.0)
+    j = np.arange(n)
+    a = orc.roemer_delay(j, tsamp, tmpl)                       # closed form
+    b = orc.roemer_delay(j, tsamp, tmpl, force_kepler=True)    # Newton path, e = 0, omega = 0
+    assert np.array_equal(a, b)                                # Newton returns E = M exactly
+    assert np.array_equal(orc.resample_indices(n, tsamp, tmpl),
+                          orc.resample_indices(n, tsamp, tmpl, force_kepler=True))
+    # omega != 0 at e = 0: tau sin(M + omega)  (A1 with E = M)
+    om = 0.7
+    c = orc.roemer_delay(j, tsamp, (47.0, 0.8, 1.3, 0.0, om))
+    d = orc.roemer_delay(j, tsamp, (47.0, 0.8, 1.3 + om, 0.0, 0.0))
+    assert np.max(np.abs(c - d)) < 1e-14
+
+
+# ------------------------------------------------------------------ T4: Kepler solve
+def _load_series():
+    C, S = {}, {}
+    with open(os.path.join(GOLDEN, "appendix_b_series.txt")) as f:
+        for line in f:
+            if line.startswith("#") or not line.strip():
+                continue
+            kind, k, pw, num, den = line.split()
+            (C if kind == "C" else S).setdefault(int(k), []).append((int(pw), Fraction(int(num), int(den))))
+    return C, S
+
+
+def test_t4_kepler_residual_and_appendix_b_series():
+    C, S = _load_series()
+    M = np.linspace(0.0, 2 * np.pi, 20001)
+    for e in (0.01, 0.05, 0.08, 0.1):
+        E = orc.kepler_solve(M, e)
+        assert np.max(np.abs(E - e * np.sin(E) - M)) <= 1e-12
+        cosE = sum(sum(float(c) * e**p for p, c in terms) * np.cos(k * M) for k, terms in C.items())
+        sinE = sum(sum(float(c) * e**p for p, c in terms) * np.sin(k * M) for k, terms in S.items())
+        # the printed series is truncated after e^6: remainder O(e^7) (measured ~1.16 e^7)
+        assert np.max(np.abs(np.cos(E) - cosE)) < 2.0 * e**7 + 1e-15
+        assert np.max(np.abs(math.sqrt(1 - e * e) * np.sin(E) - sinE)) < 2.0 * e**7 + 1e-15
+
+
+def test_kepler_against_bisection_high_eccentricity():
+    for e in (0.3, 0.7, 0.9):
+        for M in (0.1, 1.0, 2.5, 3.5, 6.0):
+            lo, hi = M - 1.0, M + 1.0
+            for _ in range(200):
+                mid = 0.5 * (lo + hi)
+                if mid - e * math.sin(mid) < M:
+                    lo = mid
+                else:
+                    hi = mid
+            assert abs(float(orc.kepler_solve(np.array([M]), e)[0]) - 0.5 * (lo + hi)) < 1e-12
+
+
+# ------------------------------------------------------------------ gather
+def test_gather_and_fill():
+    x = np.arange(8, dtype=np.float32) * 10
+    idx = np.array([0, 0, 2, 7, 8, -1, 3, 100])
+    y = orc.gather(x, idx, np.float32(-5))
+    assert y.dtype == np.float32
+    assert y.tolist() == [0, 0, 20, 70, -5, -5, 30, -5]
+    assert orc.fill_value(np.array([1, 2, 3, 6], dtype=np.float32)) == np.float32(3.0)
+
+
+# ------------------------------------------------------------------ T5 / T6: FFT
+def test_t5_parseval():
+    y = np.random.default_rng(5).standard_normal(1 << 14).astype(np.float32)
+    X = orc.rfft_forward(y)
+    n = y.size
+    lhs = np.sum(y.astype(np.float64) ** 2)
+    rhs = (abs(X[0]) ** 2 + 2 * np.sum(np.abs(X[1:-1]) ** 2) + abs(X[-1]) ** 2) / n
+    assert abs(lhs - rhs) < 1e-9 * lhs
+
+
+def test_t6_bruteforce_dft_1024():
+    n = 1024
+    y = np.random.default_rng(6).standard_normal(n).astype(np.float32)
+    jk = np.outer(np.arange(n // 2 + 1), np.arange(n))
+    brute = (np.exp(-2j * np.pi * jk / n) * y.astype(np.float64)).sum(axis=1)
+    assert np.max(np.abs(orc.rfft_forward(y) - brute)) < 1e-9
+
+
+# ------------------------------------------------------------------ T7: interbinning closed forms
+def test_t7_interbin_integer_and_half_bin_tone():
+    n, k0, A = 1 << 16, 1 << 13, 0.5
+    j = np.arange(n)
+    ref = (A * n / 2) ** 2
+    P = orc.interbin_power(orc.rfft_forward(A * np.cos(2 * np.pi * k0 * j / n)))
+    assert P.size == n // 2
+    assert abs(P[k0] / ref - 1) < 1e-9
+    assert abs(P[k0 + 1] / ref - 0.5) < 1e-9          # 1/2 |0 - X_k0|^2
+    assert P[k0 - 1] / ref < 1e-12
+    P = orc.interbin_power(orc.rfft_forward(A * np.cos(2 * np.pi * (k0 + 0.5) * j / n)))
+    assert abs(P[k0] / ref - (2 / np.pi) ** 2) < 2e-3          # raw scalloped bin: 0.405
+    assert abs(P[k0 + 1] / ref - 8 / np.pi**2) < 2e-3          # interbin recovers 0.811
+
+
+def test_dc_is_removed_before_interbinning():
+    y = np.ones(4096) * 7.0 + np.random.default_rng(1).standard_normal(4096)
+    P = orc.interbin_power(orc.rfft_forward(y))
+    assert P[0] == 0.0
+    X = orc.rfft_forward(y)
+    assert abs(P[1] - abs(X[1]) ** 2) < 1e-9 * abs(X[1]) ** 2   # no DC leakage through the difference term
+
+
+# ------------------------------------------------------------------ medians / T8
+def test_block_median_by_hand():
+    P = np.array([5, 1, 4, 2, 8, 7, 3, 6, 10, 10, 10, 10, 0, 0, 0, 1], dtype=float)
+    assert orc.block_medians(P, 8).tolist() == [4.5, 5.5]        # (4+5)/2 ; sorted 0,0,0,1,10,10,10,10 -> (1+10)/2
+
+
+def test_baseline_interpolation_by_hand():
+    m = orc.median_baseline(np.array([2.0, 4.0]), 8, 4)          # centres 1.5 and 5.5
+    assert np.allclose(m, [2, 2, 2.25, 2.75, 3.25, 3.75, 4, 4])
+
+
+def test_t8_exponential_noise_normalises_to_unit_mean():
+    P = np.random.default_rng(8).exponential(3.7, 1 << 18)
+    mb = orc.block_medians(P, 1024)
+    assert abs(np.mean(mb) / 3.7 - math.log(2)) < 0.01           # median = ln2 * mean (L77)
+    ph = orc.normalise(P, mb, 1024)
+    assert ph[0] == 0.0
+    assert abs(np.mean(ph[1:]) - 1.0) < 0.01
+
+
+# ------------------------------------------------------------------ harmonic sums
+def _round_half_up(fr: Fraction) -> int:
+    return math.floor(fr + Fraction(1, 2))
+
+
+def test_t6_harmonic_sum_bruteforce_from_eq9():
+    nb = 512
+    p = np.random.default_rng(9).exponential(1.0, nb)
+    sums = orc.harmonic_sums(p)
+    for L in range(5):
+        n = 1 << L
+        for k in range(nb):
+            s = sum(p[_round_half_up(Fraction(k * m, n))] for m in range(1, n + 1))   # eq 9
+            assert abs(sums[L][k] - s) < 1e-12
+
+
+def test_harmonic_comb():
+    nb, k0, Pk = 4096, 100, 3.0
+    p = np.zeros(nb)
+    p[[k0 * m for m in range(1, 17)]] = Pk
+    sums = orc.harmonic_sums(p)
+    for L in range(5):
+        assert sums[L][k0 << L] == Pk * (1 << L)                 # all 2^L harmonics collected
+        assert np.argmax(sums[L]) == (k0 << L) or L < 4
+    assert sums[0][k0] == Pk
+
+
+def test_harmonic_nesting_identity():
+    p = np.random.default_rng(10).exponential(1.0, 2048)
+    s = orc.harmonic_sums(p)
+    k = np.arange(2048)
+    for L in range(1, 5):
+        odd = sum(p[(k * m + (1 << (L - 1))) >> L] for m in range(1, (1 << L) + 1, 2))
+        assert np.allclose(s[L], s[L - 1] + odd, rtol=0, atol=1e-12)
+
+
+# ------------------------------------------------------------------ T9: significance
+def _golden_eq11():
+    vals, ex = {}, []
+    with open(os.path.join(GOLDEN, "eq11_constants.txt")) as f:
+        for line in f:
+            if line.startswith("#") or not line.strip():
+                continue
+            a, b, *c = line.split()
+            if a == "example":
+                ex.append((int(b), float(c[0])))
+            else:
+                vals[a] = float(b)
+    return vals, ex
+
+
+def test_t9_sigma_map_is_eq11_at_one_harmonic():
+    vals, ex = _golden_eq11()
+    mu, s = orc.sigma_constants(0)
+    assert abs(mu - vals["sqrt_pi_over_4"]) < 1e-12
+    assert abs(s - vals["sqrt_1_minus_pi_over_4"]) < 1e-12
+    for n_trials, snr in ex:
+        assert abs(float(orc.sigma_of_power(math.log(n_trials), 0)) - snr) < 5e-5
+    for L in range(5):
+        assert abs(float(orc.sigma_of_power(orc.sigma_to_power(L, 6.0), L)) - 6.0) < 1e-12
+
+
+def test_sigma_constants_against_monte_carlo():
+    rng = np.random.default_rng(17)
+    for L in range(5):
+        n = 1 << L
+        r = np.sqrt(rng.gamma(n, 1.0, 2_000_000))
+        mu, s = orc.sigma_constants(L)
+        assert abs(r.mean() - mu) < 2e-3
+        assert abs(r.std() - s) < 2e-3
+
+
+def test_lowest_bin_and_candidate_rule():
+    assert orc.lowest_bin(1 << 17, 1e-3, 0.1) == 14               # ceil(13.1072)
+    sums = {1: np.array([0.0] * 40)}
+    thr = orc.sigma_to_power(1, 6.0)
+    sums[1][27] = thr * 1.0001      # below k_lo * 2^L = 28: rejected
+    sums[1][28] = thr * 1.0001      # accepted
+    sums[1][30] = thr * 0.9999      # below threshold
+    c = orc.candidates_from_sums(sums, 5, 6.0, 14)
+    assert [(t, L, k) for t, L, k, _, _ in c] == [(5, 1, 28)]
+
+
+# ------------------------------------------------------------------ T10: end to end on C1
+def test_t10_injected_pulsar_found_with_true_template(c1):
+    x, tsamp = c1.series, c1.tsamp
+    cands = orc.search_template(x, tsamp, c1.templates[0], 0)
+    assert len(cands) > 0
+    best = max(cands, key=lambda c: c[4])
+    f_spin = 1.0 / c1.pulsars[0][0]
+    L, k = best[1], best[2]
+    assert L == 3                                   # only 10 harmonics of 50 Hz fit below Nyquist
+    assert abs(k / ((1 << L) * c1.t_obs) - f_spin) < 1.0 / c1.t_obs
+    assert best[4] > 12.0
+    # every fold peaks at the spin frequency (fold 4 at the 25 Hz alias of the 8-harmonic sum)
+    for fold, expect in ((0, 6554), (1, 13107), (2, 26214), (3, 52429)):
+        b = max((c for c in cands if c[1] == fold), key=lambda c: c[4])
+        assert abs(b[2] - expect) <= 1
+    # a wrong template and the un-resampled series do not find it
+    for tmpl in (c1.templates[5], (60.0, 0.0, 0.0, 0.0, 0.0), (60.0, 0.5, 1.0 + np.pi, 0.0, 0.0)):
+        assert orc.search_template(x, tsamp, tmpl, 1) == []
+
+
+def test_tie_distance_arbiter():
+    d = orc.tie_distance(np.array([0, 10, 100]), 1e-3, (60.0, 0.0, 0.0, 0.0, 0.0))
+    assert np.allclose(d, 0.5)                       # delta = 0 everywhere: as far from a tie as possible
+    d64 = orc.shift_in_samples(np.arange(5000), 1e-3, (60.0, 0.5, 1.0, 0.0, 0.0))
+    dl = orc.tie_distance(np.arange(5000), 1e-3, (60.0, 0.5, 1.0, 0.0, 0.0))
+    assert np.max(np.abs(np.abs((d64 - np.floor(d64)) - 0.5) - dl)) < 1e-9
