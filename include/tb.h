@@ -1,0 +1,170 @@
+/* tb.h -- C ABI of libtb: template-bank binary-pulsar search, per-template hot path on one
+ * NVIDIA B200 (sm_100a).  Method: Balakrishnan et al., arXiv:2112.11991; citations below are
+ * lines of PAPER.md (the paper text) and readings G<n> of DESIGN.md section 3.
+ *
+ * For every orbital template the library
+ *   a1  derives per-template constants and the zero offset            (Alg. 1)
+ *   a2  evaluates the Roemer delay of every output sample             (eq A1, eq 3,
+ *       circular closed form or per-sample Kepler solve                Alg. 1)
+ *   a3  gathers the nearest input sample (nearest-neighbour resampling) (L664, L702)
+ *   a4  takes the real-to-complex FFT                                   (L144, L706)
+ *   a5  forms the interbinned power spectrum                            (G12-G14)
+ *   a6  takes block medians, a7 normalises by the interpolated median   (L660 "de-reddening", G15)
+ *   a8  sums 1, 2, 4, 8, 16 harmonics                                   (eq 9, G16)
+ *   a9  thresholds in sigma and compacts candidates on the device       (eq 11, G17, G19)
+ *   a10 returns the candidate list sorted by (template, fold, bin).
+ * All of a1-a9 run in hand-written CUDA kernels plus one batched cuFFT R2C call; there is no CPU
+ * fallback: every entry point that needs the GPU fails with TB_ERR_CUDA when none is usable.
+ *
+ * Conventions
+ *   - Every function returns TB_OK (0) or a negative TB_ERR_* code; nothing throws, aborts or
+ *     prints.  tb_last_error(plan) gives a detail string owned by the plan (valid until the next
+ *     call on that plan); tb_strerror(code) a static string.
+ *   - "host" pointers are ordinary CPU memory, "device" pointers are CUDA device memory on the
+ *     plan's device.  The caller owns every buffer it passes in or receives results in; the
+ *     plan owns all memory it allocates and frees it in tb_plan_destroy.
+ *   - Work is queued on the plan's stream (opts.stream, or a stream the plan creates).
+ *     tb_search_templates returns once the work is queued (host template staging is complete);
+ *     tb_get_candidates / tb_get_timings / tb_debug_* synchronise that stream.
+ *   - No global state; plans are independent; one plan must not be used from two threads at once.
+ */
+#ifndef TB_H_
+#define TB_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(__GNUC__)
+#define TB_API __attribute__((visibility("default")))
+#else
+#define TB_API
+#endif
+
+#define TB_OK                 0
+#define TB_ERR_INVALID_ARG   -1   /* null pointer, N not a power of two >= 2*W, tsamp <= 0, fold > 4, bad template */
+#define TB_ERR_CUDA          -2   /* a CUDA runtime call failed (including "no device") */
+#define TB_ERR_CUFFT         -3   /* a cuFFT call failed */
+#define TB_ERR_NOMEM         -4   /* host or device allocation failed */
+#define TB_ERR_OVERFLOW      -5   /* more candidates than opts.max_candidates were produced */
+#define TB_ERR_CAPACITY      -6   /* caller's output buffer is too small; nothing was consumed */
+
+#define TB_MAX_FOLD           4   /* folds L = 0..4 <=> 1, 2, 4, 8, 16 summed harmonics (eq 9) */
+
+typedef struct tb_plan tb_plan;   /* opaque */
+
+/* One orbital template ({tau, Omega, alpha, psi, e}; BASELINE's names).
+ *   p_orb_s   orbital period P_orb = 2 pi / Omega, seconds, finite and > 0
+ *   tau_lts   projected semi-major axis a sin(i)/c, light-seconds, >= 0
+ *   phi0_rad  initial orbital phase alpha (mean anomaly at t = 0), radians, finite
+ *   ecc       eccentricity e, 0 <= e < 1
+ *   omega_rad longitude of periastron psi, radians, finite
+ * ecc == 0 && omega_rad == 0 selects the circular closed form Delta = tau sin(Omega t + phi0)
+ * (eq 4 L49 / eq A1 at e = 0); anything else the Kepler solve of eq 3 + eq A1. */
+typedef struct {
+    double p_orb_s, tau_lts, phi0_rad, ecc, omega_rad;
+} tb_template;                    /* 40 bytes */
+
+/* One detection: S_L[bin] >= threshold (eq 9; G19).  The fundamental spin frequency of the
+ * candidate is bin / (2^fold * N * tsamp) Hz (G16: bin indexes the highest summed harmonic). */
+typedef struct {
+    uint32_t template_id;         /* first_template_id + index in the tmpl array */
+    uint32_t fold;                /* L, 0..4 */
+    uint32_t bin;                 /* k, k_lo*2^L <= k < N/2 */
+    float    power;               /* S_L[k], normalised summed power (fp32) */
+    float    sigma;               /* (sqrt(S) - mu_n) / s_n, n = 2^L (eq 11 at n = 1; G17) */
+    uint32_t pad;                 /* 0 */
+} tb_candidate;                   /* 24 bytes */
+
+/* Plan options.  Zero-initialise, set struct_size = sizeof(tb_plan_opts), then override.
+ * A field left 0 takes the default in brackets. */
+typedef struct {
+    uint32_t struct_size;
+    int32_t  device;              /* CUDA device ordinal [0] */
+    void*    stream;              /* cudaStream_t to queue on; NULL -> the plan creates its own */
+    uint32_t median_window;       /* W: power of two, 128..2048 [1024] (BASELINE C1) */
+    double   f_min_hz;            /* lowest searched fundamental frequency [0.1] (G20); <0 -> 0 */
+    uint64_t max_candidates;      /* capacity of the device candidate buffer [1<<22] */
+    uint32_t chunk_templates;     /* templates per launch group B; 0 -> chosen from free memory */
+    int32_t  series_is_device_ptr;/* 0: series is host memory and is copied; 1: series is device
+                                     memory on `device`, borrowed, must outlive the plan */
+    int32_t  has_fill;            /* 0: out-of-range samples take the fp64 mean of the series,
+                                     rounded to fp32 (G8); 1: they take fill_value */
+    float    fill_value;
+    int32_t  enable_timings;      /* 1: record CUDA events around every stage of every chunk */
+    int32_t  reserved;
+} tb_plan_opts;
+
+/* Per-stage device time of the last tb_search_templates call (CUDA events, summed over chunks;
+ * zero unless opts.enable_timings), and the byte model of DESIGN.md section 7. */
+typedef struct {
+    double   ms_resample, ms_fft, ms_spectrum /* a5+a6: spectrum + block medians */, ms_normalise, ms_hsum, ms_total;
+    uint64_t n_templates, n_samples, n_chunks, chunk_templates;
+    uint64_t model_bytes_per_template;   /* 22*N: algorithmic HBM bytes */
+} tb_timings;
+
+/* Create a plan for one dedispersed time series S[i], i*tsamp.
+ *   out        receives the plan (set to NULL on failure)
+ *   series     float32[n_samples], host (copied) or device (borrowed) per opts
+ *   n_samples  N, a power of two, 2*W <= N <= 2^28
+ *   tsamp_s    sampling time in seconds, > 0
+ *   opts       may be NULL (all defaults)
+ * Allocates every device buffer the search needs (series, B resampled series, B spectra, the
+ * candidate buffer, the cuFFT plan and its work area): TB_ERR_NOMEM if that does not fit. */
+TB_API int tb_plan_create(tb_plan** out, const float* series, uint64_t n_samples, double tsamp_s,
+                   const tb_plan_opts* opts);
+
+/* Search `n_templates` templates (host array) and APPEND the detections to the plan's device
+ * candidate buffer (steps a1-a9).  template_id of tmpl[i] is first_template_id + i.
+ *   folds / n_folds   the harmonic folds to threshold: distinct values from {0,1,2,3,4}
+ *   sigma_threshold   candidates have sigma_L >= sigma_threshold (finite)
+ * Invalid templates make the whole call fail with TB_ERR_INVALID_ARG before any work is queued.
+ * n_templates == 0 is valid and does nothing. */
+TB_API int tb_search_templates(tb_plan* plan, const tb_template* tmpl, uint64_t n_templates,
+                        uint32_t first_template_id, const uint32_t* folds, uint32_t n_folds,
+                        double sigma_threshold);
+
+/* Copy the accumulated candidates to `out` (host, capacity entries), sorted by
+ * (template_id, fold, bin); *n_total receives the number produced since the last clear.
+ *   out == NULL or capacity < count -> TB_ERR_CAPACITY, *n_total set, nothing consumed
+ *   count > max_candidates          -> TB_ERR_OVERFLOW, *n_total = true count, the first
+ *                                      max_candidates stored entries are returned if they fit
+ * A successful full read clears the buffer (so does tb_clear_candidates). */
+TB_API int tb_get_candidates(tb_plan* plan, tb_candidate* out, uint64_t capacity, uint64_t* n_total);
+TB_API int tb_clear_candidates(tb_plan* plan);
+TB_API int tb_plan_destroy(tb_plan* plan);      /* NULL is allowed */
+
+TB_API const char* tb_strerror(int code);
+TB_API const char* tb_last_error(const tb_plan* plan);
+
+/* ---- measurement and parity taps (not on the timed path) ---- */
+TB_API int tb_get_timings(tb_plan* plan, tb_timings* out);
+
+/* Source index idx_j = j - floor(delta_j + 1/2) of every output sample of one template, exactly
+ * as the resampling kernel computes it (same device function), before the range check.
+ * idx_out: host int64[N]. */
+TB_API int tb_debug_resample_indices(tb_plan* plan, const tb_template* tmpl, int64_t* idx_out);
+
+/* Spectra of one template through the production kernels: interbinned powers P_k (a5),
+ * normalised powers P^_k (a7), both float32[N/2], and block medians float32[N/2/W] (a6).
+ * Any output pointer may be NULL.  Host buffers. */
+TB_API int tb_debug_spectrum(tb_plan* plan, const tb_template* tmpl, float* p_interbinned,
+                      float* p_normalised, float* medians);
+
+/* Resampled series y_j of one template (a3): host float32[N]. */
+TB_API int tb_debug_resampled(tb_plan* plan, const tb_template* tmpl, float* y_out);
+
+/* Host fp64: the summed power at which sigma_L equals `sigma` (G17).  fold 0..4. */
+TB_API int tb_sigma_to_power(uint32_t fold, double sigma, double* power_out);
+
+/* Plan facts for harnesses: fill value in use, chunk size B, lowest bin k_lo, and the Hermite
+ * knot spacing (log2, 0 = every sample exact) the resampler would choose for a template. */
+TB_API int tb_plan_info(const tb_plan* plan, float* fill_value, uint32_t* chunk_templates, uint32_t* k_lo);
+TB_API int tb_template_knot_log2(const tb_plan* plan, const tb_template* tmpl, int32_t* log2_h);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TB_H_ */

@@ -1,0 +1,643 @@
+// tb_api.cu -- host side of libtb: plan, template constants (a1), chunked launch sequence,
+// candidate retrieval (a10), timings and parity taps.  Boundary: include/tb.h.
+#include "../../include/tb.h"
+#include "tb_kernels.cuh"
+
+#include <cufft.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <limits>
+#include <map>
+#include <new>
+#include <string>
+#include <vector>
+
+using namespace tb;
+
+static_assert(sizeof(tb_candidate) == 24 && sizeof(Candidate) == 24, "candidate layout");
+static_assert(sizeof(tb_template) == 40, "template layout");
+
+namespace {
+
+constexpr int N_STAGE_EVENTS = 6;   // start, resample, fft, spectrum+median, normalise, hsum
+
+struct EventSet { cudaEvent_t e[N_STAGE_EVENTS]; };
+
+}  // namespace
+
+struct tb_plan {
+    int device = 0;
+    cudaStream_t stream = nullptr;
+    bool own_stream = false;
+    uint64_t n = 0, nb = 0;
+    double tsamp = 0.0;
+    uint32_t window = 1024, log2w = 10, nblk = 0;
+    double f_min = 0.1;
+    uint32_t k_lo = 0;
+    uint64_t max_cand = 0;
+    uint32_t chunk = 0;
+    bool timings = false;
+    float fill = 0.f;
+    size_t ld = 0;                                   // complex row stride of the FFT output
+
+    const float* d_series = nullptr;
+    float* d_series_owned = nullptr;
+    float* d_resampled = nullptr;                    // [chunk][n]
+    float2* d_fft = nullptr;                         // [chunk][ld]
+    float* d_power = nullptr;                        // [chunk][nb]
+    float* d_med = nullptr;                          // [chunk][nblk]
+    Candidate* d_cand = nullptr;
+    unsigned long long* d_cursor = nullptr;
+    TmplDev* d_tmpl = nullptr;
+    size_t tmpl_cap = 0;
+    TmplDev* h_tmpl = nullptr;                       // pinned staging
+    size_t h_tmpl_cap = 0;
+    cudaEvent_t ev_staged = nullptr;                 // the last template upload has been consumed
+    bool staged_pending = false;
+
+    std::map<uint32_t, cufftHandle> fft_plans;       // by batch size, sharing one work area
+    void* d_work = nullptr;
+    size_t work_bytes = 0;
+
+    std::vector<EventSet> events;
+    size_t events_used = 0;
+    tb_timings last = {};
+
+    std::string err;
+};
+
+namespace {
+
+int fail(tb_plan* p, int code, const std::string& msg)
+{
+    if (p) p->err = msg;
+    return code;
+}
+
+#define TB_CUDA(p, call)                                                                               \
+    do {                                                                                               \
+        cudaError_t e__ = (call);                                                                      \
+        if (e__ != cudaSuccess)                                                                        \
+            return fail((p), e__ == cudaErrorMemoryAllocation ? TB_ERR_NOMEM : TB_ERR_CUDA,            \
+                        std::string(#call) + ": " + cudaGetErrorString(e__));                          \
+    } while (0)
+
+#define TB_CUFFT(p, call)                                                                              \
+    do {                                                                                               \
+        cufftResult r__ = (call);                                                                      \
+        if (r__ != CUFFT_SUCCESS)                                                                      \
+            return fail((p), r__ == CUFFT_ALLOC_FAILED ? TB_ERR_NOMEM : TB_ERR_CUFFT,                  \
+                        std::string(#call) + ": cufft error " + std::to_string((int)r__));             \
+    } while (0)
+
+bool is_pow2(uint64_t v) { return v && !(v & (v - 1)); }
+uint32_t ilog2(uint64_t v) { uint32_t l = 0; while ((1ull << (l + 1)) <= v) ++l; return l; }
+
+// sigma map (G17): sqrt(S) for S ~ Gamma(n,1) has mean Gamma(n+1/2)/Gamma(n), variance n - mean^2
+void sigma_constants(uint32_t fold, double* mu, double* s)
+{
+    const uint32_t n = 1u << fold;
+    double m = 0.88622692545275801365;                 // Gamma(3/2)/Gamma(1) = sqrt(pi)/2
+    for (uint32_t i = 1; i < n; ++i) m *= ((double)i + 0.5) / (double)i;   // Gamma(i+3/2)/Gamma(i+1)
+    *mu = m;
+    *s = std::sqrt((double)n - m * m);
+}
+
+// Knot spacing of the cubic Hermite interpolation of the delay: the largest
+// h = 2^l <= 128 with  (h w)^4 / 384 * (tau/tsamp) * K(e) <= 2e-11 samples, where
+// K(e) = R^4 + 11 e R^5 + 25 e^2 R^6 + 15 e^3 R^7, R = 1/(1-e), bounds the 4th derivative of
+// A cos E + B sin E with respect to the mean anomaly.
+int knot_log2(double tau_over_tsamp, double w, double e)
+{
+    const double R = 1.0 / (1.0 - e);
+    const double K = std::pow(R, 4) + 11 * e * std::pow(R, 5) + 25 * e * e * std::pow(R, 6) + 15 * e * e * e * std::pow(R, 7);
+    int l = 7;
+    for (; l > 0; --l) {
+        const double hw = std::ldexp(w, l);
+        if (hw * hw * hw * hw / 384.0 * tau_over_tsamp * K <= 2e-11) break;
+    }
+    return l;
+}
+
+int validate_template(const tb_template& t, double tsamp, std::string* why)
+{
+    auto bad = [&](const char* m) { *why = m; return TB_ERR_INVALID_ARG; };
+    if (!std::isfinite(t.p_orb_s) || t.p_orb_s <= 0) return bad("template: p_orb_s must be finite and > 0");
+    if (!std::isfinite(t.tau_lts) || t.tau_lts < 0) return bad("template: tau_lts must be finite and >= 0");
+    if (!std::isfinite(t.phi0_rad) || !std::isfinite(t.omega_rad)) return bad("template: phi0/omega must be finite");
+    if (!(t.ecc >= 0 && t.ecc < 1)) return bad("template: ecc must be in [0, 1)");
+    if (2.0 * t.tau_lts * (1 + t.ecc) / tsamp >= 1073741824.0) return bad("template: shift exceeds 2^30 samples");
+    return TB_OK;
+}
+
+// step a1, in long double so that the constants are correctly rounded doubles
+void make_tmpl(const tb_template& t, double tsamp, TmplDev* o)
+{
+    const long double two_pi = 8.0L * atanl(1.0L);
+    const long double c = (long double)tsamp / (long double)t.p_orb_s;
+    o->c_hi = (double)c;
+    o->c_lo = (double)(c - (long double)o->c_hi);
+    o->w = (double)(two_pi * c);
+    long double phi = fmodl((long double)t.phi0_rad, two_pi);
+    if (phi < 0) phi += two_pi;
+    o->phi0 = (double)phi;
+    const long double e = t.ecc, g = (long double)t.tau_lts / (long double)tsamp;
+    const long double A = g * sinl((long double)t.omega_rad);
+    const long double B = g * sqrtl(1.0L - e * e) * cosl((long double)t.omega_rad);
+    o->A = (double)A;
+    o->B = (double)B;
+    o->ecc = t.ecc;
+    o->circular = (t.ecc == 0.0) ? 1 : 0;
+    // zero offset: E0 from M = phi0 (Alg. 1)
+    const long double M = (long double)o->phi0;
+    long double E = M + e * sinl(M);
+    for (int it = 0; it < 100; ++it) {
+        const long double dE = (E - e * sinl(E) - M) / (1.0L - e * cosl(E));
+        E -= dE;
+        if (fabsl(dE) < 1e-19L) break;
+    }
+    o->d0 = (double)((long double)o->A * cosl(E) + (long double)o->B * sinl(E));
+    o->log2h = knot_log2((double)g, o->w, t.ecc);
+}
+
+int get_fft_plan(tb_plan* p, uint32_t batch, cufftHandle* out)
+{
+    auto it = p->fft_plans.find(batch);
+    if (it != p->fft_plans.end()) { *out = it->second; return TB_OK; }
+    cufftHandle h;
+    TB_CUFFT(p, cufftCreate(&h));
+    cufftResult r = cufftSetAutoAllocation(h, 0);
+    long long nn[1] = {(long long)p->n};
+    long long inembed[1] = {(long long)p->n};
+    long long onembed[1] = {(long long)p->ld};
+    size_t ws = 0;
+    if (r == CUFFT_SUCCESS)
+        r = cufftMakePlanMany64(h, 1, nn, inembed, 1, (long long)p->n, onembed, 1, (long long)p->ld, CUFFT_R2C,
+                                (long long)batch, &ws);
+    if (r != CUFFT_SUCCESS) {
+        cufftDestroy(h);
+        return fail(p, r == CUFFT_ALLOC_FAILED ? TB_ERR_NOMEM : TB_ERR_CUFFT,
+                    "cufftMakePlanMany64 failed: " + std::to_string((int)r));
+    }
+    if (ws > p->work_bytes) {
+        TB_CUDA(p, cudaStreamSynchronize(p->stream));
+        if (p->d_work) cudaFree(p->d_work);
+        p->d_work = nullptr;
+        p->work_bytes = 0;
+        cudaError_t e = cudaMalloc(&p->d_work, ws);
+        if (e != cudaSuccess) { cufftDestroy(h); return fail(p, TB_ERR_NOMEM, "cuFFT work area allocation failed"); }
+        p->work_bytes = ws;
+        for (auto& kv : p->fft_plans) TB_CUFFT(p, cufftSetWorkArea(kv.second, p->d_work));
+    }
+    TB_CUFFT(p, cufftSetWorkArea(h, p->d_work));
+    TB_CUFFT(p, cufftSetStream(h, p->stream));
+    p->fft_plans[batch] = h;
+    *out = h;
+    return TB_OK;
+}
+
+template <int W>
+void launch_spectrum(tb_plan* p, uint32_t nt)
+{
+    const int cta_per_row = (int)((p->nblk + SP_WARPS - 1) / SP_WARPS);
+    k_spectrum_median<W><<<(unsigned)(cta_per_row * nt), SP_WARPS * 32, 0, p->stream>>>(
+        p->d_fft, p->ld, p->d_power, p->d_med, (int)p->nb, (int)p->nblk, cta_per_row);
+}
+
+// stages of one chunk of nt templates whose constants sit at d_tmpl + off
+int run_resample(tb_plan* p, size_t off, uint32_t nt, long long* d_idx)
+{
+    const int tile = (int)std::min<uint64_t>(RS_TILE, p->n);
+    const unsigned grid = (unsigned)((p->n / tile) * nt);
+    if (d_idx)
+        k_resample<true><<<grid, RS_THREADS, 0, p->stream>>>(p->d_series, p->d_resampled, p->d_tmpl + off, (int)nt,
+                                                             (int)p->n, tile, p->fill, d_idx);
+    else
+        k_resample<false><<<grid, RS_THREADS, 0, p->stream>>>(p->d_series, p->d_resampled, p->d_tmpl + off, (int)nt,
+                                                              (int)p->n, tile, p->fill, nullptr);
+    TB_CUDA(p, cudaGetLastError());
+    return TB_OK;
+}
+
+int run_fft(tb_plan* p, uint32_t nt)
+{
+    cufftHandle h;
+    int rc = get_fft_plan(p, nt, &h);
+    if (rc) return rc;
+    TB_CUFFT(p, cufftExecR2C(h, p->d_resampled, reinterpret_cast<cufftComplex*>(p->d_fft)));
+    return TB_OK;
+}
+
+int run_spectrum(tb_plan* p, uint32_t nt)
+{
+    switch (p->window) {
+        case 128: launch_spectrum<128>(p, nt); break;
+        case 256: launch_spectrum<256>(p, nt); break;
+        case 512: launch_spectrum<512>(p, nt); break;
+        case 1024: launch_spectrum<1024>(p, nt); break;
+        case 2048: launch_spectrum<2048>(p, nt); break;
+        default: return fail(p, TB_ERR_INVALID_ARG, "median_window");
+    }
+    TB_CUDA(p, cudaGetLastError());
+    return TB_OK;
+}
+
+int run_normalise(tb_plan* p, uint32_t nt)
+{
+    const int cta_per_row = (int)((p->nb + 1023) / 1024);
+    k_normalise<<<(unsigned)(cta_per_row * nt), 256, 0, p->stream>>>(p->d_power, p->d_med, (int)p->nb, (int)p->nblk,
+                                                                     (int)p->log2w, cta_per_row);
+    TB_CUDA(p, cudaGetLastError());
+    return TB_OK;
+}
+
+int run_hsum(tb_plan* p, uint32_t nt, const FoldParams& fp, uint32_t first_id)
+{
+    const int cta_per_row = (int)((p->nb + 255) / 256);
+    k_hsum_threshold<<<(unsigned)(cta_per_row * nt), 256, 0, p->stream>>>(p->d_power, (int)p->nb, cta_per_row, fp,
+                                                                          first_id, p->d_cand, p->d_cursor,
+                                                                          (unsigned long long)p->max_cand);
+    TB_CUDA(p, cudaGetLastError());
+    return TB_OK;
+}
+
+int upload_templates(tb_plan* p, const tb_template* tmpl, uint64_t k)
+{
+    for (uint64_t i = 0; i < k; ++i) {
+        std::string why;
+        if (validate_template(tmpl[i], p->tsamp, &why)) return fail(p, TB_ERR_INVALID_ARG, why + " (index " + std::to_string(i) + ")");
+    }
+    if (p->staged_pending) {
+        TB_CUDA(p, cudaEventSynchronize(p->ev_staged));
+        p->staged_pending = false;
+    }
+    if (k > p->h_tmpl_cap) {
+        if (p->h_tmpl) cudaFreeHost(p->h_tmpl);
+        p->h_tmpl = nullptr; p->h_tmpl_cap = 0;
+        TB_CUDA(p, cudaMallocHost(&p->h_tmpl, k * sizeof(TmplDev)));
+        p->h_tmpl_cap = k;
+    }
+    if (k > p->tmpl_cap) {
+        TB_CUDA(p, cudaStreamSynchronize(p->stream));
+        if (p->d_tmpl) cudaFree(p->d_tmpl);
+        p->d_tmpl = nullptr; p->tmpl_cap = 0;
+        TB_CUDA(p, cudaMalloc(&p->d_tmpl, k * sizeof(TmplDev)));
+        p->tmpl_cap = k;
+    }
+    for (uint64_t i = 0; i < k; ++i) make_tmpl(tmpl[i], p->tsamp, &p->h_tmpl[i]);
+    TB_CUDA(p, cudaMemcpyAsync(p->d_tmpl, p->h_tmpl, k * sizeof(TmplDev), cudaMemcpyHostToDevice, p->stream));
+    TB_CUDA(p, cudaEventRecord(p->ev_staged, p->stream));
+    p->staged_pending = true;
+    return TB_OK;
+}
+
+int make_fold_params(tb_plan* p, const uint32_t* folds, uint32_t n_folds, double sigma, FoldParams* fp)
+{
+    if (!std::isfinite(sigma)) return fail(p, TB_ERR_INVALID_ARG, "sigma_threshold must be finite");
+    if (n_folds > 0 && !folds) return fail(p, TB_ERR_INVALID_ARG, "folds is NULL");
+    bool seen[5] = {false, false, false, false, false};
+    for (uint32_t i = 0; i < n_folds; ++i) {
+        if (folds[i] > TB_MAX_FOLD) return fail(p, TB_ERR_INVALID_ARG, "fold > 4");
+        if (seen[folds[i]]) return fail(p, TB_ERR_INVALID_ARG, "duplicate fold");
+        seen[folds[i]] = true;
+    }
+    for (uint32_t L = 0; L < 5; ++L) {
+        double mu, s;
+        sigma_constants(L, &mu, &s);
+        fp->mu[L] = (float)mu;
+        fp->inv_s[L] = (float)(1.0 / s);
+        const double root = mu + sigma * s;
+        fp->thr[L] = seen[L] ? (root <= 0 ? 0.f : (float)(root * root)) : std::numeric_limits<float>::infinity();
+    }
+    fp->k_lo = p->k_lo;
+    return TB_OK;
+}
+
+void destroy(tb_plan* p)
+{
+    if (!p) return;
+    cudaSetDevice(p->device);
+    if (p->stream) cudaStreamSynchronize(p->stream);
+    for (auto& kv : p->fft_plans) cufftDestroy(kv.second);
+    for (auto& es : p->events) for (auto& e : es.e) cudaEventDestroy(e);
+    if (p->ev_staged) cudaEventDestroy(p->ev_staged);
+    cudaFree(p->d_work); cudaFree(p->d_series_owned); cudaFree(p->d_resampled); cudaFree(p->d_fft);
+    cudaFree(p->d_power); cudaFree(p->d_med); cudaFree(p->d_cand); cudaFree(p->d_cursor); cudaFree(p->d_tmpl);
+    if (p->h_tmpl) cudaFreeHost(p->h_tmpl);
+    if (p->own_stream && p->stream) cudaStreamDestroy(p->stream);
+    delete p;
+}
+
+int single_template_stage(tb_plan* p, const tb_template* tmpl)
+{
+    if (!p || !tmpl) return fail(p, TB_ERR_INVALID_ARG, "null argument");
+    TB_CUDA(p, cudaSetDevice(p->device));
+    return upload_templates(p, tmpl, 1);
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* tb_strerror(int code)
+{
+    switch (code) {
+        case TB_OK: return "ok";
+        case TB_ERR_INVALID_ARG: return "invalid argument";
+        case TB_ERR_CUDA: return "CUDA error";
+        case TB_ERR_CUFFT: return "cuFFT error";
+        case TB_ERR_NOMEM: return "out of memory";
+        case TB_ERR_OVERFLOW: return "candidate buffer overflow";
+        case TB_ERR_CAPACITY: return "output buffer too small";
+        default: return "unknown error";
+    }
+}
+
+const char* tb_last_error(const tb_plan* plan) { return plan ? plan->err.c_str() : "null plan"; }
+
+int tb_sigma_to_power(uint32_t fold, double sigma, double* power_out)
+{
+    if (fold > TB_MAX_FOLD || !power_out || !std::isfinite(sigma)) return TB_ERR_INVALID_ARG;
+    double mu, s;
+    sigma_constants(fold, &mu, &s);
+    const double r = mu + sigma * s;
+    *power_out = r <= 0 ? 0.0 : r * r;
+    return TB_OK;
+}
+
+int tb_plan_create(tb_plan** out, const float* series, uint64_t n_samples, double tsamp_s, const tb_plan_opts* uopts)
+{
+    if (!out) return TB_ERR_INVALID_ARG;
+    *out = nullptr;
+    tb_plan_opts o;
+    std::memset(&o, 0, sizeof(o));
+    if (uopts) {
+        if (uopts->struct_size < 8 || uopts->struct_size > sizeof(o)) return TB_ERR_INVALID_ARG;
+        std::memcpy(&o, uopts, uopts->struct_size);
+    }
+    const uint32_t W = o.median_window ? o.median_window : 1024;
+    if (!series || !(tsamp_s > 0) || !std::isfinite(tsamp_s)) return TB_ERR_INVALID_ARG;
+    if (!is_pow2(W) || W < 128 || W > 2048) return TB_ERR_INVALID_ARG;
+    if (!is_pow2(n_samples) || n_samples < 2ull * W || n_samples > (1ull << 28)) return TB_ERR_INVALID_ARG;
+
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || o.device < 0 || o.device >= ndev) return TB_ERR_CUDA;
+
+    tb_plan* p = new (std::nothrow) tb_plan;
+    if (!p) return TB_ERR_NOMEM;
+    p->device = o.device;
+    p->n = n_samples;
+    p->nb = n_samples / 2;
+    p->tsamp = tsamp_s;
+    p->window = W;
+    p->log2w = ilog2(W);
+    p->nblk = (uint32_t)(p->nb / W);
+    p->f_min = (o.f_min_hz == 0.0) ? 0.1 : (o.f_min_hz < 0 ? 0.0 : o.f_min_hz);
+    p->k_lo = (uint32_t)std::min<double>(std::ceil(p->f_min * ((double)n_samples * tsamp_s)), 4294967295.0);
+    p->max_cand = o.max_candidates ? o.max_candidates : (1ull << 22);
+    p->timings = o.enable_timings != 0;
+    p->ld = p->nb + 4;                                // N/2+1 bins padded to a multiple of 4 complex (32 B)
+
+    auto bail = [&](int code, const std::string& m) { (void)m; destroy(p); return code; };
+#define TB_TRY(call)                                                                                   \
+    do {                                                                                               \
+        cudaError_t e__ = (call);                                                                      \
+        if (e__ != cudaSuccess)                                                                        \
+            return bail(e__ == cudaErrorMemoryAllocation ? TB_ERR_NOMEM : TB_ERR_CUDA, #call);         \
+    } while (0)
+
+    TB_TRY(cudaSetDevice(p->device));
+    if (o.stream) p->stream = (cudaStream_t)o.stream;
+    else { TB_TRY(cudaStreamCreateWithFlags(&p->stream, cudaStreamNonBlocking)); p->own_stream = true; }
+    TB_TRY(cudaEventCreateWithFlags(&p->ev_staged, cudaEventDisableTiming));
+
+    // chunk size B
+    const size_t per_t = (size_t)p->n * 4 + p->ld * 8 + (size_t)p->nb * 4 + (size_t)p->nblk * 4;
+    uint32_t B = o.chunk_templates;
+    if (B == 0) {
+        size_t free_b = 0, total_b = 0;
+        TB_TRY(cudaMemGetInfo(&free_b, &total_b));
+        const uint64_t by_size = std::max<uint64_t>(1, (1ull << 29) / p->n);
+        const uint64_t by_mem = std::max<uint64_t>(1, (uint64_t)(0.5 * (double)free_b) / (per_t * 2));   // x2: cuFFT work area
+        B = (uint32_t)std::min<uint64_t>(std::min<uint64_t>(by_size, by_mem), 256);
+    }
+    p->chunk = B;
+
+    // series + fill value
+    if (o.series_is_device_ptr) {
+        p->d_series = series;
+    } else {
+        TB_TRY(cudaMalloc(&p->d_series_owned, p->n * sizeof(float)));
+        TB_TRY(cudaMemcpyAsync(p->d_series_owned, series, p->n * sizeof(float), cudaMemcpyHostToDevice, p->stream));
+        p->d_series = p->d_series_owned;
+    }
+    if (o.has_fill) {
+        p->fill = o.fill_value;
+    } else if (!o.series_is_device_ptr) {
+        long double s = 0.0L;
+        for (uint64_t i = 0; i < p->n; ++i) s += (long double)series[i];
+        p->fill = (float)(double)(s / (long double)p->n);
+    } else {
+        double* d_acc = nullptr;
+        double acc = 0.0;
+        TB_TRY(cudaMalloc(&d_acc, sizeof(double)));
+        TB_TRY(cudaMemsetAsync(d_acc, 0, sizeof(double), p->stream));
+        k_sum_f64<<<296, 256, 0, p->stream>>>(p->d_series, (size_t)p->n, d_acc);
+        TB_TRY(cudaMemcpyAsync(&acc, d_acc, sizeof(double), cudaMemcpyDeviceToHost, p->stream));
+        TB_TRY(cudaStreamSynchronize(p->stream));
+        cudaFree(d_acc);
+        p->fill = (float)(acc / (double)p->n);
+    }
+
+    TB_TRY(cudaMalloc(&p->d_resampled, (size_t)B * p->n * sizeof(float)));
+    TB_TRY(cudaMalloc(&p->d_fft, (size_t)B * p->ld * sizeof(float2)));
+    TB_TRY(cudaMalloc(&p->d_power, (size_t)B * p->nb * sizeof(float)));
+    TB_TRY(cudaMalloc(&p->d_med, (size_t)B * p->nblk * sizeof(float)));
+    TB_TRY(cudaMalloc(&p->d_cand, p->max_cand * sizeof(Candidate)));
+    TB_TRY(cudaMalloc(&p->d_cursor, sizeof(unsigned long long)));
+    TB_TRY(cudaMemsetAsync(p->d_cursor, 0, sizeof(unsigned long long), p->stream));
+#undef TB_TRY
+    cufftHandle h;
+    int rc = get_fft_plan(p, B, &h);
+    if (rc) { destroy(p); return rc; }
+    if (cudaStreamSynchronize(p->stream) != cudaSuccess) { destroy(p); return TB_ERR_CUDA; }
+    *out = p;
+    return TB_OK;
+}
+
+int tb_plan_destroy(tb_plan* plan)
+{
+    destroy(plan);
+    return TB_OK;
+}
+
+int tb_plan_info(const tb_plan* plan, float* fill_value, uint32_t* chunk_templates, uint32_t* k_lo)
+{
+    if (!plan) return TB_ERR_INVALID_ARG;
+    if (fill_value) *fill_value = plan->fill;
+    if (chunk_templates) *chunk_templates = plan->chunk;
+    if (k_lo) *k_lo = plan->k_lo;
+    return TB_OK;
+}
+
+int tb_template_knot_log2(const tb_plan* plan, const tb_template* tmpl, int32_t* log2_h)
+{
+    if (!plan || !tmpl || !log2_h) return TB_ERR_INVALID_ARG;
+    std::string why;
+    if (validate_template(*tmpl, plan->tsamp, &why)) return TB_ERR_INVALID_ARG;
+    TmplDev d;
+    make_tmpl(*tmpl, plan->tsamp, &d);
+    *log2_h = d.log2h;
+    return TB_OK;
+}
+
+int tb_search_templates(tb_plan* p, const tb_template* tmpl, uint64_t n_templates, uint32_t first_template_id,
+                        const uint32_t* folds, uint32_t n_folds, double sigma_threshold)
+{
+    if (!p) return TB_ERR_INVALID_ARG;
+    if (n_templates && !tmpl) return fail(p, TB_ERR_INVALID_ARG, "tmpl is NULL");
+    if (n_templates > 0xffffffffull - first_template_id) return fail(p, TB_ERR_INVALID_ARG, "template ids overflow 32 bits");
+    FoldParams fp;
+    int rc = make_fold_params(p, folds, n_folds, sigma_threshold, &fp);
+    if (rc) return rc;
+    TB_CUDA(p, cudaSetDevice(p->device));
+    p->last = {};
+    p->events_used = 0;
+    p->last.n_templates = n_templates;
+    p->last.n_samples = p->n;
+    p->last.chunk_templates = p->chunk;
+    p->last.model_bytes_per_template = 22ull * p->n;
+    if (n_templates == 0) return TB_OK;
+    rc = upload_templates(p, tmpl, n_templates);
+    if (rc) return rc;
+
+    for (uint64_t off = 0; off < n_templates; off += p->chunk) {
+        const uint32_t nt = (uint32_t)std::min<uint64_t>(p->chunk, n_templates - off);
+        EventSet* es = nullptr;
+        if (p->timings) {
+            if (p->events_used == p->events.size()) {
+                EventSet ne;
+                for (auto& e : ne.e) TB_CUDA(p, cudaEventCreate(&e));
+                p->events.push_back(ne);
+            }
+            es = &p->events[p->events_used++];
+            TB_CUDA(p, cudaEventRecord(es->e[0], p->stream));
+        }
+        if ((rc = run_resample(p, off, nt, nullptr))) return rc;
+        if (es) TB_CUDA(p, cudaEventRecord(es->e[1], p->stream));
+        if ((rc = run_fft(p, nt))) return rc;
+        if (es) TB_CUDA(p, cudaEventRecord(es->e[2], p->stream));
+        if ((rc = run_spectrum(p, nt))) return rc;
+        if (es) TB_CUDA(p, cudaEventRecord(es->e[3], p->stream));
+        if ((rc = run_normalise(p, nt))) return rc;
+        if (es) TB_CUDA(p, cudaEventRecord(es->e[4], p->stream));
+        if ((rc = run_hsum(p, nt, fp, first_template_id + (uint32_t)off))) return rc;
+        if (es) TB_CUDA(p, cudaEventRecord(es->e[5], p->stream));
+        p->last.n_chunks++;
+    }
+    return TB_OK;
+}
+
+int tb_get_timings(tb_plan* p, tb_timings* out)
+{
+    if (!p || !out) return TB_ERR_INVALID_ARG;
+    TB_CUDA(p, cudaSetDevice(p->device));
+    TB_CUDA(p, cudaStreamSynchronize(p->stream));
+    tb_timings t = p->last;
+    t.ms_resample = t.ms_fft = t.ms_spectrum = t.ms_normalise = t.ms_hsum = t.ms_total = 0.0;
+    for (size_t i = 0; i < p->events_used; ++i) {
+        float ms[5];
+        for (int s = 0; s < 5; ++s) TB_CUDA(p, cudaEventElapsedTime(&ms[s], p->events[i].e[s], p->events[i].e[s + 1]));
+        t.ms_resample += ms[0]; t.ms_fft += ms[1]; t.ms_spectrum += ms[2]; t.ms_normalise += ms[3]; t.ms_hsum += ms[4];
+    }
+    if (p->events_used) {
+        float tot = 0.f;
+        TB_CUDA(p, cudaEventElapsedTime(&tot, p->events[0].e[0], p->events[p->events_used - 1].e[5]));
+        t.ms_total = tot;
+    }
+    *out = t;
+    return TB_OK;
+}
+
+int tb_clear_candidates(tb_plan* p)
+{
+    if (!p) return TB_ERR_INVALID_ARG;
+    TB_CUDA(p, cudaSetDevice(p->device));
+    TB_CUDA(p, cudaMemsetAsync(p->d_cursor, 0, sizeof(unsigned long long), p->stream));
+    return TB_OK;
+}
+
+int tb_get_candidates(tb_plan* p, tb_candidate* out, uint64_t capacity, uint64_t* n_total)
+{
+    if (!p || !n_total) return fail(p, TB_ERR_INVALID_ARG, "null argument");
+    TB_CUDA(p, cudaSetDevice(p->device));
+    unsigned long long count = 0;
+    TB_CUDA(p, cudaMemcpyAsync(&count, p->d_cursor, sizeof(count), cudaMemcpyDeviceToHost, p->stream));
+    TB_CUDA(p, cudaStreamSynchronize(p->stream));
+    *n_total = count;
+    const uint64_t stored = std::min<uint64_t>(count, p->max_cand);
+    if (stored > 0 && (!out || capacity < stored)) return fail(p, TB_ERR_CAPACITY, "output buffer too small");
+    if (stored > 0) {
+        TB_CUDA(p, cudaMemcpyAsync(out, p->d_cand, stored * sizeof(Candidate), cudaMemcpyDeviceToHost, p->stream));
+        TB_CUDA(p, cudaStreamSynchronize(p->stream));
+        std::sort(out, out + stored, [](const tb_candidate& a, const tb_candidate& b) {
+            if (a.template_id != b.template_id) return a.template_id < b.template_id;
+            if (a.fold != b.fold) return a.fold < b.fold;
+            return a.bin < b.bin;
+        });
+    }
+    TB_CUDA(p, cudaMemsetAsync(p->d_cursor, 0, sizeof(unsigned long long), p->stream));
+    if (count > p->max_cand) return fail(p, TB_ERR_OVERFLOW, "candidate buffer overflow: " + std::to_string(count));
+    return TB_OK;
+}
+
+int tb_debug_resample_indices(tb_plan* p, const tb_template* tmpl, int64_t* idx_out)
+{
+    if (!idx_out) return fail(p, TB_ERR_INVALID_ARG, "null argument");
+    int rc = single_template_stage(p, tmpl);
+    if (rc) return rc;
+    long long* d_idx = nullptr;
+    TB_CUDA(p, cudaMalloc(&d_idx, p->n * sizeof(long long)));
+    rc = run_resample(p, 0, 1, d_idx);
+    if (!rc) {
+        cudaError_t e = cudaMemcpyAsync(idx_out, d_idx, p->n * sizeof(long long), cudaMemcpyDeviceToHost, p->stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(p->stream);
+        if (e != cudaSuccess) rc = fail(p, TB_ERR_CUDA, cudaGetErrorString(e));
+    }
+    cudaFree(d_idx);
+    return rc;
+}
+
+int tb_debug_resampled(tb_plan* p, const tb_template* tmpl, float* y_out)
+{
+    if (!y_out) return fail(p, TB_ERR_INVALID_ARG, "null argument");
+    int rc = single_template_stage(p, tmpl);
+    if (rc) return rc;
+    if ((rc = run_resample(p, 0, 1, nullptr))) return rc;
+    TB_CUDA(p, cudaMemcpyAsync(y_out, p->d_resampled, p->n * sizeof(float), cudaMemcpyDeviceToHost, p->stream));
+    TB_CUDA(p, cudaStreamSynchronize(p->stream));
+    return TB_OK;
+}
+
+int tb_debug_spectrum(tb_plan* p, const tb_template* tmpl, float* p_interbinned, float* p_normalised, float* medians)
+{
+    int rc = single_template_stage(p, tmpl);
+    if (rc) return rc;
+    if ((rc = run_resample(p, 0, 1, nullptr))) return rc;
+    if ((rc = run_fft(p, 1))) return rc;
+    if ((rc = run_spectrum(p, 1))) return rc;
+    if (p_interbinned)
+        TB_CUDA(p, cudaMemcpyAsync(p_interbinned, p->d_power, p->nb * sizeof(float), cudaMemcpyDeviceToHost, p->stream));
+    if (medians)
+        TB_CUDA(p, cudaMemcpyAsync(medians, p->d_med, p->nblk * sizeof(float), cudaMemcpyDeviceToHost, p->stream));
+    if ((rc = run_normalise(p, 1))) return rc;
+    if (p_normalised)
+        TB_CUDA(p, cudaMemcpyAsync(p_normalised, p->d_power, p->nb * sizeof(float), cudaMemcpyDeviceToHost, p->stream));
+    TB_CUDA(p, cudaStreamSynchronize(p->stream));
+    return TB_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,381 @@
+// tb_kernels.cuh -- device code of libtb (sm_100a).  See include/tb.h for the boundary and
+// DESIGN.md sections 6-7 for the data layout, the byte model and the roofline of each kernel.
+//
+// Nothing on this path is a dense contraction, so no tensor cores: the kernels are bound by
+// HBM (streaming 128-bit loads/stores), by the fp64 pipe (delay model) or by instruction issue
+// (median select, harmonic sum).  Citations: PAPER.md line numbers; G<n> = DESIGN.md readings.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace tb {
+
+// ---------------------------------------------------------------------------------------------
+// per-template constants (step a1), computed on the host in extended precision
+// ---------------------------------------------------------------------------------------------
+struct TmplDev {
+    double c_hi, c_lo;   // orbital turns per sample tsamp/P_orb as a double-double
+    double w;            // radians per sample 2*pi*tsamp/P_orb
+    double phi0;         // initial orbital phase reduced to [0, 2*pi)
+    double A, B;         // (tau/tsamp) sin(omega), (tau/tsamp) sqrt(1-e^2) cos(omega)   (eq A1)
+    double ecc;          // e
+    double d0;           // zero offset in samples: A cos E0 + B sin E0 at M = phi0      (L675, L682-692)
+    int32_t log2h;       // Hermite knot spacing h = 2^log2h samples (0: every sample is a knot)
+    int32_t circular;    // 1: e == 0, E = M (no Kepler solve)
+};
+
+struct FoldParams {
+    float    thr[5];     // power threshold T_L per fold, +inf for folds not requested
+    float    mu[5];      // mu_n, n = 2^L
+    float    inv_s[5];   // 1/s_n
+    uint32_t k_lo;       // lowest fundamental bin (G20); fold L starts at k_lo << L
+};
+
+struct Candidate {       // == tb_candidate
+    uint32_t template_id, fold, bin;
+    float    power, sigma;
+    uint32_t pad;
+};
+
+constexpr int RS_THREADS = 256;      // resampler CTA
+constexpr int RS_TILE    = 4096;     // output samples per CTA
+constexpr int RS_MAXSEG  = 512;      // Hermite segments held in shared memory at once
+constexpr int SP_WARPS   = 8;        // spectrum/median CTA = 8 warps, one median block per warp
+
+// ---------------------------------------------------------------------------------------------
+// a2: exact delay (in samples, zero offset removed) and its per-sample slope at sample j.
+//   phase in turns u = frac(j * tsamp/P_orb) from a double-double product, so that the mean
+//   anomaly M = 2 pi u + phi0 carries ~1e-17 rad of error instead of ulp(Omega t) (DESIGN.md
+//   section 6.1: index parity error budget).  E from Newton's method on E - e sin E = M
+//   (eq 3; Alg. 1; G9), delay from eq A1 (L666).
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ void delay_knot(const TmplDev& t, int j, double& val, double& slope)
+{
+    const double TWO_PI_HI = 6.283185307179586232;      // fl(2 pi)
+    const double TWO_PI_LO = 2.449293598294706414e-16;  // 2 pi - fl(2 pi)
+    const double jd  = (double)j;
+    const double p   = jd * t.c_hi;
+    double lo        = fma(jd, t.c_hi, -p);              // exact product error
+    lo               = fma(jd, t.c_lo, lo);
+    const double u   = p - floor(p);                     // exact
+    const double m   = u * TWO_PI_HI;
+    double me        = fma(u, TWO_PI_HI, -m);
+    me               = fma(u, TWO_PI_LO, me);
+    me               = fma(lo, TWO_PI_HI, me);
+    const double M   = m + t.phi0;                       // two-sum
+    const double bb  = M - m;
+    const double Mlo = ((m - (M - bb)) + (t.phi0 - bb)) + me;
+
+    double sE, cE, r;
+    if (t.circular) {
+        sincos(M, &sE, &cE);
+        r = 1.0;
+    } else {
+        const double e = t.ecc;
+        double sM, cM;
+        sincos(M, &sM, &cM);
+        double E = M + e * sM;
+        sE = sM; cE = cM;
+        for (int it = 0; it < 60; ++it) {
+            sincos(E, &sE, &cE);
+            const double f  = (E - M) - e * sE;
+            const double dE = f / (1.0 - e * cE);
+            E -= dE;
+            if (fabs(dE) < 1e-8) {                       // last step: second-order update, no sincos
+                const double h2 = 0.5 * dE * dE;
+                const double s2 = sE - dE * cE - h2 * sE;
+                const double c2 = cE + dE * sE - h2 * cE;
+                sE = s2; cE = c2;
+                break;
+            }
+        }
+        r = 1.0 / (1.0 - e * cE);
+    }
+    // first-order correction for the low part of M
+    const double dE = Mlo * r;
+    const double s1 = fma(dE, cE, sE);
+    const double c1 = fma(-dE, sE, cE);
+    val   = fma(t.A, c1, fma(t.B, s1, -t.d0));
+    slope = (t.B * c1 - t.A * s1) * r * t.w;
+}
+
+// floor(x) for |x| < 2^31 through the 2^52+2^51 magic constant and a round-down add: one DADD on
+// the fp64 pipe instead of a quarter-rate F2I conversion.
+__device__ __forceinline__ int floor_to_int(double x)
+{
+    return __double2loint(__dadd_rd(x, 6755399441055744.0));
+}
+
+// ---------------------------------------------------------------------------------------------
+// K1  resampler (a2 + a3).  One CTA = one tile of RS_TILE output samples of one template.
+//   phase 1: exact (value, slope) knots every h samples             (fp64, sincos / Newton)
+//   phase 2: cubic Hermite coefficients per segment in shared memory
+//   phase 3: delta_j from 3 DFMA, s = floor(delta + 1/2), idx = j - s, gather x[idx] (read-only
+//            path; the series is shared by all templates and L2-resident), 128-bit store.
+//   h is chosen per template on the host so that the interpolation error is < 2e-11 samples
+//   (DESIGN.md 6.1); h = 1 degenerates to the exact formula at every sample.
+//   Grid is flattened: blockIdx.x = tile * n_tmpl + template, so CTAs that run together read
+//   the same stretch of the series.
+// ---------------------------------------------------------------------------------------------
+template <bool DEBUG_IDX>
+__global__ void __launch_bounds__(RS_THREADS)
+k_resample(const float* __restrict__ x, float* __restrict__ y, const TmplDev* __restrict__ tmpl,
+           int n_tmpl, int n, int tile, float fill, long long* __restrict__ idx_out)
+{
+    __shared__ double s_val[RS_MAXSEG + 1];
+    __shared__ double s_slp[RS_MAXSEG + 1];
+    __shared__ __align__(16) double s_coef[RS_MAXSEG][4];
+
+    const int b     = blockIdx.x % n_tmpl;
+    const int tbase = (blockIdx.x / n_tmpl) * tile;
+    const TmplDev t = tmpl[b];
+    const int log2h = t.log2h;
+    const int h     = 1 << log2h;
+    const double inv_h = 1.0 / (double)h;
+    const int sub   = min(tile, RS_MAXSEG << log2h);
+    float* __restrict__ yrow = y + (size_t)b * (size_t)n;
+
+    for (int jsub = tbase; jsub < tbase + tile; jsub += sub) {
+        const int nseg = sub >> log2h;
+        if (jsub != tbase) __syncthreads();
+        for (int k = threadIdx.x; k <= nseg; k += RS_THREADS) {
+            double v, d;
+            delay_knot(t, jsub + (k << log2h), v, d);
+            s_val[k] = v;
+            s_slp[k] = d * (double)h;
+        }
+        __syncthreads();
+        for (int k = threadIdx.x; k < nseg; k += RS_THREADS) {
+            const double v0 = s_val[k], v1 = s_val[k + 1], d0 = s_slp[k], d1 = s_slp[k + 1];
+            const double dv = v1 - v0;
+            s_coef[k][0] = v0 + 0.5;                         // +1/2: rounding becomes a floor
+            s_coef[k][1] = d0;
+            s_coef[k][2] = 3.0 * dv - (2.0 * d0 + d1);
+            s_coef[k][3] = (d0 + d1) - 2.0 * dv;
+        }
+        __syncthreads();
+
+        for (int g = threadIdx.x; g < (sub >> 2); g += RS_THREADS) {
+            const int o = g << 2;
+            const int j = jsub + o;
+            int src[4];
+            if (log2h >= 2) {
+                const int seg = o >> log2h;
+                const double2 c01 = *reinterpret_cast<const double2*>(&s_coef[seg][0]);
+                const double2 c23 = *reinterpret_cast<const double2*>(&s_coef[seg][2]);
+                double tt = (double)(o & (h - 1)) * inv_h;
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    const double d = fma(fma(fma(c23.y, tt, c23.x), tt, c01.y), tt, c01.x);
+                    src[q] = j + q - floor_to_int(d);
+                    tt += inv_h;
+                }
+            } else {
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    const int oq  = o + q;
+                    const int seg = oq >> log2h;
+                    const double tt = (double)(oq & (h - 1)) * inv_h;
+                    const double d = fma(fma(fma(s_coef[seg][3], tt, s_coef[seg][2]), tt, s_coef[seg][1]), tt,
+                                         s_coef[seg][0]);
+                    src[q] = j + q - floor_to_int(d);
+                }
+            }
+            float4 v;
+            v.x = ((unsigned)src[0] < (unsigned)n) ? __ldg(x + src[0]) : fill;
+            v.y = ((unsigned)src[1] < (unsigned)n) ? __ldg(x + src[1]) : fill;
+            v.z = ((unsigned)src[2] < (unsigned)n) ? __ldg(x + src[2]) : fill;
+            v.w = ((unsigned)src[3] < (unsigned)n) ? __ldg(x + src[3]) : fill;
+            *reinterpret_cast<float4*>(yrow + j) = v;
+            if (DEBUG_IDX) {
+#pragma unroll
+                for (int q = 0; q < 4; ++q) idx_out[(size_t)b * (size_t)n + j + q] = (long long)src[q];
+            }
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// K2  spectrum former + block median (a5 + a6).  One warp = one median block of W bins:
+//   lane holds W/32 powers in registers, P_k = max(|X_k|^2, 1/2 |X_k - X_{k-1}|^2) with X_0 <- 0
+//   (G12-G14), written once as float4; the exact median (mean of the two middle order
+//   statistics, G15) is found by a 31-step bisection on the bit pattern of the non-negative
+//   floats with warp-wide counts (REDUX) -- no shared memory, no block barrier.
+//   ld = row stride of the cuFFT output in complex elements (even: rows are 16-byte aligned).
+// ---------------------------------------------------------------------------------------------
+template <int W>
+__global__ void __launch_bounds__(SP_WARPS * 32)
+k_spectrum_median(const float2* __restrict__ X, size_t ld, float* __restrict__ P, float* __restrict__ med,
+                  int nb, int nblk_per_row, int cta_per_row)
+{
+    constexpr int VPT  = W / 32;        // powers per lane
+    constexpr int ITER = W / 128;       // 4 consecutive bins per lane per iteration
+    const int row  = blockIdx.x / cta_per_row;
+    const int blk  = (blockIdx.x % cta_per_row) * SP_WARPS + (threadIdx.x >> 5);
+    const int lane = threadIdx.x & 31;
+    if (blk >= nblk_per_row) return;
+
+    const float2* __restrict__ Xr = X + (size_t)row * ld;
+    float* __restrict__ Pr        = P + (size_t)row * (size_t)nb;
+    const int base = blk * W;
+
+    float p[VPT];
+    float2 carry = make_float2(0.f, 0.f);                // X_{k-1} for lane 0 (X_{-1} = 0)
+    if (base > 0 && lane == 0) carry = __ldg(Xr + base - 1);
+#pragma unroll
+    for (int i = 0; i < ITER; ++i) {
+        const int k0 = base + i * 128 + lane * 4;
+        float4 a = __ldg(reinterpret_cast<const float4*>(Xr + k0));
+        float4 c = __ldg(reinterpret_cast<const float4*>(Xr + k0 + 2));
+        if (k0 == 0) { a.x = 0.f; a.y = 0.f; }           // X_0 <- 0 before differencing (G13)
+        float px = __shfl_up_sync(0xffffffffu, c.z, 1);
+        float py = __shfl_up_sync(0xffffffffu, c.w, 1);
+        if (lane == 0) { px = carry.x; py = carry.y; }
+        const float nx = __shfl_sync(0xffffffffu, c.z, 31);
+        const float ny = __shfl_sync(0xffffffffu, c.w, 31);
+        carry = make_float2(nx, ny);
+        float dx, dy;
+        float4 o;
+        dx = a.x - px;  dy = a.y - py;  o.x = fmaxf(a.x * a.x + a.y * a.y, 0.5f * (dx * dx + dy * dy));
+        dx = a.z - a.x; dy = a.w - a.y; o.y = fmaxf(a.z * a.z + a.w * a.w, 0.5f * (dx * dx + dy * dy));
+        dx = c.x - a.z; dy = c.y - a.w; o.z = fmaxf(c.x * c.x + c.y * c.y, 0.5f * (dx * dx + dy * dy));
+        dx = c.z - c.x; dy = c.w - c.y; o.w = fmaxf(c.z * c.z + c.w * c.w, 0.5f * (dx * dx + dy * dy));
+        *reinterpret_cast<float4*>(Pr + k0) = o;
+        p[4 * i + 0] = o.x; p[4 * i + 1] = o.y; p[4 * i + 2] = o.z; p[4 * i + 3] = o.w;
+    }
+
+    // exact order statistics W/2-1 and W/2 (0-based) of the W values held by the warp
+    uint32_t key[VPT];
+#pragma unroll
+    for (int v = 0; v < VPT; ++v) key[v] = __float_as_uint(p[v]);
+    constexpr int K1 = W / 2 - 1;
+    uint32_t prefix = 0;
+    for (int bit = 30; bit >= 0; --bit) {
+        const uint32_t cand = prefix | (1u << bit);
+        int c = 0;
+#pragma unroll
+        for (int v = 0; v < VPT; ++v) c += (key[v] < cand) ? 1 : 0;
+        c = __reduce_add_sync(0xffffffffu, c);
+        if (c <= K1) prefix = cand;                      // the K1-th smallest is >= cand
+    }
+    int le = 0;
+    uint32_t nxt = 0xffffffffu;
+#pragma unroll
+    for (int v = 0; v < VPT; ++v) {
+        le += (key[v] <= prefix) ? 1 : 0;
+        if (key[v] > prefix) nxt = min(nxt, key[v]);
+    }
+    le  = __reduce_add_sync(0xffffffffu, le);
+    nxt = __reduce_min_sync(0xffffffffu, nxt);
+    const uint32_t upper = (le >= W / 2 + 1) ? prefix : nxt;
+    if (lane == 0) med[(size_t)row * nblk_per_row + blk] = 0.5f * (__uint_as_float(prefix) + __uint_as_float(upper));
+}
+
+// ---------------------------------------------------------------------------------------------
+// K3  normalise (a7), in place: P^_k = P_k ln2 / m(k), m(k) = linear interpolation of the block
+//   medians between block centres bW + (W-1)/2, flat outside (G15); P^_0 = 0; m <= 0 -> 0.
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ float baseline_at(const float* __restrict__ med, int nblk, int k, int log2w)
+{
+    const int W = 1 << log2w;
+    const int a = k - (W >> 1);                          // k - c_b = (a mod W) + 1/2
+    if (a < 0) return __ldg(med);
+    const int b = a >> log2w;
+    if (b >= nblk - 1) return __ldg(med + nblk - 1);
+    const float fr = ((float)(a & (W - 1)) + 0.5f) * (1.0f / (float)W);
+    const float m0 = __ldg(med + b), m1 = __ldg(med + b + 1);
+    return fmaf(fr, m1 - m0, m0);
+}
+
+__global__ void __launch_bounds__(256)
+k_normalise(float* __restrict__ P, const float* __restrict__ med, int nb, int nblk, int log2w, int cta_per_row)
+{
+    const int row = blockIdx.x / cta_per_row;
+    const int k0  = ((blockIdx.x % cta_per_row) * 256 + threadIdx.x) * 4;
+    if (k0 >= nb) return;
+    float* __restrict__ Pr = P + (size_t)row * (size_t)nb;
+    const float* __restrict__ mr = med + (size_t)row * nblk;
+    float4 v = *reinterpret_cast<const float4*>(Pr + k0);
+    float* vv = reinterpret_cast<float*>(&v);
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+        const float m = baseline_at(mr, nblk, k0 + q, log2w);
+        vv[q] = (m > 0.f) ? vv[q] * 0.69314718055994530942f / m : 0.f;
+    }
+    if (k0 == 0) v.x = 0.f;
+    *reinterpret_cast<float4*>(Pr + k0) = v;
+}
+
+// ---------------------------------------------------------------------------------------------
+// K4  harmonic sum + threshold + compaction (a8 + a9).
+//   S_L[k] = sum_{m=1}^{2^L} P^[(k m + 2^(L-1)) >> L]  (eq 9; G16), nested:
+//   S_L = S_{L-1} + the odd-m terms.  A bin/fold over threshold becomes a candidate; the warp
+//   ballots its hits and takes one atomic per warp on the device cursor (L660 "peak detection",
+//   G19).  The cursor keeps counting past the capacity so that overflow is reported, not hidden.
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256)
+k_hsum_threshold(const float* __restrict__ Ph, int nb, int cta_per_row, FoldParams fp, uint32_t first_id,
+                 Candidate* __restrict__ out, unsigned long long* __restrict__ cursor,
+                 unsigned long long capacity)
+{
+    const int row = blockIdx.x / cta_per_row;
+    const int k   = (blockIdx.x % cta_per_row) * 256 + threadIdx.x;
+    const float* __restrict__ p = Ph + (size_t)row * (size_t)nb;
+    const unsigned lane = threadIdx.x & 31;
+
+    float S[5];
+    const bool live = k < nb;
+    if (live) {
+        const uint32_t uk = (uint32_t)k;
+        S[0] = __ldg(p + uk);
+        S[1] = S[0] + __ldg(p + ((uk + 1u) >> 1));
+        S[2] = S[1] + __ldg(p + ((uk + 2u) >> 2)) + __ldg(p + ((3u * uk + 2u) >> 2));
+        float s = S[2];
+#pragma unroll
+        for (uint32_t m = 1; m < 8; m += 2) s += __ldg(p + ((m * uk + 4u) >> 3));
+        S[3] = s;
+#pragma unroll
+        for (uint32_t m = 1; m < 16; m += 2) s += __ldg(p + ((m * uk + 8u) >> 4));
+        S[4] = s;
+    }
+    bool any = false;
+    if (live) {
+#pragma unroll
+        for (int L = 0; L < 5; ++L) any |= (S[L] >= fp.thr[L]) && ((uint32_t)k >= (fp.k_lo << L));
+    }
+    if (__ballot_sync(0xffffffffu, any) == 0u) return;
+#pragma unroll
+    for (int L = 0; L < 5; ++L) {
+        const bool hit = live && (S[L] >= fp.thr[L]) && ((uint32_t)k >= (fp.k_lo << L));
+        const unsigned mask = __ballot_sync(0xffffffffu, hit);
+        if (mask == 0u) continue;
+        unsigned long long basepos = 0;
+        if (lane == (unsigned)(__ffs(mask) - 1)) basepos = atomicAdd(cursor, (unsigned long long)__popc(mask));
+        basepos = __shfl_sync(0xffffffffu, basepos, __ffs(mask) - 1);
+        if (hit) {
+            const unsigned long long pos = basepos + (unsigned long long)__popc(mask & ((1u << lane) - 1u));
+            if (pos < capacity) {
+                Candidate c;
+                c.template_id = first_id + (uint32_t)row;
+                c.fold = (uint32_t)L;
+                c.bin = (uint32_t)k;
+                c.power = S[L];
+                c.sigma = (sqrtf(S[L]) - fp.mu[L]) * fp.inv_s[L];
+                c.pad = 0u;
+                out[pos] = c;
+            }
+        }
+    }
+}
+
+// fp64 sum of a device series (fill value when the series is borrowed device memory)
+__global__ void k_sum_f64(const float* __restrict__ x, size_t n, double* __restrict__ acc)
+{
+    double s = 0.0;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x)
+        s += (double)x[i];
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_down_sync(0xffffffffu, s, o);
+    if ((threadIdx.x & 31) == 0) atomicAdd(acc, s);
+}
+
+}  // namespace tb

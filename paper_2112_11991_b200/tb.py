@@ -1,0 +1,254 @@
+"""ctypes binding of libtb (include/tb.h).  Argument marshalling only: every step of the hot path
+runs inside the shared library's CUDA kernels.  There is no CPU fallback -- importing this module
+raises if libtb.so has not been built (``python -m paper_2112_11991_b200.build``), and every call
+raises ``TbError`` when the library reports a failure (e.g. no CUDA device).
+
+The module-level functions carry the C names (tb_plan_create, tb_search_templates, ...) and take /
+return plain Python and numpy objects; ``Plan`` is a small RAII convenience over them.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_LIB_PATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "lib", "libtb.so")
+if not os.path.exists(_LIB_PATH):
+    raise ImportError(f"{_LIB_PATH} is missing: build it with `python -m paper_2112_11991_b200.build` "
+                      "(there is no CPU fallback)")
+lib = C.CDLL(_LIB_PATH)
+
+TB_OK, TB_ERR_INVALID_ARG, TB_ERR_CUDA, TB_ERR_CUFFT, TB_ERR_NOMEM, TB_ERR_OVERFLOW, TB_ERR_CAPACITY = 0, -1, -2, -3, -4, -5, -6
+
+TEMPLATE_DTYPE = np.dtype([("p_orb_s", "<f8"), ("tau_lts", "<f8"), ("phi0_rad", "<f8"), ("ecc", "<f8"),
+                           ("omega_rad", "<f8")])
+CANDIDATE_DTYPE = np.dtype([("template_id", "<u4"), ("fold", "<u4"), ("bin", "<u4"), ("power", "<f4"),
+                            ("sigma", "<f4"), ("pad", "<u4")])
+assert TEMPLATE_DTYPE.itemsize == 40 and CANDIDATE_DTYPE.itemsize == 24
+
+
+class PlanOpts(C.Structure):
+    _fields_ = [("struct_size", C.c_uint32), ("device", C.c_int32), ("stream", C.c_void_p),
+                ("median_window", C.c_uint32), ("f_min_hz", C.c_double), ("max_candidates", C.c_uint64),
+                ("chunk_templates", C.c_uint32), ("series_is_device_ptr", C.c_int32), ("has_fill", C.c_int32),
+                ("fill_value", C.c_float), ("enable_timings", C.c_int32), ("reserved", C.c_int32)]
+
+
+class Timings(C.Structure):
+    _fields_ = [("ms_resample", C.c_double), ("ms_fft", C.c_double), ("ms_spectrum", C.c_double),
+                ("ms_normalise", C.c_double), ("ms_hsum", C.c_double), ("ms_total", C.c_double),
+                ("n_templates", C.c_uint64), ("n_samples", C.c_uint64), ("n_chunks", C.c_uint64),
+                ("chunk_templates", C.c_uint64), ("model_bytes_per_template", C.c_uint64)]
+
+    def as_dict(self):
+        return {k: getattr(self, k) for k, _ in self._fields_}
+
+
+EXPORTS = ["tb_plan_create", "tb_search_templates", "tb_get_candidates", "tb_clear_candidates", "tb_plan_destroy",
+           "tb_strerror", "tb_last_error", "tb_get_timings", "tb_debug_resample_indices", "tb_debug_spectrum",
+           "tb_debug_resampled", "tb_sigma_to_power", "tb_plan_info", "tb_template_knot_log2"]
+
+_vp, _u64, _u32 = C.c_void_p, C.c_uint64, C.c_uint32
+lib.tb_plan_create.argtypes = [C.POINTER(_vp), _vp, _u64, C.c_double, C.POINTER(PlanOpts)]
+lib.tb_search_templates.argtypes = [_vp, _vp, _u64, _u32, _vp, _u32, C.c_double]
+lib.tb_get_candidates.argtypes = [_vp, _vp, _u64, C.POINTER(_u64)]
+lib.tb_clear_candidates.argtypes = [_vp]
+lib.tb_plan_destroy.argtypes = [_vp]
+lib.tb_strerror.argtypes = [C.c_int]
+lib.tb_strerror.restype = C.c_char_p
+lib.tb_last_error.argtypes = [_vp]
+lib.tb_last_error.restype = C.c_char_p
+lib.tb_get_timings.argtypes = [_vp, C.POINTER(Timings)]
+lib.tb_debug_resample_indices.argtypes = [_vp, _vp, _vp]
+lib.tb_debug_spectrum.argtypes = [_vp, _vp, _vp, _vp, _vp]
+lib.tb_debug_resampled.argtypes = [_vp, _vp, _vp]
+lib.tb_sigma_to_power.argtypes = [_u32, C.c_double, C.POINTER(C.c_double)]
+lib.tb_plan_info.argtypes = [_vp, C.POINTER(C.c_float), C.POINTER(_u32), C.POINTER(_u32)]
+lib.tb_template_knot_log2.argtypes = [_vp, _vp, C.POINTER(C.c_int32)]
+for _name in EXPORTS:
+    if _name not in ("tb_strerror", "tb_last_error"):
+        getattr(lib, _name).restype = C.c_int
+
+
+class TbError(RuntimeError):
+    def __init__(self, code, detail=""):
+        self.code = code
+        super().__init__(f"libtb: {lib.tb_strerror(code).decode()} ({code}) {detail}")
+
+
+def _check(code, plan=None):
+    if code != TB_OK:
+        detail = lib.tb_last_error(plan).decode() if plan else ""
+        raise TbError(code, detail)
+
+
+def as_templates(templates) -> np.ndarray:
+    """float64[K,5] (P_orb, tau, phi0, e, omega) or a structured array -> contiguous tb_template[K]."""
+    t = np.asarray(templates)
+    if t.dtype == TEMPLATE_DTYPE:
+        return np.ascontiguousarray(t).reshape(-1)
+    t = np.ascontiguousarray(np.asarray(t, dtype=np.float64).reshape(-1, 5))
+    return t.view(TEMPLATE_DTYPE).reshape(-1)
+
+
+def tb_plan_create(series, n_samples, tsamp_s, *, device=0, stream=None, median_window=0, f_min_hz=0.0,
+                   max_candidates=0, chunk_templates=0, series_is_device_ptr=False, fill_value=None,
+                   enable_timings=False):
+    """series: numpy float32[N] (host) or an integer device address when series_is_device_ptr."""
+    o = PlanOpts()
+    o.struct_size = C.sizeof(PlanOpts)
+    o.device, o.stream = int(device), stream
+    o.median_window, o.f_min_hz, o.max_candidates = int(median_window), float(f_min_hz), int(max_candidates)
+    o.chunk_templates, o.series_is_device_ptr = int(chunk_templates), int(bool(series_is_device_ptr))
+    o.has_fill, o.fill_value = (0, 0.0) if fill_value is None else (1, float(fill_value))
+    o.enable_timings = int(bool(enable_timings))
+    if series_is_device_ptr:
+        ptr = int(series)
+    else:
+        series = np.ascontiguousarray(series, dtype=np.float32)
+        ptr = series.ctypes.data
+    plan = _vp()
+    _check(lib.tb_plan_create(C.byref(plan), ptr, int(n_samples), float(tsamp_s), C.byref(o)))
+    return plan
+
+
+def tb_search_templates(plan, templates, first_template_id=0, folds=(0, 1, 2, 3, 4), sigma_threshold=6.0):
+    t = as_templates(templates)
+    f = np.ascontiguousarray(folds, dtype=np.uint32)
+    _check(lib.tb_search_templates(plan, t.ctypes.data, t.size, int(first_template_id), f.ctypes.data, f.size,
+                                   float(sigma_threshold)), plan)
+
+
+def tb_get_candidates(plan, capacity=None):
+    """Returns (candidates structured array sorted by (template, fold, bin), n_total).  Raises
+    TbError(TB_ERR_OVERFLOW) if the device buffer overflowed (``.n_total`` on the exception)."""
+    n = _u64(0)
+    if capacity is None:
+        code = lib.tb_get_candidates(plan, None, 0, C.byref(n))
+        if code == TB_OK:
+            return np.zeros(0, dtype=CANDIDATE_DTYPE), 0
+        if code not in (TB_ERR_CAPACITY,):
+            _check(code, plan)
+        capacity = n.value
+    out = np.zeros(int(capacity), dtype=CANDIDATE_DTYPE)
+    code = lib.tb_get_candidates(plan, out.ctypes.data, out.size, C.byref(n))
+    if code == TB_ERR_OVERFLOW:
+        err = TbError(code, lib.tb_last_error(plan).decode())
+        err.n_total = n.value
+        err.partial = out
+        raise err
+    _check(code, plan)
+    return out[: n.value], n.value
+
+
+def tb_clear_candidates(plan):
+    _check(lib.tb_clear_candidates(plan), plan)
+
+
+def tb_plan_destroy(plan):
+    _check(lib.tb_plan_destroy(plan))
+
+
+def tb_get_timings(plan) -> dict:
+    t = Timings()
+    _check(lib.tb_get_timings(plan, C.byref(t)), plan)
+    return t.as_dict()
+
+
+def tb_plan_info(plan):
+    f, b, k = C.c_float(), _u32(), _u32()
+    _check(lib.tb_plan_info(plan, C.byref(f), C.byref(b), C.byref(k)), plan)
+    return {"fill_value": np.float32(f.value), "chunk_templates": b.value, "k_lo": k.value}
+
+
+def tb_template_knot_log2(plan, template) -> int:
+    t = as_templates(template)
+    v = C.c_int32()
+    _check(lib.tb_template_knot_log2(plan, t.ctypes.data, C.byref(v)), plan)
+    return v.value
+
+
+def tb_debug_resample_indices(plan, template, n_samples) -> np.ndarray:
+    t = as_templates(template)
+    out = np.empty(int(n_samples), dtype=np.int64)
+    _check(lib.tb_debug_resample_indices(plan, t.ctypes.data, out.ctypes.data), plan)
+    return out
+
+
+def tb_debug_resampled(plan, template, n_samples) -> np.ndarray:
+    t = as_templates(template)
+    out = np.empty(int(n_samples), dtype=np.float32)
+    _check(lib.tb_debug_resampled(plan, t.ctypes.data, out.ctypes.data), plan)
+    return out
+
+
+def tb_debug_spectrum(plan, template, n_samples, median_window=1024):
+    t = as_templates(template)
+    nb = int(n_samples) // 2
+    p = np.empty(nb, dtype=np.float32)
+    ph = np.empty(nb, dtype=np.float32)
+    m = np.empty(nb // int(median_window), dtype=np.float32)
+    _check(lib.tb_debug_spectrum(plan, t.ctypes.data, p.ctypes.data, ph.ctypes.data, m.ctypes.data), plan)
+    return p, ph, m
+
+
+def tb_sigma_to_power(fold, sigma) -> float:
+    v = C.c_double()
+    _check(lib.tb_sigma_to_power(int(fold), float(sigma), C.byref(v)))
+    return v.value
+
+
+class Plan:
+    """RAII wrapper: ``with Plan(series, tsamp) as p: p.search(templates); cands, n = p.candidates()``."""
+
+    def __init__(self, series, tsamp_s, n_samples=None, **opts):
+        self.n_samples = int(n_samples if n_samples is not None else len(series))
+        self.tsamp = float(tsamp_s)
+        self.median_window = int(opts.get("median_window", 0) or 1024)
+        self._series = series                        # keep host/device memory alive
+        self.handle = tb_plan_create(series, self.n_samples, tsamp_s, **opts)
+
+    def search(self, templates, first_template_id=0, folds=(0, 1, 2, 3, 4), sigma_threshold=6.0):
+        tb_search_templates(self.handle, templates, first_template_id, folds, sigma_threshold)
+
+    def candidates(self, capacity=None):
+        return tb_get_candidates(self.handle, capacity)
+
+    def clear(self):
+        tb_clear_candidates(self.handle)
+
+    def timings(self):
+        return tb_get_timings(self.handle)
+
+    def info(self):
+        return tb_plan_info(self.handle)
+
+    def knot_log2(self, template):
+        return tb_template_knot_log2(self.handle, template)
+
+    def debug_indices(self, template):
+        return tb_debug_resample_indices(self.handle, template, self.n_samples)
+
+    def debug_resampled(self, template):
+        return tb_debug_resampled(self.handle, template, self.n_samples)
+
+    def debug_spectrum(self, template):
+        return tb_debug_spectrum(self.handle, template, self.n_samples, self.median_window)
+
+    def close(self):
+        if self.handle is not None:
+            tb_plan_destroy(self.handle)
+            self.handle = None
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *a):
+        self.close()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

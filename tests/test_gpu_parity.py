@@ -1,0 +1,219 @@
+"""-m gpu: the CUDA path (through the C-ABI binding) against the CPU oracle, element by element.
+
+Small cases are compared in full; BASELINE.json's full-size configs are run in full on the GPU in
+the launch configuration bench.py times, and compared on (i) every true-signal template,
+(ii) every template the GPU reported a candidate for (bounded), (iii) a seeded sample of the rest
+-- the "parity economy" of SURVEY 8(d) -- because the oracle needs seconds per template there.
+"""
+import numpy as np
+import pytest
+
+from oracle import tb_oracle as orc
+from paper_2112_11991_b200 import workloads as wl_mod
+
+from parity import by_template, check_indices, check_template
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def tb():
+    import torch
+    assert torch.cuda.is_available(), "these tests need a CUDA device"
+    from paper_2112_11991_b200 import build
+    build.build()
+    from paper_2112_11991_b200 import tb
+    return tb
+
+
+def full_bank_parity(tb, wl, sigma, check_ids, max_hit_templates=6, **opts):
+    """Search the whole bank on the GPU, then compare the listed templates with the oracle."""
+    with tb.Plan(wl.series, wl.tsamp, **opts) as plan:
+        plan.search(wl.templates, 0, wl.folds, sigma)
+        cands, n = plan.candidates()
+        assert n == len(cands)
+        key = np.stack([cands["template_id"], cands["fold"], cands["bin"]], axis=1).astype(np.int64)
+        assert np.all(np.diff(key[:, 0] * (1 << 40) + key[:, 1] * (1 << 32) + key[:, 2]) > 0), "not sorted / duplicates"
+        per = by_template(cands)
+        hit = [t for t in per if t not in check_ids][:max_hit_templates]
+        reports = {}
+        for tid in list(check_ids) + hit:
+            reports[tid] = check_template(plan, wl, tid, sigma, wl.folds, per.get(tid, cands[:0]))
+    return cands, reports
+
+
+# ------------------------------------------------------------------ C1 in full
+def test_c1_full_parity_6sigma(tb, c1):
+    cands, rep = full_bank_parity(tb, c1, 6.0, range(len(c1.templates)))
+    assert set(np.unique(cands["template_id"])) == {0}            # only the true template detects
+    best = cands[np.argmax(cands["sigma"])]
+    assert (int(best["fold"]), int(best["bin"])) == (3, 52429)    # 50 Hz in the 8-harmonic fold
+    assert sum(r["n_oracle"] for r in rep.values()) == 76
+    assert max(r["err_power"] for r in rep.values()) <= 1e-4
+
+
+def test_c1_low_threshold_stresses_the_compactor(tb, c1):
+    cands, rep = full_bank_parity(tb, c1, 4.0, range(0, 64, 7))
+    assert len(cands) > 100
+    cands, rep = full_bank_parity(tb, c1, 2.5, (0, 31))
+    assert len(cands) > 100000
+    assert all(r["n_gpu"] > 0 for r in rep.values())
+
+
+def test_chunking_and_ids_do_not_change_the_result(tb, c1):
+    t = c1.templates[:13]
+    with tb.Plan(c1.series, c1.tsamp, chunk_templates=64) as a, tb.Plan(c1.series, c1.tsamp, chunk_templates=5) as b:
+        a.search(t, 100, c1.folds, 4.5)
+        ca, _ = a.candidates()
+        b.search(t[:6], 100, c1.folds, 4.5)                      # two calls append
+        b.search(t[6:], 106, c1.folds, 4.5)
+        cb, _ = b.candidates()
+    assert len(ca) > 0 and ca["template_id"].min() >= 100
+    assert np.array_equal(ca, cb)
+
+
+def test_fold_subset_and_window(tb, c1):
+    with tb.Plan(c1.series, c1.tsamp, median_window=256) as plan:
+        plan.search(c1.templates[:2], 0, (1, 3), 5.0)
+        cands, _ = plan.candidates()
+        assert set(np.unique(cands["fold"])) <= {1, 3} and len(cands) > 0
+        rep = check_template(plan, c1, 0, 5.0, (1, 3), by_template(cands).get(0))
+        assert rep["n_oracle"] == rep["n_gpu"] or rep["n_band"] > 0
+
+
+# ------------------------------------------------------------------ degenerate and edge cases
+def test_tau_zero_is_identity_and_empty_inputs(tb, c1):
+    with tb.Plan(c1.series, c1.tsamp) as plan:
+        idx = plan.debug_indices((60.0, 0.0, 0.3, 0.0, 0.0))
+        assert np.array_equal(idx, np.arange(c1.n_samples))
+        assert np.array_equal(plan.debug_resampled((60.0, 0.0, 0.3, 0.2, 1.0)), c1.series)
+        plan.search(np.zeros((0, 5)), 0, c1.folds, 6.0)          # empty bank
+        cands, n = plan.candidates()
+        assert n == 0 and len(cands) == 0
+        plan.search(c1.templates[:1], 0, (), 6.0)                # no folds requested
+        assert plan.candidates()[1] == 0
+
+
+def test_minimum_length_series(tb):
+    rng = np.random.default_rng(1)
+    x = rng.standard_normal(2048).astype(np.float32)
+    w = wl_mod.Workload("tiny", 2048, 1e-3, x, np.array([[1.0, 0.05, 0.5, 0.0, 0.0], [0.9, 0.04, 2.0, 0.3, 1.0]]), (), ())
+    cands, rep = full_bank_parity(tb, w, 2.0, (0, 1))
+    assert len(cands) > 0
+
+
+def test_exact_fallback_when_the_orbit_is_too_fast_for_interpolation(tb, c1):
+    """P_orb of a few hundred samples: the Hermite spacing collapses to 1 (every sample exact)."""
+    with tb.Plan(c1.series, c1.tsamp) as plan:
+        for tmpl in [(0.4, 0.02, 1.0, 0.0, 0.0), (0.5, 0.02, 1.0, 0.4, 2.0), (3.0, 0.2, 0.1, 0.1, 0.3)]:
+            assert plan.knot_log2(tmpl) <= 2
+            check_indices(plan, c1, np.array(tmpl))
+        assert plan.knot_log2(c1.templates[0]) >= 3
+
+
+def test_out_of_range_samples_take_the_fill_value(tb, c1):
+    tmpl = np.array([100.0, 3.0, 4.0, 0.0, 0.0])                 # shifts of thousands of samples
+    with tb.Plan(c1.series, c1.tsamp, fill_value=123.5) as plan:
+        idx = plan.debug_indices(tmpl)
+        y = plan.debug_resampled(tmpl)
+    assert np.array_equal(idx, orc.resample_indices(c1.n_samples, c1.tsamp, tmpl))
+    oob = (idx < 0) | (idx >= c1.n_samples)
+    assert oob.sum() > 100 and np.all(y[oob] == np.float32(123.5))
+    assert np.array_equal(y, orc.gather(c1.series, idx, np.float32(123.5)))
+
+
+def test_default_fill_is_the_series_mean(tb, c1):
+    with tb.Plan(c1.series + np.float32(3.0), c1.tsamp) as plan:
+        assert plan.info()["fill_value"] == orc.fill_value(c1.series + np.float32(3.0))
+
+
+def test_overflow_and_capacity_errors(tb, c1):
+    with tb.Plan(c1.series, c1.tsamp, max_candidates=100) as plan:
+        plan.search(c1.templates[:4], 0, c1.folds, 3.0)
+        with pytest.raises(tb.TbError) as ei:
+            plan.candidates()
+        assert ei.value.code == tb.TB_ERR_OVERFLOW and ei.value.n_total > 100
+        plan.search(c1.templates[:1], 0, (0,), 5.0)              # buffer was cleared by the read
+        cands, n = plan.candidates()
+        assert 0 < n <= 100
+        plan.search(c1.templates[:1], 0, (0,), 5.0)
+        n_total = tb._u64(0)
+        small = np.zeros(1, dtype=tb.CANDIDATE_DTYPE)
+        assert tb.lib.tb_get_candidates(plan.handle, small.ctypes.data, 1, n_total) == tb.TB_ERR_CAPACITY
+        assert n_total.value == n                                # nothing consumed
+        assert plan.candidates()[1] == n
+
+
+def test_invalid_templates_and_folds(tb, c1):
+    with tb.Plan(c1.series, c1.tsamp) as plan:
+        for bad in [(0.0, 1, 0, 0, 0), (60, -1, 0, 0, 0), (60, 1, 0, 1.0, 0), (60, 1, np.nan, 0, 0), (60, 1e9, 0, 0, 0)]:
+            with pytest.raises(tb.TbError) as ei:
+                plan.search(np.array([bad], dtype=np.float64))
+            assert ei.value.code == tb.TB_ERR_INVALID_ARG
+        for folds in [(5,), (1, 1)]:
+            with pytest.raises(tb.TbError):
+                plan.search(c1.templates[:1], 0, folds)
+
+
+def test_device_resident_series(tb, c1):
+    import torch
+    x = torch.from_numpy(c1.series).cuda()
+    s = torch.cuda.Stream()
+    with tb.Plan(x.data_ptr(), c1.tsamp, n_samples=c1.n_samples, series_is_device_ptr=True, stream=s.cuda_stream,
+                 enable_timings=True) as plan:
+        assert abs(float(plan.info()["fill_value"]) - float(orc.fill_value(c1.series))) < 1e-6
+        plan.search(c1.templates, 0, c1.folds, 6.0)
+        cands, n = plan.candidates()
+        t = plan.timings()
+    assert n == 76
+    assert t["n_templates"] == 64 and t["ms_total"] > 0 and t["ms_fft"] > 0
+
+
+# ------------------------------------------------------------------ elliptical, small
+def test_elliptical_small_full_parity(tb):
+    w = wl_mod.config4(n_templates=24, log2n=18)
+    cands, rep = full_bank_parity(tb, w, 5.0, range(24))
+    assert 0 in by_template(cands)                                # the injected pulsar is found
+    w2 = wl_mod.Workload("hi-e", w.n_samples, w.tsamp, w.series,
+                         np.array([[5.0, 0.3, 1.0, 0.6, 0.5], [7.0, 0.5, 2.0, 0.9, 4.0], [4.0, 0.2, 6.0, 0.3, 3.0]]), (), ())
+    with tb.Plan(w2.series, w2.tsamp) as plan:
+        for t in w2.templates:
+            check_indices(plan, w2, t)
+
+
+# ------------------------------------------------------------------ full-size configs (sampled oracle)
+def _sample(k, n, seed, exclude=()):
+    rng = np.random.default_rng(seed)
+    return [int(i) for i in rng.permutation(k) if int(i) not in exclude][:n]
+
+
+def test_c2_full_size(tb):
+    w = wl_mod.config2()
+    cands, rep = full_bank_parity(tb, w, 6.0, list(w.true_ids) + _sample(4096, 3, 22, w.true_ids), max_hit_templates=3)
+    per = by_template(cands)
+    assert all(t in per for t in w.true_ids)                      # all three pulsars detected
+
+
+def test_c4_full_size_elliptical(tb):
+    w = wl_mod.config4()
+    cands, rep = full_bank_parity(tb, w, 6.0, [0] + _sample(8192, 2, 44, (0,)), max_hit_templates=2)
+    assert 0 in by_template(cands)
+    best = by_template(cands)[0]
+    best = best[np.argmax(best["sigma"])]
+    f = best["bin"] / ((1 << int(best["fold"])) * w.t_obs)
+    assert abs(f - 40.0) < 2.0 / w.t_obs                          # 25 ms pulsar
+
+
+def test_c3_full_size_quantised(tb):
+    w = wl_mod.config3()
+    cands, rep = full_bank_parity(tb, w, 6.0, [0] + _sample(16384, 1, 33, (0,)), max_hit_templates=1)
+    assert 0 in by_template(cands)
+
+
+@pytest.mark.parametrize("log2n,n_check", [(20, 6), (22, 4), (23, 2), (24, 2), (26, 1)])
+def test_c5_sweep(tb, log2n, n_check):
+    w = wl_mod.config5(log2n=log2n)
+    half = n_check // 2 or 1
+    ids = _sample(256, half, log2n) + [256 + i for i in _sample(256, n_check - half, log2n + 1)]
+    cands, rep = full_bank_parity(tb, w, 6.0, ids, max_hit_templates=1)
+    assert max(r["flips"] for r in rep.values()) <= 2
