@@ -103,6 +103,7 @@ typedef struct {
     double   ms_resample, ms_fft, ms_spectrum /* a5+a6: spectrum + block medians */, ms_normalise, ms_hsum, ms_total;
     uint64_t n_templates, n_samples, n_chunks, chunk_templates;
     uint64_t model_bytes_per_template;   /* 22*N: algorithmic HBM bytes */
+    uint64_t n_kernel_launches;          /* libtb's own kernels launched by that call (cuFFT's not counted) */
 } tb_timings;
 
 /* Create a plan for one dedispersed time series S[i], i*tsamp.
@@ -115,6 +116,13 @@ typedef struct {
  * candidate buffer, the cuFFT plan and its work area): TB_ERR_NOMEM if that does not fit. */
 TB_API int tb_plan_create(tb_plan** out, const float* series, uint64_t n_samples, double tsamp_s,
                    const tb_plan_opts* opts);
+
+/* Replace the plan's time series by another of the same length and sampling time (the next
+ * DM trial / beam: PAPER.md L448, L660), reusing every buffer and FFT plan.  `series` is host
+ * memory (copied on the plan's stream; pinned memory makes the copy asynchronous) unless the
+ * plan was created with series_is_device_ptr, in which case it is a borrowed device pointer.
+ * The fill value is recomputed unless the plan was created with has_fill. */
+TB_API int tb_plan_set_series(tb_plan* plan, const float* series);
 
 /* Search `n_templates` templates (host array) and APPEND the detections to the plan's device
  * candidate buffer (steps a1-a9).  template_id of tmpl[i] is first_template_id + i.

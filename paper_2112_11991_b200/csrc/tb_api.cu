@@ -40,6 +40,7 @@ struct tb_plan {
     uint64_t max_cand = 0;
     uint32_t chunk = 0;
     bool timings = false;
+    bool user_fill = false, borrowed = false;
     float fill = 0.f;
     size_t ld = 0;                                   // complex row stride of the FFT output
 
@@ -60,6 +61,7 @@ struct tb_plan {
 
     std::map<uint32_t, cufftHandle> fft_plans;       // by batch size, sharing one work area
     void* d_work = nullptr;
+    double* d_acc = nullptr;
     size_t work_bytes = 0;
 
     std::vector<EventSet> events;
@@ -161,6 +163,36 @@ void make_tmpl(const tb_template& t, double tsamp, TmplDev* o)
     }
     o->d0 = (double)((long double)o->A * cosl(E) + (long double)o->B * sinl(E));
     o->log2h = knot_log2((double)g, o->w, t.ecc);
+}
+
+// copy (or borrow) the series and derive the fill value (G8)
+int load_series(tb_plan* p, const float* series)
+{
+    if (p->borrowed) {
+        p->d_series = series;
+    } else {
+        if (!p->d_series_owned) TB_CUDA(p, cudaMalloc(&p->d_series_owned, p->n * sizeof(float)));
+        TB_CUDA(p, cudaMemcpyAsync(p->d_series_owned, series, p->n * sizeof(float), cudaMemcpyHostToDevice, p->stream));
+        p->d_series = p->d_series_owned;
+    }
+    if (p->user_fill) return TB_OK;
+    if (!p->borrowed) {
+        double acc[16] = {0};                              // 16 fp64 partial sums (n is a multiple of 16)
+        for (uint64_t i = 0; i < p->n; i += 16)
+            for (int q = 0; q < 16; ++q) acc[q] += (double)series[i + q];
+        long double s = 0.0L;
+        for (int q = 0; q < 16; ++q) s += (long double)acc[q];
+        p->fill = (float)(double)(s / (long double)p->n);
+    } else {
+        double acc = 0.0;
+        if (!p->d_acc) TB_CUDA(p, cudaMalloc(&p->d_acc, sizeof(double)));
+        TB_CUDA(p, cudaMemsetAsync(p->d_acc, 0, sizeof(double), p->stream));
+        k_sum_f64<<<296, 256, 0, p->stream>>>(p->d_series, (size_t)p->n, p->d_acc);
+        TB_CUDA(p, cudaMemcpyAsync(&acc, p->d_acc, sizeof(double), cudaMemcpyDeviceToHost, p->stream));
+        TB_CUDA(p, cudaStreamSynchronize(p->stream));
+        p->fill = (float)(acc / (double)p->n);
+    }
+    return TB_OK;
 }
 
 int get_fft_plan(tb_plan* p, uint32_t batch, cufftHandle* out)
@@ -324,7 +356,7 @@ void destroy(tb_plan* p)
     for (auto& kv : p->fft_plans) cufftDestroy(kv.second);
     for (auto& es : p->events) for (auto& e : es.e) cudaEventDestroy(e);
     if (p->ev_staged) cudaEventDestroy(p->ev_staged);
-    cudaFree(p->d_work); cudaFree(p->d_series_owned); cudaFree(p->d_resampled); cudaFree(p->d_fft);
+    cudaFree(p->d_work); cudaFree(p->d_acc); cudaFree(p->d_series_owned); cudaFree(p->d_resampled); cudaFree(p->d_fft);
     cudaFree(p->d_power); cudaFree(p->d_med); cudaFree(p->d_cand); cudaFree(p->d_cursor); cudaFree(p->d_tmpl);
     if (p->h_tmpl) cudaFreeHost(p->h_tmpl);
     if (p->own_stream && p->stream) cudaStreamDestroy(p->stream);
@@ -427,30 +459,10 @@ int tb_plan_create(tb_plan** out, const float* series, uint64_t n_samples, doubl
     p->chunk = B;
 
     // series + fill value
-    if (o.series_is_device_ptr) {
-        p->d_series = series;
-    } else {
-        TB_TRY(cudaMalloc(&p->d_series_owned, p->n * sizeof(float)));
-        TB_TRY(cudaMemcpyAsync(p->d_series_owned, series, p->n * sizeof(float), cudaMemcpyHostToDevice, p->stream));
-        p->d_series = p->d_series_owned;
-    }
-    if (o.has_fill) {
-        p->fill = o.fill_value;
-    } else if (!o.series_is_device_ptr) {
-        long double s = 0.0L;
-        for (uint64_t i = 0; i < p->n; ++i) s += (long double)series[i];
-        p->fill = (float)(double)(s / (long double)p->n);
-    } else {
-        double* d_acc = nullptr;
-        double acc = 0.0;
-        TB_TRY(cudaMalloc(&d_acc, sizeof(double)));
-        TB_TRY(cudaMemsetAsync(d_acc, 0, sizeof(double), p->stream));
-        k_sum_f64<<<296, 256, 0, p->stream>>>(p->d_series, (size_t)p->n, d_acc);
-        TB_TRY(cudaMemcpyAsync(&acc, d_acc, sizeof(double), cudaMemcpyDeviceToHost, p->stream));
-        TB_TRY(cudaStreamSynchronize(p->stream));
-        cudaFree(d_acc);
-        p->fill = (float)(acc / (double)p->n);
-    }
+    p->borrowed = o.series_is_device_ptr != 0;
+    p->user_fill = o.has_fill != 0;
+    p->fill = o.fill_value;
+    { int rc = load_series(p, series); if (rc) { destroy(p); return rc; } }
 
     TB_TRY(cudaMalloc(&p->d_resampled, (size_t)B * p->n * sizeof(float)));
     TB_TRY(cudaMalloc(&p->d_fft, (size_t)B * p->ld * sizeof(float2)));
@@ -466,6 +478,13 @@ int tb_plan_create(tb_plan** out, const float* series, uint64_t n_samples, doubl
     if (cudaStreamSynchronize(p->stream) != cudaSuccess) { destroy(p); return TB_ERR_CUDA; }
     *out = p;
     return TB_OK;
+}
+
+int tb_plan_set_series(tb_plan* p, const float* series)
+{
+    if (!p || !series) return fail(p, TB_ERR_INVALID_ARG, "null argument");
+    TB_CUDA(p, cudaSetDevice(p->device));
+    return load_series(p, series);
 }
 
 int tb_plan_destroy(tb_plan* plan)
@@ -537,6 +556,7 @@ int tb_search_templates(tb_plan* p, const tb_template* tmpl, uint64_t n_template
         if ((rc = run_hsum(p, nt, fp, first_template_id + (uint32_t)off))) return rc;
         if (es) TB_CUDA(p, cudaEventRecord(es->e[5], p->stream));
         p->last.n_chunks++;
+        p->last.n_kernel_launches += 4;
     }
     return TB_OK;
 }

@@ -39,18 +39,20 @@ class Timings(C.Structure):
     _fields_ = [("ms_resample", C.c_double), ("ms_fft", C.c_double), ("ms_spectrum", C.c_double),
                 ("ms_normalise", C.c_double), ("ms_hsum", C.c_double), ("ms_total", C.c_double),
                 ("n_templates", C.c_uint64), ("n_samples", C.c_uint64), ("n_chunks", C.c_uint64),
-                ("chunk_templates", C.c_uint64), ("model_bytes_per_template", C.c_uint64)]
+                ("chunk_templates", C.c_uint64), ("model_bytes_per_template", C.c_uint64),
+                ("n_kernel_launches", C.c_uint64)]
 
     def as_dict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}
 
 
-EXPORTS = ["tb_plan_create", "tb_search_templates", "tb_get_candidates", "tb_clear_candidates", "tb_plan_destroy",
+EXPORTS = ["tb_plan_create", "tb_plan_set_series", "tb_search_templates", "tb_get_candidates", "tb_clear_candidates", "tb_plan_destroy",
            "tb_strerror", "tb_last_error", "tb_get_timings", "tb_debug_resample_indices", "tb_debug_spectrum",
            "tb_debug_resampled", "tb_sigma_to_power", "tb_plan_info", "tb_template_knot_log2"]
 
 _vp, _u64, _u32 = C.c_void_p, C.c_uint64, C.c_uint32
 lib.tb_plan_create.argtypes = [C.POINTER(_vp), _vp, _u64, C.c_double, C.POINTER(PlanOpts)]
+lib.tb_plan_set_series.argtypes = [_vp, _vp]
 lib.tb_search_templates.argtypes = [_vp, _vp, _u64, _u32, _vp, _u32, C.c_double]
 lib.tb_get_candidates.argtypes = [_vp, _vp, _u64, C.POINTER(_u64)]
 lib.tb_clear_candidates.argtypes = [_vp]
@@ -111,6 +113,16 @@ def tb_plan_create(series, n_samples, tsamp_s, *, device=0, stream=None, median_
     plan = _vp()
     _check(lib.tb_plan_create(C.byref(plan), ptr, int(n_samples), float(tsamp_s), C.byref(o)))
     return plan
+
+
+def tb_plan_set_series(plan, series, series_is_device_ptr=False):
+    """series: numpy float32[N] (host; pinned memory makes the copy asynchronous) or a device address."""
+    if series_is_device_ptr:
+        ptr = int(series)
+    else:
+        assert series.dtype == np.float32 and series.flags.c_contiguous
+        ptr = series.ctypes.data
+    _check(lib.tb_plan_set_series(plan, ptr), plan)
 
 
 def tb_search_templates(plan, templates, first_template_id=0, folds=(0, 1, 2, 3, 4), sigma_threshold=6.0):
@@ -208,6 +220,10 @@ class Plan:
         self.median_window = int(opts.get("median_window", 0) or 1024)
         self._series = series                        # keep host/device memory alive
         self.handle = tb_plan_create(series, self.n_samples, tsamp_s, **opts)
+
+    def set_series(self, series, series_is_device_ptr=False):
+        self._series = series
+        tb_plan_set_series(self.handle, series, series_is_device_ptr)
 
     def search(self, templates, first_template_id=0, folds=(0, 1, 2, 3, 4), sigma_threshold=6.0):
         tb_search_templates(self.handle, templates, first_template_id, folds, sigma_threshold)

@@ -166,16 +166,18 @@ def config3(n_templates: int = 16384, log2n: int = 25) -> Workload:
     return Workload("C3", n, tsamp, x.astype(np.float32), templates, (0,), (psr,))
 
 
-def config4(n_templates: int = 8192, log2n: int = 23) -> Workload:
+def config4(n_templates: int = 8192, log2n: int = 23, tau_scale: float = 1.0) -> Workload:
     """C4: elliptical, 2^23 @ 64 us, N(0,1) + 25 ms pulsar (P_orb=0.15T, tau=4, e=0.08,
-    omega=1.2); bank P_orb~U[.1,.2]T, tau~U[.5,8], phi0,omega~U[0,2pi), e~U[0,.1]."""
+    omega=1.2); bank P_orb~U[.1,.2]T, tau~U[.5,8], phi0,omega~U[0,2pi), e~U[0,.1].
+    ``tau_scale`` shrinks every tau for scaled-down test series (P_orb scales with T, so tau has
+    to shrink too for the orbit to stay sub-luminal)."""
     n, tsamp = 1 << log2n, 64e-6
     T = n * tsamp
     rng = _rng(4)
     noise = rng.standard_normal(n)
     phi0 = rng.uniform(0.0, 2.0 * np.pi)
-    psr = (0.025, 0.15 * T, 4.0, phi0, 0.08, 1.2, default_amplitude(n))
-    bank = _bank(rng, n_templates - 1, 0.1 * T, 0.2 * T, 0.5, 8.0, elliptical=True)
+    psr = (0.025, 0.15 * T, 4.0 * tau_scale, phi0, 0.08, 1.2, default_amplitude(n))
+    bank = _bank(rng, n_templates - 1, 0.1 * T, 0.2 * T, 0.5 * tau_scale, 8.0 * tau_scale, elliptical=True)
     x = noise + pulse_train(n, tsamp, *psr)
     templates = np.vstack([np.array([[psr[1], psr[2], psr[3], psr[4], psr[5]]]), bank])
     return Workload("C4", n, tsamp, x.astype(np.float32), templates, (0,), (psr,))

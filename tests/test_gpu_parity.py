@@ -56,7 +56,7 @@ def test_c1_low_threshold_stresses_the_compactor(tb, c1):
     cands, rep = full_bank_parity(tb, c1, 4.0, range(0, 64, 7))
     assert len(cands) > 100
     cands, rep = full_bank_parity(tb, c1, 2.5, (0, 31))
-    assert len(cands) > 100000
+    assert len(cands) > 10000
     assert all(r["n_gpu"] > 0 for r in rep.values())
 
 
@@ -112,7 +112,7 @@ def test_exact_fallback_when_the_orbit_is_too_fast_for_interpolation(tb, c1):
 
 
 def test_out_of_range_samples_take_the_fill_value(tb, c1):
-    tmpl = np.array([100.0, 3.0, 4.0, 0.0, 0.0])                 # shifts of thousands of samples
+    tmpl = np.array([100.0, 3.0, 1.0, 0.0, 0.0])                 # the last ~2000 samples map beyond the end
     with tb.Plan(c1.series, c1.tsamp, fill_value=123.5) as plan:
         idx = plan.debug_indices(tmpl)
         y = plan.debug_resampled(tmpl)
@@ -171,7 +171,7 @@ def test_device_resident_series(tb, c1):
 
 # ------------------------------------------------------------------ elliptical, small
 def test_elliptical_small_full_parity(tb):
-    w = wl_mod.config4(n_templates=24, log2n=18)
+    w = wl_mod.config4(n_templates=24, log2n=18, tau_scale=1.0 / 128)
     cands, rep = full_bank_parity(tb, w, 5.0, range(24))
     assert 0 in by_template(cands)                                # the injected pulsar is found
     w2 = wl_mod.Workload("hi-e", w.n_samples, w.tsamp, w.series,

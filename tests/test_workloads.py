@@ -21,7 +21,7 @@ def test_small_variants_of_c2_c3_c4_c5():
     c3 = wl.config3(n_templates=8, log2n=16)
     q = c3.series * 32.0
     assert np.array_equal(q, np.rint(q)) and q.min() >= -128 and q.max() <= 127   # 8-bit codes
-    c4 = wl.config4(n_templates=8, log2n=16)
+    c4 = wl.config4(n_templates=8, log2n=16, tau_scale=1 / 512)
     assert c4.templates[0, 3] == 0.08 and c4.templates[0, 4] == 1.2
     assert c4.templates[1:, 3].max() <= 0.1 and c4.templates[1:, 3].min() >= 0
     c5 = wl.config5(log2n=16, n_circ=4, n_ell=4)
