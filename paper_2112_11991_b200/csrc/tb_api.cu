@@ -288,6 +288,20 @@ int run_normalise(tb_plan* p, uint32_t nt)
 
 int run_hsum(tb_plan* p, uint32_t nt, const FoldParams& fp, uint32_t first_id)
 {
+    if (p->nb >= (uint64_t)HS_T) {
+        const int tiles = (int)(p->nb / HS_T);
+        const size_t smem = HS_SMEM_FLOATS * sizeof(float);
+        static bool attr_set = false;
+        if (!attr_set) {
+            TB_CUDA(p, cudaFuncSetAttribute(k_hsum_tile, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            attr_set = true;
+        }
+        k_hsum_tile<<<(unsigned)(tiles * nt), HS_THREADS, smem, p->stream>>>(p->d_power, (int)p->nb, tiles, fp, first_id,
+                                                                             p->d_cand, p->d_cursor,
+                                                                             (unsigned long long)p->max_cand);
+        TB_CUDA(p, cudaGetLastError());
+        return TB_OK;
+    }
     const int cta_per_row = (int)((p->nb + 255) / 256);
     k_hsum_threshold<<<(unsigned)(cta_per_row * nt), 256, 0, p->stream>>>(p->d_power, (int)p->nb, cta_per_row, fp,
                                                                           first_id, p->d_cand, p->d_cursor,

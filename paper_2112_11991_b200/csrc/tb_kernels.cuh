@@ -368,6 +368,198 @@ k_hsum_threshold(const float* __restrict__ Ph, int nb, int cta_per_row, FoldPara
     }
 }
 
+// ---------------------------------------------------------------------------------------------
+// K4t  tiled harmonic summer (a8 + a9) for Nb >= HS_T.  Same sums as k_hsum_threshold.
+//   One CTA = HS_T consecutive top-harmonic bins of one template; one thread = 16 consecutive
+//   bins k = k0 + 16 q + r.  For harmonic m/2^L (odd m) those 16 bins read the m*(16>>L)+1
+//   consecutive values starting at (m k0 >> L) + m q (16>>L), and WHICH of them bin r takes,
+//   (m r + 2^(L-1)) >> L, is a compile-time constant: after unrolling there is no index
+//   arithmetic left, 9.4 loads per bin instead of 16, and every add is register-to-register.
+//   The 14 regions (m/4, m/8, m/16) of the normalised spectrum are staged in shared memory by
+//   TMA 1-D bulk copies (cp.async.bulk + mbarrier: no load/store instructions spent on staging);
+//   lane strides m*(16>>L) words with 32/64/128-bit accesses are bank-conflict free for odd m.
+//   Folds 0 and 1 come straight from global memory with coalesced 128-bit loads.
+//   Templates are processed row-major so that one template's spectrum (2N bytes) stays in L2
+//   while its 8.5 reads per bin are served (L2 -> SM traffic 17N bytes per template).
+// ---------------------------------------------------------------------------------------------
+constexpr int HS_T = 2048;
+constexpr int HS_THREADS = HS_T / 16;
+
+__host__ __device__ constexpr int hs_len(int L, int m) { return m * (HS_T >> L) + 4; }
+__host__ __device__ constexpr int hs_off(int L, int m)
+{
+    int o = 0;
+    for (int l = 2; l <= 4; ++l)
+        for (int mm = 1; mm < (1 << l); mm += 2) {
+            if (l == L && mm == m) return o;
+            o += hs_len(l, mm);
+        }
+    return o;
+}
+constexpr int HS_SMEM_FLOATS = hs_off(5, 1);
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "WAIT_%=:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+        "@p bra DONE_%=;\n\t"
+        "bra WAIT_%=;\n\t"
+        "DONE_%=:\n\t}" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                     smem_u32(dst)),
+                 "l"(src), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+
+// acc[r] += span[(M r + 2^(L-1)) >> L], span = the M*(16>>L)+1 staged values of this thread
+template <int L, int M>
+__device__ __forceinline__ void hs_accumulate(const float* __restrict__ sm, int q, float (&acc)[16])
+{
+    constexpr int STEP = M * (16 >> L);              // words between consecutive threads' spans
+    constexpr int NV = STEP + 1;
+    const float* sp = sm + hs_off(L, M) + q * STEP;
+    float v[NV];
+    if constexpr (L == 2) {                          // STEP multiple of 4: 128-bit loads
+#pragma unroll
+        for (int i = 0; i < STEP; i += 4) {
+            const float4 t = *reinterpret_cast<const float4*>(sp + i);
+            v[i] = t.x; v[i + 1] = t.y; v[i + 2] = t.z; v[i + 3] = t.w;
+        }
+    } else if constexpr (L == 3) {                   // STEP multiple of 2: 64-bit loads
+#pragma unroll
+        for (int i = 0; i < STEP; i += 2) {
+            const float2 t = *reinterpret_cast<const float2*>(sp + i);
+            v[i] = t.x; v[i + 1] = t.y;
+        }
+    } else {
+#pragma unroll
+        for (int i = 0; i < STEP; ++i) v[i] = sp[i];
+    }
+    v[STEP] = sp[STEP];
+#pragma unroll
+    for (int r = 0; r < 16; ++r) acc[r] += v[(M * r + (1 << (L - 1))) >> L];
+}
+
+// rare path: emit the hits of one fold with a warp-aggregated atomic per bin offset
+template <int L>
+__device__ __forceinline__ void hs_emit(const float (&acc)[16], uint32_t kq, const FoldParams& fp, uint32_t tid,
+                                        Candidate* __restrict__ out, unsigned long long* __restrict__ cursor,
+                                        unsigned long long capacity)
+{
+    const unsigned lane = threadIdx.x & 31;
+#pragma unroll
+    for (int r = 0; r < 16; ++r) {                   // unrolled: acc[] must stay in registers
+        const uint32_t k = kq + (uint32_t)r;
+        const bool hit = (acc[r] >= fp.thr[L]) && (k >= (fp.k_lo << L));
+        const unsigned mask = __ballot_sync(0xffffffffu, hit);
+        if (mask == 0u) continue;
+        const int leader = __ffs(mask) - 1;
+        unsigned long long basepos = 0;
+        if ((int)lane == leader) basepos = atomicAdd(cursor, (unsigned long long)__popc(mask));
+        basepos = __shfl_sync(0xffffffffu, basepos, leader);
+        if (hit) {
+            const unsigned long long pos = basepos + (unsigned long long)__popc(mask & ((1u << lane) - 1u));
+            if (pos < capacity) {
+                Candidate c;
+                c.template_id = tid; c.fold = (uint32_t)L; c.bin = k; c.power = acc[r];
+                c.sigma = (sqrtf(acc[r]) - fp.mu[L]) * fp.inv_s[L];
+                c.pad = 0u;
+                out[pos] = c;
+            }
+        }
+    }
+}
+
+template <int L>
+__device__ __forceinline__ void hs_check(const float (&acc)[16], uint32_t kq, const FoldParams& fp, uint32_t tid,
+                                         Candidate* __restrict__ out, unsigned long long* __restrict__ cursor,
+                                         unsigned long long capacity)
+{
+    bool any = false;
+    const float thr = fp.thr[L];
+#pragma unroll
+    for (int r = 0; r < 16; ++r) any |= (acc[r] >= thr);
+    if (__any_sync(0xffffffffu, any)) hs_emit<L>(acc, kq, fp, tid, out, cursor, capacity);
+}
+
+__global__ void __launch_bounds__(HS_THREADS)
+k_hsum_tile(const float* __restrict__ Ph, int nb, int tiles_per_row, FoldParams fp, uint32_t first_id,
+            Candidate* __restrict__ out, unsigned long long* __restrict__ cursor, unsigned long long capacity)
+{
+    extern __shared__ __align__(16) float hs_sm[];
+    __shared__ __align__(8) uint64_t bar;
+    const int row = blockIdx.x / tiles_per_row;
+    const int k0  = (blockIdx.x % tiles_per_row) * HS_T;
+    const float* __restrict__ p = Ph + (size_t)row * (size_t)nb;
+    const uint32_t tid = first_id + (uint32_t)row;
+
+    if (threadIdx.x == 0) mbar_init(&bar, 1);
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        mbar_expect_tx(&bar, (uint32_t)(HS_SMEM_FLOATS * sizeof(float)));
+#pragma unroll
+        for (int L = 2; L <= 4; ++L)
+#pragma unroll
+            for (int m = 1; m < (1 << L); m += 2)
+                bulk_g2s(hs_sm + hs_off(L, m), p + (((size_t)m * (size_t)k0) >> L), (uint32_t)(hs_len(L, m) * sizeof(float)), &bar);
+    }
+
+    const int q = threadIdx.x;
+    const uint32_t kq = (uint32_t)(k0 + 16 * q);
+    float acc[16];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {                    // fold 0: the bin itself
+        const float4 t = __ldg(reinterpret_cast<const float4*>(p + kq) + i);
+        acc[4 * i] = t.x; acc[4 * i + 1] = t.y; acc[4 * i + 2] = t.z; acc[4 * i + 3] = t.w;
+    }
+    hs_check<0>(acc, kq, fp, tid, out, cursor, capacity);
+    {                                                // fold 1: + P^[(k+1)>>1], 9 values from 8 q'
+        const float* h = p + (kq >> 1);
+        const float4 a = __ldg(reinterpret_cast<const float4*>(h));
+        const float4 b = __ldg(reinterpret_cast<const float4*>(h) + 1);
+        const float  c = __ldg(h + 8);
+        const float v[9] = {a.x, a.y, a.z, a.w, b.x, b.y, b.z, b.w, c};
+#pragma unroll
+        for (int r = 0; r < 16; ++r) acc[r] += v[(r + 1) >> 1];
+    }
+    hs_check<1>(acc, kq, fp, tid, out, cursor, capacity);
+
+    mbar_wait(&bar, 0);
+    hs_accumulate<2, 1>(hs_sm, q, acc);
+    hs_accumulate<2, 3>(hs_sm, q, acc);
+    hs_check<2>(acc, kq, fp, tid, out, cursor, capacity);
+    hs_accumulate<3, 1>(hs_sm, q, acc);
+    hs_accumulate<3, 3>(hs_sm, q, acc);
+    hs_accumulate<3, 5>(hs_sm, q, acc);
+    hs_accumulate<3, 7>(hs_sm, q, acc);
+    hs_check<3>(acc, kq, fp, tid, out, cursor, capacity);
+    hs_accumulate<4, 1>(hs_sm, q, acc);
+    hs_accumulate<4, 3>(hs_sm, q, acc);
+    hs_accumulate<4, 5>(hs_sm, q, acc);
+    hs_accumulate<4, 7>(hs_sm, q, acc);
+    hs_accumulate<4, 9>(hs_sm, q, acc);
+    hs_accumulate<4, 11>(hs_sm, q, acc);
+    hs_accumulate<4, 13>(hs_sm, q, acc);
+    hs_accumulate<4, 15>(hs_sm, q, acc);
+    hs_check<4>(acc, kq, fp, tid, out, cursor, capacity);
+}
+
 // fp64 sum of a device series (fill value when the series is borrowed device memory)
 __global__ void k_sum_f64(const float* __restrict__ x, size_t n, double* __restrict__ acc)
 {
