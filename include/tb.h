@@ -94,7 +94,9 @@ typedef struct {
                                      rounded to fp32 (G8); 1: they take fill_value */
     float    fill_value;
     int32_t  enable_timings;      /* 1: record CUDA events around every stage of every chunk */
-    int32_t  reserved;
+    int32_t  fft_path;            /* 0: automatic (hand-written two-pass FFT with fused gather where it
+                                     applies: 2^17 <= N <= 2^23 and knot spacing >= 8, batched cuFFT
+                                     otherwise); 1: always cuFFT; 2: hand-written or TB_ERR_INVALID_ARG */
 } tb_plan_opts;
 
 /* Per-stage device time of the last tb_search_templates call (CUDA events, summed over chunks;

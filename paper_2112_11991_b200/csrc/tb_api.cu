@@ -2,6 +2,7 @@
 // candidate retrieval (a10), timings and parity taps.  Boundary: include/tb.h.
 #include "../../include/tb.h"
 #include "tb_kernels.cuh"
+#include "tb_fft.cuh"
 
 #include <cufft.h>
 
@@ -58,6 +59,14 @@ struct tb_plan {
     size_t h_tmpl_cap = 0;
     cudaEvent_t ev_staged = nullptr;                 // the last template upload has been consumed
     bool staged_pending = false;
+
+    // hand-written FFT path (tb_fft.cuh): M = N/2 = M1 * M2
+    bool own_fft = false;
+    int log2m1 = 0, log2m2 = 0;
+    SegRec* d_seg = nullptr;                         // [chunk][n >> MIN_LOG2H]
+    size_t seg_stride = 0;
+    float2 *d_tw1a = nullptr, *d_tw1b = nullptr, *d_tw2 = nullptr, *d_twn = nullptr;
+    int min_log2h = 0;                               // smallest knot spacing among the staged templates
 
     std::map<uint32_t, cufftHandle> fft_plans;       // by batch size, sharing one work area
     void* d_work = nullptr;
@@ -231,12 +240,115 @@ int get_fft_plan(tb_plan* p, uint32_t batch, cufftHandle* out)
     return TB_OK;
 }
 
+constexpr int OWN_MIN_LOG2H = 3;                     // the fused path needs >= 2 samples per segment; 8 bounds the table
+
 template <int W>
-void launch_spectrum(tb_plan* p, uint32_t nt)
+void launch_spectrum(tb_plan* p, uint32_t nt, bool unpack)
 {
     const int cta_per_row = (int)((p->nblk + SP_WARPS - 1) / SP_WARPS);
-    k_spectrum_median<W><<<(unsigned)(cta_per_row * nt), SP_WARPS * 32, 0, p->stream>>>(
-        p->d_fft, p->ld, p->d_power, p->d_med, (int)p->nb, (int)p->nblk, cta_per_row);
+    if (unpack)
+        k_spectrum_median<W, true><<<(unsigned)(cta_per_row * nt), SP_WARPS * 32, 0, p->stream>>>(
+            p->d_fft, (size_t)p->nb, p->d_power, p->d_med, (int)p->nb, (int)p->nblk, cta_per_row, p->d_twn);
+    else
+        k_spectrum_median<W, false><<<(unsigned)(cta_per_row * nt), SP_WARPS * 32, 0, p->stream>>>(
+            p->d_fft, p->ld, p->d_power, p->d_med, (int)p->nb, (int)p->nblk, cta_per_row, nullptr);
+}
+
+// ---- hand-written FFT path -------------------------------------------------------------------
+template <int R1> constexpr int fft_bundle() { return R1 >= 8 ? 4 : 8; }       // C (pass 1) and R (pass 2)
+template <int R1> constexpr size_t fft_smem() { return (size_t)(fft_bundle<R1>() * (R1 * FFT_PA + 16 / fft_bundle<R1>()) + 256) * sizeof(float2); }
+
+template <int R1, bool DEBUG>
+int launch_cols(tb_plan* p, size_t off, uint32_t nt, long long* d_idx, float* d_y)
+{
+    constexpr int C = fft_bundle<R1>();
+    auto kern = k_fft_cols<R1, C, DEBUG>;
+    static bool attr = false;
+    if (!attr) { TB_CUDA(p, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_smem<R1>())); attr = true; }
+    const unsigned grid = (unsigned)(((1u << p->log2m2) / C) * nt);
+    kern<<<grid, FFT_THREADS, fft_smem<R1>(), p->stream>>>(p->d_series, p->d_seg, p->seg_stride, p->d_tmpl + off, (int)nt,
+                                                          (int)p->n, p->log2m2, p->fill, p->d_tw1a, p->d_tw2,
+                                                          reinterpret_cast<float2*>(p->d_resampled), d_idx, d_y);
+    TB_CUDA(p, cudaGetLastError());
+    return TB_OK;
+}
+
+template <int R1>
+int launch_rows(tb_plan* p, uint32_t nt)
+{
+    constexpr int R = fft_bundle<R1>();
+    auto kern = k_fft_rows<R1, R>;
+    static bool attr = false;
+    if (!attr) { TB_CUDA(p, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_smem<R1>())); attr = true; }
+    const unsigned grid = (unsigned)(((1u << p->log2m1) / R) * nt);
+    kern<<<grid, FFT_THREADS, fft_smem<R1>(), p->stream>>>(reinterpret_cast<const float2*>(p->d_resampled), p->d_fft,
+                                                          p->log2m1, p->d_tw1b, p->d_tw2);
+    TB_CUDA(p, cudaGetLastError());
+    return TB_OK;
+}
+
+// K0 + P1: delay segments, then gather + column FFTs into T (the buffer the legacy path uses for y)
+int run_own_pass1(tb_plan* p, size_t off, uint32_t nt, long long* d_idx, float* d_y)
+{
+    const int cta_per_tmpl = (int)(((p->n >> OWN_MIN_LOG2H) + 255) / 256);
+    k_delay_segments<<<(unsigned)(cta_per_tmpl * nt), 256, 0, p->stream>>>(p->d_tmpl + off, (int)nt, (int)p->n, p->d_seg,
+                                                                           p->seg_stride, cta_per_tmpl);
+    TB_CUDA(p, cudaGetLastError());
+    const bool dbg = d_idx != nullptr;
+    switch (p->log2m1 - 8) {
+        case 0: return dbg ? launch_cols<1, true>(p, off, nt, d_idx, d_y) : launch_cols<1, false>(p, off, nt, nullptr, nullptr);
+        case 1: return dbg ? launch_cols<2, true>(p, off, nt, d_idx, d_y) : launch_cols<2, false>(p, off, nt, nullptr, nullptr);
+        case 2: return dbg ? launch_cols<4, true>(p, off, nt, d_idx, d_y) : launch_cols<4, false>(p, off, nt, nullptr, nullptr);
+        case 3: return dbg ? launch_cols<8, true>(p, off, nt, d_idx, d_y) : launch_cols<8, false>(p, off, nt, nullptr, nullptr);
+    }
+    return fail(p, TB_ERR_INVALID_ARG, "unsupported M1");
+}
+
+int run_own_pass2(tb_plan* p, uint32_t nt)
+{
+    switch (p->log2m2 - 8) {
+        case 0: return launch_rows<1>(p, nt);
+        case 1: return launch_rows<2>(p, nt);
+        case 2: return launch_rows<4>(p, nt);
+        case 3: return launch_rows<8>(p, nt);
+    }
+    return fail(p, TB_ERR_INVALID_ARG, "unsupported M2");
+}
+
+// twiddle tables of the hand-written FFT, in long double, rounded once to fp32
+int make_twiddles(tb_plan* p)
+{
+    const long double two_pi = 8.0L * atanl(1.0L);
+    auto upload = [&](std::vector<float2>& h, float2** d) -> int {
+        TB_CUDA(p, cudaMalloc(d, h.size() * sizeof(float2)));
+        TB_CUDA(p, cudaMemcpy(*d, h.data(), h.size() * sizeof(float2), cudaMemcpyHostToDevice));
+        return TB_OK;
+    };
+    auto tw1 = [&](int log2l, float2** d) -> int {       // [ka*256 + w] = W_L^{w ka}
+        const int L = 1 << log2l, R1 = L / 256;
+        std::vector<float2> h((size_t)L);
+        for (int ka = 0; ka < R1; ++ka)
+            for (int w = 0; w < 256; ++w) {
+                const long double a = -two_pi * (long double)((long long)w * ka % L) / (long double)L;
+                h[(size_t)ka * 256 + w] = make_float2((float)cosl(a), (float)sinl(a));
+            }
+        return upload(h, d);
+    };
+    int rc;
+    if ((rc = tw1(p->log2m1, &p->d_tw1a))) return rc;
+    if ((rc = tw1(p->log2m2, &p->d_tw1b))) return rc;
+    std::vector<float2> h2(256), hn(p->window);
+    for (int kb = 0; kb < 16; ++kb)
+        for (int c = 0; c < 16; ++c) {
+            const long double a = -two_pi * (long double)(kb * c) / 256.0L;
+            h2[kb * 16 + c] = make_float2((float)cosl(a), (float)sinl(a));
+        }
+    for (uint32_t i = 0; i < p->window; ++i) {
+        const long double a = -two_pi * (long double)i / (long double)p->n;
+        hn[i] = make_float2((float)cosl(a), (float)sinl(a));
+    }
+    if ((rc = upload(h2, &p->d_tw2))) return rc;
+    return upload(hn, &p->d_twn);
 }
 
 // stages of one chunk of nt templates whose constants sit at d_tmpl + off
@@ -263,14 +375,14 @@ int run_fft(tb_plan* p, uint32_t nt)
     return TB_OK;
 }
 
-int run_spectrum(tb_plan* p, uint32_t nt)
+int run_spectrum(tb_plan* p, uint32_t nt, bool unpack)
 {
     switch (p->window) {
-        case 128: launch_spectrum<128>(p, nt); break;
-        case 256: launch_spectrum<256>(p, nt); break;
-        case 512: launch_spectrum<512>(p, nt); break;
-        case 1024: launch_spectrum<1024>(p, nt); break;
-        case 2048: launch_spectrum<2048>(p, nt); break;
+        case 128: launch_spectrum<128>(p, nt, unpack); break;
+        case 256: launch_spectrum<256>(p, nt, unpack); break;
+        case 512: launch_spectrum<512>(p, nt, unpack); break;
+        case 1024: launch_spectrum<1024>(p, nt, unpack); break;
+        case 2048: launch_spectrum<2048>(p, nt, unpack); break;
         default: return fail(p, TB_ERR_INVALID_ARG, "median_window");
     }
     TB_CUDA(p, cudaGetLastError());
@@ -333,7 +445,11 @@ int upload_templates(tb_plan* p, const tb_template* tmpl, uint64_t k)
         TB_CUDA(p, cudaMalloc(&p->d_tmpl, k * sizeof(TmplDev)));
         p->tmpl_cap = k;
     }
-    for (uint64_t i = 0; i < k; ++i) make_tmpl(tmpl[i], p->tsamp, &p->h_tmpl[i]);
+    p->min_log2h = 7;
+    for (uint64_t i = 0; i < k; ++i) {
+        make_tmpl(tmpl[i], p->tsamp, &p->h_tmpl[i]);
+        p->min_log2h = std::min(p->min_log2h, (int)p->h_tmpl[i].log2h);
+    }
     TB_CUDA(p, cudaMemcpyAsync(p->d_tmpl, p->h_tmpl, k * sizeof(TmplDev), cudaMemcpyHostToDevice, p->stream));
     TB_CUDA(p, cudaEventRecord(p->ev_staged, p->stream));
     p->staged_pending = true;
@@ -370,6 +486,7 @@ void destroy(tb_plan* p)
     for (auto& kv : p->fft_plans) cufftDestroy(kv.second);
     for (auto& es : p->events) for (auto& e : es.e) cudaEventDestroy(e);
     if (p->ev_staged) cudaEventDestroy(p->ev_staged);
+    cudaFree(p->d_seg); cudaFree(p->d_tw1a); cudaFree(p->d_tw1b); cudaFree(p->d_tw2); cudaFree(p->d_twn);
     cudaFree(p->d_work); cudaFree(p->d_acc); cudaFree(p->d_series_owned); cudaFree(p->d_resampled); cudaFree(p->d_fft);
     cudaFree(p->d_power); cudaFree(p->d_med); cudaFree(p->d_cand); cudaFree(p->d_cursor); cudaFree(p->d_tmpl);
     if (p->h_tmpl) cudaFreeHost(p->h_tmpl);
@@ -461,7 +578,7 @@ int tb_plan_create(tb_plan** out, const float* series, uint64_t n_samples, doubl
     TB_TRY(cudaEventCreateWithFlags(&p->ev_staged, cudaEventDisableTiming));
 
     // chunk size B
-    const size_t per_t = (size_t)p->n * 4 + p->ld * 8 + (size_t)p->nb * 4 + (size_t)p->nblk * 4;
+    const size_t per_t = (size_t)p->n * 4 + p->ld * 8 + (size_t)p->nb * 4 + (size_t)p->nblk * 4 + (size_t)p->n * 8;
     uint32_t B = o.chunk_templates;
     if (B == 0) {
         size_t free_b = 0, total_b = 0;
@@ -478,6 +595,21 @@ int tb_plan_create(tb_plan** out, const float* series, uint64_t n_samples, doubl
     p->fill = o.fill_value;
     { int rc = load_series(p, series); if (rc) { destroy(p); return rc; } }
 
+    // FFT path: hand-written two-pass FFT for 2^17 <= N <= 2^23, batched cuFFT otherwise
+    {
+        const int lm = (int)ilog2(p->nb);
+        p->log2m1 = lm / 2;
+        p->log2m2 = lm - p->log2m1;
+        const bool fits = p->log2m1 >= 8 && p->log2m2 <= 11;
+        if (o.fft_path == 2 && !fits) { destroy(p); return TB_ERR_INVALID_ARG; }
+        p->own_fft = fits && o.fft_path != 1;
+    }
+    if (p->own_fft) {
+        p->seg_stride = (size_t)(p->n >> OWN_MIN_LOG2H);
+        TB_TRY(cudaMalloc(&p->d_seg, (size_t)B * p->seg_stride * sizeof(SegRec)));
+        int rc = make_twiddles(p);
+        if (rc) { destroy(p); return rc; }
+    }
     TB_TRY(cudaMalloc(&p->d_resampled, (size_t)B * p->n * sizeof(float)));
     TB_TRY(cudaMalloc(&p->d_fft, (size_t)B * p->ld * sizeof(float2)));
     TB_TRY(cudaMalloc(&p->d_power, (size_t)B * p->nb * sizeof(float)));
@@ -547,6 +679,7 @@ int tb_search_templates(tb_plan* p, const tb_template* tmpl, uint64_t n_template
     rc = upload_templates(p, tmpl, n_templates);
     if (rc) return rc;
 
+    const bool own = p->own_fft && p->min_log2h >= OWN_MIN_LOG2H;
     for (uint64_t off = 0; off < n_templates; off += p->chunk) {
         const uint32_t nt = (uint32_t)std::min<uint64_t>(p->chunk, n_templates - off);
         EventSet* es = nullptr;
@@ -559,11 +692,18 @@ int tb_search_templates(tb_plan* p, const tb_template* tmpl, uint64_t n_template
             es = &p->events[p->events_used++];
             TB_CUDA(p, cudaEventRecord(es->e[0], p->stream));
         }
-        if ((rc = run_resample(p, off, nt, nullptr))) return rc;
-        if (es) TB_CUDA(p, cudaEventRecord(es->e[1], p->stream));
-        if ((rc = run_fft(p, nt))) return rc;
+        if (own) {                                       // K0 + P1 | P2 | unpack + spectrum + median
+            if ((rc = run_own_pass1(p, off, nt, nullptr, nullptr))) return rc;
+            if (es) TB_CUDA(p, cudaEventRecord(es->e[1], p->stream));
+            if ((rc = run_own_pass2(p, nt))) return rc;
+            p->last.n_kernel_launches += 2;
+        } else {
+            if ((rc = run_resample(p, off, nt, nullptr))) return rc;
+            if (es) TB_CUDA(p, cudaEventRecord(es->e[1], p->stream));
+            if ((rc = run_fft(p, nt))) return rc;
+        }
         if (es) TB_CUDA(p, cudaEventRecord(es->e[2], p->stream));
-        if ((rc = run_spectrum(p, nt))) return rc;
+        if ((rc = run_spectrum(p, nt, own))) return rc;
         if (es) TB_CUDA(p, cudaEventRecord(es->e[3], p->stream));
         if ((rc = run_normalise(p, nt))) return rc;
         if (es) TB_CUDA(p, cudaEventRecord(es->e[4], p->stream));
@@ -635,6 +775,14 @@ int tb_debug_resample_indices(tb_plan* p, const tb_template* tmpl, int64_t* idx_
     if (rc) return rc;
     long long* d_idx = nullptr;
     TB_CUDA(p, cudaMalloc(&d_idx, p->n * sizeof(long long)));
+    if (p->own_fft && p->min_log2h >= OWN_MIN_LOG2H) {
+        float* d_y = nullptr;
+        cudaError_t e = cudaMalloc(&d_y, p->n * sizeof(float));
+        if (e != cudaSuccess) { cudaFree(d_idx); return fail(p, TB_ERR_NOMEM, "debug buffer"); }
+        rc = run_own_pass1(p, 0, 1, d_idx, d_y);
+        cudaStreamSynchronize(p->stream);
+        cudaFree(d_y);
+    } else
     rc = run_resample(p, 0, 1, d_idx);
     if (!rc) {
         cudaError_t e = cudaMemcpyAsync(idx_out, d_idx, p->n * sizeof(long long), cudaMemcpyDeviceToHost, p->stream);
@@ -650,6 +798,22 @@ int tb_debug_resampled(tb_plan* p, const tb_template* tmpl, float* y_out)
     if (!y_out) return fail(p, TB_ERR_INVALID_ARG, "null argument");
     int rc = single_template_stage(p, tmpl);
     if (rc) return rc;
+    if (p->own_fft && p->min_log2h >= OWN_MIN_LOG2H) {
+        long long* d_idx = nullptr;
+        float* d_y = nullptr;
+        TB_CUDA(p, cudaMalloc(&d_idx, p->n * sizeof(long long)));
+        cudaError_t e = cudaMalloc(&d_y, p->n * sizeof(float));
+        if (e != cudaSuccess) { cudaFree(d_idx); return fail(p, TB_ERR_NOMEM, "debug buffer"); }
+        rc = run_own_pass1(p, 0, 1, d_idx, d_y);
+        if (!rc) {
+            e = cudaMemcpyAsync(y_out, d_y, p->n * sizeof(float), cudaMemcpyDeviceToHost, p->stream);
+            if (e == cudaSuccess) e = cudaStreamSynchronize(p->stream);
+            if (e != cudaSuccess) rc = fail(p, TB_ERR_CUDA, cudaGetErrorString(e));
+        }
+        cudaStreamSynchronize(p->stream);
+        cudaFree(d_idx); cudaFree(d_y);
+        return rc;
+    }
     if ((rc = run_resample(p, 0, 1, nullptr))) return rc;
     TB_CUDA(p, cudaMemcpyAsync(y_out, p->d_resampled, p->n * sizeof(float), cudaMemcpyDeviceToHost, p->stream));
     TB_CUDA(p, cudaStreamSynchronize(p->stream));
@@ -660,9 +824,15 @@ int tb_debug_spectrum(tb_plan* p, const tb_template* tmpl, float* p_interbinned,
 {
     int rc = single_template_stage(p, tmpl);
     if (rc) return rc;
-    if ((rc = run_resample(p, 0, 1, nullptr))) return rc;
-    if ((rc = run_fft(p, 1))) return rc;
-    if ((rc = run_spectrum(p, 1))) return rc;
+    const bool own = p->own_fft && p->min_log2h >= OWN_MIN_LOG2H;
+    if (own) {
+        if ((rc = run_own_pass1(p, 0, 1, nullptr, nullptr))) return rc;
+        if ((rc = run_own_pass2(p, 1))) return rc;
+    } else {
+        if ((rc = run_resample(p, 0, 1, nullptr))) return rc;
+        if ((rc = run_fft(p, 1))) return rc;
+    }
+    if ((rc = run_spectrum(p, 1, own))) return rc;
     if (p_interbinned)
         TB_CUDA(p, cudaMemcpyAsync(p_interbinned, p->d_power, p->nb * sizeof(float), cudaMemcpyDeviceToHost, p->stream));
     if (medians)

@@ -1,0 +1,321 @@
+// tb_fft.cuh -- hand-written two-pass (four-step) FFT of the resampled series, with the
+// nearest-neighbour gather fused into the first pass's load (steps a2+a3+a4 of include/tb.h).
+//
+// The real series y[0..N) of one template is transformed as the complex series
+// z_j = y_{2j} + i y_{2j+1}, j < M = N/2, with M = M1 * M2 ("apply the
+// resampling ... and then calculate an FFT"; G11: forward, unnormalised):
+//
+//   j = j1*M2 + j2,  k = k1 + M1*k2
+//   Z[k1 + M1 k2] = sum_{j2} W_M^{j2 k1} ( sum_{j1} z[j1 M2 + j2] W_M1^{j1 k1} ) W_M2^{j2 k2}
+//
+//   K0  k_delay_segments  exact (value, slope) knots of the delay every h samples -> one cubic
+//                         Hermite record per segment (fp64 + an fp32 copy with a safety margin)
+//   P1  k_fft_cols        per CTA a bundle of C columns j2: gathers z straight from the series
+//                         (the resampled series is never written), M1-point FFTs in shared
+//                         memory, times W_M^{j2 k1}, writes T[k1][j2]            (4N bytes out)
+//   P2  k_fft_rows        per CTA R rows k1: M2-point FFTs, writes Z[k1 + M1 k2] (4N in, 4N out)
+//   the R2C unpack X_k = E_k + W_N^k O_k is fused into the spectrum former (tb_kernels.cuh).
+//
+// In-CTA FFT of length L = R1*256 (R1 in {1,2,4,8}): three in-place steps over a 3-D view
+// [a < R1][b < 16][c < 16] of the data, physical index a*272 + b*17 + c (pitch 17 on the unit
+// stride axis makes all three access patterns bank-conflict free for 64-bit elements):
+//   step 1 over a (radix R1, fused with the global load), twiddle W_L^{(16b+c) ka}
+//   step 2 over b (radix 16),                              twiddle W_256^{c kb}
+//   step 3 over c (radix 16, fused with the global store); output k = ka + R1 kb + 16 R1 kc.
+#pragma once
+#include "tb_kernels.cuh"
+
+namespace tb {
+
+constexpr int FFT_PB = 17;            // pitch of the b axis (16 + 1)
+constexpr int FFT_PA = 16 * FFT_PB;   // pitch of the a axis
+constexpr int FFT_THREADS = 256;
+
+struct SegRec {                       // one Hermite segment of the delay, 64 bytes
+    float  f0, f1, f2, f3;            // fp32 cubic in t in [0,1): delta - i0 = f0 + t(f1 + t(f2 + t f3))
+    int    i0;                        // nearest integer to the segment's first delta
+    float  eps;                       // |rounding residual| beyond 0.5 - eps -> decide in fp64
+    int    pad0, pad1;
+    double d0, d1, d2, d3;            // fp64 cubic of delta + 1/2 (the k_resample coefficients)
+};
+static_assert(sizeof(SegRec) == 64, "segment record");
+
+__device__ __forceinline__ float2 cmul(float2 a, float2 w) { return make_float2(a.x * w.x - a.y * w.y, a.x * w.y + a.y * w.x); }
+__device__ __forceinline__ float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
+__device__ __forceinline__ float2 csub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
+__device__ __forceinline__ float2 mul_mi(float2 a) { return make_float2(a.y, -a.x); }   // a * (-i)
+
+// forward 4-point DFT of (x0,x1,x2,x3), natural order in and out
+__device__ __forceinline__ void fft4(float2& x0, float2& x1, float2& x2, float2& x3)
+{
+    const float2 t0 = cadd(x0, x2), t1 = csub(x0, x2), t2 = cadd(x1, x3), t3 = mul_mi(csub(x1, x3));
+    x0 = cadd(t0, t2); x2 = csub(t0, t2); x1 = cadd(t1, t3); x3 = csub(t1, t3);
+}
+
+template <int R> __device__ __forceinline__ void fft_reg(float2 (&v)[R]);
+
+template <> __device__ __forceinline__ void fft_reg<1>(float2 (&)[1]) {}
+template <> __device__ __forceinline__ void fft_reg<2>(float2 (&v)[2])
+{
+    const float2 a = v[0], b = v[1];
+    v[0] = cadd(a, b); v[1] = csub(a, b);
+}
+template <> __device__ __forceinline__ void fft_reg<4>(float2 (&v)[4]) { fft4(v[0], v[1], v[2], v[3]); }
+template <> __device__ __forceinline__ void fft_reg<8>(float2 (&v)[8])
+{
+    // n = 2 n1 + n2, k = k1 + 4 k2: 4-point over n1, twiddle W8^{n2 k1}, 2-point over n2
+    constexpr float H = 0.70710678118654752440f;
+    fft4(v[0], v[2], v[4], v[6]);                 // n2 = 0 -> A[k1][0] in v[0],v[2],v[4],v[6]
+    fft4(v[1], v[3], v[5], v[7]);                 // n2 = 1 -> A[k1][1] in v[1],v[3],v[5],v[7]
+    v[3] = cmul(v[3], make_float2(H, -H));        // W8^1
+    v[5] = mul_mi(v[5]);                          // W8^2
+    v[7] = cmul(v[7], make_float2(-H, -H));       // W8^3
+    float2 o[8];
+#pragma unroll
+    for (int k1 = 0; k1 < 4; ++k1) {
+        o[k1]     = cadd(v[2 * k1], v[2 * k1 + 1]);
+        o[k1 + 4] = csub(v[2 * k1], v[2 * k1 + 1]);
+    }
+#pragma unroll
+    for (int i = 0; i < 8; ++i) v[i] = o[i];
+}
+template <> __device__ __forceinline__ void fft_reg<16>(float2 (&v)[16])
+{
+    // n = 4 n1 + n2, k = k1 + 4 k2: 4-point over n1, twiddle W16^{n2 k1}, 4-point over n2
+    constexpr float C1 = 0.92387953251128675613f, S1 = 0.38268343236508977173f, H = 0.70710678118654752440f;
+#pragma unroll
+    for (int n2 = 0; n2 < 4; ++n2) fft4(v[n2], v[4 + n2], v[8 + n2], v[12 + n2]);   // A[k1][n2] at v[4 k1 + n2]
+    v[5]  = cmul(v[5],  make_float2(C1, -S1));    // k1=1,n2=1: W16^1
+    v[6]  = cmul(v[6],  make_float2(H, -H));      // W16^2
+    v[7]  = cmul(v[7],  make_float2(S1, -C1));    // W16^3
+    v[9]  = cmul(v[9],  make_float2(H, -H));      // k1=2,n2=1: W16^2
+    v[10] = mul_mi(v[10]);                        // W16^4
+    v[11] = cmul(v[11], make_float2(-H, -H));     // W16^6
+    v[13] = cmul(v[13], make_float2(S1, -C1));    // k1=3,n2=1: W16^3
+    v[14] = cmul(v[14], make_float2(-H, -H));     // W16^6
+    v[15] = cmul(v[15], make_float2(-C1, S1));    // W16^9
+    float2 o[16];
+#pragma unroll
+    for (int k1 = 0; k1 < 4; ++k1) {
+        float2 a = v[4 * k1], b = v[4 * k1 + 1], c = v[4 * k1 + 2], d = v[4 * k1 + 3];
+        fft4(a, b, c, d);                         // over n2 -> k2
+        o[k1] = a; o[k1 + 4] = b; o[k1 + 8] = c; o[k1 + 12] = d;
+    }
+#pragma unroll
+    for (int i = 0; i < 16; ++i) v[i] = o[i];
+}
+
+// step 2 of the in-CTA FFT for one slot: work item w in [0, 16 R1): (ka, c) = (w >> 4, w & 15)
+__device__ __forceinline__ void fft_step2(float2* __restrict__ slot, int w, const float2* __restrict__ tw2)
+{
+    const int c = w & 15;
+    float2* p = slot + (w >> 4) * FFT_PA + c;
+    float2 v[16];
+#pragma unroll
+    for (int b = 0; b < 16; ++b) v[b] = p[b * FFT_PB];
+    fft_reg<16>(v);
+#pragma unroll
+    for (int kb = 1; kb < 16; ++kb) v[kb] = cmul(v[kb], tw2[kb * 16 + c]);
+#pragma unroll
+    for (int kb = 0; kb < 16; ++kb) p[kb * FFT_PB] = v[kb];
+}
+
+// ---------------------------------------------------------------------------------------------
+// K0  Hermite segment records of the delay for every template of the chunk.
+//   One CTA = 256 consecutive segments of one template (257 exact knots).  Output record s of
+//   template b at seg[b * seg_stride + s].  Same knots and fp64 coefficients as k_resample.
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256)
+k_delay_segments(const TmplDev* __restrict__ tmpl, int n_tmpl, int n, SegRec* __restrict__ seg, size_t seg_stride,
+                 int cta_per_tmpl)
+{
+    __shared__ double s_val[257], s_slp[257];
+    const int b = blockIdx.x % n_tmpl;
+    const int s0 = (blockIdx.x / n_tmpl) * 256;
+    const TmplDev t = tmpl[b];
+    const int log2h = t.log2h;
+    const int nseg = n >> log2h;
+    if (s0 >= nseg) return;
+    const double h = (double)(1 << log2h);
+    for (int k = threadIdx.x; k <= 256; k += 256) {
+        double v, d;
+        delay_knot(t, (s0 + k) << log2h, v, d);
+        s_val[k] = v; s_slp[k] = d * h;
+    }
+    __syncthreads();
+    const int s = s0 + threadIdx.x;
+    if (s >= nseg) return;
+    const double v0 = s_val[threadIdx.x], v1 = s_val[threadIdx.x + 1], g0 = s_slp[threadIdx.x], g1 = s_slp[threadIdx.x + 1];
+    const double dv = v1 - v0;
+    SegRec r;
+    r.d0 = v0 + 0.5; r.d1 = g0; r.d2 = 3.0 * dv - (2.0 * g0 + g1); r.d3 = (g0 + g1) - 2.0 * dv;
+    const double i0 = rint(v0);
+    r.i0 = (int)i0;
+    r.f0 = (float)(v0 - i0); r.f1 = (float)r.d1; r.f2 = (float)r.d2; r.f3 = (float)r.d3;
+    r.eps = (float)((fabs(r.d1) + fabs(r.d2) + fabs(r.d3) + 2.0) * 1e-6);
+    r.pad0 = 0; r.pad1 = 0;
+    seg[(size_t)b * seg_stride + s] = r;
+}
+
+// source index of output sample nn (a3): fp32 cubic, re-decided in fp64 within eps of a tie
+__device__ __forceinline__ int source_index(const SegRec* __restrict__ segs, int nn, int log2h, float inv_h)
+{
+    const SegRec* r = segs + (nn >> log2h);
+    const float4 f = __ldg(reinterpret_cast<const float4*>(r));
+    const int2 ie = __ldg(reinterpret_cast<const int2*>(r) + 2);
+    const int o = nn & ((1 << log2h) - 1);
+    const float tt = (float)o * inv_h;
+    const float y = fmaf(fmaf(fmaf(f.w, tt, f.z), tt, f.y), tt, f.x);
+    const float z = y + 12582912.0f;                         // 1.5 * 2^23: round to nearest integer
+    int s = __float_as_int(z) - 0x4B400000;
+    const float res = y - (z - 12582912.0f);
+    if (fabsf(res) > 0.5f - __int_as_float(ie.y)) {          // too close to a tie for fp32: fp64 decision
+        const double2 c01 = __ldg(reinterpret_cast<const double2*>(r) + 2);
+        const double2 c23 = __ldg(reinterpret_cast<const double2*>(r) + 3);
+        const double td = (double)o * (double)inv_h;
+        s = floor_to_int(fma(fma(fma(c23.y, td, c23.x), td, c01.y), td, c01.x)) - ie.x;
+    }
+    return nn - (ie.x + s);
+}
+
+// ---------------------------------------------------------------------------------------------
+// P1  gather + column FFTs.  CTA = C columns [c0, c0+C) of template b, all M1 = R1*256 rows.
+//   blockIdx.x = bundle * n_tmpl + b (template fastest: co-resident CTAs gather from the same
+//   stretch of the series, which stays in L2).
+// ---------------------------------------------------------------------------------------------
+template <int R1, int C, bool DEBUG>
+__global__ void __launch_bounds__(FFT_THREADS)
+k_fft_cols(const float* __restrict__ x, const SegRec* __restrict__ seg, size_t seg_stride,
+           const TmplDev* __restrict__ tmpl, int n_tmpl, int n, int log2m2, float fill,
+           const float2* __restrict__ tw1, const float2* __restrict__ tw2g, float2* __restrict__ T,
+           long long* __restrict__ idx_out, float* __restrict__ y_out)
+{
+    constexpr int L = R1 * 256;                    // M1
+    constexpr int LP = R1 * FFT_PA + 16 / C;       // slot pitch: 16/C mod 16 keeps the column-fastest accesses conflict free
+    extern __shared__ __align__(16) float2 fsm[];
+    float2* tw2 = fsm + C * LP;
+    const int b  = blockIdx.x % n_tmpl;
+    const int c0 = (blockIdx.x / n_tmpl) * C;
+    const int m2 = 1 << log2m2;
+    const size_t m = (size_t)L << log2m2;          // M
+    const int log2h = tmpl[b].log2h;
+    const float inv_h = 1.0f / (float)(1 << log2h);
+    const SegRec* __restrict__ segs = seg + (size_t)b * seg_stride;
+    float2* __restrict__ Tb = T + (size_t)b * m;
+
+    tw2[threadIdx.x] = __ldg(tw2g + threadIdx.x);
+
+    // phase A: gather, radix-R1 over a, twiddle, to shared memory.  item i: col = i % C, w = i / C
+    for (int i = threadIdx.x; i < 256 * C; i += FFT_THREADS) {
+        const int col = i % C, w = i / C;
+        float2 v[R1];
+#pragma unroll
+        for (int a = 0; a < R1; ++a) {
+            const int j1 = a * 256 + w;
+            const int nn = (int)((((size_t)j1 << log2m2) + c0 + col) << 1);     // first of the two samples
+            const int s0 = source_index(segs, nn, log2h, inv_h);
+            const int s1 = source_index(segs, nn + 1, log2h, inv_h);
+            v[a].x = ((unsigned)s0 < (unsigned)n) ? __ldg(x + s0) : fill;
+            v[a].y = ((unsigned)s1 < (unsigned)n) ? __ldg(x + s1) : fill;
+            if (DEBUG) {
+                idx_out[(size_t)b * n + nn] = s0; idx_out[(size_t)b * n + nn + 1] = s1;
+                y_out[(size_t)b * n + nn] = v[a].x; y_out[(size_t)b * n + nn + 1] = v[a].y;
+            }
+        }
+        fft_reg<R1>(v);
+#pragma unroll
+        for (int ka = 1; ka < R1; ++ka) v[ka] = cmul(v[ka], __ldg(tw1 + ka * 256 + w));
+        float2* p = fsm + col * LP + (w >> 4) * FFT_PB + (w & 15);
+#pragma unroll
+        for (int ka = 0; ka < R1; ++ka) p[ka * FFT_PA] = v[ka];
+    }
+    __syncthreads();
+    // phase B: radix 16 over b
+    for (int i = threadIdx.x; i < 16 * R1 * C; i += FFT_THREADS) fft_step2(fsm + (i / (16 * R1)) * LP, i % (16 * R1), tw2);
+    __syncthreads();
+    // phase C: radix 16 over c, four-step twiddle W_M^{j2 k1}, store T[k1][j2].  item: col fastest
+    for (int i = threadIdx.x; i < 16 * R1 * C; i += FFT_THREADS) {
+        const int col = i % C, w = i / C;          // w = ka*16 + kb
+        const int ka = w >> 4, kb = w & 15;
+        const float2* p = fsm + col * LP + ka * FFT_PA + kb * FFT_PB;
+        float2 v[16];
+#pragma unroll
+        for (int c = 0; c < 16; ++c) v[c] = p[c];
+        fft_reg<16>(v);
+        const int j2 = c0 + col;
+        const int kbase = ka + R1 * kb;            // k1 = kbase + 16 R1 kc
+        // W_M^{j2 k1} = W_M^{j2 kbase} * g^kc, g = W_M^{16 R1 j2}; both arguments are exact in fp32
+        const float inv_m = 1.0f / (float)m;
+        float sb, cb, sg, cg;
+        sincospif(-2.0f * (float)(j2 * kbase) * inv_m, &sb, &cb);
+        sincospif(-2.0f * (float)(j2 * 16 * R1) * inv_m, &sg, &cg);
+        const float2 g1 = make_float2(cg, sg);
+        const float2 g2 = cmul(g1, g1), g4 = cmul(g2, g2), g8 = cmul(g4, g4);
+        float2 pw[16];
+        pw[0] = make_float2(cb, sb);
+        pw[1] = cmul(pw[0], g1);
+        pw[2] = cmul(pw[0], g2); pw[3] = cmul(pw[1], g2);
+#pragma unroll
+        for (int q = 0; q < 4; ++q) pw[4 + q] = cmul(pw[q], g4);
+#pragma unroll
+        for (int q = 0; q < 8; ++q) pw[8 + q] = cmul(pw[q], g8);
+        float2* out = Tb + ((size_t)kbase << log2m2) + j2;
+        const size_t kstep = (size_t)(16 * R1) << log2m2;
+#pragma unroll
+        for (int kc = 0; kc < 16; ++kc) out[kc * kstep] = cmul(v[kc], pw[kc]);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// P2  row FFTs.  CTA = R rows [k1, k1+R) of template b, row length M2 = R1*256; output
+//   Z[(k1 + r) + M1 k2] (runs of R consecutive elements).  blockIdx.x = b * (M1/R) + row group.
+// ---------------------------------------------------------------------------------------------
+template <int R1, int R>
+__global__ void __launch_bounds__(FFT_THREADS)
+k_fft_rows(const float2* __restrict__ T, float2* __restrict__ Z, int log2m1, const float2* __restrict__ tw1,
+           const float2* __restrict__ tw2g)
+{
+    constexpr int L = R1 * 256;                    // M2
+    constexpr int LP = R1 * FFT_PA + 16 / R;       // slot pitch: 16/R mod 16 keeps the row-fastest accesses conflict free
+    extern __shared__ __align__(16) float2 fsm[];
+    float2* tw2 = fsm + R * LP;
+    const int groups = (1 << log2m1) / R;
+    const int b  = blockIdx.x / groups;
+    const int k1 = (blockIdx.x % groups) * R;
+    const size_t m = (size_t)L << log2m1;
+    const float2* __restrict__ Tb = T + (size_t)b * m + (size_t)k1 * L;
+    float2* __restrict__ Zb = Z + (size_t)b * m + k1;
+
+    tw2[threadIdx.x] = __ldg(tw2g + threadIdx.x);
+
+    for (int i = threadIdx.x; i < 256 * R; i += FFT_THREADS) {      // phase A: item (r, w), w fastest
+        const int r = i >> 8, w = i & 255;
+        float2 v[R1];
+#pragma unroll
+        for (int a = 0; a < R1; ++a) v[a] = __ldg(Tb + (size_t)r * L + a * 256 + w);
+        fft_reg<R1>(v);
+#pragma unroll
+        for (int ka = 1; ka < R1; ++ka) v[ka] = cmul(v[ka], __ldg(tw1 + ka * 256 + w));
+        float2* p = fsm + r * LP + (w >> 4) * FFT_PB + (w & 15);
+#pragma unroll
+        for (int ka = 0; ka < R1; ++ka) p[ka * FFT_PA] = v[ka];
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i < 16 * R1 * R; i += FFT_THREADS) fft_step2(fsm + (i / (16 * R1)) * LP, i % (16 * R1), tw2);
+    __syncthreads();
+    for (int i = threadIdx.x; i < 16 * R1 * R; i += FFT_THREADS) {  // phase C: item (w, r), r fastest
+        const int r = i % R, w = i / R;
+        const int ka = w >> 4, kb = w & 15;
+        const float2* p = fsm + r * LP + ka * FFT_PA + kb * FFT_PB;
+        float2 v[16];
+#pragma unroll
+        for (int c = 0; c < 16; ++c) v[c] = p[c];
+        fft_reg<16>(v);
+        float2* out = Zb + (((size_t)(ka + R1 * kb)) << log2m1) + r;
+        const size_t kstep = (size_t)(16 * R1) << log2m1;
+#pragma unroll
+        for (int kc = 0; kc < 16; ++kc) out[kc * kstep] = v[kc];
+    }
+}
+
+}  // namespace tb

@@ -203,10 +203,21 @@ k_resample(const float* __restrict__ x, float* __restrict__ y, const TmplDev* __
 //   floats with warp-wide counts (REDUX) -- no shared memory, no block barrier.
 //   ld = row stride of the cuFFT output in complex elements (even: rows are 16-byte aligned).
 // ---------------------------------------------------------------------------------------------
-template <int W>
+//   UNPACK = true: the input is Z, the length-N/2 complex FFT of z_j = y_2j + i y_2j+1 (row
+//   stride ld = N/2), and the real-series spectrum is formed on the fly,
+//       X_k = E_k + W_N^k O_k,  E = (Z_k + conj Z_{M-k})/2,  O = -i (Z_k - conj Z_{M-k})/2,
+//   with W_N^k = W_N^{block start} (one fp64 sincospi per warp) * twn[k - block start] (table).
+__device__ __forceinline__ float2 r2c_unpack(float2 zk, float2 zm, float2 w)
+{
+    const float er = 0.5f * (zk.x + zm.x), ei = 0.5f * (zk.y - zm.y);
+    const float orr = 0.5f * (zk.y + zm.y), oi = -0.5f * (zk.x - zm.x);
+    return make_float2(er + (w.x * orr - w.y * oi), ei + (w.x * oi + w.y * orr));
+}
+
+template <int W, bool UNPACK>
 __global__ void __launch_bounds__(SP_WARPS * 32)
 k_spectrum_median(const float2* __restrict__ X, size_t ld, float* __restrict__ P, float* __restrict__ med,
-                  int nb, int nblk_per_row, int cta_per_row)
+                  int nb, int nblk_per_row, int cta_per_row, const float2* __restrict__ twn)
 {
     constexpr int VPT  = W / 32;        // powers per lane
     constexpr int ITER = W / 128;       // 4 consecutive bins per lane per iteration
@@ -221,12 +232,34 @@ k_spectrum_median(const float2* __restrict__ X, size_t ld, float* __restrict__ P
 
     float p[VPT];
     float2 carry = make_float2(0.f, 0.f);                // X_{k-1} for lane 0 (X_{-1} = 0)
-    if (base > 0 && lane == 0) carry = __ldg(Xr + base - 1);
+    float2 wbase = make_float2(1.f, 0.f);
+    if (UNPACK) {
+        double sb, cb;
+        sincospi(-(double)base / (double)nb, &sb, &cb);  // W_N^base, N = 2 nb
+        wbase = make_float2((float)cb, (float)sb);
+        if (base > 0 && lane == 0) {
+            double s1, c1;
+            sincospi(-(double)(base - 1) / (double)nb, &s1, &c1);
+            carry = r2c_unpack(__ldg(Xr + base - 1), __ldg(Xr + (nb - base + 1)), make_float2((float)c1, (float)s1));
+        }
+    } else if (base > 0 && lane == 0) carry = __ldg(Xr + base - 1);
 #pragma unroll
     for (int i = 0; i < ITER; ++i) {
         const int k0 = base + i * 128 + lane * 4;
         float4 a = __ldg(reinterpret_cast<const float4*>(Xr + k0));
         float4 c = __ldg(reinterpret_cast<const float4*>(Xr + k0 + 2));
+        if (UNPACK) {
+            const float2* zm = Xr + (nb - k0);           // Z_{M-k0}; bins k0+q mirror at zm[-q]
+            const float2 m0 = __ldg(k0 == 0 ? Xr : zm), m1 = __ldg(zm - 1), m2 = __ldg(zm - 2), m3 = __ldg(zm - 3);
+            const float4 t01 = __ldg(reinterpret_cast<const float4*>(twn + (k0 - base)));
+            const float4 t23 = __ldg(reinterpret_cast<const float4*>(twn + (k0 - base) + 2));
+            const float2 x0 = r2c_unpack(make_float2(a.x, a.y), m0, make_float2(wbase.x * t01.x - wbase.y * t01.y, wbase.x * t01.y + wbase.y * t01.x));
+            const float2 x1 = r2c_unpack(make_float2(a.z, a.w), m1, make_float2(wbase.x * t01.z - wbase.y * t01.w, wbase.x * t01.w + wbase.y * t01.z));
+            const float2 x2 = r2c_unpack(make_float2(c.x, c.y), m2, make_float2(wbase.x * t23.x - wbase.y * t23.y, wbase.x * t23.y + wbase.y * t23.x));
+            const float2 x3 = r2c_unpack(make_float2(c.z, c.w), m3, make_float2(wbase.x * t23.z - wbase.y * t23.w, wbase.x * t23.w + wbase.y * t23.z));
+            a = make_float4(x0.x, x0.y, x1.x, x1.y);
+            c = make_float4(x2.x, x2.y, x3.x, x3.y);
+        }
         if (k0 == 0) { a.x = 0.f; a.y = 0.f; }           // X_0 <- 0 before differencing (G13)
         float px = __shfl_up_sync(0xffffffffu, c.z, 1);
         float py = __shfl_up_sync(0xffffffffu, c.w, 1);

@@ -32,7 +32,7 @@ class PlanOpts(C.Structure):
     _fields_ = [("struct_size", C.c_uint32), ("device", C.c_int32), ("stream", C.c_void_p),
                 ("median_window", C.c_uint32), ("f_min_hz", C.c_double), ("max_candidates", C.c_uint64),
                 ("chunk_templates", C.c_uint32), ("series_is_device_ptr", C.c_int32), ("has_fill", C.c_int32),
-                ("fill_value", C.c_float), ("enable_timings", C.c_int32), ("reserved", C.c_int32)]
+                ("fill_value", C.c_float), ("enable_timings", C.c_int32), ("fft_path", C.c_int32)]
 
 
 class Timings(C.Structure):
@@ -96,7 +96,7 @@ def as_templates(templates) -> np.ndarray:
 
 def tb_plan_create(series, n_samples, tsamp_s, *, device=0, stream=None, median_window=0, f_min_hz=0.0,
                    max_candidates=0, chunk_templates=0, series_is_device_ptr=False, fill_value=None,
-                   enable_timings=False):
+                   enable_timings=False, fft_path=0):
     """series: numpy float32[N] (host) or an integer device address when series_is_device_ptr."""
     o = PlanOpts()
     o.struct_size = C.sizeof(PlanOpts)
@@ -105,6 +105,7 @@ def tb_plan_create(series, n_samples, tsamp_s, *, device=0, stream=None, median_
     o.chunk_templates, o.series_is_device_ptr = int(chunk_templates), int(bool(series_is_device_ptr))
     o.has_fill, o.fill_value = (0, 0.0) if fill_value is None else (1, float(fill_value))
     o.enable_timings = int(bool(enable_timings))
+    o.fft_path = int(fft_path)
     if series_is_device_ptr:
         ptr = int(series)
     else:
