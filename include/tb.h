@@ -106,6 +106,7 @@ typedef struct {
     uint64_t n_templates, n_samples, n_chunks, chunk_templates;
     uint64_t model_bytes_per_template;   /* 22*N: algorithmic HBM bytes */
     uint64_t n_kernel_launches;          /* libtb's own kernels launched by that call (cuFFT's not counted) */
+    uint64_t n_median_fallbacks;         /* median blocks that took the data-independent bisection path */
 } tb_timings;
 
 /* Create a plan for one dedispersed time series S[i], i*tsamp.

@@ -41,7 +41,7 @@ struct tb_plan {
     uint64_t max_cand = 0;
     uint32_t chunk = 0;
     bool timings = false;
-    bool user_fill = false, borrowed = false;
+    bool user_fill = false, borrowed = false, l2_pinned = false;
     float fill = 0.f;
     size_t ld = 0;                                   // complex row stride of the FFT output
 
@@ -204,6 +204,25 @@ int load_series(tb_plan* p, const float* series)
     return TB_OK;
 }
 
+// Keep the series resident in L2 (persisting access-policy window on the plan's stream): every
+// template gathers from the same 4N bytes while tens of GB of scratch stream through the cache.
+void pin_series_in_l2(tb_plan* p)
+{
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, p->device) != cudaSuccess || prop.persistingL2CacheMaxSize <= 0) return;
+    const size_t bytes = std::min<size_t>(p->n * sizeof(float), (size_t)prop.accessPolicyMaxWindowSize);
+    cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, std::min<size_t>(bytes, (size_t)prop.persistingL2CacheMaxSize));
+    cudaStreamAttrValue attr;
+    std::memset(&attr, 0, sizeof(attr));
+    attr.accessPolicyWindow.base_ptr = const_cast<float*>(p->d_series);
+    attr.accessPolicyWindow.num_bytes = bytes;
+    attr.accessPolicyWindow.hitRatio = std::min(1.0f, (float)prop.persistingL2CacheMaxSize / (float)bytes);
+    attr.accessPolicyWindow.hitProp = cudaAccessPropertyPersisting;
+    attr.accessPolicyWindow.missProp = cudaAccessPropertyStreaming;
+    if (cudaStreamSetAttribute(p->stream, cudaStreamAttributeAccessPolicyWindow, &attr) == cudaSuccess) p->l2_pinned = true;
+    cudaGetLastError();
+}
+
 int get_fft_plan(tb_plan* p, uint32_t batch, cufftHandle* out)
 {
     auto it = p->fft_plans.find(batch);
@@ -248,10 +267,10 @@ void launch_spectrum(tb_plan* p, uint32_t nt, bool unpack)
     const int cta_per_row = (int)((p->nblk + SP_WARPS - 1) / SP_WARPS);
     if (unpack)
         k_spectrum_median<W, true><<<(unsigned)(cta_per_row * nt), SP_WARPS * 32, 0, p->stream>>>(
-            p->d_fft, (size_t)p->nb, p->d_power, p->d_med, (int)p->nb, (int)p->nblk, cta_per_row, p->d_twn);
+            p->d_fft, (size_t)p->nb, p->d_power, p->d_med, (int)p->nb, (int)p->nblk, cta_per_row, p->d_twn, p->d_cursor + 1);
     else
         k_spectrum_median<W, false><<<(unsigned)(cta_per_row * nt), SP_WARPS * 32, 0, p->stream>>>(
-            p->d_fft, p->ld, p->d_power, p->d_med, (int)p->nb, (int)p->nblk, cta_per_row, nullptr);
+            p->d_fft, p->ld, p->d_power, p->d_med, (int)p->nb, (int)p->nblk, cta_per_row, nullptr, p->d_cursor + 1);
 }
 
 // ---- hand-written FFT path -------------------------------------------------------------------
@@ -483,6 +502,12 @@ void destroy(tb_plan* p)
     if (!p) return;
     cudaSetDevice(p->device);
     if (p->stream) cudaStreamSynchronize(p->stream);
+    if (p->l2_pinned) {
+        cudaStreamAttrValue attr;
+        std::memset(&attr, 0, sizeof(attr));
+        cudaStreamSetAttribute(p->stream, cudaStreamAttributeAccessPolicyWindow, &attr);
+        cudaCtxResetPersistingL2Cache();
+    }
     for (auto& kv : p->fft_plans) cufftDestroy(kv.second);
     for (auto& es : p->events) for (auto& e : es.e) cudaEventDestroy(e);
     if (p->ev_staged) cudaEventDestroy(p->ev_staged);
@@ -594,6 +619,7 @@ int tb_plan_create(tb_plan** out, const float* series, uint64_t n_samples, doubl
     p->user_fill = o.has_fill != 0;
     p->fill = o.fill_value;
     { int rc = load_series(p, series); if (rc) { destroy(p); return rc; } }
+    pin_series_in_l2(p);
 
     // FFT path: hand-written two-pass FFT for 2^17 <= N <= 2^23, batched cuFFT otherwise
     {
@@ -615,8 +641,8 @@ int tb_plan_create(tb_plan** out, const float* series, uint64_t n_samples, doubl
     TB_TRY(cudaMalloc(&p->d_power, (size_t)B * p->nb * sizeof(float)));
     TB_TRY(cudaMalloc(&p->d_med, (size_t)B * p->nblk * sizeof(float)));
     TB_TRY(cudaMalloc(&p->d_cand, p->max_cand * sizeof(Candidate)));
-    TB_TRY(cudaMalloc(&p->d_cursor, sizeof(unsigned long long)));
-    TB_TRY(cudaMemsetAsync(p->d_cursor, 0, sizeof(unsigned long long), p->stream));
+    TB_TRY(cudaMalloc(&p->d_cursor, 2 * sizeof(unsigned long long)));   // [0] candidate cursor, [1] median fallbacks
+    TB_TRY(cudaMemsetAsync(p->d_cursor, 0, 2 * sizeof(unsigned long long), p->stream));
 #undef TB_TRY
     cufftHandle h;
     int rc = get_fft_plan(p, B, &h);
@@ -630,7 +656,9 @@ int tb_plan_set_series(tb_plan* p, const float* series)
 {
     if (!p || !series) return fail(p, TB_ERR_INVALID_ARG, "null argument");
     TB_CUDA(p, cudaSetDevice(p->device));
-    return load_series(p, series);
+    const int rc = load_series(p, series);
+    if (!rc && p->borrowed) pin_series_in_l2(p);
+    return rc;
 }
 
 int tb_plan_destroy(tb_plan* plan)
@@ -676,6 +704,7 @@ int tb_search_templates(tb_plan* p, const tb_template* tmpl, uint64_t n_template
     p->last.chunk_templates = p->chunk;
     p->last.model_bytes_per_template = 22ull * p->n;
     if (n_templates == 0) return TB_OK;
+    TB_CUDA(p, cudaMemsetAsync(p->d_cursor + 1, 0, sizeof(unsigned long long), p->stream));
     rc = upload_templates(p, tmpl, n_templates);
     if (rc) return rc;
 
@@ -721,6 +750,11 @@ int tb_get_timings(tb_plan* p, tb_timings* out)
     TB_CUDA(p, cudaSetDevice(p->device));
     TB_CUDA(p, cudaStreamSynchronize(p->stream));
     tb_timings t = p->last;
+    {
+        unsigned long long fb = 0;
+        TB_CUDA(p, cudaMemcpy(&fb, p->d_cursor + 1, sizeof(fb), cudaMemcpyDeviceToHost));
+        t.n_median_fallbacks = fb;
+    }
     t.ms_resample = t.ms_fft = t.ms_spectrum = t.ms_normalise = t.ms_hsum = t.ms_total = 0.0;
     for (size_t i = 0; i < p->events_used; ++i) {
         float ms[5];

@@ -157,25 +157,31 @@ k_delay_segments(const TmplDev* __restrict__ tmpl, int n_tmpl, int n, SegRec* __
     seg[(size_t)b * seg_stride + s] = r;
 }
 
-// source index of output sample nn (a3): fp32 cubic, re-decided in fp64 within eps of a tie
-__device__ __forceinline__ int source_index(const SegRec* __restrict__ segs, int nn, int log2h, float inv_h)
+// source indices of the output sample pair (nn, nn+1), nn even (a3): fp32 cubic of the segment
+// the pair lies in; a sample whose rounding residual is within eps of a tie is re-decided in
+// fp64 with k_resample's coefficients, so the integer decision is the fp64 one everywhere.
+__device__ __forceinline__ int2 source_pair(const SegRec* __restrict__ segs, int nn, int log2h, float inv_h)
 {
     const SegRec* r = segs + (nn >> log2h);
     const float4 f = __ldg(reinterpret_cast<const float4*>(r));
     const int2 ie = __ldg(reinterpret_cast<const int2*>(r) + 2);
     const int o = nn & ((1 << log2h) - 1);
-    const float tt = (float)o * inv_h;
-    const float y = fmaf(fmaf(fmaf(f.w, tt, f.z), tt, f.y), tt, f.x);
-    const float z = y + 12582912.0f;                         // 1.5 * 2^23: round to nearest integer
-    int s = __float_as_int(z) - 0x4B400000;
-    const float res = y - (z - 12582912.0f);
-    if (fabsf(res) > 0.5f - __int_as_float(ie.y)) {          // too close to a tie for fp32: fp64 decision
+    const float t0 = (float)o * inv_h, t1 = t0 + inv_h;
+    const float y0 = fmaf(fmaf(fmaf(f.w, t0, f.z), t0, f.y), t0, f.x);
+    const float y1 = fmaf(fmaf(fmaf(f.w, t1, f.z), t1, f.y), t1, f.x);
+    const float z0 = y0 + 12582912.0f, z1 = y1 + 12582912.0f;      // 1.5 * 2^23: round to nearest integer
+    const int base = nn - ie.x + 0x4B400000;
+    int2 src = make_int2(base - __float_as_int(z0), base + 1 - __float_as_int(z1));
+    const float lim = 0.5f - __int_as_float(ie.y);
+    const bool tie0 = fabsf(y0 - (z0 - 12582912.0f)) > lim, tie1 = fabsf(y1 - (z1 - 12582912.0f)) > lim;
+    if (tie0 || tie1) {                                           // rare (about 2 eps per sample)
         const double2 c01 = __ldg(reinterpret_cast<const double2*>(r) + 2);
         const double2 c23 = __ldg(reinterpret_cast<const double2*>(r) + 3);
-        const double td = (double)o * (double)inv_h;
-        s = floor_to_int(fma(fma(fma(c23.y, td, c23.x), td, c01.y), td, c01.x)) - ie.x;
+        const double ta = (double)o * (double)inv_h, tb = (double)(o + 1) * (double)inv_h;
+        if (tie0) src.x = nn - floor_to_int(fma(fma(fma(c23.y, ta, c23.x), ta, c01.y), ta, c01.x));
+        if (tie1) src.y = nn + 1 - floor_to_int(fma(fma(fma(c23.y, tb, c23.x), tb, c01.y), tb, c01.x));
     }
-    return nn - (ie.x + s);
+    return src;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -184,7 +190,7 @@ __device__ __forceinline__ int source_index(const SegRec* __restrict__ segs, int
 //   stretch of the series, which stays in L2).
 // ---------------------------------------------------------------------------------------------
 template <int R1, int C, bool DEBUG>
-__global__ void __launch_bounds__(FFT_THREADS)
+__global__ void __launch_bounds__(FFT_THREADS, 3)
 k_fft_cols(const float* __restrict__ x, const SegRec* __restrict__ seg, size_t seg_stride,
            const TmplDev* __restrict__ tmpl, int n_tmpl, int n, int log2m2, float fill,
            const float2* __restrict__ tw1, const float2* __restrict__ tw2g, float2* __restrict__ T,
@@ -213,8 +219,8 @@ k_fft_cols(const float* __restrict__ x, const SegRec* __restrict__ seg, size_t s
         for (int a = 0; a < R1; ++a) {
             const int j1 = a * 256 + w;
             const int nn = (int)((((size_t)j1 << log2m2) + c0 + col) << 1);     // first of the two samples
-            const int s0 = source_index(segs, nn, log2h, inv_h);
-            const int s1 = source_index(segs, nn + 1, log2h, inv_h);
+            const int2 sp = source_pair(segs, nn, log2h, inv_h);
+            const int s0 = sp.x, s1 = sp.y;
             v[a].x = ((unsigned)s0 < (unsigned)n) ? __ldg(x + s0) : fill;
             v[a].y = ((unsigned)s1 < (unsigned)n) ? __ldg(x + s1) : fill;
             if (DEBUG) {
@@ -262,7 +268,7 @@ k_fft_cols(const float* __restrict__ x, const SegRec* __restrict__ seg, size_t s
         float2* out = Tb + ((size_t)kbase << log2m2) + j2;
         const size_t kstep = (size_t)(16 * R1) << log2m2;
 #pragma unroll
-        for (int kc = 0; kc < 16; ++kc) out[kc * kstep] = cmul(v[kc], pw[kc]);
+        for (int kc = 0; kc < 16; ++kc) __stcs(out + kc * kstep, cmul(v[kc], pw[kc]));   // streamed: read once by pass 2
     }
 }
 
@@ -271,7 +277,7 @@ k_fft_cols(const float* __restrict__ x, const SegRec* __restrict__ seg, size_t s
 //   Z[(k1 + r) + M1 k2] (runs of R consecutive elements).  blockIdx.x = b * (M1/R) + row group.
 // ---------------------------------------------------------------------------------------------
 template <int R1, int R>
-__global__ void __launch_bounds__(FFT_THREADS)
+__global__ void __launch_bounds__(FFT_THREADS, 3)
 k_fft_rows(const float2* __restrict__ T, float2* __restrict__ Z, int log2m1, const float2* __restrict__ tw1,
            const float2* __restrict__ tw2g)
 {
@@ -292,7 +298,7 @@ k_fft_rows(const float2* __restrict__ T, float2* __restrict__ Z, int log2m1, con
         const int r = i >> 8, w = i & 255;
         float2 v[R1];
 #pragma unroll
-        for (int a = 0; a < R1; ++a) v[a] = __ldg(Tb + (size_t)r * L + a * 256 + w);
+        for (int a = 0; a < R1; ++a) v[a] = __ldcs(Tb + (size_t)r * L + a * 256 + w);
         fft_reg<R1>(v);
 #pragma unroll
         for (int ka = 1; ka < R1; ++ka) v[ka] = cmul(v[ka], __ldg(tw1 + ka * 256 + w));
@@ -314,7 +320,7 @@ k_fft_rows(const float2* __restrict__ T, float2* __restrict__ Z, int log2m1, con
         float2* out = Zb + (((size_t)(ka + R1 * kb)) << log2m1) + r;
         const size_t kstep = (size_t)(16 * R1) << log2m1;
 #pragma unroll
-        for (int kc = 0; kc < 16; ++kc) out[kc * kstep] = v[kc];
+        for (int kc = 0; kc < 16; ++kc) __stcs(out + kc * kstep, v[kc]);
     }
 }
 

@@ -217,7 +217,8 @@ __device__ __forceinline__ float2 r2c_unpack(float2 zk, float2 zm, float2 w)
 template <int W, bool UNPACK>
 __global__ void __launch_bounds__(SP_WARPS * 32)
 k_spectrum_median(const float2* __restrict__ X, size_t ld, float* __restrict__ P, float* __restrict__ med,
-                  int nb, int nblk_per_row, int cta_per_row, const float2* __restrict__ twn)
+                  int nb, int nblk_per_row, int cta_per_row, const float2* __restrict__ twn,
+                  unsigned long long* __restrict__ fallbacks)
 {
     constexpr int VPT  = W / 32;        // powers per lane
     constexpr int ITER = W / 128;       // 4 consecutive bins per lane per iteration
@@ -277,30 +278,85 @@ k_spectrum_median(const float2* __restrict__ X, size_t ld, float* __restrict__ P
         p[4 * i + 0] = o.x; p[4 * i + 1] = o.y; p[4 * i + 2] = o.z; p[4 * i + 3] = o.w;
     }
 
-    // exact order statistics W/2-1 and W/2 (0-based) of the W values held by the warp
-    uint32_t key[VPT];
-#pragma unroll
-    for (int v = 0; v < VPT; ++v) key[v] = __float_as_uint(p[v]);
+    // Exact order statistics W/2-1 and W/2 (0-based) of the W values held by the warp.
+    // Fast path: the median of noise-like powers sits near 0.78 x the block mean, so count the
+    // values below lo = 0.66 mean, compact those in [lo, hi = 0.90 mean) (ballot + popc prefix
+    // into a per-warp shared list, about 13 % of the block) and select among them; if the two
+    // middle ranks are not both inside the bracket (or it overflows) fall back to the
+    // data-independent bisection over all W values.  Both paths are exact.
     constexpr int K1 = W / 2 - 1;
-    uint32_t prefix = 0;
-    for (int bit = 30; bit >= 0; --bit) {
-        const uint32_t cand = prefix | (1u << bit);
-        int c = 0;
+    constexpr int CAP = (W >= 512) ? W / 4 : W;          // candidate list capacity
+    constexpr int CPL = CAP / 32;                        // candidates per lane
+    __shared__ float s_cand[SP_WARPS][CAP];
+    float* cand = s_cand[threadIdx.x >> 5];
+    float sum = 0.f;
 #pragma unroll
-        for (int v = 0; v < VPT; ++v) c += (key[v] < cand) ? 1 : 0;
-        c = __reduce_add_sync(0xffffffffu, c);
-        if (c <= K1) prefix = cand;                      // the K1-th smallest is >= cand
-    }
-    int le = 0;
-    uint32_t nxt = 0xffffffffu;
+    for (int v = 0; v < VPT; ++v) sum += p[v];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
+    const float lo = sum * (0.66f / (float)W), hi = sum * (0.90f / (float)W);
+    const unsigned lt_mask = (1u << lane) - 1u;
+    int below = 0, nmid = 0;
 #pragma unroll
     for (int v = 0; v < VPT; ++v) {
-        le += (key[v] <= prefix) ? 1 : 0;
-        if (key[v] > prefix) nxt = min(nxt, key[v]);
+        const bool isb = p[v] < lo;
+        const bool ism = !isb && p[v] < hi;
+        below += isb ? 1 : 0;
+        const unsigned mm = __ballot_sync(0xffffffffu, ism);
+        const int pos = nmid + __popc(mm & lt_mask);
+        if (ism && pos < CAP) cand[pos] = p[v];
+        nmid += __popc(mm);
     }
-    le  = __reduce_add_sync(0xffffffffu, le);
-    nxt = __reduce_min_sync(0xffffffffu, nxt);
-    const uint32_t upper = (le >= W / 2 + 1) ? prefix : nxt;
+    below = __reduce_add_sync(0xffffffffu, below);
+    uint32_t prefix = 0, upper;
+    if (below <= K1 && below + nmid >= K1 + 2 && nmid <= CAP) {
+        __syncwarp();
+        uint32_t ck[CPL];
+#pragma unroll
+        for (int q = 0; q < CPL; ++q) ck[q] = (q * 32 + lane < nmid) ? __float_as_uint(cand[q * 32 + lane]) : 0xffffffffu;
+        const int r1 = K1 - below;                       // rank among the candidates
+        for (int bit = 30; bit >= 0; --bit) {
+            const uint32_t cnd = prefix | (1u << bit);
+            int c = 0;
+#pragma unroll
+            for (int q = 0; q < CPL; ++q) c += (ck[q] < cnd) ? 1 : 0;
+            c = __reduce_add_sync(0xffffffffu, c);
+            if (c <= r1) prefix = cnd;
+        }
+        int le = 0;
+        uint32_t nxt = 0xffffffffu;
+#pragma unroll
+        for (int q = 0; q < CPL; ++q) {
+            le += (ck[q] <= prefix) ? 1 : 0;
+            if (ck[q] > prefix) nxt = min(nxt, ck[q]);
+        }
+        le  = __reduce_add_sync(0xffffffffu, le);
+        nxt = __reduce_min_sync(0xffffffffu, nxt);
+        upper = (le >= r1 + 2) ? prefix : nxt;
+    } else {
+        if (lane == 0 && fallbacks) atomicAdd(fallbacks, 1ull);
+        uint32_t key[VPT];
+#pragma unroll
+        for (int v = 0; v < VPT; ++v) key[v] = __float_as_uint(p[v]);
+        for (int bit = 30; bit >= 0; --bit) {
+            const uint32_t cnd = prefix | (1u << bit);
+            int c = 0;
+#pragma unroll
+            for (int v = 0; v < VPT; ++v) c += (key[v] < cnd) ? 1 : 0;
+            c = __reduce_add_sync(0xffffffffu, c);
+            if (c <= K1) prefix = cnd;                   // the K1-th smallest is >= cnd
+        }
+        int le = 0;
+        uint32_t nxt = 0xffffffffu;
+#pragma unroll
+        for (int v = 0; v < VPT; ++v) {
+            le += (key[v] <= prefix) ? 1 : 0;
+            if (key[v] > prefix) nxt = min(nxt, key[v]);
+        }
+        le  = __reduce_add_sync(0xffffffffu, le);
+        nxt = __reduce_min_sync(0xffffffffu, nxt);
+        upper = (le >= W / 2 + 1) ? prefix : nxt;
+    }
     if (lane == 0) med[(size_t)row * nblk_per_row + blk] = 0.5f * (__uint_as_float(prefix) + __uint_as_float(upper));
 }
 
