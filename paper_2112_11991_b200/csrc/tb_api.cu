@@ -61,7 +61,8 @@ struct tb_plan {
     bool staged_pending = false;
 
     // hand-written FFT path (tb_fft.cuh): M = N/2 = M1 * M2
-    bool own_fft = false;
+    bool own_fft = false, unfused = false;
+    float2* d_T = nullptr;
     int log2m1 = 0, log2m2 = 0;
     SegRec* d_seg = nullptr;                         // [chunk][n >> MIN_LOG2H]
     size_t seg_stride = 0;
@@ -262,32 +263,49 @@ int get_fft_plan(tb_plan* p, uint32_t batch, cufftHandle* out)
 constexpr int OWN_MIN_LOG2H = 3;                     // the fused path needs >= 2 samples per segment; 8 bounds the table
 
 template <int W>
-void launch_spectrum(tb_plan* p, uint32_t nt, bool unpack)
+void launch_spectrum(tb_plan* p, uint32_t nt, bool unpack, float* d_raw)
 {
     const int cta_per_row = (int)((p->nblk + SP_WARPS - 1) / SP_WARPS);
-    if (unpack)
-        k_spectrum_median<W, true><<<(unsigned)(cta_per_row * nt), SP_WARPS * 32, 0, p->stream>>>(
-            p->d_fft, (size_t)p->nb, p->d_power, p->d_med, (int)p->nb, (int)p->nblk, cta_per_row, p->d_twn, p->d_cursor + 1);
-    else
-        k_spectrum_median<W, false><<<(unsigned)(cta_per_row * nt), SP_WARPS * 32, 0, p->stream>>>(
-            p->d_fft, p->ld, p->d_power, p->d_med, (int)p->nb, (int)p->nblk, cta_per_row, nullptr, p->d_cursor + 1);
+    const unsigned grid = (unsigned)(cta_per_row * nt), threads = (SP_WARPS + 2) * 32;
+    const float2* in = p->d_fft;
+    const size_t ld = unpack ? (size_t)p->nb : p->ld;
+    const float2* tw = unpack ? p->d_twn : nullptr;
+    unsigned long long* fb = p->d_cursor + 1;
+    if (unpack && d_raw)       k_spectrum_median<W, true, true><<<grid, threads, 0, p->stream>>>(in, ld, p->d_power, p->d_med, (int)p->nb, (int)p->nblk, cta_per_row, tw, fb, d_raw);
+    else if (unpack)           k_spectrum_median<W, true, false><<<grid, threads, 0, p->stream>>>(in, ld, p->d_power, p->d_med, (int)p->nb, (int)p->nblk, cta_per_row, tw, fb, nullptr);
+    else if (d_raw)            k_spectrum_median<W, false, true><<<grid, threads, 0, p->stream>>>(in, ld, p->d_power, p->d_med, (int)p->nb, (int)p->nblk, cta_per_row, tw, fb, d_raw);
+    else                       k_spectrum_median<W, false, false><<<grid, threads, 0, p->stream>>>(in, ld, p->d_power, p->d_med, (int)p->nb, (int)p->nblk, cta_per_row, tw, fb, nullptr);
 }
 
 // ---- hand-written FFT path -------------------------------------------------------------------
 template <int R1> constexpr int fft_bundle() { return R1 >= 8 ? 4 : 8; }       // C (pass 1) and R (pass 2)
 template <int R1> constexpr size_t fft_smem() { return (size_t)(fft_bundle<R1>() * (R1 * FFT_PA + 16 / fft_bundle<R1>()) + 256) * sizeof(float2); }
 
+template <int R1>
+int launch_cols_unfused(tb_plan* p, uint32_t nt)
+{
+    constexpr int C = fft_bundle<R1>();
+    auto kern = k_fft_cols<R1, C, false, false>;
+    static bool attr = false;
+    if (!attr) { TB_CUDA(p, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_smem<R1>())); attr = true; }
+    const unsigned grid = (unsigned)(((1u << p->log2m2) / C) * nt);
+    kern<<<grid, FFT_THREADS, fft_smem<R1>(), p->stream>>>(p->d_resampled, nullptr, 0, p->d_tmpl, (int)nt, (int)p->n, p->log2m2,
+                                                          p->fill, p->d_tw1a, p->d_tw2, p->d_T, nullptr, nullptr);
+    TB_CUDA(p, cudaGetLastError());
+    return TB_OK;
+}
+
 template <int R1, bool DEBUG>
 int launch_cols(tb_plan* p, size_t off, uint32_t nt, long long* d_idx, float* d_y)
 {
     constexpr int C = fft_bundle<R1>();
-    auto kern = k_fft_cols<R1, C, DEBUG>;
+    auto kern = k_fft_cols<R1, C, DEBUG, true>;
     static bool attr = false;
     if (!attr) { TB_CUDA(p, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_smem<R1>())); attr = true; }
     const unsigned grid = (unsigned)(((1u << p->log2m2) / C) * nt);
     kern<<<grid, FFT_THREADS, fft_smem<R1>(), p->stream>>>(p->d_series, p->d_seg, p->seg_stride, p->d_tmpl + off, (int)nt,
                                                           (int)p->n, p->log2m2, p->fill, p->d_tw1a, p->d_tw2,
-                                                          reinterpret_cast<float2*>(p->d_resampled), d_idx, d_y);
+                                                          p->unfused ? p->d_T : reinterpret_cast<float2*>(p->d_resampled), d_idx, d_y);
     TB_CUDA(p, cudaGetLastError());
     return TB_OK;
 }
@@ -300,7 +318,7 @@ int launch_rows(tb_plan* p, uint32_t nt)
     static bool attr = false;
     if (!attr) { TB_CUDA(p, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_smem<R1>())); attr = true; }
     const unsigned grid = (unsigned)(((1u << p->log2m1) / R) * nt);
-    kern<<<grid, FFT_THREADS, fft_smem<R1>(), p->stream>>>(reinterpret_cast<const float2*>(p->d_resampled), p->d_fft,
+    kern<<<grid, FFT_THREADS, fft_smem<R1>(), p->stream>>>(p->unfused ? p->d_T : reinterpret_cast<const float2*>(p->d_resampled), p->d_fft,
                                                           p->log2m1, p->d_tw1b, p->d_tw2);
     TB_CUDA(p, cudaGetLastError());
     return TB_OK;
@@ -319,6 +337,17 @@ int run_own_pass1(tb_plan* p, size_t off, uint32_t nt, long long* d_idx, float* 
         case 1: return dbg ? launch_cols<2, true>(p, off, nt, d_idx, d_y) : launch_cols<2, false>(p, off, nt, nullptr, nullptr);
         case 2: return dbg ? launch_cols<4, true>(p, off, nt, d_idx, d_y) : launch_cols<4, false>(p, off, nt, nullptr, nullptr);
         case 3: return dbg ? launch_cols<8, true>(p, off, nt, d_idx, d_y) : launch_cols<8, false>(p, off, nt, nullptr, nullptr);
+    }
+    return fail(p, TB_ERR_INVALID_ARG, "unsupported M1");
+}
+
+int run_unfused_pass1(tb_plan* p, uint32_t nt)
+{
+    switch (p->log2m1 - 8) {
+        case 0: return launch_cols_unfused<1>(p, nt);
+        case 1: return launch_cols_unfused<2>(p, nt);
+        case 2: return launch_cols_unfused<4>(p, nt);
+        case 3: return launch_cols_unfused<8>(p, nt);
     }
     return fail(p, TB_ERR_INVALID_ARG, "unsupported M1");
 }
@@ -394,25 +423,16 @@ int run_fft(tb_plan* p, uint32_t nt)
     return TB_OK;
 }
 
-int run_spectrum(tb_plan* p, uint32_t nt, bool unpack)
+int run_spectrum(tb_plan* p, uint32_t nt, bool unpack, float* d_raw = nullptr)
 {
     switch (p->window) {
-        case 128: launch_spectrum<128>(p, nt, unpack); break;
-        case 256: launch_spectrum<256>(p, nt, unpack); break;
-        case 512: launch_spectrum<512>(p, nt, unpack); break;
-        case 1024: launch_spectrum<1024>(p, nt, unpack); break;
-        case 2048: launch_spectrum<2048>(p, nt, unpack); break;
+        case 128: launch_spectrum<128>(p, nt, unpack, d_raw); break;
+        case 256: launch_spectrum<256>(p, nt, unpack, d_raw); break;
+        case 512: launch_spectrum<512>(p, nt, unpack, d_raw); break;
+        case 1024: launch_spectrum<1024>(p, nt, unpack, d_raw); break;
+        case 2048: launch_spectrum<2048>(p, nt, unpack, d_raw); break;
         default: return fail(p, TB_ERR_INVALID_ARG, "median_window");
     }
-    TB_CUDA(p, cudaGetLastError());
-    return TB_OK;
-}
-
-int run_normalise(tb_plan* p, uint32_t nt)
-{
-    const int cta_per_row = (int)((p->nb + 1023) / 1024);
-    k_normalise<<<(unsigned)(cta_per_row * nt), 256, 0, p->stream>>>(p->d_power, p->d_med, (int)p->nb, (int)p->nblk,
-                                                                     (int)p->log2w, cta_per_row);
     TB_CUDA(p, cudaGetLastError());
     return TB_OK;
 }
@@ -511,7 +531,7 @@ void destroy(tb_plan* p)
     for (auto& kv : p->fft_plans) cufftDestroy(kv.second);
     for (auto& es : p->events) for (auto& e : es.e) cudaEventDestroy(e);
     if (p->ev_staged) cudaEventDestroy(p->ev_staged);
-    cudaFree(p->d_seg); cudaFree(p->d_tw1a); cudaFree(p->d_tw1b); cudaFree(p->d_tw2); cudaFree(p->d_twn);
+    cudaFree(p->d_T); cudaFree(p->d_seg); cudaFree(p->d_tw1a); cudaFree(p->d_tw1b); cudaFree(p->d_tw2); cudaFree(p->d_twn);
     cudaFree(p->d_work); cudaFree(p->d_acc); cudaFree(p->d_series_owned); cudaFree(p->d_resampled); cudaFree(p->d_fft);
     cudaFree(p->d_power); cudaFree(p->d_med); cudaFree(p->d_cand); cudaFree(p->d_cursor); cudaFree(p->d_tmpl);
     if (p->h_tmpl) cudaFreeHost(p->h_tmpl);
@@ -627,14 +647,16 @@ int tb_plan_create(tb_plan** out, const float* series, uint64_t n_samples, doubl
         p->log2m1 = lm / 2;
         p->log2m2 = lm - p->log2m1;
         const bool fits = p->log2m1 >= 8 && p->log2m2 <= 11;
-        if (o.fft_path == 2 && !fits) { destroy(p); return TB_ERR_INVALID_ARG; }
+        if (o.fft_path >= 2 && !fits) { destroy(p); return TB_ERR_INVALID_ARG; }
         p->own_fft = fits && o.fft_path != 1;
+        p->unfused = p->own_fft && o.fft_path == 3;
     }
     if (p->own_fft) {
         p->seg_stride = (size_t)(p->n >> OWN_MIN_LOG2H);
         TB_TRY(cudaMalloc(&p->d_seg, (size_t)B * p->seg_stride * sizeof(SegRec)));
         int rc = make_twiddles(p);
         if (rc) { destroy(p); return rc; }
+        if (p->unfused) TB_TRY(cudaMalloc(&p->d_T, (size_t)B * p->nb * sizeof(float2)));
     }
     TB_TRY(cudaMalloc(&p->d_resampled, (size_t)B * p->n * sizeof(float)));
     TB_TRY(cudaMalloc(&p->d_fft, (size_t)B * p->ld * sizeof(float2)));
@@ -721,7 +743,13 @@ int tb_search_templates(tb_plan* p, const tb_template* tmpl, uint64_t n_template
             es = &p->events[p->events_used++];
             TB_CUDA(p, cudaEventRecord(es->e[0], p->stream));
         }
-        if (own) {                                       // K0 + P1 | P2 | unpack + spectrum + median
+        if (own && p->unfused) {                         // experiment: k_resample | P1 without gather, P2
+            if ((rc = run_resample(p, off, nt, nullptr))) return rc;
+            if (es) TB_CUDA(p, cudaEventRecord(es->e[1], p->stream));
+            if ((rc = run_unfused_pass1(p, nt))) return rc;
+            if ((rc = run_own_pass2(p, nt))) return rc;
+            p->last.n_kernel_launches += 2;
+        } else if (own) {                                // K0 + P1 | P2 | unpack + spectrum + median
             if ((rc = run_own_pass1(p, off, nt, nullptr, nullptr))) return rc;
             if (es) TB_CUDA(p, cudaEventRecord(es->e[1], p->stream));
             if ((rc = run_own_pass2(p, nt))) return rc;
@@ -734,12 +762,11 @@ int tb_search_templates(tb_plan* p, const tb_template* tmpl, uint64_t n_template
         if (es) TB_CUDA(p, cudaEventRecord(es->e[2], p->stream));
         if ((rc = run_spectrum(p, nt, own))) return rc;
         if (es) TB_CUDA(p, cudaEventRecord(es->e[3], p->stream));
-        if ((rc = run_normalise(p, nt))) return rc;
-        if (es) TB_CUDA(p, cudaEventRecord(es->e[4], p->stream));
+        if (es) TB_CUDA(p, cudaEventRecord(es->e[4], p->stream));   // a7 is fused into the spectrum kernel
         if ((rc = run_hsum(p, nt, fp, first_template_id + (uint32_t)off))) return rc;
         if (es) TB_CUDA(p, cudaEventRecord(es->e[5], p->stream));
         p->last.n_chunks++;
-        p->last.n_kernel_launches += 4;
+        p->last.n_kernel_launches += 3;
     }
     return TB_OK;
 }
@@ -866,15 +893,19 @@ int tb_debug_spectrum(tb_plan* p, const tb_template* tmpl, float* p_interbinned,
         if ((rc = run_resample(p, 0, 1, nullptr))) return rc;
         if ((rc = run_fft(p, 1))) return rc;
     }
-    if ((rc = run_spectrum(p, 1, own))) return rc;
-    if (p_interbinned)
-        TB_CUDA(p, cudaMemcpyAsync(p_interbinned, p->d_power, p->nb * sizeof(float), cudaMemcpyDeviceToHost, p->stream));
-    if (medians)
-        TB_CUDA(p, cudaMemcpyAsync(medians, p->d_med, p->nblk * sizeof(float), cudaMemcpyDeviceToHost, p->stream));
-    if ((rc = run_normalise(p, 1))) return rc;
-    if (p_normalised)
-        TB_CUDA(p, cudaMemcpyAsync(p_normalised, p->d_power, p->nb * sizeof(float), cudaMemcpyDeviceToHost, p->stream));
-    TB_CUDA(p, cudaStreamSynchronize(p->stream));
+    float* d_raw = nullptr;
+    TB_CUDA(p, cudaMalloc(&d_raw, p->nb * sizeof(float)));
+    rc = run_spectrum(p, 1, own, d_raw);
+    cudaError_t e = cudaSuccess;
+    if (!rc && p_interbinned) e = cudaMemcpyAsync(p_interbinned, d_raw, p->nb * sizeof(float), cudaMemcpyDeviceToHost, p->stream);
+    if (!rc && e == cudaSuccess && medians)
+        e = cudaMemcpyAsync(medians, p->d_med, p->nblk * sizeof(float), cudaMemcpyDeviceToHost, p->stream);
+    if (!rc && e == cudaSuccess && p_normalised)
+        e = cudaMemcpyAsync(p_normalised, p->d_power, p->nb * sizeof(float), cudaMemcpyDeviceToHost, p->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(p->stream);
+    cudaFree(d_raw);
+    if (rc) return rc;
+    if (e != cudaSuccess) return fail(p, TB_ERR_CUDA, cudaGetErrorString(e));
     return TB_OK;
 }
 

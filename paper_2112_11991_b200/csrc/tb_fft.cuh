@@ -189,7 +189,7 @@ __device__ __forceinline__ int2 source_pair(const SegRec* __restrict__ segs, int
 //   blockIdx.x = bundle * n_tmpl + b (template fastest: co-resident CTAs gather from the same
 //   stretch of the series, which stays in L2).
 // ---------------------------------------------------------------------------------------------
-template <int R1, int C, bool DEBUG>
+template <int R1, int C, bool DEBUG, bool GATHER>
 __global__ void __launch_bounds__(FFT_THREADS, 3)
 k_fft_cols(const float* __restrict__ x, const SegRec* __restrict__ seg, size_t seg_stride,
            const TmplDev* __restrict__ tmpl, int n_tmpl, int n, int log2m2, float fill,
@@ -200,9 +200,11 @@ k_fft_cols(const float* __restrict__ x, const SegRec* __restrict__ seg, size_t s
     constexpr int LP = R1 * FFT_PA + 16 / C;       // slot pitch: 16/C mod 16 keeps the column-fastest accesses conflict free
     extern __shared__ __align__(16) float2 fsm[];
     float2* tw2 = fsm + C * LP;
-    const int b  = blockIdx.x % n_tmpl;
-    const int c0 = (blockIdx.x / n_tmpl) * C;
-    const int m2 = 1 << log2m2;
+    // fused gather: template fastest (co-resident CTAs gather from the same stretch of the series);
+    // plain load: bundle fastest (co-resident CTAs touch adjacent sectors of the same lines)
+    const int nbund = (1 << log2m2) / C;
+    const int b  = GATHER ? blockIdx.x % n_tmpl : blockIdx.x / nbund;
+    const int c0 = (GATHER ? blockIdx.x / n_tmpl : blockIdx.x % nbund) * C;
     const size_t m = (size_t)L << log2m2;          // M
     const int log2h = tmpl[b].log2h;
     const float inv_h = 1.0f / (float)(1 << log2h);
@@ -212,6 +214,28 @@ k_fft_cols(const float* __restrict__ x, const SegRec* __restrict__ seg, size_t s
     tw2[threadIdx.x] = __ldg(tw2g + threadIdx.x);
 
     // phase A: gather, radix-R1 over a, twiddle, to shared memory.  item i: col = i % C, w = i / C
+    if (!GATHER) {
+        // x holds the resampled series of this chunk [n_tmpl][n]; all loads are issued first
+        const float2* __restrict__ yb = reinterpret_cast<const float2*>(x + (size_t)b * n);
+        float2 v[C][R1];
+#pragma unroll
+        for (int it = 0; it < C; ++it) {
+            const int i = it * FFT_THREADS + threadIdx.x;
+            const int col = i % C, w = i / C;
+#pragma unroll
+            for (int a = 0; a < R1; ++a) v[it][a] = __ldcs(yb + (((size_t)(a * 256 + w)) << log2m2) + c0 + col);
+        }
+#pragma unroll
+        for (int it = 0; it < C; ++it) {
+            const int i = it * FFT_THREADS + threadIdx.x;
+            const int col = i % C, w = i / C;
+            fft_reg<R1>(v[it]);
+            float2* p = fsm + col * LP + (w >> 4) * FFT_PB + (w & 15);
+            p[0] = v[it][0];
+#pragma unroll
+            for (int ka = 1; ka < R1; ++ka) p[ka * FFT_PA] = cmul(v[it][ka], __ldg(tw1 + ka * 256 + w));
+        }
+    } else
     for (int i = threadIdx.x; i < 256 * C; i += FFT_THREADS) {
         const int col = i % C, w = i / C;
         float2 v[R1];
@@ -294,17 +318,26 @@ k_fft_rows(const float2* __restrict__ T, float2* __restrict__ Z, int log2m1, con
 
     tw2[threadIdx.x] = __ldg(tw2g + threadIdx.x);
 
-    for (int i = threadIdx.x; i < 256 * R; i += FFT_THREADS) {      // phase A: item (r, w), w fastest
-        const int r = i >> 8, w = i & 255;
-        float2 v[R1];
+    {   // phase A: item (r, w) = (it, threadIdx.x); every global load of the thread is issued before
+        // the first butterfly so that one memory round trip covers the whole tile
+        static_assert(FFT_THREADS == 256, "one work item per thread and row");
+        const int w = threadIdx.x;
+        float2 v[R][R1];
 #pragma unroll
-        for (int a = 0; a < R1; ++a) v[a] = __ldcs(Tb + (size_t)r * L + a * 256 + w);
-        fft_reg<R1>(v);
+        for (int r = 0; r < R; ++r)
 #pragma unroll
-        for (int ka = 1; ka < R1; ++ka) v[ka] = cmul(v[ka], __ldg(tw1 + ka * 256 + w));
-        float2* p = fsm + r * LP + (w >> 4) * FFT_PB + (w & 15);
+            for (int a = 0; a < R1; ++a) v[r][a] = __ldcs(Tb + (size_t)r * L + a * 256 + w);
+        float2 tw[R1];
 #pragma unroll
-        for (int ka = 0; ka < R1; ++ka) p[ka * FFT_PA] = v[ka];
+        for (int ka = 1; ka < R1; ++ka) tw[ka] = __ldg(tw1 + ka * 256 + w);
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            fft_reg<R1>(v[r]);
+            float2* p = fsm + r * LP + (w >> 4) * FFT_PB + (w & 15);
+            p[0] = v[r][0];
+#pragma unroll
+            for (int ka = 1; ka < R1; ++ka) p[ka * FFT_PA] = cmul(v[r][ka], tw[ka]);
+        }
     }
     __syncthreads();
     for (int i = threadIdx.x; i < 16 * R1 * R; i += FFT_THREADS) fft_step2(fsm + (i / (16 * R1)) * LP, i % (16 * R1), tw2);

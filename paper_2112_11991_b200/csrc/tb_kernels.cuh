@@ -125,6 +125,8 @@ k_resample(const float* __restrict__ x, float* __restrict__ y, const TmplDev* __
     __shared__ double s_val[RS_MAXSEG + 1];
     __shared__ double s_slp[RS_MAXSEG + 1];
     __shared__ __align__(16) double s_coef[RS_MAXSEG][4];
+    __shared__ __align__(16) float4 s_cf[RS_MAXSEG];     // fp32 copy of the cubic, relative to s_ci.x
+    __shared__ int2 s_ci[RS_MAXSEG];                     // (nearest integer to the first delta, tie margin bits)
 
     const int b     = blockIdx.x % n_tmpl;
     const int tbase = (blockIdx.x / n_tmpl) * tile;
@@ -152,6 +154,9 @@ k_resample(const float* __restrict__ x, float* __restrict__ y, const TmplDev* __
             s_coef[k][1] = d0;
             s_coef[k][2] = 3.0 * dv - (2.0 * d0 + d1);
             s_coef[k][3] = (d0 + d1) - 2.0 * dv;
+            const double i0 = rint(v0);
+            s_cf[k] = make_float4((float)(v0 - i0), (float)d0, (float)s_coef[k][2], (float)s_coef[k][3]);
+            s_ci[k] = make_int2((int)i0, __float_as_int((float)((fabs(d0) + fabs(s_coef[k][2]) + fabs(s_coef[k][3]) + 2.0) * 1e-6)));
         }
         __syncthreads();
 
@@ -160,15 +165,35 @@ k_resample(const float* __restrict__ x, float* __restrict__ y, const TmplDev* __
             const int j = jsub + o;
             int src[4];
             if (log2h >= 2) {
+                // fp32 cubic relative to the segment's integer offset; a sample whose rounding
+                // residual is within the margin of a tie is re-decided with the fp64 cubic, so the
+                // integer decision is the fp64 one everywhere (3 FFMA instead of 3 DFMA per sample)
                 const int seg = o >> log2h;
-                const double2 c01 = *reinterpret_cast<const double2*>(&s_coef[seg][0]);
-                const double2 c23 = *reinterpret_cast<const double2*>(&s_coef[seg][2]);
-                double tt = (double)(o & (h - 1)) * inv_h;
+                const float4 f = s_cf[seg];
+                const int2 ie = s_ci[seg];
+                const float lim = 0.5f - __int_as_float(ie.y);
+                const float inv_hf = (float)inv_h;
+                float tf = (float)(o & (h - 1)) * inv_hf;
+                const int jb = j - ie.x + 0x4B400000;
+                bool tie = false;
 #pragma unroll
                 for (int q = 0; q < 4; ++q) {
-                    const double d = fma(fma(fma(c23.y, tt, c23.x), tt, c01.y), tt, c01.x);
-                    src[q] = j + q - floor_to_int(d);
-                    tt += inv_h;
+                    const float yv = fmaf(fmaf(fmaf(f.w, tf, f.z), tf, f.y), tf, f.x);
+                    const float z = yv + 12582912.0f;            // 1.5 * 2^23: nearest integer in the low bits
+                    src[q] = jb + q - __float_as_int(z);
+                    tie |= fabsf(yv - (z - 12582912.0f)) > lim;
+                    tf += inv_hf;
+                }
+                if (tie) {
+                    const double2 c01 = *reinterpret_cast<const double2*>(&s_coef[seg][0]);
+                    const double2 c23 = *reinterpret_cast<const double2*>(&s_coef[seg][2]);
+                    double tt = (double)(o & (h - 1)) * inv_h;
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) {
+                        const double d = fma(fma(fma(c23.y, tt, c23.x), tt, c01.y), tt, c01.x);
+                        src[q] = j + q - floor_to_int(d);
+                        tt += inv_h;
+                    }
                 }
             } else {
 #pragma unroll
@@ -196,17 +221,22 @@ k_resample(const float* __restrict__ x, float* __restrict__ y, const TmplDev* __
 }
 
 // ---------------------------------------------------------------------------------------------
-// K2  spectrum former + block median (a5 + a6).  One warp = one median block of W bins:
-//   lane holds W/32 powers in registers, P_k = max(|X_k|^2, 1/2 |X_k - X_{k-1}|^2) with X_0 <- 0
-//   (G12-G14), written once as float4; the exact median (mean of the two middle order
-//   statistics, G15) is found by a 31-step bisection on the bit pattern of the non-negative
-//   floats with warp-wide counts (REDUX) -- no shared memory, no block barrier.
-//   ld = row stride of the cuFFT output in complex elements (even: rows are 16-byte aligned).
-// ---------------------------------------------------------------------------------------------
+// K2  spectrum former + block median + normalisation (a5 + a6 + a7).
+//   One warp = one median block of W bins; a CTA = SP_WARPS consecutive blocks plus one halo
+//   block on each side (their medians are needed to interpolate the baseline; they are
+//   recomputed rather than exchanged through global memory, 2/SP_WARPS extra work).
+//   Each lane keeps W/32 powers in registers, P_k = max(|X_k|^2, 1/2 |X_k - X_{k-1}|^2) with
+//   X_0 <- 0 (G12-G14).  Exact block median (mean of the two middle order statistics, G15) by
+//   bracket-and-select with warp ballots, exact bisection fallback.  After one block barrier
+//   the powers are normalised in registers, P^_k = P_k ln2 / m(k), m(k) interpolated linearly
+//   between block centres bW + (W-1)/2, flat outside (G15), P^_0 = 0, m <= 0 -> 0, and written
+//   once as float4: the raw powers never reach HBM (RAW = true writes them too, parity tap).
 //   UNPACK = true: the input is Z, the length-N/2 complex FFT of z_j = y_2j + i y_2j+1 (row
 //   stride ld = N/2), and the real-series spectrum is formed on the fly,
 //       X_k = E_k + W_N^k O_k,  E = (Z_k + conj Z_{M-k})/2,  O = -i (Z_k - conj Z_{M-k})/2,
 //   with W_N^k = W_N^{block start} (one fp64 sincospi per warp) * twn[k - block start] (table).
+//   UNPACK = false: the input is the cuFFT R2C output (row stride ld, padded to 16 bytes).
+// ---------------------------------------------------------------------------------------------
 __device__ __forceinline__ float2 r2c_unpack(float2 zk, float2 zm, float2 w)
 {
     const float er = 0.5f * (zk.x + zm.x), ei = 0.5f * (zk.y - zm.y);
@@ -214,81 +244,20 @@ __device__ __forceinline__ float2 r2c_unpack(float2 zk, float2 zm, float2 w)
     return make_float2(er + (w.x * orr - w.y * oi), ei + (w.x * oi + w.y * orr));
 }
 
-template <int W, bool UNPACK>
-__global__ void __launch_bounds__(SP_WARPS * 32)
-k_spectrum_median(const float2* __restrict__ X, size_t ld, float* __restrict__ P, float* __restrict__ med,
-                  int nb, int nblk_per_row, int cta_per_row, const float2* __restrict__ twn,
-                  unsigned long long* __restrict__ fallbacks)
+// exact order statistics W/2-1 and W/2 of the W non-negative floats held by a warp (VPT per
+// lane); returns their mean.  cand = this warp's shared scratch of CAP floats.
+template <int W>
+__device__ __forceinline__ float warp_median(const float (&p)[W / 32], float* cand, int lane,
+                                             unsigned long long* __restrict__ fallbacks)
 {
-    constexpr int VPT  = W / 32;        // powers per lane
-    constexpr int ITER = W / 128;       // 4 consecutive bins per lane per iteration
-    const int row  = blockIdx.x / cta_per_row;
-    const int blk  = (blockIdx.x % cta_per_row) * SP_WARPS + (threadIdx.x >> 5);
-    const int lane = threadIdx.x & 31;
-    if (blk >= nblk_per_row) return;
-
-    const float2* __restrict__ Xr = X + (size_t)row * ld;
-    float* __restrict__ Pr        = P + (size_t)row * (size_t)nb;
-    const int base = blk * W;
-
-    float p[VPT];
-    float2 carry = make_float2(0.f, 0.f);                // X_{k-1} for lane 0 (X_{-1} = 0)
-    float2 wbase = make_float2(1.f, 0.f);
-    if (UNPACK) {
-        double sb, cb;
-        sincospi(-(double)base / (double)nb, &sb, &cb);  // W_N^base, N = 2 nb
-        wbase = make_float2((float)cb, (float)sb);
-        if (base > 0 && lane == 0) {
-            double s1, c1;
-            sincospi(-(double)(base - 1) / (double)nb, &s1, &c1);
-            carry = r2c_unpack(__ldg(Xr + base - 1), __ldg(Xr + (nb - base + 1)), make_float2((float)c1, (float)s1));
-        }
-    } else if (base > 0 && lane == 0) carry = __ldg(Xr + base - 1);
-#pragma unroll
-    for (int i = 0; i < ITER; ++i) {
-        const int k0 = base + i * 128 + lane * 4;
-        float4 a = __ldg(reinterpret_cast<const float4*>(Xr + k0));
-        float4 c = __ldg(reinterpret_cast<const float4*>(Xr + k0 + 2));
-        if (UNPACK) {
-            const float2* zm = Xr + (nb - k0);           // Z_{M-k0}; bins k0+q mirror at zm[-q]
-            const float2 m0 = __ldg(k0 == 0 ? Xr : zm), m1 = __ldg(zm - 1), m2 = __ldg(zm - 2), m3 = __ldg(zm - 3);
-            const float4 t01 = __ldg(reinterpret_cast<const float4*>(twn + (k0 - base)));
-            const float4 t23 = __ldg(reinterpret_cast<const float4*>(twn + (k0 - base) + 2));
-            const float2 x0 = r2c_unpack(make_float2(a.x, a.y), m0, make_float2(wbase.x * t01.x - wbase.y * t01.y, wbase.x * t01.y + wbase.y * t01.x));
-            const float2 x1 = r2c_unpack(make_float2(a.z, a.w), m1, make_float2(wbase.x * t01.z - wbase.y * t01.w, wbase.x * t01.w + wbase.y * t01.z));
-            const float2 x2 = r2c_unpack(make_float2(c.x, c.y), m2, make_float2(wbase.x * t23.x - wbase.y * t23.y, wbase.x * t23.y + wbase.y * t23.x));
-            const float2 x3 = r2c_unpack(make_float2(c.z, c.w), m3, make_float2(wbase.x * t23.z - wbase.y * t23.w, wbase.x * t23.w + wbase.y * t23.z));
-            a = make_float4(x0.x, x0.y, x1.x, x1.y);
-            c = make_float4(x2.x, x2.y, x3.x, x3.y);
-        }
-        if (k0 == 0) { a.x = 0.f; a.y = 0.f; }           // X_0 <- 0 before differencing (G13)
-        float px = __shfl_up_sync(0xffffffffu, c.z, 1);
-        float py = __shfl_up_sync(0xffffffffu, c.w, 1);
-        if (lane == 0) { px = carry.x; py = carry.y; }
-        const float nx = __shfl_sync(0xffffffffu, c.z, 31);
-        const float ny = __shfl_sync(0xffffffffu, c.w, 31);
-        carry = make_float2(nx, ny);
-        float dx, dy;
-        float4 o;
-        dx = a.x - px;  dy = a.y - py;  o.x = fmaxf(a.x * a.x + a.y * a.y, 0.5f * (dx * dx + dy * dy));
-        dx = a.z - a.x; dy = a.w - a.y; o.y = fmaxf(a.z * a.z + a.w * a.w, 0.5f * (dx * dx + dy * dy));
-        dx = c.x - a.z; dy = c.y - a.w; o.z = fmaxf(c.x * c.x + c.y * c.y, 0.5f * (dx * dx + dy * dy));
-        dx = c.z - c.x; dy = c.w - c.y; o.w = fmaxf(c.z * c.z + c.w * c.w, 0.5f * (dx * dx + dy * dy));
-        *reinterpret_cast<float4*>(Pr + k0) = o;
-        p[4 * i + 0] = o.x; p[4 * i + 1] = o.y; p[4 * i + 2] = o.z; p[4 * i + 3] = o.w;
-    }
-
-    // Exact order statistics W/2-1 and W/2 (0-based) of the W values held by the warp.
-    // Fast path: the median of noise-like powers sits near 0.78 x the block mean, so count the
-    // values below lo = 0.66 mean, compact those in [lo, hi = 0.90 mean) (ballot + popc prefix
-    // into a per-warp shared list, about 13 % of the block) and select among them; if the two
-    // middle ranks are not both inside the bracket (or it overflows) fall back to the
-    // data-independent bisection over all W values.  Both paths are exact.
+    constexpr int VPT = W / 32;
     constexpr int K1 = W / 2 - 1;
     constexpr int CAP = (W >= 512) ? W / 4 : W;          // candidate list capacity
     constexpr int CPL = CAP / 32;                        // candidates per lane
-    __shared__ float s_cand[SP_WARPS][CAP];
-    float* cand = s_cand[threadIdx.x >> 5];
+    // Fast path: the median of noise-like powers sits near 0.78 x the block mean, so count the
+    // values below lo = 0.66 mean, compact those in [lo, hi = 0.90 mean) (ballot + popc prefix,
+    // about 13 % of the block) and select among them.  If the two middle ranks are not both
+    // inside the bracket (or it overflows) fall back to the bisection over all W values.
     float sum = 0.f;
 #pragma unroll
     for (int v = 0; v < VPT; ++v) sum += p[v];
@@ -315,7 +284,7 @@ k_spectrum_median(const float2* __restrict__ X, size_t ld, float* __restrict__ P
 #pragma unroll
         for (int q = 0; q < CPL; ++q) ck[q] = (q * 32 + lane < nmid) ? __float_as_uint(cand[q * 32 + lane]) : 0xffffffffu;
         const int r1 = K1 - below;                       // rank among the candidates
-        for (int bit = 30; bit >= 0; --bit) {
+        for (int bit = 30; bit >= 0; --bit) {            // non-negative floats order like their bit patterns
             const uint32_t cnd = prefix | (1u << bit);
             int c = 0;
 #pragma unroll
@@ -333,6 +302,7 @@ k_spectrum_median(const float2* __restrict__ X, size_t ld, float* __restrict__ P
         le  = __reduce_add_sync(0xffffffffu, le);
         nxt = __reduce_min_sync(0xffffffffu, nxt);
         upper = (le >= r1 + 2) ? prefix : nxt;
+        __syncwarp();
     } else {
         if (lane == 0 && fallbacks) atomicAdd(fallbacks, 1ull);
         uint32_t key[VPT];
@@ -357,42 +327,108 @@ k_spectrum_median(const float2* __restrict__ X, size_t ld, float* __restrict__ P
         nxt = __reduce_min_sync(0xffffffffu, nxt);
         upper = (le >= W / 2 + 1) ? prefix : nxt;
     }
-    if (lane == 0) med[(size_t)row * nblk_per_row + blk] = 0.5f * (__uint_as_float(prefix) + __uint_as_float(upper));
+    return 0.5f * (__uint_as_float(prefix) + __uint_as_float(upper));
 }
 
-// ---------------------------------------------------------------------------------------------
-// K3  normalise (a7), in place: P^_k = P_k ln2 / m(k), m(k) = linear interpolation of the block
-//   medians between block centres bW + (W-1)/2, flat outside (G15); P^_0 = 0; m <= 0 -> 0.
-// ---------------------------------------------------------------------------------------------
-__device__ __forceinline__ float baseline_at(const float* __restrict__ med, int nblk, int k, int log2w)
+template <int W, bool UNPACK, bool RAW>
+__global__ void __launch_bounds__((SP_WARPS + 2) * 32)
+k_spectrum_median(const float2* __restrict__ X, size_t ld, float* __restrict__ P, float* __restrict__ med,
+                  int nb, int nblk_per_row, int cta_per_row, const float2* __restrict__ twn,
+                  unsigned long long* __restrict__ fallbacks, float* __restrict__ Praw)
 {
-    const int W = 1 << log2w;
-    const int a = k - (W >> 1);                          // k - c_b = (a mod W) + 1/2
-    if (a < 0) return __ldg(med);
-    const int b = a >> log2w;
-    if (b >= nblk - 1) return __ldg(med + nblk - 1);
-    const float fr = ((float)(a & (W - 1)) + 0.5f) * (1.0f / (float)W);
-    const float m0 = __ldg(med + b), m1 = __ldg(med + b + 1);
-    return fmaf(fr, m1 - m0, m0);
-}
+    constexpr int VPT  = W / 32;        // powers per lane
+    constexpr int ITER = W / 128;       // 4 consecutive bins per lane per iteration
+    constexpr int CAP  = (W >= 512) ? W / 4 : W;
+    __shared__ float s_cand[SP_WARPS + 2][CAP];
+    __shared__ float s_med[SP_WARPS + 2];
+    const int row  = blockIdx.x / cta_per_row;
+    const int wid  = threadIdx.x >> 5;
+    const int lane = threadIdx.x & 31;
+    const int blk  = (blockIdx.x % cta_per_row) * SP_WARPS - 1 + wid;      // wid 0 and SP_WARPS+1 are halo blocks
+    const bool active = blk >= 0 && blk < nblk_per_row;
+    const bool writer = active && wid >= 1 && wid <= SP_WARPS;
 
-__global__ void __launch_bounds__(256)
-k_normalise(float* __restrict__ P, const float* __restrict__ med, int nb, int nblk, int log2w, int cta_per_row)
-{
-    const int row = blockIdx.x / cta_per_row;
-    const int k0  = ((blockIdx.x % cta_per_row) * 256 + threadIdx.x) * 4;
-    if (k0 >= nb) return;
-    float* __restrict__ Pr = P + (size_t)row * (size_t)nb;
-    const float* __restrict__ mr = med + (size_t)row * nblk;
-    float4 v = *reinterpret_cast<const float4*>(Pr + k0);
-    float* vv = reinterpret_cast<float*>(&v);
+    const float2* __restrict__ Xr = X + (size_t)row * ld;
+    const int base = blk * W;
+
+    float p[VPT];
+    float m_cur = 0.f;
+    if (active) {
+        float2 carry = make_float2(0.f, 0.f);            // X_{k-1} for lane 0 (X_{-1} = 0)
+        float2 wbase = make_float2(1.f, 0.f);
+        if (UNPACK) {
+            double sb, cb;
+            sincospi(-(double)base / (double)nb, &sb, &cb);      // W_N^base, N = 2 nb
+            wbase = make_float2((float)cb, (float)sb);
+            if (base > 0 && lane == 0) {
+                double s1, c1;
+                sincospi(-(double)(base - 1) / (double)nb, &s1, &c1);
+                carry = r2c_unpack(__ldg(Xr + base - 1), __ldg(Xr + (nb - base + 1)), make_float2((float)c1, (float)s1));
+            }
+        } else if (base > 0 && lane == 0) carry = __ldg(Xr + base - 1);
 #pragma unroll
-    for (int q = 0; q < 4; ++q) {
-        const float m = baseline_at(mr, nblk, k0 + q, log2w);
-        vv[q] = (m > 0.f) ? vv[q] * 0.69314718055994530942f / m : 0.f;
+        for (int i = 0; i < ITER; ++i) {
+            const int k0 = base + i * 128 + lane * 4;
+            float4 a = __ldg(reinterpret_cast<const float4*>(Xr + k0));
+            float4 c = __ldg(reinterpret_cast<const float4*>(Xr + k0 + 2));
+            if (UNPACK) {
+                const float2* zm = Xr + (nb - k0);       // Z_{M-k0}; bins k0+q mirror at zm[-q]
+                const float2 m0 = __ldg(k0 == 0 ? Xr : zm), m1 = __ldg(zm - 1), m2 = __ldg(zm - 2), m3 = __ldg(zm - 3);
+                const float4 t01 = __ldg(reinterpret_cast<const float4*>(twn + (k0 - base)));
+                const float4 t23 = __ldg(reinterpret_cast<const float4*>(twn + (k0 - base) + 2));
+                const float2 x0 = r2c_unpack(make_float2(a.x, a.y), m0, make_float2(wbase.x * t01.x - wbase.y * t01.y, wbase.x * t01.y + wbase.y * t01.x));
+                const float2 x1 = r2c_unpack(make_float2(a.z, a.w), m1, make_float2(wbase.x * t01.z - wbase.y * t01.w, wbase.x * t01.w + wbase.y * t01.z));
+                const float2 x2 = r2c_unpack(make_float2(c.x, c.y), m2, make_float2(wbase.x * t23.x - wbase.y * t23.y, wbase.x * t23.y + wbase.y * t23.x));
+                const float2 x3 = r2c_unpack(make_float2(c.z, c.w), m3, make_float2(wbase.x * t23.z - wbase.y * t23.w, wbase.x * t23.w + wbase.y * t23.z));
+                a = make_float4(x0.x, x0.y, x1.x, x1.y);
+                c = make_float4(x2.x, x2.y, x3.x, x3.y);
+            }
+            if (k0 == 0) { a.x = 0.f; a.y = 0.f; }       // X_0 <- 0 before differencing (G13)
+            float px = __shfl_up_sync(0xffffffffu, c.z, 1);
+            float py = __shfl_up_sync(0xffffffffu, c.w, 1);
+            if (lane == 0) { px = carry.x; py = carry.y; }
+            const float nx = __shfl_sync(0xffffffffu, c.z, 31);
+            const float ny = __shfl_sync(0xffffffffu, c.w, 31);
+            carry = make_float2(nx, ny);
+            float dx, dy;
+            float4 o;
+            dx = a.x - px;  dy = a.y - py;  o.x = fmaxf(a.x * a.x + a.y * a.y, 0.5f * (dx * dx + dy * dy));
+            dx = a.z - a.x; dy = a.w - a.y; o.y = fmaxf(a.z * a.z + a.w * a.w, 0.5f * (dx * dx + dy * dy));
+            dx = c.x - a.z; dy = c.y - a.w; o.z = fmaxf(c.x * c.x + c.y * c.y, 0.5f * (dx * dx + dy * dy));
+            dx = c.z - c.x; dy = c.w - c.y; o.w = fmaxf(c.z * c.z + c.w * c.w, 0.5f * (dx * dx + dy * dy));
+            if (RAW && writer) *reinterpret_cast<float4*>(Praw + (size_t)row * (size_t)nb + k0) = o;
+            p[4 * i + 0] = o.x; p[4 * i + 1] = o.y; p[4 * i + 2] = o.z; p[4 * i + 3] = o.w;
+        }
+        m_cur = warp_median<W>(p, s_cand[wid], lane, (wid >= 1 && wid <= SP_WARPS) ? fallbacks : nullptr);
+        if (lane == 0) {
+            s_med[wid] = m_cur;
+            if (writer) med[(size_t)row * nblk_per_row + blk] = m_cur;
+        }
     }
-    if (k0 == 0) v.x = 0.f;
-    *reinterpret_cast<float4*>(Pr + k0) = v;
+    __syncthreads();
+    if (!writer) return;
+    const float m_prev = (blk > 0) ? s_med[wid - 1] : m_cur;                     // flat below the first centre
+    const float m_next = (blk + 1 < nblk_per_row) ? s_med[wid + 1] : m_cur;      // flat above the last centre
+    float* __restrict__ Pr = P + (size_t)row * (size_t)nb;
+    constexpr float LN2 = 0.69314718055994530942f;
+    constexpr float INV_W = 1.0f / (float)W;
+#pragma unroll
+    for (int i = 0; i < ITER; ++i) {
+        const int e0 = i * 128 + lane * 4;               // offset of the 4 bins inside the block
+        const bool second = e0 >= W / 2;
+        const float ma = second ? m_cur : m_prev, mb = second ? m_next : m_cur;
+        const float f0 = ((float)(second ? e0 - W / 2 : e0 + W / 2) + 0.5f) * INV_W;
+        const float dm = (mb - ma);
+        float4 o;
+        float* ov = reinterpret_cast<float*>(&o);
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            const float m = fmaf(f0 + (float)q * INV_W, dm, ma);
+            ov[q] = (m > 0.f) ? __fdividef(p[4 * i + q] * LN2, m) : 0.f;
+        }
+        if (base + e0 == 0) o.x = 0.f;                   // P^_0 = 0
+        *reinterpret_cast<float4*>(Pr + base + e0) = o;
+    }
 }
 
 // ---------------------------------------------------------------------------------------------
