@@ -186,7 +186,7 @@ def run_ours(args, wl):
     pinned = torch.from_numpy(wl.series).pin_memory()
     host_series = pinned.numpy()
     plan = tb.Plan(host_series, wl.tsamp, device=local, stream=stream.cuda_stream, enable_timings=True,
-                   chunk_templates=args.chunk)
+                   chunk_templates=args.chunk, fft_path=args.fft_path)
     chunk = plan.info()["chunk_templates"]
     stage_keys = ["ms_resample", "ms_fft", "ms_spectrum", "ms_normalise", "ms_hsum", "ms_total"]
 
@@ -302,6 +302,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--log2n", type=int, default=23)
     ap.add_argument("--chunk", type=int, default=0)
+    ap.add_argument("--fft-path", type=int, default=0, help="tb_plan_opts.fft_path (0 auto, 1 cuFFT, 2 own fused, 3 own unfused)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
 
