@@ -66,7 +66,7 @@ struct tb_plan {
     int log2m1 = 0, log2m2 = 0;
     SegRec* d_seg = nullptr;                         // [chunk][n >> MIN_LOG2H]
     size_t seg_stride = 0;
-    float2 *d_tw1a = nullptr, *d_tw1b = nullptr, *d_tw2 = nullptr, *d_twn = nullptr;
+    float2 *d_tw1a = nullptr, *d_tw1b = nullptr, *d_tw2 = nullptr, *d_twn = nullptr, *d_twb = nullptr;
     int min_log2h = 0;                               // smallest knot spacing among the staged templates
 
     std::map<uint32_t, cufftHandle> fft_plans;       // by batch size, sharing one work area
@@ -266,15 +266,16 @@ template <int W>
 void launch_spectrum(tb_plan* p, uint32_t nt, bool unpack, float* d_raw)
 {
     const int cta_per_row = (int)((p->nblk + SP_WARPS - 1) / SP_WARPS);
-    const unsigned grid = (unsigned)(cta_per_row * nt), threads = (SP_WARPS + 2) * 32;
+    const unsigned grid = (unsigned)(cta_per_row * nt), threads = (SP_WARPS + 1) * 32;
     const float2* in = p->d_fft;
     const size_t ld = unpack ? (size_t)p->nb : p->ld;
-    const float2* tw = unpack ? p->d_twn : nullptr;
+    const float2 *tw = unpack ? p->d_twn : nullptr, *tb = unpack ? p->d_twb : nullptr;
     unsigned long long* fb = p->d_cursor + 1;
-    if (unpack && d_raw)       k_spectrum_median<W, true, true><<<grid, threads, 0, p->stream>>>(in, ld, p->d_power, p->d_med, (int)p->nb, (int)p->nblk, cta_per_row, tw, fb, d_raw);
-    else if (unpack)           k_spectrum_median<W, true, false><<<grid, threads, 0, p->stream>>>(in, ld, p->d_power, p->d_med, (int)p->nb, (int)p->nblk, cta_per_row, tw, fb, nullptr);
-    else if (d_raw)            k_spectrum_median<W, false, true><<<grid, threads, 0, p->stream>>>(in, ld, p->d_power, p->d_med, (int)p->nb, (int)p->nblk, cta_per_row, tw, fb, d_raw);
-    else                       k_spectrum_median<W, false, false><<<grid, threads, 0, p->stream>>>(in, ld, p->d_power, p->d_med, (int)p->nb, (int)p->nblk, cta_per_row, tw, fb, nullptr);
+    const int nb = (int)p->nb, nblk = (int)p->nblk;
+    if (unpack && d_raw)       k_spectrum_median<W, true, true><<<grid, threads, 0, p->stream>>>(in, ld, p->d_power, p->d_med, nb, nblk, cta_per_row, tw, tb, fb, d_raw);
+    else if (unpack)           k_spectrum_median<W, true, false><<<grid, threads, 0, p->stream>>>(in, ld, p->d_power, p->d_med, nb, nblk, cta_per_row, tw, tb, fb, nullptr);
+    else if (d_raw)            k_spectrum_median<W, false, true><<<grid, threads, 0, p->stream>>>(in, ld, p->d_power, p->d_med, nb, nblk, cta_per_row, tw, tb, fb, d_raw);
+    else                       k_spectrum_median<W, false, false><<<grid, threads, 0, p->stream>>>(in, ld, p->d_power, p->d_med, nb, nblk, cta_per_row, tw, tb, fb, nullptr);
 }
 
 // ---- hand-written FFT path -------------------------------------------------------------------
@@ -385,7 +386,7 @@ int make_twiddles(tb_plan* p)
     int rc;
     if ((rc = tw1(p->log2m1, &p->d_tw1a))) return rc;
     if ((rc = tw1(p->log2m2, &p->d_tw1b))) return rc;
-    std::vector<float2> h2(256), hn(p->window);
+    std::vector<float2> h2(256), hn(p->window), hb(p->nblk);
     for (int kb = 0; kb < 16; ++kb)
         for (int c = 0; c < 16; ++c) {
             const long double a = -two_pi * (long double)(kb * c) / 256.0L;
@@ -395,7 +396,12 @@ int make_twiddles(tb_plan* p)
         const long double a = -two_pi * (long double)i / (long double)p->n;
         hn[i] = make_float2((float)cosl(a), (float)sinl(a));
     }
+    for (uint32_t b = 0; b < p->nblk; ++b) {             // W_N^{b W}: the R2C twiddle at the start of median block b
+        const long double a = -two_pi * (long double)((uint64_t)b * p->window) / (long double)p->n;
+        hb[b] = make_float2((float)cosl(a), (float)sinl(a));
+    }
     if ((rc = upload(h2, &p->d_tw2))) return rc;
+    if ((rc = upload(hb, &p->d_twb))) return rc;
     return upload(hn, &p->d_twn);
 }
 
@@ -441,15 +447,16 @@ int run_hsum(tb_plan* p, uint32_t nt, const FoldParams& fp, uint32_t first_id)
 {
     if (p->nb >= (uint64_t)HS_T) {
         const int tiles = (int)(p->nb / HS_T);
-        const size_t smem = HS_SMEM_FLOATS * sizeof(float);
+        const int tpc = std::min(tiles, 8);                                  // tiles walked by one CTA (double-buffered)
+        const size_t smem = 2 * HS_SMEM_FLOATS * sizeof(float);
         static bool attr_set = false;
         if (!attr_set) {
             TB_CUDA(p, cudaFuncSetAttribute(k_hsum_tile, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
             attr_set = true;
         }
-        k_hsum_tile<<<(unsigned)(tiles * nt), HS_THREADS, smem, p->stream>>>(p->d_power, (int)p->nb, tiles, fp, first_id,
-                                                                             p->d_cand, p->d_cursor,
-                                                                             (unsigned long long)p->max_cand);
+        k_hsum_tile<<<(unsigned)((tiles / tpc) * nt), HS_THREADS, smem, p->stream>>>(p->d_power, (int)p->nb, tiles / tpc, tpc, fp,
+                                                                                     first_id, p->d_cand, p->d_cursor,
+                                                                                     (unsigned long long)p->max_cand);
         TB_CUDA(p, cudaGetLastError());
         return TB_OK;
     }
@@ -531,7 +538,7 @@ void destroy(tb_plan* p)
     for (auto& kv : p->fft_plans) cufftDestroy(kv.second);
     for (auto& es : p->events) for (auto& e : es.e) cudaEventDestroy(e);
     if (p->ev_staged) cudaEventDestroy(p->ev_staged);
-    cudaFree(p->d_T); cudaFree(p->d_seg); cudaFree(p->d_tw1a); cudaFree(p->d_tw1b); cudaFree(p->d_tw2); cudaFree(p->d_twn);
+    cudaFree(p->d_T); cudaFree(p->d_seg); cudaFree(p->d_tw1a); cudaFree(p->d_tw1b); cudaFree(p->d_tw2); cudaFree(p->d_twn); cudaFree(p->d_twb);
     cudaFree(p->d_work); cudaFree(p->d_acc); cudaFree(p->d_series_owned); cudaFree(p->d_resampled); cudaFree(p->d_fft);
     cudaFree(p->d_power); cudaFree(p->d_med); cudaFree(p->d_cand); cudaFree(p->d_cursor); cudaFree(p->d_tmpl);
     if (p->h_tmpl) cudaFreeHost(p->h_tmpl);

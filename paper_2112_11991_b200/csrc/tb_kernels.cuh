@@ -222,26 +222,31 @@ k_resample(const float* __restrict__ x, float* __restrict__ y, const TmplDev* __
 
 // ---------------------------------------------------------------------------------------------
 // K2  spectrum former + block median + normalisation (a5 + a6 + a7).
-//   One warp = one median block of W bins; a CTA = SP_WARPS consecutive blocks plus one halo
-//   block on each side (their medians are needed to interpolate the baseline; they are
-//   recomputed rather than exchanged through global memory, 2/SP_WARPS extra work).
+//   One warp = one median block of W bins.  A CTA has SP_WARPS + 1 warps on SP_WARPS + 1
+//   consecutive blocks B0 .. B0 + SP_WARPS and writes the SP_WARPS * W normalised bins between the
+//   centres of its first and last block (the baseline of a bin is interpolated between the two
+//   block centres that enclose it): warp 0 writes the second half of its block, the last warp the
+//   first half, the others their whole block.  The boundary block is therefore formed twice (by
+//   two CTAs, 1/SP_WARPS extra work) instead of being exchanged through global memory.
 //   Each lane keeps W/32 powers in registers, P_k = max(|X_k|^2, 1/2 |X_k - X_{k-1}|^2) with
 //   X_0 <- 0 (G12-G14).  Exact block median (mean of the two middle order statistics, G15) by
-//   bracket-and-select with warp ballots, exact bisection fallback.  After one block barrier
-//   the powers are normalised in registers, P^_k = P_k ln2 / m(k), m(k) interpolated linearly
-//   between block centres bW + (W-1)/2, flat outside (G15), P^_0 = 0, m <= 0 -> 0, and written
-//   once as float4: the raw powers never reach HBM (RAW = true writes them too, parity tap).
+//   bracket-and-select, exact bisection fallback.  After one block barrier the powers are
+//   normalised in registers, P^_k = P_k ln2 / m(k), m(k) interpolated linearly between block
+//   centres bW + (W-1)/2, flat outside (G15), P^_0 = 0, m <= 0 -> 0, and written once as float4:
+//   the raw powers never reach HBM (RAW = true writes them too, parity tap).
 //   UNPACK = true: the input is Z, the length-N/2 complex FFT of z_j = y_2j + i y_2j+1 (row
 //   stride ld = N/2), and the real-series spectrum is formed on the fly,
-//       X_k = E_k + W_N^k O_k,  E = (Z_k + conj Z_{M-k})/2,  O = -i (Z_k - conj Z_{M-k})/2,
-//   with W_N^k = W_N^{block start} (one fp64 sincospi per warp) * twn[k - block start] (table).
+//       2 X_k = (Z_k + conj Z_{M-k}) - i W_N^k (Z_k - conj Z_{M-k}),
+//   with W_N^k = twb[block] * twn[k - block start] (two small tables made on the host in
+//   extended precision).  The factor 2 is carried through the median (powers are 4x) and only
+//   removed where a raw power or a median is written: it cancels in P^.
 //   UNPACK = false: the input is the cuFFT R2C output (row stride ld, padded to 16 bytes).
 // ---------------------------------------------------------------------------------------------
-__device__ __forceinline__ float2 r2c_unpack(float2 zk, float2 zm, float2 w)
+__device__ __forceinline__ float2 r2c_unpack2(float2 zk, float2 zm, float2 w)     // 2 X_k
 {
-    const float er = 0.5f * (zk.x + zm.x), ei = 0.5f * (zk.y - zm.y);
-    const float orr = 0.5f * (zk.y + zm.y), oi = -0.5f * (zk.x - zm.x);
-    return make_float2(er + (w.x * orr - w.y * oi), ei + (w.x * oi + w.y * orr));
+    const float er = zk.x + zm.x, ei = zk.y - zm.y;
+    const float orr = zk.y + zm.y, oi = zm.x - zk.x;
+    return make_float2(fmaf(w.x, orr, fmaf(-w.y, oi, er)), fmaf(w.x, oi, fmaf(w.y, orr, ei)));
 }
 
 // exact order statistics W/2-1 and W/2 of the W non-negative floats held by a warp (VPT per
@@ -254,60 +259,83 @@ __device__ __forceinline__ float warp_median(const float (&p)[W / 32], float* ca
     constexpr int K1 = W / 2 - 1;
     constexpr int CAP = (W >= 512) ? W / 4 : W;          // candidate list capacity
     constexpr int CPL = CAP / 32;                        // candidates per lane
+    constexpr int NMW = (VPT + 31) / 32;
     // Fast path: the median of noise-like powers sits near 0.78 x the block mean, so count the
-    // values below lo = 0.66 mean, compact those in [lo, hi = 0.90 mean) (ballot + popc prefix,
-    // about 13 % of the block) and select among them.  If the two middle ranks are not both
-    // inside the bracket (or it overflows) fall back to the bisection over all W values.
+    // values below lo = 0.66 mean and compact those in [lo, hi = 0.90 mean) (about 13 % of the
+    // block: per-lane bit masks, one warp scan of the per-lane counts, lane-major list), then
+    // select among them.  If the two middle ranks are not both inside the bracket (or it
+    // overflows) fall back to the bisection over all W values.
     float sum = 0.f;
 #pragma unroll
     for (int v = 0; v < VPT; ++v) sum += p[v];
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
     const float lo = sum * (0.66f / (float)W), hi = sum * (0.90f / (float)W);
-    const unsigned lt_mask = (1u << lane) - 1u;
-    int below = 0, nmid = 0;
+    int below = 0, mine = 0;
+    uint32_t mask[NMW];
+#pragma unroll
+    for (int i = 0; i < NMW; ++i) mask[i] = 0u;
 #pragma unroll
     for (int v = 0; v < VPT; ++v) {
         const bool isb = p[v] < lo;
         const bool ism = !isb && p[v] < hi;
         below += isb ? 1 : 0;
-        const unsigned mm = __ballot_sync(0xffffffffu, ism);
-        const int pos = nmid + __popc(mm & lt_mask);
-        if (ism && pos < CAP) cand[pos] = p[v];
-        nmid += __popc(mm);
+        mine  += ism ? 1 : 0;
+        mask[v >> 5] |= ism ? (1u << (v & 31)) : 0u;
     }
     below = __reduce_add_sync(0xffffffffu, below);
-    uint32_t prefix = 0, upper;
+    int incl = mine;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const int t = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += t;
+    }
+    const int nmid = __shfl_sync(0xffffffffu, incl, 31);
+    uint32_t lower, upper;
     if (below <= K1 && below + nmid >= K1 + 2 && nmid <= CAP) {
+        int pos = incl - mine;
+#pragma unroll
+        for (int v = 0; v < VPT; ++v)
+            if (mask[v >> 5] & (1u << (v & 31))) cand[pos++] = p[v];
         __syncwarp();
         uint32_t ck[CPL];
 #pragma unroll
         for (int q = 0; q < CPL; ++q) ck[q] = (q * 32 + lane < nmid) ? __float_as_uint(cand[q * 32 + lane]) : 0xffffffffu;
+        // bisection in key space (non-negative floats order like their bit patterns) on the
+        // bracket [L, H) until exactly one candidate (or one key) is left around rank r1
         const int r1 = K1 - below;                       // rank among the candidates
-        for (int bit = 30; bit >= 0; --bit) {            // non-negative floats order like their bit patterns
-            const uint32_t cnd = prefix | (1u << bit);
+        uint32_t L = __float_as_uint(lo), H = __float_as_uint(hi);
+        int cl = 0, ch = nmid;                           // candidates below L, below H
+        while (ch - cl > 1 && H - L > 1u) {
+            const uint32_t mid = L + ((H - L) >> 1);
             int c = 0;
 #pragma unroll
-            for (int q = 0; q < CPL; ++q) c += (ck[q] < cnd) ? 1 : 0;
+            for (int q = 0; q < CPL; ++q) c += (ck[q] < mid) ? 1 : 0;
             c = __reduce_add_sync(0xffffffffu, c);
-            if (c <= r1) prefix = cnd;
+            if (c <= r1) { L = mid; cl = c; } else { H = mid; ch = c; }
         }
+        uint32_t v1 = 0xffffffffu;
+#pragma unroll
+        for (int q = 0; q < CPL; ++q) v1 = min(v1, ck[q] >= L ? ck[q] : 0xffffffffu);
+        v1 = __reduce_min_sync(0xffffffffu, v1);         // the candidate of rank r1
         int le = 0;
         uint32_t nxt = 0xffffffffu;
 #pragma unroll
         for (int q = 0; q < CPL; ++q) {
-            le += (ck[q] <= prefix) ? 1 : 0;
-            if (ck[q] > prefix) nxt = min(nxt, ck[q]);
+            le += (ck[q] <= v1) ? 1 : 0;
+            nxt = min(nxt, ck[q] > v1 ? ck[q] : 0xffffffffu);
         }
         le  = __reduce_add_sync(0xffffffffu, le);
         nxt = __reduce_min_sync(0xffffffffu, nxt);
-        upper = (le >= r1 + 2) ? prefix : nxt;
+        lower = v1;
+        upper = (le >= r1 + 2) ? v1 : nxt;
         __syncwarp();
     } else {
         if (lane == 0 && fallbacks) atomicAdd(fallbacks, 1ull);
         uint32_t key[VPT];
 #pragma unroll
         for (int v = 0; v < VPT; ++v) key[v] = __float_as_uint(p[v]);
+        uint32_t prefix = 0;
         for (int bit = 30; bit >= 0; --bit) {
             const uint32_t cnd = prefix | (1u << bit);
             int c = 0;
@@ -325,28 +353,31 @@ __device__ __forceinline__ float warp_median(const float (&p)[W / 32], float* ca
         }
         le  = __reduce_add_sync(0xffffffffu, le);
         nxt = __reduce_min_sync(0xffffffffu, nxt);
+        lower = prefix;
         upper = (le >= W / 2 + 1) ? prefix : nxt;
     }
-    return 0.5f * (__uint_as_float(prefix) + __uint_as_float(upper));
+    return 0.5f * (__uint_as_float(lower) + __uint_as_float(upper));
 }
 
 template <int W, bool UNPACK, bool RAW>
-__global__ void __launch_bounds__((SP_WARPS + 2) * 32)
+__global__ void __launch_bounds__((SP_WARPS + 1) * 32)
 k_spectrum_median(const float2* __restrict__ X, size_t ld, float* __restrict__ P, float* __restrict__ med,
                   int nb, int nblk_per_row, int cta_per_row, const float2* __restrict__ twn,
-                  unsigned long long* __restrict__ fallbacks, float* __restrict__ Praw)
+                  const float2* __restrict__ twb, unsigned long long* __restrict__ fallbacks,
+                  float* __restrict__ Praw)
 {
     constexpr int VPT  = W / 32;        // powers per lane
     constexpr int ITER = W / 128;       // 4 consecutive bins per lane per iteration
     constexpr int CAP  = (W >= 512) ? W / 4 : W;
-    __shared__ float s_cand[SP_WARPS + 2][CAP];
-    __shared__ float s_med[SP_WARPS + 2];
+    constexpr float SCALE = UNPACK ? 0.25f : 1.0f;       // powers are held as 4 P_k on the unpack path
+    __shared__ float s_cand[SP_WARPS + 1][CAP];
+    __shared__ float s_med[SP_WARPS + 1];
     const int row  = blockIdx.x / cta_per_row;
     const int wid  = threadIdx.x >> 5;
     const int lane = threadIdx.x & 31;
-    const int blk  = (blockIdx.x % cta_per_row) * SP_WARPS - 1 + wid;      // wid 0 and SP_WARPS+1 are halo blocks
-    const bool active = blk >= 0 && blk < nblk_per_row;
-    const bool writer = active && wid >= 1 && wid <= SP_WARPS;
+    const int blk  = (blockIdx.x % cta_per_row) * SP_WARPS + wid;     // warp SP_WARPS: the next CTA's first block
+    const bool active = blk < nblk_per_row;
+    const bool owner = active && wid < SP_WARPS;                      // writes the median and the raw powers
 
     const float2* __restrict__ Xr = X + (size_t)row * ld;
     const int base = blk * W;
@@ -357,18 +388,20 @@ k_spectrum_median(const float2* __restrict__ X, size_t ld, float* __restrict__ P
         float2 carry = make_float2(0.f, 0.f);            // X_{k-1} for lane 0 (X_{-1} = 0)
         float2 wbase = make_float2(1.f, 0.f);
         if (UNPACK) {
-            double sb, cb;
-            sincospi(-(double)base / (double)nb, &sb, &cb);      // W_N^base, N = 2 nb
-            wbase = make_float2((float)cb, (float)sb);
+            wbase = __ldg(twb + blk);                    // W_N^base, N = 2 nb
             if (base > 0 && lane == 0) {
-                double s1, c1;
-                sincospi(-(double)(base - 1) / (double)nb, &s1, &c1);
-                carry = r2c_unpack(__ldg(Xr + base - 1), __ldg(Xr + (nb - base + 1)), make_float2((float)c1, (float)s1));
+                const float2 wp = __ldg(twb + blk - 1), wl = __ldg(twn + W - 1);
+                carry = r2c_unpack2(__ldg(Xr + base - 1), __ldg(Xr + (nb - base + 1)),
+                                    make_float2(wp.x * wl.x - wp.y * wl.y, wp.x * wl.y + wp.y * wl.x));
             }
         } else if (base > 0 && lane == 0) carry = __ldg(Xr + base - 1);
 #pragma unroll
         for (int i = 0; i < ITER; ++i) {
             const int k0 = base + i * 128 + lane * 4;
+            if (i + 2 < ITER) {                          // pull the lines of iteration i+2 into L2 (no registers held)
+                asm volatile("prefetch.global.L2 [%0];" ::"l"(Xr + k0 + 256));
+                if (UNPACK) asm volatile("prefetch.global.L2 [%0];" ::"l"(Xr + (nb - k0 - 256) - 3));
+            }
             float4 a = __ldg(reinterpret_cast<const float4*>(Xr + k0));
             float4 c = __ldg(reinterpret_cast<const float4*>(Xr + k0 + 2));
             if (UNPACK) {
@@ -376,10 +409,10 @@ k_spectrum_median(const float2* __restrict__ X, size_t ld, float* __restrict__ P
                 const float2 m0 = __ldg(k0 == 0 ? Xr : zm), m1 = __ldg(zm - 1), m2 = __ldg(zm - 2), m3 = __ldg(zm - 3);
                 const float4 t01 = __ldg(reinterpret_cast<const float4*>(twn + (k0 - base)));
                 const float4 t23 = __ldg(reinterpret_cast<const float4*>(twn + (k0 - base) + 2));
-                const float2 x0 = r2c_unpack(make_float2(a.x, a.y), m0, make_float2(wbase.x * t01.x - wbase.y * t01.y, wbase.x * t01.y + wbase.y * t01.x));
-                const float2 x1 = r2c_unpack(make_float2(a.z, a.w), m1, make_float2(wbase.x * t01.z - wbase.y * t01.w, wbase.x * t01.w + wbase.y * t01.z));
-                const float2 x2 = r2c_unpack(make_float2(c.x, c.y), m2, make_float2(wbase.x * t23.x - wbase.y * t23.y, wbase.x * t23.y + wbase.y * t23.x));
-                const float2 x3 = r2c_unpack(make_float2(c.z, c.w), m3, make_float2(wbase.x * t23.z - wbase.y * t23.w, wbase.x * t23.w + wbase.y * t23.z));
+                const float2 x0 = r2c_unpack2(make_float2(a.x, a.y), m0, make_float2(wbase.x * t01.x - wbase.y * t01.y, wbase.x * t01.y + wbase.y * t01.x));
+                const float2 x1 = r2c_unpack2(make_float2(a.z, a.w), m1, make_float2(wbase.x * t01.z - wbase.y * t01.w, wbase.x * t01.w + wbase.y * t01.z));
+                const float2 x2 = r2c_unpack2(make_float2(c.x, c.y), m2, make_float2(wbase.x * t23.x - wbase.y * t23.y, wbase.x * t23.y + wbase.y * t23.x));
+                const float2 x3 = r2c_unpack2(make_float2(c.z, c.w), m3, make_float2(wbase.x * t23.z - wbase.y * t23.w, wbase.x * t23.w + wbase.y * t23.z));
                 a = make_float4(x0.x, x0.y, x1.x, x1.y);
                 c = make_float4(x2.x, x2.y, x3.x, x3.y);
             }
@@ -396,19 +429,23 @@ k_spectrum_median(const float2* __restrict__ X, size_t ld, float* __restrict__ P
             dx = a.z - a.x; dy = a.w - a.y; o.y = fmaxf(a.z * a.z + a.w * a.w, 0.5f * (dx * dx + dy * dy));
             dx = c.x - a.z; dy = c.y - a.w; o.z = fmaxf(c.x * c.x + c.y * c.y, 0.5f * (dx * dx + dy * dy));
             dx = c.z - c.x; dy = c.w - c.y; o.w = fmaxf(c.z * c.z + c.w * c.w, 0.5f * (dx * dx + dy * dy));
-            if (RAW && writer) *reinterpret_cast<float4*>(Praw + (size_t)row * (size_t)nb + k0) = o;
+            if (RAW && owner)
+                *reinterpret_cast<float4*>(Praw + (size_t)row * (size_t)nb + k0) = make_float4(SCALE * o.x, SCALE * o.y, SCALE * o.z, SCALE * o.w);
             p[4 * i + 0] = o.x; p[4 * i + 1] = o.y; p[4 * i + 2] = o.z; p[4 * i + 3] = o.w;
         }
-        m_cur = warp_median<W>(p, s_cand[wid], lane, (wid >= 1 && wid <= SP_WARPS) ? fallbacks : nullptr);
+        m_cur = warp_median<W>(p, s_cand[wid], lane, owner ? fallbacks : nullptr);
         if (lane == 0) {
             s_med[wid] = m_cur;
-            if (writer) med[(size_t)row * nblk_per_row + blk] = m_cur;
+            if (owner) med[(size_t)row * nblk_per_row + blk] = SCALE * m_cur;
         }
     }
     __syncthreads();
-    if (!writer) return;
-    const float m_prev = (blk > 0) ? s_med[wid - 1] : m_cur;                     // flat below the first centre
-    const float m_next = (blk + 1 < nblk_per_row) ? s_med[wid + 1] : m_cur;      // flat above the last centre
+    if (!active) return;
+    // first half of the block: between the previous centre and this one; second half: this and the next
+    const bool can_first  = wid > 0 || blk == 0;
+    const bool can_second = wid < SP_WARPS;
+    const float m_prev = (wid > 0) ? s_med[wid - 1] : m_cur;                                  // flat below the first centre
+    const float m_next = (wid < SP_WARPS && blk + 1 < nblk_per_row) ? s_med[wid + 1] : m_cur; // flat above the last centre
     float* __restrict__ Pr = P + (size_t)row * (size_t)nb;
     constexpr float LN2 = 0.69314718055994530942f;
     constexpr float INV_W = 1.0f / (float)W;
@@ -416,15 +453,26 @@ k_spectrum_median(const float2* __restrict__ X, size_t ld, float* __restrict__ P
     for (int i = 0; i < ITER; ++i) {
         const int e0 = i * 128 + lane * 4;               // offset of the 4 bins inside the block
         const bool second = e0 >= W / 2;
+        if (!(second ? can_second : can_first)) continue;
         const float ma = second ? m_cur : m_prev, mb = second ? m_next : m_cur;
         const float f0 = ((float)(second ? e0 - W / 2 : e0 + W / 2) + 0.5f) * INV_W;
-        const float dm = (mb - ma);
+        const float st = (mb - ma) * INV_W;              // baseline step per bin
+        const float b0 = fmaf(f0, mb - ma, ma);          // baseline at the first of the 4 bins
+        const float b2 = fmaf(2.0f, st, b0);
         float4 o;
-        float* ov = reinterpret_cast<float*>(&o);
+        if (b0 > 0.f && b2 + st > 0.f && fminf(ma, mb) > 0.f) {
+            // two reciprocals per four bins; the odd bins use 1/(m + st) = (1/m)(1 - st/m) + O((st/m)^2),
+            // st/m < 2^-10 |mb - ma| / m: relative error < 1e-6 for baseline ratios up to 2
+            const float r0 = __fdividef(LN2, b0), r2 = __fdividef(LN2, b2);
+            const float r1 = r0 * (1.0f - st * r0 * (1.0f / LN2)), r3 = r2 * (1.0f - st * r2 * (1.0f / LN2));
+            o = make_float4(p[4 * i] * r0, p[4 * i + 1] * r1, p[4 * i + 2] * r2, p[4 * i + 3] * r3);
+        } else {
+            float* ov = reinterpret_cast<float*>(&o);
 #pragma unroll
-        for (int q = 0; q < 4; ++q) {
-            const float m = fmaf(f0 + (float)q * INV_W, dm, ma);
-            ov[q] = (m > 0.f) ? __fdividef(p[4 * i + q] * LN2, m) : 0.f;
+            for (int q = 0; q < 4; ++q) {
+                const float m = fmaf((float)q, st, b0);
+                ov[q] = (m > 0.f) ? __fdividef(p[4 * i + q] * LN2, m) : 0.f;
+            }
         }
         if (base + e0 == 0) o.x = 0.f;                   // P^_0 = 0
         *reinterpret_cast<float4*>(Pr + base + e0) = o;
@@ -623,66 +671,93 @@ __device__ __forceinline__ void hs_check(const float (&acc)[16], uint32_t kq, co
     if (__any_sync(0xffffffffu, any)) hs_emit<L>(acc, kq, fp, tid, out, cursor, capacity);
 }
 
+// issue the 14 bulk copies of one tile's regions into `sm`, completion on `bar` (one thread)
+__device__ __forceinline__ void hs_stage(float* sm, const float* __restrict__ p, int k0, uint64_t* bar)
+{
+    mbar_expect_tx(bar, (uint32_t)(HS_SMEM_FLOATS * sizeof(float)));
+#pragma unroll
+    for (int L = 2; L <= 4; ++L)
+#pragma unroll
+        for (int m = 1; m < (1 << L); m += 2)
+            bulk_g2s(sm + hs_off(L, m), p + (((size_t)m * (size_t)k0) >> L), (uint32_t)(hs_len(L, m) * sizeof(float)), bar);
+}
+
+struct HsDirect {                                    // folds 0 and 1 of one thread's 16 bins, from global memory
+    float4 a0, a1, a2, a3, h0, h1;
+    float  h2;
+};
+__device__ __forceinline__ HsDirect hs_load_direct(const float* __restrict__ p, uint32_t kq)
+{
+    HsDirect d;
+    const float4* a = reinterpret_cast<const float4*>(p + kq);
+    d.a0 = __ldg(a); d.a1 = __ldg(a + 1); d.a2 = __ldg(a + 2); d.a3 = __ldg(a + 3);
+    const float* h = p + (kq >> 1);
+    d.h0 = __ldg(reinterpret_cast<const float4*>(h));
+    d.h1 = __ldg(reinterpret_cast<const float4*>(h) + 1);
+    d.h2 = __ldg(h + 8);
+    return d;
+}
+
+// A CTA walks `tpc` consecutive tiles of one template with two staging buffers: while tile t is
+// summed out of one buffer the bulk copies of tile t+1 land in the other, and the fold-0/1
+// values of tile t+1 are already on their way to registers, so no warp waits on memory once the
+// first tile is in (the single-buffered version spent 2/3 of its issue slots waiting).
 __global__ void __launch_bounds__(HS_THREADS)
-k_hsum_tile(const float* __restrict__ Ph, int nb, int tiles_per_row, FoldParams fp, uint32_t first_id,
+k_hsum_tile(const float* __restrict__ Ph, int nb, int groups_per_row, int tpc, FoldParams fp, uint32_t first_id,
             Candidate* __restrict__ out, unsigned long long* __restrict__ cursor, unsigned long long capacity)
 {
-    extern __shared__ __align__(16) float hs_sm[];
-    __shared__ __align__(8) uint64_t bar;
-    const int row = blockIdx.x / tiles_per_row;
-    const int k0  = (blockIdx.x % tiles_per_row) * HS_T;
+    extern __shared__ __align__(16) float hs_sm[];   // two buffers of HS_SMEM_FLOATS
+    __shared__ __align__(8) uint64_t bar[2];
+    const int row   = blockIdx.x / groups_per_row;
+    const int tile0 = (blockIdx.x % groups_per_row) * tpc;
     const float* __restrict__ p = Ph + (size_t)row * (size_t)nb;
     const uint32_t tid = first_id + (uint32_t)row;
-
-    if (threadIdx.x == 0) mbar_init(&bar, 1);
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        mbar_expect_tx(&bar, (uint32_t)(HS_SMEM_FLOATS * sizeof(float)));
-#pragma unroll
-        for (int L = 2; L <= 4; ++L)
-#pragma unroll
-            for (int m = 1; m < (1 << L); m += 2)
-                bulk_g2s(hs_sm + hs_off(L, m), p + (((size_t)m * (size_t)k0) >> L), (uint32_t)(hs_len(L, m) * sizeof(float)), &bar);
-    }
-
     const int q = threadIdx.x;
-    const uint32_t kq = (uint32_t)(k0 + 16 * q);
-    float acc[16];
-#pragma unroll
-    for (int i = 0; i < 4; ++i) {                    // fold 0: the bin itself
-        const float4 t = __ldg(reinterpret_cast<const float4*>(p + kq) + i);
-        acc[4 * i] = t.x; acc[4 * i + 1] = t.y; acc[4 * i + 2] = t.z; acc[4 * i + 3] = t.w;
-    }
-    hs_check<0>(acc, kq, fp, tid, out, cursor, capacity);
-    {                                                // fold 1: + P^[(k+1)>>1], 9 values from 8 q'
-        const float* h = p + (kq >> 1);
-        const float4 a = __ldg(reinterpret_cast<const float4*>(h));
-        const float4 b = __ldg(reinterpret_cast<const float4*>(h) + 1);
-        const float  c = __ldg(h + 8);
-        const float v[9] = {a.x, a.y, a.z, a.w, b.x, b.y, b.z, b.w, c};
-#pragma unroll
-        for (int r = 0; r < 16; ++r) acc[r] += v[(r + 1) >> 1];
-    }
-    hs_check<1>(acc, kq, fp, tid, out, cursor, capacity);
 
-    mbar_wait(&bar, 0);
-    hs_accumulate<2, 1>(hs_sm, q, acc);
-    hs_accumulate<2, 3>(hs_sm, q, acc);
-    hs_check<2>(acc, kq, fp, tid, out, cursor, capacity);
-    hs_accumulate<3, 1>(hs_sm, q, acc);
-    hs_accumulate<3, 3>(hs_sm, q, acc);
-    hs_accumulate<3, 5>(hs_sm, q, acc);
-    hs_accumulate<3, 7>(hs_sm, q, acc);
-    hs_check<3>(acc, kq, fp, tid, out, cursor, capacity);
-    hs_accumulate<4, 1>(hs_sm, q, acc);
-    hs_accumulate<4, 3>(hs_sm, q, acc);
-    hs_accumulate<4, 5>(hs_sm, q, acc);
-    hs_accumulate<4, 7>(hs_sm, q, acc);
-    hs_accumulate<4, 9>(hs_sm, q, acc);
-    hs_accumulate<4, 11>(hs_sm, q, acc);
-    hs_accumulate<4, 13>(hs_sm, q, acc);
-    hs_accumulate<4, 15>(hs_sm, q, acc);
-    hs_check<4>(acc, kq, fp, tid, out, cursor, capacity);
+    if (threadIdx.x == 0) { mbar_init(&bar[0], 1); mbar_init(&bar[1], 1); }
+    __syncthreads();
+    if (threadIdx.x == 0) hs_stage(hs_sm, p, tile0 * HS_T, &bar[0]);
+    HsDirect nxt = hs_load_direct(p, (uint32_t)(tile0 * HS_T + 16 * q));
+
+    for (int t = 0; t < tpc; ++t) {
+        const int k0 = (tile0 + t) * HS_T;
+        const uint32_t kq = (uint32_t)(k0 + 16 * q);
+        const float* sm = hs_sm + (t & 1) * HS_SMEM_FLOATS;
+        if (t + 1 < tpc && threadIdx.x == 0)         // the other buffer was released by the barrier that ended tile t-1
+            hs_stage(hs_sm + ((t + 1) & 1) * HS_SMEM_FLOATS, p, k0 + HS_T, &bar[(t + 1) & 1]);
+        const HsDirect d = nxt;
+        if (t + 1 < tpc) nxt = hs_load_direct(p, kq + HS_T);
+
+        float acc[16] = {d.a0.x, d.a0.y, d.a0.z, d.a0.w, d.a1.x, d.a1.y, d.a1.z, d.a1.w,
+                         d.a2.x, d.a2.y, d.a2.z, d.a2.w, d.a3.x, d.a3.y, d.a3.z, d.a3.w};   // fold 0: the bin itself
+        hs_check<0>(acc, kq, fp, tid, out, cursor, capacity);
+        {                                            // fold 1: + P^[(k+1)>>1], 9 values from 8 q'
+            const float v[9] = {d.h0.x, d.h0.y, d.h0.z, d.h0.w, d.h1.x, d.h1.y, d.h1.z, d.h1.w, d.h2};
+#pragma unroll
+            for (int r = 0; r < 16; ++r) acc[r] += v[(r + 1) >> 1];
+        }
+        hs_check<1>(acc, kq, fp, tid, out, cursor, capacity);
+
+        mbar_wait(&bar[t & 1], (uint32_t)((t >> 1) & 1));
+        hs_accumulate<2, 1>(sm, q, acc);
+        hs_accumulate<2, 3>(sm, q, acc);
+        hs_check<2>(acc, kq, fp, tid, out, cursor, capacity);
+        hs_accumulate<3, 1>(sm, q, acc);
+        hs_accumulate<3, 3>(sm, q, acc);
+        hs_accumulate<3, 5>(sm, q, acc);
+        hs_accumulate<3, 7>(sm, q, acc);
+        hs_check<3>(acc, kq, fp, tid, out, cursor, capacity);
+        hs_accumulate<4, 1>(sm, q, acc);
+        hs_accumulate<4, 3>(sm, q, acc);
+        hs_accumulate<4, 5>(sm, q, acc);
+        hs_accumulate<4, 7>(sm, q, acc);
+        hs_accumulate<4, 9>(sm, q, acc);
+        hs_accumulate<4, 11>(sm, q, acc);
+        hs_accumulate<4, 13>(sm, q, acc);
+        hs_accumulate<4, 15>(sm, q, acc);
+        hs_check<4>(acc, kq, fp, tid, out, cursor, capacity);
+        __syncthreads();                             // every thread is done with buffer t&1: it may be refilled
+    }
 }
 
 // fp64 sum of a device series (fill value when the series is borrowed device memory)
