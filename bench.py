@@ -302,7 +302,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--log2n", type=int, default=23)
     ap.add_argument("--chunk", type=int, default=0)
-    ap.add_argument("--fft-path", type=int, default=0, help="tb_plan_opts.fft_path (0 auto, 1 cuFFT, 2 own fused, 3 own unfused)")
+    ap.add_argument("--fft-path", type=int, default=0, help="tb_plan_opts.fft_path (0 auto, 1 cuFFT, 2 hand-written or error)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
 

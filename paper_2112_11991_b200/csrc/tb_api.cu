@@ -61,8 +61,7 @@ struct tb_plan {
     bool staged_pending = false;
 
     // hand-written FFT path (tb_fft.cuh): M = N/2 = M1 * M2
-    bool own_fft = false, unfused = false;
-    float2* d_T = nullptr;
+    bool own_fft = false;
     int log2m1 = 0, log2m2 = 0;
     SegRec* d_seg = nullptr;                         // [chunk][n >> MIN_LOG2H]
     size_t seg_stride = 0;
@@ -263,50 +262,30 @@ int get_fft_plan(tb_plan* p, uint32_t batch, cufftHandle* out)
 constexpr int OWN_MIN_LOG2H = 3;                     // the fused path needs >= 2 samples per segment; 8 bounds the table
 
 template <int W>
-void launch_spectrum(tb_plan* p, uint32_t nt, bool unpack, float* d_raw)
+void launch_spectrum(tb_plan* p, uint32_t nt, float* d_raw)
 {
     const int cta_per_row = (int)((p->nblk + SP_WARPS - 1) / SP_WARPS);
     const unsigned grid = (unsigned)(cta_per_row * nt), threads = (SP_WARPS + 1) * 32;
-    const float2* in = p->d_fft;
-    const size_t ld = unpack ? (size_t)p->nb : p->ld;
-    const float2 *tw = unpack ? p->d_twn : nullptr, *tb = unpack ? p->d_twb : nullptr;
     unsigned long long* fb = p->d_cursor + 1;
     const int nb = (int)p->nb, nblk = (int)p->nblk;
-    if (unpack && d_raw)       k_spectrum_median<W, true, true><<<grid, threads, 0, p->stream>>>(in, ld, p->d_power, p->d_med, nb, nblk, cta_per_row, tw, tb, fb, d_raw);
-    else if (unpack)           k_spectrum_median<W, true, false><<<grid, threads, 0, p->stream>>>(in, ld, p->d_power, p->d_med, nb, nblk, cta_per_row, tw, tb, fb, nullptr);
-    else if (d_raw)            k_spectrum_median<W, false, true><<<grid, threads, 0, p->stream>>>(in, ld, p->d_power, p->d_med, nb, nblk, cta_per_row, tw, tb, fb, d_raw);
-    else                       k_spectrum_median<W, false, false><<<grid, threads, 0, p->stream>>>(in, ld, p->d_power, p->d_med, nb, nblk, cta_per_row, tw, tb, fb, nullptr);
+    if (d_raw) k_spectrum_median<W, false, true><<<grid, threads, 0, p->stream>>>(p->d_fft, p->ld, p->d_power, p->d_med, nb, nblk, cta_per_row, nullptr, nullptr, fb, d_raw);
+    else       k_spectrum_median<W, false, false><<<grid, threads, 0, p->stream>>>(p->d_fft, p->ld, p->d_power, p->d_med, nb, nblk, cta_per_row, nullptr, nullptr, fb, nullptr);
 }
 
 // ---- hand-written FFT path -------------------------------------------------------------------
-template <int R1> constexpr int fft_bundle() { return R1 >= 8 ? 4 : 8; }       // C (pass 1) and R (pass 2)
-template <int R1> constexpr size_t fft_smem() { return (size_t)(fft_bundle<R1>() * (R1 * FFT_PA + 16 / fft_bundle<R1>()) + 256) * sizeof(float2); }
-
-template <int R1>
-int launch_cols_unfused(tb_plan* p, uint32_t nt)
-{
-    constexpr int C = fft_bundle<R1>();
-    auto kern = k_fft_cols<R1, C, false, false>;
-    static bool attr = false;
-    if (!attr) { TB_CUDA(p, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_smem<R1>())); attr = true; }
-    const unsigned grid = (unsigned)(((1u << p->log2m2) / C) * nt);
-    kern<<<grid, FFT_THREADS, fft_smem<R1>(), p->stream>>>(p->d_resampled, nullptr, 0, p->d_tmpl, (int)nt, (int)p->n, p->log2m2,
-                                                          p->fill, p->d_tw1a, p->d_tw2, p->d_T, nullptr, nullptr);
-    TB_CUDA(p, cudaGetLastError());
-    return TB_OK;
-}
+constexpr int FFT_C = 16;                            // columns per CTA of pass 1 (runs of 32 samples / 128 bytes)
+template <int R1> constexpr size_t cols_smem() { return (size_t)(FFT_C * (R1 * FFT_PA + 16 / FFT_C) + 256) * sizeof(float2); }
 
 template <int R1, bool DEBUG>
 int launch_cols(tb_plan* p, size_t off, uint32_t nt, long long* d_idx, float* d_y)
 {
-    constexpr int C = fft_bundle<R1>();
-    auto kern = k_fft_cols<R1, C, DEBUG, true>;
+    auto kern = k_fft_cols<R1, FFT_C, DEBUG>;
     static bool attr = false;
-    if (!attr) { TB_CUDA(p, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_smem<R1>())); attr = true; }
-    const unsigned grid = (unsigned)(((1u << p->log2m2) / C) * nt);
-    kern<<<grid, FFT_THREADS, fft_smem<R1>(), p->stream>>>(p->d_series, p->d_seg, p->seg_stride, p->d_tmpl + off, (int)nt,
-                                                          (int)p->n, p->log2m2, p->fill, p->d_tw1a, p->d_tw2,
-                                                          p->unfused ? p->d_T : reinterpret_cast<float2*>(p->d_resampled), d_idx, d_y);
+    if (!attr) { TB_CUDA(p, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cols_smem<R1>())); attr = true; }
+    const unsigned grid = (unsigned)(((1u << p->log2m2) / FFT_C) * nt);
+    kern<<<grid, FFT_THREADS, cols_smem<R1>(), p->stream>>>(p->d_series, p->d_seg, p->seg_stride, p->d_tmpl + off, (int)nt,
+                                                           (int)p->n, p->log2m2, p->fill, p->d_tw1a, p->d_tw2,
+                                                           reinterpret_cast<float2*>(p->d_resampled), d_idx, d_y);
     TB_CUDA(p, cudaGetLastError());
     return TB_OK;
 }
@@ -314,13 +293,13 @@ int launch_cols(tb_plan* p, size_t off, uint32_t nt, long long* d_idx, float* d_
 template <int R1>
 int launch_rows(tb_plan* p, uint32_t nt)
 {
-    constexpr int R = fft_bundle<R1>();
-    auto kern = k_fft_rows<R1, R>;
+    using Cfg = RowsCfg<R1>;
+    auto kern = k_fft_rows_t<R1>;
     static bool attr = false;
-    if (!attr) { TB_CUDA(p, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_smem<R1>())); attr = true; }
-    const unsigned grid = (unsigned)(((1u << p->log2m1) / R) * nt);
-    kern<<<grid, FFT_THREADS, fft_smem<R1>(), p->stream>>>(p->unfused ? p->d_T : reinterpret_cast<const float2*>(p->d_resampled), p->d_fft,
-                                                          p->log2m1, p->d_tw1b, p->d_tw2);
+    if (!attr) { TB_CUDA(p, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM)); attr = true; }
+    const unsigned grid = (unsigned)(((1u << p->log2m1) / Cfg::R) * nt);
+    kern<<<grid, FFT_THREADS, Cfg::SMEM, p->stream>>>(reinterpret_cast<const float2*>(p->d_resampled), p->d_fft, p->log2m1,
+                                                     p->d_tw1b, p->d_tw2);
     TB_CUDA(p, cudaGetLastError());
     return TB_OK;
 }
@@ -336,19 +315,6 @@ int run_own_pass1(tb_plan* p, size_t off, uint32_t nt, long long* d_idx, float* 
     switch (p->log2m1 - 8) {
         case 0: return dbg ? launch_cols<1, true>(p, off, nt, d_idx, d_y) : launch_cols<1, false>(p, off, nt, nullptr, nullptr);
         case 1: return dbg ? launch_cols<2, true>(p, off, nt, d_idx, d_y) : launch_cols<2, false>(p, off, nt, nullptr, nullptr);
-        case 2: return dbg ? launch_cols<4, true>(p, off, nt, d_idx, d_y) : launch_cols<4, false>(p, off, nt, nullptr, nullptr);
-        case 3: return dbg ? launch_cols<8, true>(p, off, nt, d_idx, d_y) : launch_cols<8, false>(p, off, nt, nullptr, nullptr);
-    }
-    return fail(p, TB_ERR_INVALID_ARG, "unsupported M1");
-}
-
-int run_unfused_pass1(tb_plan* p, uint32_t nt)
-{
-    switch (p->log2m1 - 8) {
-        case 0: return launch_cols_unfused<1>(p, nt);
-        case 1: return launch_cols_unfused<2>(p, nt);
-        case 2: return launch_cols_unfused<4>(p, nt);
-        case 3: return launch_cols_unfused<8>(p, nt);
     }
     return fail(p, TB_ERR_INVALID_ARG, "unsupported M1");
 }
@@ -360,8 +326,43 @@ int run_own_pass2(tb_plan* p, uint32_t nt)
         case 1: return launch_rows<2>(p, nt);
         case 2: return launch_rows<4>(p, nt);
         case 3: return launch_rows<8>(p, nt);
+        case 4: return launch_rows<16>(p, nt);
+        case 5: return launch_rows<32>(p, nt);
     }
     return fail(p, TB_ERR_INVALID_ARG, "unsupported M2");
+}
+
+template <int W>
+int launch_spectrum_t(tb_plan* p, uint32_t nt, float* d_raw)
+{
+    const size_t smem = st_smem_bytes(W, p->log2m1);
+    const unsigned grid = (unsigned)((p->nblk / 16) * nt);
+    unsigned long long* fb = p->d_cursor + 1;
+    if (d_raw) {
+        auto kern = k_spectrum_t<W, true>;
+        TB_CUDA(p, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)st_smem_bytes(W, 8)));
+        kern<<<grid, ST_THREADS, smem, p->stream>>>(p->d_fft, p->d_power, p->d_med, p->log2m1, p->log2m2, (int)p->nblk,
+                                                   p->d_twn, p->d_twb, fb, d_raw);
+    } else {
+        auto kern = k_spectrum_t<W, false>;
+        static bool attr = false;
+        if (!attr) { TB_CUDA(p, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)st_smem_bytes(W, 8))); attr = true; }
+        kern<<<grid, ST_THREADS, smem, p->stream>>>(p->d_fft, p->d_power, p->d_med, p->log2m1, p->log2m2, (int)p->nblk,
+                                                   p->d_twn, p->d_twb, fb, nullptr);
+    }
+    TB_CUDA(p, cudaGetLastError());
+    return TB_OK;
+}
+
+int run_spectrum_t(tb_plan* p, uint32_t nt, float* d_raw = nullptr)
+{
+    switch (p->window) {
+        case 256: return launch_spectrum_t<256>(p, nt, d_raw);
+        case 512: return launch_spectrum_t<512>(p, nt, d_raw);
+        case 1024: return launch_spectrum_t<1024>(p, nt, d_raw);
+        case 2048: return launch_spectrum_t<2048>(p, nt, d_raw);
+    }
+    return fail(p, TB_ERR_INVALID_ARG, "median_window");
 }
 
 // twiddle tables of the hand-written FFT, in long double, rounded once to fp32
@@ -386,18 +387,18 @@ int make_twiddles(tb_plan* p)
     int rc;
     if ((rc = tw1(p->log2m1, &p->d_tw1a))) return rc;
     if ((rc = tw1(p->log2m2, &p->d_tw1b))) return rc;
-    std::vector<float2> h2(256), hn(p->window), hb(p->nblk);
+    std::vector<float2> h2(256), hn((size_t)1 << p->log2m1), hb((size_t)1 << p->log2m2);
     for (int kb = 0; kb < 16; ++kb)
         for (int c = 0; c < 16; ++c) {
             const long double a = -two_pi * (long double)(kb * c) / 256.0L;
             h2[kb * 16 + c] = make_float2((float)cosl(a), (float)sinl(a));
         }
-    for (uint32_t i = 0; i < p->window; ++i) {
+    for (size_t i = 0; i < hn.size(); ++i) {             // R2C twiddle W_N^k = W_N^{k1} * W_N^{M1 k2}
         const long double a = -two_pi * (long double)i / (long double)p->n;
         hn[i] = make_float2((float)cosl(a), (float)sinl(a));
     }
-    for (uint32_t b = 0; b < p->nblk; ++b) {             // W_N^{b W}: the R2C twiddle at the start of median block b
-        const long double a = -two_pi * (long double)((uint64_t)b * p->window) / (long double)p->n;
+    for (size_t b = 0; b < hb.size(); ++b) {
+        const long double a = -two_pi * (long double)((uint64_t)b << p->log2m1) / (long double)p->n;
         hb[b] = make_float2((float)cosl(a), (float)sinl(a));
     }
     if ((rc = upload(h2, &p->d_tw2))) return rc;
@@ -429,14 +430,14 @@ int run_fft(tb_plan* p, uint32_t nt)
     return TB_OK;
 }
 
-int run_spectrum(tb_plan* p, uint32_t nt, bool unpack, float* d_raw = nullptr)
+int run_spectrum(tb_plan* p, uint32_t nt, float* d_raw = nullptr)
 {
     switch (p->window) {
-        case 128: launch_spectrum<128>(p, nt, unpack, d_raw); break;
-        case 256: launch_spectrum<256>(p, nt, unpack, d_raw); break;
-        case 512: launch_spectrum<512>(p, nt, unpack, d_raw); break;
-        case 1024: launch_spectrum<1024>(p, nt, unpack, d_raw); break;
-        case 2048: launch_spectrum<2048>(p, nt, unpack, d_raw); break;
+        case 128: launch_spectrum<128>(p, nt, d_raw); break;
+        case 256: launch_spectrum<256>(p, nt, d_raw); break;
+        case 512: launch_spectrum<512>(p, nt, d_raw); break;
+        case 1024: launch_spectrum<1024>(p, nt, d_raw); break;
+        case 2048: launch_spectrum<2048>(p, nt, d_raw); break;
         default: return fail(p, TB_ERR_INVALID_ARG, "median_window");
     }
     TB_CUDA(p, cudaGetLastError());
@@ -538,7 +539,7 @@ void destroy(tb_plan* p)
     for (auto& kv : p->fft_plans) cufftDestroy(kv.second);
     for (auto& es : p->events) for (auto& e : es.e) cudaEventDestroy(e);
     if (p->ev_staged) cudaEventDestroy(p->ev_staged);
-    cudaFree(p->d_T); cudaFree(p->d_seg); cudaFree(p->d_tw1a); cudaFree(p->d_tw1b); cudaFree(p->d_tw2); cudaFree(p->d_twn); cudaFree(p->d_twb);
+    cudaFree(p->d_seg); cudaFree(p->d_tw1a); cudaFree(p->d_tw1b); cudaFree(p->d_tw2); cudaFree(p->d_twn); cudaFree(p->d_twb);
     cudaFree(p->d_work); cudaFree(p->d_acc); cudaFree(p->d_series_owned); cudaFree(p->d_resampled); cudaFree(p->d_fft);
     cudaFree(p->d_power); cudaFree(p->d_med); cudaFree(p->d_cand); cudaFree(p->d_cursor); cudaFree(p->d_tmpl);
     if (p->h_tmpl) cudaFreeHost(p->h_tmpl);
@@ -648,22 +649,21 @@ int tb_plan_create(tb_plan** out, const float* series, uint64_t n_samples, doubl
     { int rc = load_series(p, series); if (rc) { destroy(p); return rc; } }
     pin_series_in_l2(p);
 
-    // FFT path: hand-written two-pass FFT for 2^17 <= N <= 2^23, batched cuFFT otherwise
+    // FFT path: hand-written two-pass FFT (M = N/2 = M1 * M2, M1 = 512, or 256 at 2^17) when
+    // 2^17 <= N <= 2^23, W >= M1 and the median blocks pair up in groups of 16; batched cuFFT otherwise
     {
         const int lm = (int)ilog2(p->nb);
-        p->log2m1 = lm / 2;
+        p->log2m1 = lm >= 17 ? 9 : 8;
         p->log2m2 = lm - p->log2m1;
-        const bool fits = p->log2m1 >= 8 && p->log2m2 <= 11;
+        const bool fits = p->log2m2 >= 8 && p->log2m2 <= 13 && W >= (1u << p->log2m1) && p->nblk >= 16 && p->nblk % 16 == 0;
         if (o.fft_path >= 2 && !fits) { destroy(p); return TB_ERR_INVALID_ARG; }
         p->own_fft = fits && o.fft_path != 1;
-        p->unfused = p->own_fft && o.fft_path == 3;
     }
     if (p->own_fft) {
         p->seg_stride = (size_t)(p->n >> OWN_MIN_LOG2H);
         TB_TRY(cudaMalloc(&p->d_seg, (size_t)B * p->seg_stride * sizeof(SegRec)));
         int rc = make_twiddles(p);
         if (rc) { destroy(p); return rc; }
-        if (p->unfused) TB_TRY(cudaMalloc(&p->d_T, (size_t)B * p->nb * sizeof(float2)));
     }
     TB_TRY(cudaMalloc(&p->d_resampled, (size_t)B * p->n * sizeof(float)));
     TB_TRY(cudaMalloc(&p->d_fft, (size_t)B * p->ld * sizeof(float2)));
@@ -750,24 +750,20 @@ int tb_search_templates(tb_plan* p, const tb_template* tmpl, uint64_t n_template
             es = &p->events[p->events_used++];
             TB_CUDA(p, cudaEventRecord(es->e[0], p->stream));
         }
-        if (own && p->unfused) {                         // experiment: k_resample | P1 without gather, P2
-            if ((rc = run_resample(p, off, nt, nullptr))) return rc;
-            if (es) TB_CUDA(p, cudaEventRecord(es->e[1], p->stream));
-            if ((rc = run_unfused_pass1(p, nt))) return rc;
-            if ((rc = run_own_pass2(p, nt))) return rc;
-            p->last.n_kernel_launches += 2;
-        } else if (own) {                                // K0 + P1 | P2 | unpack + spectrum + median
+        if (own) {                                       // K0 + P1 | P2 | transpose + unpack + spectrum + median + normalise
             if ((rc = run_own_pass1(p, off, nt, nullptr, nullptr))) return rc;
             if (es) TB_CUDA(p, cudaEventRecord(es->e[1], p->stream));
             if ((rc = run_own_pass2(p, nt))) return rc;
+            if (es) TB_CUDA(p, cudaEventRecord(es->e[2], p->stream));
+            if ((rc = run_spectrum_t(p, nt))) return rc;
             p->last.n_kernel_launches += 2;
         } else {
             if ((rc = run_resample(p, off, nt, nullptr))) return rc;
             if (es) TB_CUDA(p, cudaEventRecord(es->e[1], p->stream));
             if ((rc = run_fft(p, nt))) return rc;
+            if (es) TB_CUDA(p, cudaEventRecord(es->e[2], p->stream));
+            if ((rc = run_spectrum(p, nt))) return rc;
         }
-        if (es) TB_CUDA(p, cudaEventRecord(es->e[2], p->stream));
-        if ((rc = run_spectrum(p, nt, own))) return rc;
         if (es) TB_CUDA(p, cudaEventRecord(es->e[3], p->stream));
         if (es) TB_CUDA(p, cudaEventRecord(es->e[4], p->stream));   // a7 is fused into the spectrum kernel
         if ((rc = run_hsum(p, nt, fp, first_template_id + (uint32_t)off))) return rc;
@@ -902,7 +898,7 @@ int tb_debug_spectrum(tb_plan* p, const tb_template* tmpl, float* p_interbinned,
     }
     float* d_raw = nullptr;
     TB_CUDA(p, cudaMalloc(&d_raw, p->nb * sizeof(float)));
-    rc = run_spectrum(p, 1, own, d_raw);
+    rc = own ? run_spectrum_t(p, 1, d_raw) : run_spectrum(p, 1, d_raw);
     cudaError_t e = cudaSuccess;
     if (!rc && p_interbinned) e = cudaMemcpyAsync(p_interbinned, d_raw, p->nb * sizeof(float), cudaMemcpyDeviceToHost, p->stream);
     if (!rc && e == cudaSuccess && medians)

@@ -10,15 +10,19 @@
 //
 //   K0  k_delay_segments  exact (value, slope) knots of the delay every h samples -> one cubic
 //                         Hermite record per segment (fp64 + an fp32 copy with a safety margin)
-//   P1  k_fft_cols        per CTA a bundle of C columns j2: gathers z straight from the series
-//                         (the resampled series is never written), M1-point FFTs in shared
-//                         memory, times W_M^{j2 k1}, writes T[k1][j2]            (4N bytes out)
-//   P2  k_fft_rows        per CTA R rows k1: M2-point FFTs, writes Z[k1 + M1 k2] (4N in, 4N out)
-//   the R2C unpack X_k = E_k + W_N^k O_k is fused into the spectrum former (tb_kernels.cuh).
+//   P1  k_fft_cols        per CTA a bundle of C = 16 columns j2 (M1 = 512 rows, 256 at 2^17):
+//                         gathers z straight from the series in runs of 32 samples (the
+//                         resampled series is never written), M1-point FFTs in shared memory,
+//                         times W_M^{j2 k1}, writes T[k1][j2] in 128-byte runs   (4N bytes out)
+//   P2  k_fft_rows_t      per CTA R rows k1: M2-point FFTs (M2 = 256..8192), writes the
+//                         TRANSPOSED spectrum Zt[k1][k2] (bin k = k1 + M1 k2), so that both its
+//                         loads and its stores are fully contiguous              (4N in, 4N out)
+//   the transposition back to bin order and the R2C unpack X_k = E_k + W_N^k O_k are fused into
+//   the spectrum former k_spectrum_t (below), which reads Zt in runs of >= 128 bytes.
 //
-// In-CTA FFT of length L = R1*256 (R1 in {1,2,4,8}): three in-place steps over a 3-D view
-// [a < R1][b < 16][c < 16] of the data, physical index a*272 + b*17 + c (pitch 17 on the unit
-// stride axis makes all three access patterns bank-conflict free for 64-bit elements):
+// In-CTA FFT of length L = R1*256 (R1 in {1,...,32}): three in-place steps over a 3-D view
+// [a < R1][b < 16][c < 16] of the data, physical index a*PA + b*PB + c (the pitches are chosen per
+// kernel so that all three access patterns are bank-conflict free for 64-bit elements):
 //   step 1 over a (radix R1, fused with the global load), twiddle W_L^{(16b+c) ka}
 //   step 2 over b (radix 16),                              twiddle W_256^{c kb}
 //   step 3 over c (radix 16, fused with the global store); output k = ka + R1 kb + 16 R1 kc.
@@ -105,19 +109,47 @@ template <> __device__ __forceinline__ void fft_reg<16>(float2 (&v)[16])
     for (int i = 0; i < 16; ++i) v[i] = o[i];
 }
 
+template <> __device__ __forceinline__ void fft_reg<32>(float2 (&v)[32])
+{
+    // decimation in frequency: u_i = v_i + v_{i+16}, d_i = (v_i - v_{i+16}) W32^i;
+    // X[2k] = FFT16(u)[k], X[2k+1] = FFT16(d)[k]
+    constexpr float C32[16] = {1.0f, 0.98078528040323044913f, 0.92387953251128675613f, 0.83146961230254523708f,
+                               0.70710678118654752440f, 0.55557023301960222474f, 0.38268343236508977173f,
+                               0.19509032201612826785f, 0.0f, -0.19509032201612826785f, -0.38268343236508977173f,
+                               -0.55557023301960222474f, -0.70710678118654752440f, -0.83146961230254523708f,
+                               -0.92387953251128675613f, -0.98078528040323044913f};
+    constexpr float S32[16] = {0.0f, 0.19509032201612826785f, 0.38268343236508977173f, 0.55557023301960222474f,
+                               0.70710678118654752440f, 0.83146961230254523708f, 0.92387953251128675613f,
+                               0.98078528040323044913f, 1.0f, 0.98078528040323044913f, 0.92387953251128675613f,
+                               0.83146961230254523708f, 0.70710678118654752440f, 0.55557023301960222474f,
+                               0.38268343236508977173f, 0.19509032201612826785f};
+    float2 u[16], d[16];
+#pragma unroll
+    for (int i = 0; i < 16; ++i) {
+        u[i] = cadd(v[i], v[i + 16]);
+        const float2 t = csub(v[i], v[i + 16]);
+        d[i] = (i == 0) ? t : (i == 8) ? mul_mi(t) : cmul(t, make_float2(C32[i], -S32[i]));
+    }
+    fft_reg<16>(u);
+    fft_reg<16>(d);
+#pragma unroll
+    for (int k = 0; k < 16; ++k) { v[2 * k] = u[k]; v[2 * k + 1] = d[k]; }
+}
+
 // step 2 of the in-CTA FFT for one slot: work item w in [0, 16 R1): (ka, c) = (w >> 4, w & 15)
+template <int PA, int PB>
 __device__ __forceinline__ void fft_step2(float2* __restrict__ slot, int w, const float2* __restrict__ tw2)
 {
     const int c = w & 15;
-    float2* p = slot + (w >> 4) * FFT_PA + c;
+    float2* p = slot + (w >> 4) * PA + c;
     float2 v[16];
 #pragma unroll
-    for (int b = 0; b < 16; ++b) v[b] = p[b * FFT_PB];
+    for (int b = 0; b < 16; ++b) v[b] = p[b * PB];
     fft_reg<16>(v);
 #pragma unroll
     for (int kb = 1; kb < 16; ++kb) v[kb] = cmul(v[kb], tw2[kb * 16 + c]);
 #pragma unroll
-    for (int kb = 0; kb < 16; ++kb) p[kb * FFT_PB] = v[kb];
+    for (int kb = 0; kb < 16; ++kb) p[kb * PB] = v[kb];
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -187,24 +219,24 @@ __device__ __forceinline__ int2 source_pair(const SegRec* __restrict__ segs, int
 // ---------------------------------------------------------------------------------------------
 // P1  gather + column FFTs.  CTA = C columns [c0, c0+C) of template b, all M1 = R1*256 rows.
 //   blockIdx.x = bundle * n_tmpl + b (template fastest: co-resident CTAs gather from the same
-//   stretch of the series, which stays in L2).
+//   stretch of the series, which stays in L2).  A row of the CTA's tile is a run of 2C
+//   consecutive output samples: with C = 16 one 128-byte stretch of the series (shifted by the
+//   delay) and one segment record serve 16 threads.
 // ---------------------------------------------------------------------------------------------
-template <int R1, int C, bool DEBUG, bool GATHER>
+template <int R1, int C, bool DEBUG>
 __global__ void __launch_bounds__(FFT_THREADS, 3)
 k_fft_cols(const float* __restrict__ x, const SegRec* __restrict__ seg, size_t seg_stride,
            const TmplDev* __restrict__ tmpl, int n_tmpl, int n, int log2m2, float fill,
            const float2* __restrict__ tw1, const float2* __restrict__ tw2g, float2* __restrict__ T,
            long long* __restrict__ idx_out, float* __restrict__ y_out)
 {
+    constexpr int PB = FFT_PB, PA = FFT_PA;
     constexpr int L = R1 * 256;                    // M1
-    constexpr int LP = R1 * FFT_PA + 16 / C;       // slot pitch: 16/C mod 16 keeps the column-fastest accesses conflict free
+    constexpr int LP = R1 * PA + 16 / C;           // slot pitch: 16/C mod 16 keeps the column-fastest accesses conflict free
     extern __shared__ __align__(16) float2 fsm[];
     float2* tw2 = fsm + C * LP;
-    // fused gather: template fastest (co-resident CTAs gather from the same stretch of the series);
-    // plain load: bundle fastest (co-resident CTAs touch adjacent sectors of the same lines)
-    const int nbund = (1 << log2m2) / C;
-    const int b  = GATHER ? blockIdx.x % n_tmpl : blockIdx.x / nbund;
-    const int c0 = (GATHER ? blockIdx.x / n_tmpl : blockIdx.x % nbund) * C;
+    const int b  = blockIdx.x % n_tmpl;
+    const int c0 = (blockIdx.x / n_tmpl) * C;
     const size_t m = (size_t)L << log2m2;          // M
     const int log2h = tmpl[b].log2h;
     const float inv_h = 1.0f / (float)(1 << log2h);
@@ -214,28 +246,7 @@ k_fft_cols(const float* __restrict__ x, const SegRec* __restrict__ seg, size_t s
     tw2[threadIdx.x] = __ldg(tw2g + threadIdx.x);
 
     // phase A: gather, radix-R1 over a, twiddle, to shared memory.  item i: col = i % C, w = i / C
-    if (!GATHER) {
-        // x holds the resampled series of this chunk [n_tmpl][n]; all loads are issued first
-        const float2* __restrict__ yb = reinterpret_cast<const float2*>(x + (size_t)b * n);
-        float2 v[C][R1];
-#pragma unroll
-        for (int it = 0; it < C; ++it) {
-            const int i = it * FFT_THREADS + threadIdx.x;
-            const int col = i % C, w = i / C;
-#pragma unroll
-            for (int a = 0; a < R1; ++a) v[it][a] = __ldcs(yb + (((size_t)(a * 256 + w)) << log2m2) + c0 + col);
-        }
-#pragma unroll
-        for (int it = 0; it < C; ++it) {
-            const int i = it * FFT_THREADS + threadIdx.x;
-            const int col = i % C, w = i / C;
-            fft_reg<R1>(v[it]);
-            float2* p = fsm + col * LP + (w >> 4) * FFT_PB + (w & 15);
-            p[0] = v[it][0];
-#pragma unroll
-            for (int ka = 1; ka < R1; ++ka) p[ka * FFT_PA] = cmul(v[it][ka], __ldg(tw1 + ka * 256 + w));
-        }
-    } else
+#pragma unroll 2
     for (int i = threadIdx.x; i < 256 * C; i += FFT_THREADS) {
         const int col = i % C, w = i / C;
         float2 v[R1];
@@ -255,19 +266,19 @@ k_fft_cols(const float* __restrict__ x, const SegRec* __restrict__ seg, size_t s
         fft_reg<R1>(v);
 #pragma unroll
         for (int ka = 1; ka < R1; ++ka) v[ka] = cmul(v[ka], __ldg(tw1 + ka * 256 + w));
-        float2* p = fsm + col * LP + (w >> 4) * FFT_PB + (w & 15);
+        float2* p = fsm + col * LP + (w >> 4) * PB + (w & 15);
 #pragma unroll
-        for (int ka = 0; ka < R1; ++ka) p[ka * FFT_PA] = v[ka];
+        for (int ka = 0; ka < R1; ++ka) p[ka * PA] = v[ka];
     }
     __syncthreads();
     // phase B: radix 16 over b
-    for (int i = threadIdx.x; i < 16 * R1 * C; i += FFT_THREADS) fft_step2(fsm + (i / (16 * R1)) * LP, i % (16 * R1), tw2);
+    for (int i = threadIdx.x; i < 16 * R1 * C; i += FFT_THREADS) fft_step2<PA, PB>(fsm + (i / (16 * R1)) * LP, i % (16 * R1), tw2);
     __syncthreads();
     // phase C: radix 16 over c, four-step twiddle W_M^{j2 k1}, store T[k1][j2].  item: col fastest
     for (int i = threadIdx.x; i < 16 * R1 * C; i += FFT_THREADS) {
         const int col = i % C, w = i / C;          // w = ka*16 + kb
         const int ka = w >> 4, kb = w & 15;
-        const float2* p = fsm + col * LP + ka * FFT_PA + kb * FFT_PB;
+        const float2* p = fsm + col * LP + ka * PA + kb * PB;
         float2 v[16];
 #pragma unroll
         for (int c = 0; c < 16; ++c) v[c] = p[c];
@@ -297,24 +308,38 @@ k_fft_cols(const float* __restrict__ x, const SegRec* __restrict__ seg, size_t s
 }
 
 // ---------------------------------------------------------------------------------------------
-// P2  row FFTs.  CTA = R rows [k1, k1+R) of template b, row length M2 = R1*256; output
-//   Z[(k1 + r) + M1 k2] (runs of R consecutive elements).  blockIdx.x = b * (M1/R) + row group.
+// P2  row FFTs, transposed output.  CTA = R rows [k1, k1+R) of template b, row length
+//   M2 = R1*256 (R1 up to 32: 8192 points, 32 values per thread in the first radix step).
+//   Output Zt[k1][k2], k2 = ka + R1 kb + 16 R1 kc: the last step's work items run ka-fastest so
+//   that a warp stores 32 consecutive k2 (256 bytes); the pitches PB = 16 + R1 (mod 16) and
+//   PA = 16 PB + 1 keep that access, and the two before it, free of bank conflicts.
+//   blockIdx.x = b * (M1/R) + row group.
 // ---------------------------------------------------------------------------------------------
-template <int R1, int R>
-__global__ void __launch_bounds__(FFT_THREADS, 3)
-k_fft_rows(const float2* __restrict__ T, float2* __restrict__ Z, int log2m1, const float2* __restrict__ tw1,
-           const float2* __restrict__ tw2g)
+template <int R1> struct RowsCfg {
+    static constexpr int PB = (R1 < 16) ? 16 + R1 : 17;
+    static constexpr int PA = 16 * PB + 1;
+    static constexpr int R = (R1 >= 8) ? 1 : 8 / R1;       // rows per CTA
+    static constexpr int LP = R1 * PA;
+    static constexpr int MINB = (R1 >= 32) ? 2 : 3;        // CTAs per SM the register budget is set for
+    static constexpr size_t SMEM = (size_t)(R * LP + 256) * sizeof(float2);
+};
+
+template <int R1>
+__global__ void __launch_bounds__(FFT_THREADS, RowsCfg<R1>::MINB)
+k_fft_rows_t(const float2* __restrict__ T, float2* __restrict__ Zt, int log2m1, const float2* __restrict__ tw1,
+             const float2* __restrict__ tw2g)
 {
+    using Cfg = RowsCfg<R1>;
+    constexpr int PA = Cfg::PA, PB = Cfg::PB, R = Cfg::R, LP = Cfg::LP;
     constexpr int L = R1 * 256;                    // M2
-    constexpr int LP = R1 * FFT_PA + 16 / R;       // slot pitch: 16/R mod 16 keeps the row-fastest accesses conflict free
     extern __shared__ __align__(16) float2 fsm[];
     float2* tw2 = fsm + R * LP;
     const int groups = (1 << log2m1) / R;
     const int b  = blockIdx.x / groups;
     const int k1 = (blockIdx.x % groups) * R;
-    const size_t m = (size_t)L << log2m1;
-    const float2* __restrict__ Tb = T + (size_t)b * m + (size_t)k1 * L;
-    float2* __restrict__ Zb = Z + (size_t)b * m + k1;
+    const size_t off = ((size_t)b << log2m1) * L + (size_t)k1 * L;
+    const float2* __restrict__ Tb = T + off;
+    float2* __restrict__ Zb = Zt + off;
 
     tw2[threadIdx.x] = __ldg(tw2g + threadIdx.x);
 
@@ -327,33 +352,29 @@ k_fft_rows(const float2* __restrict__ T, float2* __restrict__ Z, int log2m1, con
         for (int r = 0; r < R; ++r)
 #pragma unroll
             for (int a = 0; a < R1; ++a) v[r][a] = __ldcs(Tb + (size_t)r * L + a * 256 + w);
-        float2 tw[R1];
-#pragma unroll
-        for (int ka = 1; ka < R1; ++ka) tw[ka] = __ldg(tw1 + ka * 256 + w);
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             fft_reg<R1>(v[r]);
-            float2* p = fsm + r * LP + (w >> 4) * FFT_PB + (w & 15);
+            float2* p = fsm + r * LP + (w >> 4) * PB + (w & 15);
             p[0] = v[r][0];
 #pragma unroll
-            for (int ka = 1; ka < R1; ++ka) p[ka * FFT_PA] = cmul(v[r][ka], tw[ka]);
+            for (int ka = 1; ka < R1; ++ka) p[ka * PA] = cmul(v[r][ka], __ldg(tw1 + ka * 256 + w));
         }
     }
     __syncthreads();
-    for (int i = threadIdx.x; i < 16 * R1 * R; i += FFT_THREADS) fft_step2(fsm + (i / (16 * R1)) * LP, i % (16 * R1), tw2);
+    for (int i = threadIdx.x; i < 16 * R1 * R; i += FFT_THREADS) fft_step2<PA, PB>(fsm + (i / (16 * R1)) * LP, i % (16 * R1), tw2);
     __syncthreads();
-    for (int i = threadIdx.x; i < 16 * R1 * R; i += FFT_THREADS) {  // phase C: item (w, r), r fastest
-        const int r = i % R, w = i / R;
-        const int ka = w >> 4, kb = w & 15;
-        const float2* p = fsm + r * LP + ka * FFT_PA + kb * FFT_PB;
+    for (int i = threadIdx.x; i < 16 * R1 * R; i += FFT_THREADS) {  // phase C: item (r, w'), ka fastest
+        const int r = i / (16 * R1), wp = i % (16 * R1);
+        const int ka = wp % R1, kb = wp / R1;
+        const float2* p = fsm + r * LP + ka * PA + kb * PB;
         float2 v[16];
 #pragma unroll
         for (int c = 0; c < 16; ++c) v[c] = p[c];
         fft_reg<16>(v);
-        float2* out = Zb + (((size_t)(ka + R1 * kb)) << log2m1) + r;
-        const size_t kstep = (size_t)(16 * R1) << log2m1;
+        float2* out = Zb + (size_t)r * L + wp;     // k2 = wp + 16 R1 kc
 #pragma unroll
-        for (int kc = 0; kc < 16; ++kc) __stcs(out + kc * kstep, v[kc]);
+        for (int kc = 0; kc < 16; ++kc) __stcs(out + kc * (16 * R1), v[kc]);
     }
 }
 

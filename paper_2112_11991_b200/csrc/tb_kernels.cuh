@@ -480,6 +480,158 @@ k_spectrum_median(const float2* __restrict__ X, size_t ld, float* __restrict__ P
 }
 
 // ---------------------------------------------------------------------------------------------
+// K2t  spectrum former for the hand-written FFT (a5 + a6 + a7), input = the TRANSPOSED complex
+//   spectrum Zt[k1][k2] of z_j = y_2j + i y_2j+1 (tb_fft.cuh; bin k = k1 + M1 k2, M = M1 M2 = N/2).
+//   The real-series spectrum is formed on the fly (R2C unpack),
+//       2 X_k = (Z_k + conj Z_{M-k}) - i W_N^k (Z_k - conj Z_{M-k}),   W_N^k = twa[k1] * twb[k2],
+//   and the SAME pair (Z_k, Z_{M-k}) also gives X_{M-k} (W_N^{M-k} = -conj W_N^k), so one CTA
+//   serves two mirrored tiles of 9 median blocks each and every element of Zt is read once:
+//       low  tile: bins [kL0, kL0 + 9W),  kL0 = 8 g W           (blocks 8g .. 8g+8)
+//       high tile: bins [hH0, hH0 + 9W),  hH0 = M - kL0 - 9W    (blocks nblk-8g-9 .. nblk-8g-1)
+//   for g < nblk/16.  A tile is 9 W/M1 columns k2 of every row k1: runs of 18 complex values
+//   (144 bytes) at W = 1024, M1 = 512.  Thread (k2, chunk of W/32 consecutive k1) walks k
+//   upwards keeping X_{k-1} and X_{M-k+1} in registers, so each step yields the interbinned
+//   powers P_k and P_{M-k+1} (G12-G14); they go to shared memory in bin order (rows of M1 + 1
+//   floats: conflict-free for the transposing store and the block-order load).  Then, per side,
+//   warp w takes block w of the tile into registers, selects the exact median (warp_median, its
+//   own block's shared memory as scratch), and after one barrier normalises between block
+//   centres exactly like k_spectrum_median and writes 8 W bins with coalesced stores.
+//   Powers are carried as 4 P_k (the 1/2 of the unpack is skipped); the factor cancels in P^.
+// ---------------------------------------------------------------------------------------------
+constexpr int ST_WARPS = 9;
+constexpr int ST_THREADS = ST_WARPS * 32;
+
+__host__ __device__ constexpr size_t st_smem_bytes(int W, int log2m1)
+{
+    return (size_t)2 * (9 * W + 9 * (W >> log2m1)) * sizeof(float);
+}
+
+// (2 X_k, 2 X_{M-k}) of bin k = k1 + M1 k2; wb = W_N^{M1 k2}
+__device__ __forceinline__ void st_unpack(const float2* __restrict__ Zr, int k1, int k2, int m1, int log2m2,
+                                          const float2* __restrict__ twa, float2 wb, float2& xk, float2& xm)
+{
+    const int m2 = 1 << log2m2;
+    const int mr = k1 ? m1 - k1 : 0;
+    const int mc = k1 ? m2 - 1 - k2 : ((m2 - k2) & (m2 - 1));          // k = 0: Z_M = Z_0
+    const float2 zk = __ldg(Zr + ((size_t)k1 << log2m2) + k2);
+    const float2 zm = __ldg(Zr + ((size_t)mr << log2m2) + mc);
+    const float2 wa = __ldg(twa + k1);
+    const float2 w = make_float2(wa.x * wb.x - wa.y * wb.y, wa.x * wb.y + wa.y * wb.x);
+    xk = r2c_unpack2(zk, zm, w);
+    xm = r2c_unpack2(zm, zk, make_float2(-w.x, w.y));
+    if ((k1 | k2) == 0) xk = make_float2(0.f, 0.f);                     // X_0 <- 0 before differencing (G13)
+}
+
+__device__ __forceinline__ float st_interbin(float2 x, float2 prev)
+{
+    const float dx = x.x - prev.x, dy = x.y - prev.y;
+    return fmaxf(x.x * x.x + x.y * x.y, 0.5f * (dx * dx + dy * dy));
+}
+
+template <int W, bool RAW>
+__global__ void __launch_bounds__(ST_THREADS, (W <= 1024) ? 3 : 1)
+k_spectrum_t(const float2* __restrict__ Zt, float* __restrict__ P, float* __restrict__ med, int log2m1, int log2m2,
+             int nblk, const float2* __restrict__ twa, const float2* __restrict__ twb,
+             unsigned long long* __restrict__ fallbacks, float* __restrict__ Praw)
+{
+    constexpr int VPT = W / 32;
+    constexpr int LC = W / 32;                           // consecutive k1 per thread
+    constexpr int CAP = (W >= 512) ? W / 4 : W;
+    extern __shared__ __align__(16) float st_sm[];
+    __shared__ float s_med[2][ST_WARPS];
+    const int m1 = 1 << log2m1;
+    const int q = W >> log2m1;                           // columns k2 per median block
+    const int nk2 = 9 * q;
+    const int side_floats = 9 * W + nk2;
+    float* __restrict__ s_lo = st_sm;
+    float* __restrict__ s_hi = st_sm + side_floats;
+    const int groups = nblk >> 4;
+    const int row = blockIdx.x / groups, g = blockIdx.x % groups;
+    const size_t m = (size_t)1 << (log2m1 + log2m2);     // bins per template
+    const float2* __restrict__ Zr = Zt + (size_t)row * m;
+    const int a = 8 * g * q;                             // first column of the low tile
+    const int wid = threadIdx.x >> 5, lane = threadIdx.x & 31;
+
+    {   // ---- phase 1: unpack + interbin, powers to shared memory in bin order ----
+        const int k2off = threadIdx.x % nk2, k1s = (threadIdx.x / nk2) * LC;
+        const int k2 = a + k2off;
+        const float2 wb = __ldg(twb + k2);
+        float2 pl = make_float2(0.f, 0.f), ph = make_float2(0.f, 0.f);      // 2 X_{k-1}, 2 X_{M-k+1}
+        if (k1s > 0) st_unpack(Zr, k1s - 1, k2, m1, log2m2, twa, wb, pl, ph);
+        else if (k2 > 0) st_unpack(Zr, m1 - 1, k2 - 1, m1, log2m2, twa, __ldg(twb + k2 - 1), pl, ph);
+        const int e0 = k1s + (k2off << log2m1);          // k - kL0 at the first step
+#pragma unroll 4
+        for (int it = 0; it < LC; ++it) {
+            float2 xk, xm;
+            st_unpack(Zr, k1s + it, k2, m1, log2m2, twa, wb, xk, xm);
+            const int e = e0 + it;
+            s_lo[e + k2off] = st_interbin(xk, pl);
+            const int eh = 9 * W + 1 - e;                // (M - k + 1) - hH0
+            if (eh < 9 * W) s_hi[eh + (eh >> log2m1)] = st_interbin(ph, xm);
+            pl = xk; ph = xm;
+        }
+        if (threadIdx.x < 2) {                           // the two steps above the low tile: high bins hH0 + 1, hH0
+            const int kc2 = a + nk2;                     // k = kL0 + 9W + t = (k1 = t, k2 = a + 9q)
+            const float2 wc = __ldg(twb + kc2);
+            float2 x0, h0, x1, h1;
+            if (threadIdx.x == 0) st_unpack(Zr, m1 - 1, kc2 - 1, m1, log2m2, twa, __ldg(twb + kc2 - 1), x0, h0);
+            else                  st_unpack(Zr, 0, kc2, m1, log2m2, twa, wc, x0, h0);
+            st_unpack(Zr, (int)threadIdx.x, kc2, m1, log2m2, twa, wc, x1, h1);
+            s_hi[1 - (int)threadIdx.x] = st_interbin(h0, h1);
+        }
+    }
+    __syncthreads();
+
+    constexpr float LN2 = 0.69314718055994530942f;
+    constexpr float INV_W = 1.0f / (float)W;
+    const bool last_pair = g == groups - 1;
+#pragma unroll 1
+    for (int side = 0; side < 2; ++side) {
+        float* __restrict__ sm = side ? s_hi : s_lo;
+        const int blk = side ? nblk - 8 * g - 9 + wid : 8 * g + wid;
+        const bool owner = side ? wid > 0 : wid < ST_WARPS - 1;      // writes the median (and the raw powers)
+        float p[VPT];
+        const int eb = wid * W;
+#pragma unroll
+        for (int i = 0; i < VPT; ++i) { const int e = eb + i * 32 + lane; p[i] = sm[e + (e >> log2m1)]; }
+        __syncwarp();
+        if (RAW && owner) {
+#pragma unroll
+            for (int i = 0; i < VPT; ++i) Praw[(size_t)row * m + (size_t)blk * W + i * 32 + lane] = 0.25f * p[i];
+        }
+        // scratch for the bracket list: the first CAP floats of this warp's own block (CAP <= M1)
+        const float m_cur = warp_median<W>(p, sm + eb + (eb >> log2m1), lane, owner ? fallbacks : nullptr);
+        if (lane == 0) {
+            s_med[side][wid] = m_cur;
+            if (owner) med[(size_t)row * nblk + blk] = 0.25f * m_cur;
+        }
+        __syncthreads();
+        // first half of the block: between the previous centre and this one; second half: this and the next
+        bool can_first = wid > 0 || blk == 0;
+        bool can_second = wid < ST_WARPS - 1 || blk == nblk - 1;
+        if (side && last_pair) {                         // [centre(nblk/2-1), centre(nblk/2)) belongs to the low tile
+            if (wid == 0) can_second = false;
+            if (wid == 1) can_first = false;
+        }
+        const float m_prev = (wid > 0) ? s_med[side][wid - 1] : m_cur;              // flat below the first centre
+        const float m_next = (wid < ST_WARPS - 1) ? s_med[side][wid + 1] : m_cur;   // flat above the last centre
+        float* __restrict__ Pr = P + (size_t)row * m + (size_t)blk * W;
+#pragma unroll
+        for (int i = 0; i < VPT; ++i) {
+            const bool second = i >= VPT / 2;            // compile-time after unrolling
+            if (!(second ? can_second : can_first)) continue;
+            const int eo = i * 32 + lane;
+            const float ma = second ? m_cur : m_prev, mb = second ? m_next : m_cur;
+            const float f = ((float)(second ? eo - W / 2 : eo + W / 2) + 0.5f) * INV_W;
+            const float bl = fmaf(f, mb - ma, ma);
+            float o = (bl > 0.f) ? __fdividef(p[i] * LN2, bl) : 0.f;
+            if (blk == 0 && eo == 0) o = 0.f;            // P^_0 = 0
+            Pr[eo] = o;
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
 // K4  harmonic sum + threshold + compaction (a8 + a9).
 //   S_L[k] = sum_{m=1}^{2^L} P^[(k m + 2^(L-1)) >> L]  (eq 9; G16), nested:
 //   S_L = S_{L-1} + the odd-m terms.  A bin/fold over threshold becomes a candidate; the warp
