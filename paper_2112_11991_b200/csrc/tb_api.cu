@@ -307,7 +307,7 @@ int launch_rows(tb_plan* p, uint32_t nt)
 // K0 + P1: delay segments, then gather + column FFTs into T (the buffer the legacy path uses for y)
 int run_own_pass1(tb_plan* p, size_t off, uint32_t nt, long long* d_idx, float* d_y)
 {
-    const int cta_per_tmpl = (int)(((p->n >> OWN_MIN_LOG2H) + 255) / 256);
+    const int cta_per_tmpl = (int)(((p->n >> p->min_log2h) + 255) / 256);   // min_log2h: smallest knot spacing staged
     k_delay_segments<<<(unsigned)(cta_per_tmpl * nt), 256, 0, p->stream>>>(p->d_tmpl + off, (int)nt, (int)p->n, p->d_seg,
                                                                            p->seg_stride, cta_per_tmpl);
     TB_CUDA(p, cudaGetLastError());
@@ -332,35 +332,41 @@ int run_own_pass2(tb_plan* p, uint32_t nt)
     return fail(p, TB_ERR_INVALID_ARG, "unsupported M2");
 }
 
-template <int W>
+template <int W, int LOG2M1>
 int launch_spectrum_t(tb_plan* p, uint32_t nt, float* d_raw)
 {
-    const size_t smem = st_smem_bytes(W, p->log2m1);
+    constexpr size_t smem = st_smem_bytes(W, LOG2M1);
     const unsigned grid = (unsigned)((p->nblk / 16) * nt);
     unsigned long long* fb = p->d_cursor + 1;
     if (d_raw) {
-        auto kern = k_spectrum_t<W, true>;
-        TB_CUDA(p, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)st_smem_bytes(W, 8)));
-        kern<<<grid, ST_THREADS, smem, p->stream>>>(p->d_fft, p->d_power, p->d_med, p->log2m1, p->log2m2, (int)p->nblk,
-                                                   p->d_twn, p->d_twb, fb, d_raw);
-    } else {
-        auto kern = k_spectrum_t<W, false>;
+        auto kern = k_spectrum_t<W, LOG2M1, true>;
         static bool attr = false;
-        if (!attr) { TB_CUDA(p, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)st_smem_bytes(W, 8))); attr = true; }
-        kern<<<grid, ST_THREADS, smem, p->stream>>>(p->d_fft, p->d_power, p->d_med, p->log2m1, p->log2m2, (int)p->nblk,
-                                                   p->d_twn, p->d_twb, fb, nullptr);
+        if (!attr) { TB_CUDA(p, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); attr = true; }
+        kern<<<grid, ST_THREADS, smem, p->stream>>>(p->d_fft, p->d_power, p->d_med, p->log2m2, (int)p->nblk, p->d_twn, p->d_twb, fb, d_raw);
+    } else {
+        auto kern = k_spectrum_t<W, LOG2M1, false>;
+        static bool attr = false;
+        if (!attr) { TB_CUDA(p, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); attr = true; }
+        kern<<<grid, ST_THREADS, smem, p->stream>>>(p->d_fft, p->d_power, p->d_med, p->log2m2, (int)p->nblk, p->d_twn, p->d_twb, fb, nullptr);
     }
     TB_CUDA(p, cudaGetLastError());
     return TB_OK;
 }
 
+// (median window, log2 M1) pairs the transposing spectrum former is instantiated for
+bool spectrum_t_supported(uint32_t w, int log2m1)
+{
+    return (log2m1 == 8 && (w == 256 || w == 1024)) || (log2m1 == 9 && (w == 512 || w == 1024 || w == 2048));
+}
+
 int run_spectrum_t(tb_plan* p, uint32_t nt, float* d_raw = nullptr)
 {
-    switch (p->window) {
-        case 256: return launch_spectrum_t<256>(p, nt, d_raw);
-        case 512: return launch_spectrum_t<512>(p, nt, d_raw);
-        case 1024: return launch_spectrum_t<1024>(p, nt, d_raw);
-        case 2048: return launch_spectrum_t<2048>(p, nt, d_raw);
+    switch (p->window * 16 + (uint32_t)p->log2m1) {
+        case 256 * 16 + 8: return launch_spectrum_t<256, 8>(p, nt, d_raw);
+        case 1024 * 16 + 8: return launch_spectrum_t<1024, 8>(p, nt, d_raw);
+        case 512 * 16 + 9: return launch_spectrum_t<512, 9>(p, nt, d_raw);
+        case 1024 * 16 + 9: return launch_spectrum_t<1024, 9>(p, nt, d_raw);
+        case 2048 * 16 + 9: return launch_spectrum_t<2048, 9>(p, nt, d_raw);
     }
     return fail(p, TB_ERR_INVALID_ARG, "median_window");
 }
@@ -655,7 +661,7 @@ int tb_plan_create(tb_plan** out, const float* series, uint64_t n_samples, doubl
         const int lm = (int)ilog2(p->nb);
         p->log2m1 = lm >= 17 ? 9 : 8;
         p->log2m2 = lm - p->log2m1;
-        const bool fits = p->log2m2 >= 8 && p->log2m2 <= 13 && W >= (1u << p->log2m1) && p->nblk >= 16 && p->nblk % 16 == 0;
+        const bool fits = p->log2m2 >= 8 && p->log2m2 <= 13 && spectrum_t_supported(W, p->log2m1) && p->nblk >= 16 && p->nblk % 16 == 0;
         if (o.fft_path >= 2 && !fits) { destroy(p); return TB_ERR_INVALID_ARG; }
         p->own_fft = fits && o.fft_path != 1;
     }

@@ -257,7 +257,7 @@ __device__ __forceinline__ float warp_median(const float (&p)[W / 32], float* ca
 {
     constexpr int VPT = W / 32;
     constexpr int K1 = W / 2 - 1;
-    constexpr int CAP = (W >= 512) ? W / 4 : W;          // candidate list capacity
+    constexpr int CAP = (W >= 512) ? W / 4 : W / 2;          // candidate list capacity
     constexpr int CPL = CAP / 32;                        // candidates per lane
     constexpr int NMW = (VPT + 31) / 32;
     // Fast path: the median of noise-like powers sits near 0.78 x the block mean, so count the
@@ -306,13 +306,25 @@ __device__ __forceinline__ float warp_median(const float (&p)[W / 32], float* ca
         const int r1 = K1 - below;                       // rank among the candidates
         uint32_t L = __float_as_uint(lo), H = __float_as_uint(hi);
         int cl = 0, ch = nmid;                           // candidates below L, below H
+        // interpolation search: the keys inside the bracket are close to uniform, so the guess
+        // L + (H-L)(r1 + 1/2 - cl)/(ch - cl) leaves about sqrt(n) of n candidates; a step that
+        // fails to halve the candidate count is followed by a plain bisection step
+        bool bisect = false;
         while (ch - cl > 1 && H - L > 1u) {
-            const uint32_t mid = L + ((H - L) >> 1);
+            const uint32_t span = H - L;
+            uint32_t mid = L + (span >> 1);
+            if (!bisect) {
+                const float fr = ((float)(r1 - cl) + 0.5f) * __frcp_rn((float)(ch - cl));
+                mid = L + (uint32_t)(fr * (float)span);
+                mid = min(max(mid, L + 1u), H - 1u);
+            }
             int c = 0;
 #pragma unroll
             for (int q = 0; q < CPL; ++q) c += (ck[q] < mid) ? 1 : 0;
             c = __reduce_add_sync(0xffffffffu, c);
+            const int before = ch - cl;
             if (c <= r1) { L = mid; cl = c; } else { H = mid; ch = c; }
+            bisect = !bisect && 2 * (ch - cl) > before;
         }
         uint32_t v1 = 0xffffffffu;
 #pragma unroll
@@ -368,7 +380,7 @@ k_spectrum_median(const float2* __restrict__ X, size_t ld, float* __restrict__ P
 {
     constexpr int VPT  = W / 32;        // powers per lane
     constexpr int ITER = W / 128;       // 4 consecutive bins per lane per iteration
-    constexpr int CAP  = (W >= 512) ? W / 4 : W;
+    constexpr int CAP  = (W >= 512) ? W / 4 : W / 2;
     constexpr float SCALE = UNPACK ? 0.25f : 1.0f;       // powers are held as 4 P_k on the unpack path
     __shared__ float s_cand[SP_WARPS + 1][CAP];
     __shared__ float s_med[SP_WARPS + 1];
@@ -501,83 +513,116 @@ k_spectrum_median(const float2* __restrict__ X, size_t ld, float* __restrict__ P
 constexpr int ST_WARPS = 9;
 constexpr int ST_THREADS = ST_WARPS * 32;
 
-__host__ __device__ constexpr size_t st_smem_bytes(int W, int log2m1)
+// floats per tile in shared memory: 9 W/M1 rows of M1 + 1 floats; the high tile is stored from
+// float 3 on, shifted down by two bins (see phase 1), so it needs 4 more
+__host__ __device__ constexpr int st_side_floats(int W, int log2m1) { return 9 * W + 9 * (W >> log2m1) + 4; }
+__host__ __device__ constexpr size_t st_smem_bytes(int W, int log2m1) { return (size_t)2 * st_side_floats(W, log2m1) * sizeof(float); }
+
+// 2 X_k and 2 X_{M-k} from Z_k, Z_{M-k} and w = W_N^k:  E = Z_k + conj Z_{M-k}, D = Z_k - conj Z_{M-k},
+// 2 X_k = E - i w D,  2 X_{M-k} = conj E - i w' D',  w' = -conj w,  D' = -conj D
+__device__ __forceinline__ void st_unpack2(float2 zk, float2 zm, float2 w, float2& xk, float2& xm)
 {
-    return (size_t)2 * (9 * W + 9 * (W >> log2m1)) * sizeof(float);
+    const float er = zk.x + zm.x, ei = zk.y - zm.y;
+    const float dx = zk.x - zm.x, dy = zk.y + zm.y;
+    const float A = fmaf(w.x, dy, w.y * dx);
+    const float B = fmaf(w.y, dy, -w.x * dx);
+    xk = make_float2(er + A, ei + B);
+    xm = make_float2(er - A, B - ei);
 }
 
-// (2 X_k, 2 X_{M-k}) of bin k = k1 + M1 k2; wb = W_N^{M1 k2}
-__device__ __forceinline__ void st_unpack(const float2* __restrict__ Zr, int k1, int k2, int m1, int log2m2,
-                                          const float2* __restrict__ twa, float2 wb, float2& xk, float2& xm)
+// one-off version with its own loads, for the steps just outside a thread's run; wb = W_N^{M1 k2}
+template <int LOG2M1>
+__device__ __forceinline__ void st_unpack_at(const float2* __restrict__ Zr, int k1, int k2, int log2m2,
+                                             const float2* __restrict__ twa, float2 wb, float2& xk, float2& xm)
 {
+    constexpr int M1 = 1 << LOG2M1;
     const int m2 = 1 << log2m2;
-    const int mr = k1 ? m1 - k1 : 0;
+    const int mr = k1 ? M1 - k1 : 0;
     const int mc = k1 ? m2 - 1 - k2 : ((m2 - k2) & (m2 - 1));          // k = 0: Z_M = Z_0
     const float2 zk = __ldg(Zr + ((size_t)k1 << log2m2) + k2);
     const float2 zm = __ldg(Zr + ((size_t)mr << log2m2) + mc);
     const float2 wa = __ldg(twa + k1);
-    const float2 w = make_float2(wa.x * wb.x - wa.y * wb.y, wa.x * wb.y + wa.y * wb.x);
-    xk = r2c_unpack2(zk, zm, w);
-    xm = r2c_unpack2(zm, zk, make_float2(-w.x, w.y));
+    st_unpack2(zk, zm, make_float2(wa.x * wb.x - wa.y * wb.y, wa.x * wb.y + wa.y * wb.x), xk, xm);
     if ((k1 | k2) == 0) xk = make_float2(0.f, 0.f);                     // X_0 <- 0 before differencing (G13)
 }
 
 __device__ __forceinline__ float st_interbin(float2 x, float2 prev)
 {
     const float dx = x.x - prev.x, dy = x.y - prev.y;
-    return fmaxf(x.x * x.x + x.y * x.y, 0.5f * (dx * dx + dy * dy));
+    return fmaxf(fmaf(x.y, x.y, x.x * x.x), 0.5f * fmaf(dy, dy, dx * dx));
 }
 
-template <int W, bool RAW>
+template <int W, int LOG2M1, bool RAW>
 __global__ void __launch_bounds__(ST_THREADS, (W <= 1024) ? 3 : 1)
-k_spectrum_t(const float2* __restrict__ Zt, float* __restrict__ P, float* __restrict__ med, int log2m1, int log2m2,
+k_spectrum_t(const float2* __restrict__ Zt, float* __restrict__ P, float* __restrict__ med, int log2m2,
              int nblk, const float2* __restrict__ twa, const float2* __restrict__ twb,
              unsigned long long* __restrict__ fallbacks, float* __restrict__ Praw)
 {
+    static_assert(W >= (1 << LOG2M1), "a median block is a whole number of columns");
+    constexpr int M1 = 1 << LOG2M1;
     constexpr int VPT = W / 32;
     constexpr int LC = W / 32;                           // consecutive k1 per thread
-    constexpr int CAP = (W >= 512) ? W / 4 : W;
+    constexpr int Q = W >> LOG2M1;                       // columns k2 per median block
+    constexpr int NK2 = 9 * Q;
+    constexpr int SIDE = st_side_floats(W, LOG2M1);
     extern __shared__ __align__(16) float st_sm[];
     __shared__ float s_med[2][ST_WARPS];
-    const int m1 = 1 << log2m1;
-    const int q = W >> log2m1;                           // columns k2 per median block
-    const int nk2 = 9 * q;
-    const int side_floats = 9 * W + nk2;
     float* __restrict__ s_lo = st_sm;
-    float* __restrict__ s_hi = st_sm + side_floats;
+    float* __restrict__ s_hi = st_sm + SIDE + 3;         // bin hH0 + eh lives at s_hi[(eh - 2) + ((eh - 2) >> LOG2M1)]
     const int groups = nblk >> 4;
     const int row = blockIdx.x / groups, g = blockIdx.x % groups;
-    const size_t m = (size_t)1 << (log2m1 + log2m2);     // bins per template
+    const size_t m = (size_t)M1 << log2m2;               // bins per template
     const float2* __restrict__ Zr = Zt + (size_t)row * m;
-    const int a = 8 * g * q;                             // first column of the low tile
+    const int a = 8 * g * Q;                             // first column of the low tile
     const int wid = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
     {   // ---- phase 1: unpack + interbin, powers to shared memory in bin order ----
-        const int k2off = threadIdx.x % nk2, k1s = (threadIdx.x / nk2) * LC;
+        const int k2off = threadIdx.x % NK2, k1s = (threadIdx.x / NK2) * LC;
         const int k2 = a + k2off;
+        const size_t m2 = (size_t)1 << log2m2;
         const float2 wb = __ldg(twb + k2);
         float2 pl = make_float2(0.f, 0.f), ph = make_float2(0.f, 0.f);      // 2 X_{k-1}, 2 X_{M-k+1}
-        if (k1s > 0) st_unpack(Zr, k1s - 1, k2, m1, log2m2, twa, wb, pl, ph);
-        else if (k2 > 0) st_unpack(Zr, m1 - 1, k2 - 1, m1, log2m2, twa, __ldg(twb + k2 - 1), pl, ph);
-        const int e0 = k1s + (k2off << log2m1);          // k - kL0 at the first step
-#pragma unroll 4
-        for (int it = 0; it < LC; ++it) {
-            float2 xk, xm;
-            st_unpack(Zr, k1s + it, k2, m1, log2m2, twa, wb, xk, xm);
-            const int e = e0 + it;
-            s_lo[e + k2off] = st_interbin(xk, pl);
-            const int eh = 9 * W + 1 - e;                // (M - k + 1) - hH0
-            if (eh < 9 * W) s_hi[eh + (eh >> log2m1)] = st_interbin(ph, xm);
-            pl = xk; ph = xm;
+        if (k1s > 0) st_unpack_at<LOG2M1>(Zr, k1s - 1, k2, log2m2, twa, wb, pl, ph);
+        else if (k2 > 0) st_unpack_at<LOG2M1>(Zr, M1 - 1, k2 - 1, log2m2, twa, __ldg(twb + k2 - 1), pl, ph);
+        // low bin e = k - kL0 = k1 + M1 k2off at s_lo[e + k2off]; the same step yields the high bin
+        // eh = 9W + 1 - e, and eh - 2 = (M1 - 1 - k1) + M1 (9Q - 1 - k2off): both addresses move by
+        // one float per step (steps e = 0, 1 land in two unused floats at the top of the high tile)
+        float* __restrict__ lo = s_lo + k1s + k2off * (M1 + 1);
+        float* __restrict__ hi = s_hi + (M1 - 1 - k1s) + (9 * Q - 1 - k2off) * (M1 + 1);
+        const float2* __restrict__ zkp = Zr + (size_t)k1s * m2 + k2;
+        const float2* __restrict__ zmp = Zr + (size_t)(M1 - k1s) * m2 + (m2 - 1 - k2);     // row M1 is never read (k1s = 0 below)
+        const float2* __restrict__ wap = twa + k1s;
+        constexpr int UN = 4;
+#pragma unroll 1
+        for (int i0 = 0; i0 < LC; i0 += UN) {
+            float2 zk[UN], zm[UN], wa[UN];
+#pragma unroll
+            for (int u = 0; u < UN; ++u) {
+                const int it = i0 + u;
+                zk[u] = __ldg(zkp + (size_t)it * m2);
+                if (it == 0 && k1s == 0) zm[u] = __ldg(Zr + ((m2 - k2) & (m2 - 1)));          // k1 = 0 mirrors inside row 0
+                else                     zm[u] = __ldg(zmp - (size_t)it * m2);
+                wa[u] = __ldg(wap + it);
+            }
+#pragma unroll
+            for (int u = 0; u < UN; ++u) {
+                const int it = i0 + u;
+                float2 xk, xm;
+                st_unpack2(zk[u], zm[u], make_float2(wa[u].x * wb.x - wa[u].y * wb.y, wa[u].x * wb.y + wa[u].y * wb.x), xk, xm);
+                if (it == 0 && (k1s | k2) == 0) xk = make_float2(0.f, 0.f);                   // X_0 <- 0 (G13)
+                lo[it] = st_interbin(xk, pl);
+                hi[-it] = st_interbin(ph, xm);
+                pl = xk; ph = xm;
+            }
         }
         if (threadIdx.x < 2) {                           // the two steps above the low tile: high bins hH0 + 1, hH0
-            const int kc2 = a + nk2;                     // k = kL0 + 9W + t = (k1 = t, k2 = a + 9q)
+            const int kc2 = a + NK2;                     // k = kL0 + 9W + t = (k1 = t, k2 = a + 9Q)
             const float2 wc = __ldg(twb + kc2);
             float2 x0, h0, x1, h1;
-            if (threadIdx.x == 0) st_unpack(Zr, m1 - 1, kc2 - 1, m1, log2m2, twa, __ldg(twb + kc2 - 1), x0, h0);
-            else                  st_unpack(Zr, 0, kc2, m1, log2m2, twa, wc, x0, h0);
-            st_unpack(Zr, (int)threadIdx.x, kc2, m1, log2m2, twa, wc, x1, h1);
-            s_hi[1 - (int)threadIdx.x] = st_interbin(h0, h1);
+            if (threadIdx.x == 0) st_unpack_at<LOG2M1>(Zr, M1 - 1, kc2 - 1, log2m2, twa, __ldg(twb + kc2 - 1), x0, h0);
+            else                  st_unpack_at<LOG2M1>(Zr, 0, kc2, log2m2, twa, wc, x0, h0);
+            st_unpack_at<LOG2M1>(Zr, (int)threadIdx.x, kc2, log2m2, twa, wc, x1, h1);
+            s_hi[-2 - (int)threadIdx.x] = st_interbin(h0, h1);           // eh = 1 - t: (eh - 2) + ((eh - 2) >> LOG2M1)
         }
     }
     __syncthreads();
@@ -587,20 +632,26 @@ k_spectrum_t(const float2* __restrict__ Zt, float* __restrict__ P, float* __rest
     const bool last_pair = g == groups - 1;
 #pragma unroll 1
     for (int side = 0; side < 2; ++side) {
-        float* __restrict__ sm = side ? s_hi : s_lo;
         const int blk = side ? nblk - 8 * g - 9 + wid : 8 * g + wid;
         const bool owner = side ? wid > 0 : wid < ST_WARPS - 1;      // writes the median (and the raw powers)
+        // block `wid` of the tile: bins wid W + i 32 + lane, row (wid Q + (i 32 + lane) / M1) of the tile
+        float* __restrict__ sb = (side ? s_hi - 2 - (lane < 2 ? 1 : 0) : s_lo) + wid * (W + Q) + lane;
         float p[VPT];
-        const int eb = wid * W;
 #pragma unroll
-        for (int i = 0; i < VPT; ++i) { const int e = eb + i * 32 + lane; p[i] = sm[e + (e >> log2m1)]; }
+        for (int i = 0; i < VPT; ++i) {
+            // high tile: bin eh sits at (eh - 2) + ((eh - 2) >> LOG2M1); eh - 2 falls into the previous row
+            // only for the first two bins of a row, i.e. lanes 0, 1 of the steps with 32 i a multiple of M1
+            const int pad = (32 * i) >> LOG2M1;
+            if (side && (32 * i) % M1 != 0) p[i] = sb[32 * i + pad + ((lane < 2) ? 1 : 0)];
+            else                            p[i] = sb[32 * i + pad];
+        }
         __syncwarp();
         if (RAW && owner) {
 #pragma unroll
             for (int i = 0; i < VPT; ++i) Praw[(size_t)row * m + (size_t)blk * W + i * 32 + lane] = 0.25f * p[i];
         }
-        // scratch for the bracket list: the first CAP floats of this warp's own block (CAP <= M1)
-        const float m_cur = warp_median<W>(p, sm + eb + (eb >> log2m1), lane, owner ? fallbacks : nullptr);
+        // scratch for the bracket list: floats of this warp's own block (all of them are in registers now)
+        const float m_cur = warp_median<W>(p, (side ? s_hi : s_lo) + wid * (W + Q), lane, owner ? fallbacks : nullptr);
         if (lane == 0) {
             s_med[side][wid] = m_cur;
             if (owner) med[(size_t)row * nblk + blk] = 0.25f * m_cur;
@@ -615,18 +666,22 @@ k_spectrum_t(const float2* __restrict__ Zt, float* __restrict__ P, float* __rest
         }
         const float m_prev = (wid > 0) ? s_med[side][wid - 1] : m_cur;              // flat below the first centre
         const float m_next = (wid < ST_WARPS - 1) ? s_med[side][wid + 1] : m_cur;   // flat above the last centre
-        float* __restrict__ Pr = P + (size_t)row * m + (size_t)blk * W;
+        float* __restrict__ Pr = P + (size_t)row * m + (size_t)blk * W + lane;
 #pragma unroll
-        for (int i = 0; i < VPT; ++i) {
-            const bool second = i >= VPT / 2;            // compile-time after unrolling
-            if (!(second ? can_second : can_first)) continue;
-            const int eo = i * 32 + lane;
-            const float ma = second ? m_cur : m_prev, mb = second ? m_next : m_cur;
-            const float f = ((float)(second ? eo - W / 2 : eo + W / 2) + 0.5f) * INV_W;
-            const float bl = fmaf(f, mb - ma, ma);
-            float o = (bl > 0.f) ? __fdividef(p[i] * LN2, bl) : 0.f;
-            if (blk == 0 && eo == 0) o = 0.f;            // P^_0 = 0
-            Pr[eo] = o;
+        for (int h = 0; h < 2; ++h) {
+            if (!(h ? can_second : can_first)) continue;
+            const float ma = h ? m_cur : m_prev, mb = h ? m_next : m_cur;
+            // baseline at bin offset eo: ma + ((eo -+ W/2) + 1/2)/W (mb - ma) = b0 + i * st32
+            const float st32 = 32.0f * INV_W * (mb - ma);
+            const float b0 = fmaf(((float)(lane + (h ? 0 : W / 2)) + 0.5f) * INV_W, mb - ma, ma);
+#pragma unroll
+            for (int ii = 0; ii < VPT / 2; ++ii) {
+                const int i = h * (VPT / 2) + ii;
+                const float bl = fmaf((float)ii, st32, b0);
+                float o = (bl > 0.f) ? __fdividef(p[i] * LN2, bl) : 0.f;
+                if (i == 0 && blk == 0 && lane == 0) o = 0.f;        // P^_0 = 0
+                Pr[32 * i] = o;
+            }
         }
     }
 }
