@@ -66,6 +66,7 @@ struct tb_plan {
     SegRec* d_seg = nullptr;                         // [chunk][n >> MIN_LOG2H]
     size_t seg_stride = 0;
     float2 *d_tw1a = nullptr, *d_tw1b = nullptr, *d_tw2 = nullptr, *d_twn = nullptr, *d_twb = nullptr;
+    float2 rot = {1.f, 0.f};                         // W_N^1
     int min_log2h = 0;                               // smallest knot spacing among the staged templates
 
     std::map<uint32_t, cufftHandle> fft_plans;       // by batch size, sharing one work area
@@ -342,12 +343,12 @@ int launch_spectrum_t(tb_plan* p, uint32_t nt, float* d_raw)
         auto kern = k_spectrum_t<W, LOG2M1, true>;
         static bool attr = false;
         if (!attr) { TB_CUDA(p, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); attr = true; }
-        kern<<<grid, ST_THREADS, smem, p->stream>>>(p->d_fft, p->d_power, p->d_med, p->log2m2, (int)p->nblk, p->d_twn, p->d_twb, fb, d_raw);
+        kern<<<grid, ST_THREADS, smem, p->stream>>>(p->d_fft, p->d_power, p->d_med, p->log2m2, (int)p->nblk, p->d_twn, p->d_twb, p->rot, fb, d_raw);
     } else {
         auto kern = k_spectrum_t<W, LOG2M1, false>;
         static bool attr = false;
         if (!attr) { TB_CUDA(p, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); attr = true; }
-        kern<<<grid, ST_THREADS, smem, p->stream>>>(p->d_fft, p->d_power, p->d_med, p->log2m2, (int)p->nblk, p->d_twn, p->d_twb, fb, nullptr);
+        kern<<<grid, ST_THREADS, smem, p->stream>>>(p->d_fft, p->d_power, p->d_med, p->log2m2, (int)p->nblk, p->d_twn, p->d_twb, p->rot, fb, nullptr);
     }
     TB_CUDA(p, cudaGetLastError());
     return TB_OK;
@@ -407,6 +408,7 @@ int make_twiddles(tb_plan* p)
         const long double a = -two_pi * (long double)((uint64_t)b << p->log2m1) / (long double)p->n;
         hb[b] = make_float2((float)cosl(a), (float)sinl(a));
     }
+    p->rot = make_float2((float)cosl(two_pi / (long double)p->n), (float)-sinl(two_pi / (long double)p->n));
     if ((rc = upload(h2, &p->d_tw2))) return rc;
     if ((rc = upload(hb, &p->d_twb))) return rc;
     return upload(hn, &p->d_twn);

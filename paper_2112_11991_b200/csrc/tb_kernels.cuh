@@ -250,21 +250,23 @@ __device__ __forceinline__ float2 r2c_unpack2(float2 zk, float2 zm, float2 w)   
 }
 
 // exact order statistics W/2-1 and W/2 of the W non-negative floats held by a warp (VPT per
-// lane); returns their mean.  cand = this warp's shared scratch of CAP floats.
+// lane); returns their mean.  cand = this warp's shared scratch of med_scratch_floats<W>() floats.
+template <int W> __host__ __device__ constexpr int med_slots() { return (W / 32 >= 16) ? 12 : W / 32; }
+template <int W> __host__ __device__ constexpr int med_scratch_floats() { return 32 * med_slots<W>(); }
+
 template <int W>
 __device__ __forceinline__ float warp_median(const float (&p)[W / 32], float* cand, int lane,
                                              unsigned long long* __restrict__ fallbacks)
 {
     constexpr int VPT = W / 32;
     constexpr int K1 = W / 2 - 1;
-    constexpr int CAP = (W >= 512) ? W / 4 : W / 2;          // candidate list capacity
-    constexpr int CPL = CAP / 32;                        // candidates per lane
-    constexpr int NMW = (VPT + 31) / 32;
+    constexpr int CPL = med_slots<W>();                  // bracket values a lane can keep
     // Fast path: the median of noise-like powers sits near 0.78 x the block mean, so count the
-    // values below lo = 0.66 mean and compact those in [lo, hi = 0.90 mean) (about 13 % of the
-    // block: per-lane bit masks, one warp scan of the per-lane counts, lane-major list), then
-    // select among them.  If the two middle ranks are not both inside the bracket (or it
-    // overflows) fall back to the bisection over all W values.
+    // values below lo = 0.66 mean and keep those in [lo, hi = 0.90 mean) (about 13 % of the block,
+    // 4 per lane) in a private per-lane list in shared memory (slot q of lane l at cand[l + 32 q]:
+    // no scan, no compaction, no bank conflicts), then select among them.  If the two middle ranks
+    // are not both inside the bracket, or a lane holds more than CPL bracket values, fall back to
+    // the bisection over all W values.
     float sum = 0.f;
 #pragma unroll
     for (int v = 0; v < VPT; ++v) sum += p[v];
@@ -272,59 +274,35 @@ __device__ __forceinline__ float warp_median(const float (&p)[W / 32], float* ca
     for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
     const float lo = sum * (0.66f / (float)W), hi = sum * (0.90f / (float)W);
     int below = 0, mine = 0;
-    uint32_t mask[NMW];
-#pragma unroll
-    for (int i = 0; i < NMW; ++i) mask[i] = 0u;
+    float* __restrict__ cp = cand + lane;
 #pragma unroll
     for (int v = 0; v < VPT; ++v) {
         const bool isb = p[v] < lo;
         const bool ism = !isb && p[v] < hi;
         below += isb ? 1 : 0;
-        mine  += ism ? 1 : 0;
-        mask[v >> 5] |= ism ? (1u << (v & 31)) : 0u;
+        if (ism && mine < CPL) cp[32 * mine] = p[v];
+        mine += ism ? 1 : 0;
     }
     below = __reduce_add_sync(0xffffffffu, below);
-    int incl = mine;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-        const int t = __shfl_up_sync(0xffffffffu, incl, o);
-        if (lane >= o) incl += t;
-    }
-    const int nmid = __shfl_sync(0xffffffffu, incl, 31);
+    const int nmid = __reduce_add_sync(0xffffffffu, mine);
+    const int most = __reduce_max_sync(0xffffffffu, mine);
     uint32_t lower, upper;
-    if (below <= K1 && below + nmid >= K1 + 2 && nmid <= CAP) {
-        int pos = incl - mine;
-#pragma unroll
-        for (int v = 0; v < VPT; ++v)
-            if (mask[v >> 5] & (1u << (v & 31))) cand[pos++] = p[v];
-        __syncwarp();
+    if (below <= K1 && below + nmid >= K1 + 2 && most <= CPL) {
         uint32_t ck[CPL];
 #pragma unroll
-        for (int q = 0; q < CPL; ++q) ck[q] = (q * 32 + lane < nmid) ? __float_as_uint(cand[q * 32 + lane]) : 0xffffffffu;
+        for (int q = 0; q < CPL; ++q) ck[q] = (q < mine) ? __float_as_uint(cp[32 * q]) : 0xffffffffu;
         // bisection in key space (non-negative floats order like their bit patterns) on the
         // bracket [L, H) until exactly one candidate (or one key) is left around rank r1
         const int r1 = K1 - below;                       // rank among the candidates
         uint32_t L = __float_as_uint(lo), H = __float_as_uint(hi);
         int cl = 0, ch = nmid;                           // candidates below L, below H
-        // interpolation search: the keys inside the bracket are close to uniform, so the guess
-        // L + (H-L)(r1 + 1/2 - cl)/(ch - cl) leaves about sqrt(n) of n candidates; a step that
-        // fails to halve the candidate count is followed by a plain bisection step
-        bool bisect = false;
         while (ch - cl > 1 && H - L > 1u) {
-            const uint32_t span = H - L;
-            uint32_t mid = L + (span >> 1);
-            if (!bisect) {
-                const float fr = ((float)(r1 - cl) + 0.5f) * __frcp_rn((float)(ch - cl));
-                mid = L + (uint32_t)(fr * (float)span);
-                mid = min(max(mid, L + 1u), H - 1u);
-            }
+            const uint32_t mid = L + ((H - L) >> 1);
             int c = 0;
 #pragma unroll
             for (int q = 0; q < CPL; ++q) c += (ck[q] < mid) ? 1 : 0;
             c = __reduce_add_sync(0xffffffffu, c);
-            const int before = ch - cl;
             if (c <= r1) { L = mid; cl = c; } else { H = mid; ch = c; }
-            bisect = !bisect && 2 * (ch - cl) > before;
         }
         uint32_t v1 = 0xffffffffu;
 #pragma unroll
@@ -380,7 +358,7 @@ k_spectrum_median(const float2* __restrict__ X, size_t ld, float* __restrict__ P
 {
     constexpr int VPT  = W / 32;        // powers per lane
     constexpr int ITER = W / 128;       // 4 consecutive bins per lane per iteration
-    constexpr int CAP  = (W >= 512) ? W / 4 : W / 2;
+    constexpr int CAP  = med_scratch_floats<W>();
     constexpr float SCALE = UNPACK ? 0.25f : 1.0f;       // powers are held as 4 P_k on the unpack path
     __shared__ float s_cand[SP_WARPS + 1][CAP];
     __shared__ float s_med[SP_WARPS + 1];
@@ -555,7 +533,7 @@ __device__ __forceinline__ float st_interbin(float2 x, float2 prev)
 template <int W, int LOG2M1, bool RAW>
 __global__ void __launch_bounds__(ST_THREADS, (W <= 1024) ? 3 : 1)
 k_spectrum_t(const float2* __restrict__ Zt, float* __restrict__ P, float* __restrict__ med, int log2m2,
-             int nblk, const float2* __restrict__ twa, const float2* __restrict__ twb,
+             int nblk, const float2* __restrict__ twa, const float2* __restrict__ twb, float2 rot,
              unsigned long long* __restrict__ fallbacks, float* __restrict__ Praw)
 {
     static_assert(W >= (1 << LOG2M1), "a median block is a whole number of columns");
@@ -581,38 +559,48 @@ k_spectrum_t(const float2* __restrict__ Zt, float* __restrict__ P, float* __rest
         const int k2 = a + k2off;
         const size_t m2 = (size_t)1 << log2m2;
         const float2 wb = __ldg(twb + k2);
-        float2 pl = make_float2(0.f, 0.f), ph = make_float2(0.f, 0.f);      // 2 X_{k-1}, 2 X_{M-k+1}
-        if (k1s > 0) st_unpack_at<LOG2M1>(Zr, k1s - 1, k2, log2m2, twa, wb, pl, ph);
-        else if (k2 > 0) st_unpack_at<LOG2M1>(Zr, M1 - 1, k2 - 1, log2m2, twa, __ldg(twb + k2 - 1), pl, ph);
+        // 2 X_{k-1} and 2 X_{M-k+1} of the step before the run (zero before bin 0); the loads are
+        // unconditional so that they are issued together with the first group of the run
+        float2 pl, ph;
+        {
+            const bool first = (k1s | k2) == 0;
+            const int pk1 = k1s > 0 ? k1s - 1 : M1 - 1;
+            const int pk2 = k1s > 0 ? k2 : (first ? 0 : k2 - 1);
+            st_unpack_at<LOG2M1>(Zr, pk1, pk2, log2m2, twa, k1s > 0 ? wb : __ldg(twb + pk2), pl, ph);
+            if (first) { pl = make_float2(0.f, 0.f); ph = make_float2(0.f, 0.f); }
+        }
         // low bin e = k - kL0 = k1 + M1 k2off at s_lo[e + k2off]; the same step yields the high bin
         // eh = 9W + 1 - e, and eh - 2 = (M1 - 1 - k1) + M1 (9Q - 1 - k2off): both addresses move by
         // one float per step (steps e = 0, 1 land in two unused floats at the top of the high tile)
         float* __restrict__ lo = s_lo + k1s + k2off * (M1 + 1);
         float* __restrict__ hi = s_hi + (M1 - 1 - k1s) + (9 * Q - 1 - k2off) * (M1 + 1);
-        const float2* __restrict__ zkp = Zr + (size_t)k1s * m2 + k2;
-        const float2* __restrict__ zmp = Zr + (size_t)(M1 - k1s) * m2 + (m2 - 1 - k2);     // row M1 is never read (k1s = 0 below)
+        const float2* zkp = Zr + (size_t)k1s * m2 + k2;                                   // walks down the rows
+        const float2* zmp = Zr + (size_t)(M1 - k1s) * m2 + (m2 - 1 - k2);                 // walks up; row M1 is never read (k1s = 0 below)
         const float2* __restrict__ wap = twa + k1s;
-        constexpr int UN = 4;
+        constexpr int UN = (LC % 8 == 0) ? 8 : 4;
 #pragma unroll 1
         for (int i0 = 0; i0 < LC; i0 += UN) {
-            float2 zk[UN], zm[UN], wa[UN];
+            float2 zk[UN], zm[UN];
 #pragma unroll
             for (int u = 0; u < UN; ++u) {
-                const int it = i0 + u;
-                zk[u] = __ldg(zkp + (size_t)it * m2);
-                if (it == 0 && k1s == 0) zm[u] = __ldg(Zr + ((m2 - k2) & (m2 - 1)));          // k1 = 0 mirrors inside row 0
-                else                     zm[u] = __ldg(zmp - (size_t)it * m2);
-                wa[u] = __ldg(wap + it);
+                zk[u] = __ldg(zkp);
+                zm[u] = __ldg((i0 + u == 0 && k1s == 0) ? Zr + ((m2 - k2) & (m2 - 1)) : zmp);   // k1 = 0 mirrors inside row 0
+                zkp += m2; zmp -= m2;
             }
+            // W_N^k = W_N^{k1} W_N^{M1 k2}: exact table value at the head of the group, then rotated
+            // by rot = W_N^1 (UN - 1 fp32 rotations: relative error below 1e-6)
+            const float2 wa = __ldg(wap + i0);
+            float2 w = make_float2(wa.x * wb.x - wa.y * wb.y, wa.x * wb.y + wa.y * wb.x);
 #pragma unroll
             for (int u = 0; u < UN; ++u) {
                 const int it = i0 + u;
                 float2 xk, xm;
-                st_unpack2(zk[u], zm[u], make_float2(wa[u].x * wb.x - wa[u].y * wb.y, wa[u].x * wb.y + wa[u].y * wb.x), xk, xm);
+                st_unpack2(zk[u], zm[u], w, xk, xm);
                 if (it == 0 && (k1s | k2) == 0) xk = make_float2(0.f, 0.f);                   // X_0 <- 0 (G13)
                 lo[it] = st_interbin(xk, pl);
                 hi[-it] = st_interbin(ph, xm);
                 pl = xk; ph = xm;
+                w = make_float2(w.x * rot.x - w.y * rot.y, w.x * rot.y + w.y * rot.x);
             }
         }
         if (threadIdx.x < 2) {                           // the two steps above the low tile: high bins hH0 + 1, hH0
@@ -651,7 +639,7 @@ k_spectrum_t(const float2* __restrict__ Zt, float* __restrict__ P, float* __rest
             for (int i = 0; i < VPT; ++i) Praw[(size_t)row * m + (size_t)blk * W + i * 32 + lane] = 0.25f * p[i];
         }
         // scratch for the bracket list: floats of this warp's own block (all of them are in registers now)
-        const float m_cur = warp_median<W>(p, (side ? s_hi : s_lo) + wid * (W + Q), lane, owner ? fallbacks : nullptr);
+        const float m_cur = warp_median<W>(p, (side ? s_hi - 3 : s_lo) + wid * (W + Q), lane, owner ? fallbacks : nullptr);
         if (lane == 0) {
             s_med[side][wid] = m_cur;
             if (owner) med[(size_t)row * nblk + blk] = 0.25f * m_cur;
