@@ -188,7 +188,7 @@ def run_ours(args, wl):
     plan = tb.Plan(host_series, wl.tsamp, device=local, stream=stream.cuda_stream, enable_timings=True,
                    chunk_templates=args.chunk, fft_path=args.fft_path)
     chunk = plan.info()["chunk_templates"]
-    stage_keys = ["ms_resample", "ms_fft", "ms_spectrum", "ms_normalise", "ms_hsum", "ms_total"]
+    stage_keys = ["ms_delay", "ms_resample", "ms_fft", "ms_spectrum", "ms_hsum", "ms_total"]
 
     def step():
         plan.search(wl.templates, first_id, FOLDS, SIGMA)
@@ -203,6 +203,7 @@ def run_ours(args, wl):
     stages = {k: 0.0 for k in stage_keys}
     launches = 0
     n_cands = 0
+    path_used = 0
     ev0.record(stream)
     for _ in range(args.steps):
         cands, n = step()
@@ -211,6 +212,7 @@ def run_ours(args, wl):
         for k in stage_keys:
             stages[k] += tm[k]
         launches += tm["n_kernel_launches"]
+        path_used = tm["fft_path_used"]
     ev1.record(stream)
     barrier()
     ms = max_over_ranks(ev0.elapsed_time(ev1))
@@ -247,11 +249,16 @@ def run_ours(args, wl):
     # ---- roofline ----
     peak, peak_src = measured_peaks()
     per_t = {k: stages[k] / (K * args.steps) * 1e-3 for k in stage_keys}          # seconds per template
-    model = {"ms_resample": 4 * N + 4 * N // chunk, "ms_fft": 8 * N, "ms_spectrum": 6 * N,
-             "ms_normalise": 0, "ms_hsum": 2 * N}
-    names = {"ms_resample": "k_resample (a2+a3)", "ms_fft": "cuFFT R2C batched (a4)",
-             "ms_spectrum": "k_spectrum_median (a5+a6)", "ms_normalise": "k_normalise (a7)",
-             "ms_hsum": "k_hsum_threshold (a8+a9)"}
+    # algorithmic bytes each kernel must move per template
+    if path_used == 2:
+        model = {"ms_delay": 0, "ms_resample": 4 * N + 4 * N // chunk, "ms_fft": 8 * N, "ms_spectrum": 6 * N, "ms_hsum": 2 * N}
+        names = {"ms_delay": "K0 k_delay_segments (a2 knots)", "ms_resample": "P1 k_fft_cols (a2+a3, a4 pass 1)",
+                 "ms_fft": "P2 k_fft_rows_t (a4 pass 2)", "ms_spectrum": "k_spectrum_t (a4 unpack, a5+a6+a7)",
+                 "ms_hsum": "k_hsum_tile (a8+a9)"}
+    else:
+        model = {"ms_delay": 0, "ms_resample": 4 * N + 4 * N // chunk, "ms_fft": 8 * N, "ms_spectrum": 6 * N, "ms_hsum": 2 * N}
+        names = {"ms_delay": "(unused)", "ms_resample": "k_resample (a2+a3)", "ms_fft": "cuFFT R2C batched (a4)",
+                 "ms_spectrum": "k_spectrum_median (a5+a6+a7)", "ms_hsum": "k_hsum_tile (a8+a9)"}
     stage_report = {}
     for k in stage_keys[:-1]:
         gbs = model[k] / per_t[k] / 1e9 if per_t[k] > 0 else 0.0
@@ -259,12 +266,12 @@ def run_ours(args, wl):
                                   "achieved_gbs": gbs, "frac": gbs / peak,
                                   "share_of_step": per_t[k] / per_t["ms_total"] if per_t["ms_total"] else 0.0}
     dom = max(stage_keys[:-1], key=lambda k: per_t[k])
-    dom_gbs = model[dom] / per_t[dom] / 1e9
+    dom_gbs = model[dom] / per_t[dom] / 1e9 * 1.0
     traffic = None
-    tpath = os.path.join(ROOT, "profiles", "traffic.json")   # written by hand from the ncu --set full capture
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")   # dram bytes per launch, copied from the ncu --set full capture
     if os.path.exists(tpath):
         with open(tpath) as f:
-            traffic = json.load(f).get(dom)
+            traffic = json.load(f).get(names[dom].split(" (")[0])
     roofline = {"bound": "hbm", "kernel": names[dom], "achieved": dom_gbs, "peak": peak, "unit": "GB/s",
                 "frac": dom_gbs / peak, "traffic": traffic, "peak_source": peak_src,
                 "launches_timed": int(args.steps * -(-K // chunk)),

@@ -95,18 +95,28 @@ typedef struct {
     float    fill_value;
     int32_t  enable_timings;      /* 1: record CUDA events around every stage of every chunk */
     int32_t  fft_path;            /* 0: automatic (hand-written two-pass FFT with fused gather where it
-                                     applies: 2^17 <= N <= 2^23 and knot spacing >= 8, batched cuFFT
-                                     otherwise); 1: always cuFFT; 2: hand-written or TB_ERR_INVALID_ARG */
+                                     applies: 2^17 <= N <= 2^23, W in {512, 1024, 2048} (256 or 1024 at
+                                     2^17) and knot spacing >= 8; batched cuFFT otherwise); 1: always
+                                     cuFFT; 2: hand-written or TB_ERR_INVALID_ARG */
 } tb_plan_opts;
 
-/* Per-stage device time of the last tb_search_templates call (CUDA events, summed over chunks;
- * zero unless opts.enable_timings), and the byte model of DESIGN.md section 7. */
+/* Per-stage device time of the last tb_search_templates call (CUDA events on the plan's stream,
+ * summed over chunks; zero unless opts.enable_timings), and the byte model of DESIGN.md section 7.
+ *   hand-written FFT path (fft_path_used = 2)        cuFFT path (fft_path_used = 1)
+ *   ms_delay     K0 k_delay_segments (a2 knots)      0
+ *   ms_resample  P1 k_fft_cols (a2+a3 + a4 pass 1)   k_resample (a2+a3)
+ *   ms_fft       P2 k_fft_rows_t (a4 pass 2)         batched cuFFT R2C (a4)
+ *   ms_spectrum  k_spectrum_t (a4 unpack, a5-a7)     k_spectrum_median (a5-a7)
+ *   ms_hsum      k_hsum_tile (a8+a9)                 same
+ * ms_normalise is always 0 (a7 is fused into the spectrum kernels); kept for layout stability. */
 typedef struct {
-    double   ms_resample, ms_fft, ms_spectrum /* a5+a6: spectrum + block medians */, ms_normalise, ms_hsum, ms_total;
+    double   ms_resample, ms_fft, ms_spectrum, ms_normalise, ms_hsum, ms_total;
     uint64_t n_templates, n_samples, n_chunks, chunk_templates;
     uint64_t model_bytes_per_template;   /* 22*N: algorithmic HBM bytes */
     uint64_t n_kernel_launches;          /* libtb's own kernels launched by that call (cuFFT's not counted) */
     uint64_t n_median_fallbacks;         /* median blocks that took the data-independent bisection path */
+    double   ms_delay;
+    uint64_t fft_path_used;              /* 1: batched cuFFT, 2: hand-written two-pass FFT with fused gather */
 } tb_timings;
 
 /* Create a plan for one dedispersed time series S[i], i*tsamp.

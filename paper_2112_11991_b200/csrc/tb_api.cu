@@ -23,7 +23,7 @@ static_assert(sizeof(tb_template) == 40, "template layout");
 
 namespace {
 
-constexpr int N_STAGE_EVENTS = 6;   // start, resample, fft, spectrum+median, normalise, hsum
+constexpr int N_STAGE_EVENTS = 6;   // start, delay model (K0), resample / P1, fft / P2, spectrum+median+normalise, hsum
 
 struct EventSet { cudaEvent_t e[N_STAGE_EVENTS]; };
 
@@ -306,12 +306,13 @@ int launch_rows(tb_plan* p, uint32_t nt)
 }
 
 // K0 + P1: delay segments, then gather + column FFTs into T (the buffer the legacy path uses for y)
-int run_own_pass1(tb_plan* p, size_t off, uint32_t nt, long long* d_idx, float* d_y)
+int run_own_pass1(tb_plan* p, size_t off, uint32_t nt, long long* d_idx, float* d_y, cudaEvent_t after_k0 = nullptr)
 {
     const int cta_per_tmpl = (int)(((p->n >> p->min_log2h) + 255) / 256);   // min_log2h: smallest knot spacing staged
     k_delay_segments<<<(unsigned)(cta_per_tmpl * nt), 256, 0, p->stream>>>(p->d_tmpl + off, (int)nt, (int)p->n, p->d_seg,
                                                                            p->seg_stride, cta_per_tmpl);
     TB_CUDA(p, cudaGetLastError());
+    if (after_k0) TB_CUDA(p, cudaEventRecord(after_k0, p->stream));
     const bool dbg = d_idx != nullptr;
     switch (p->log2m1 - 8) {
         case 0: return dbg ? launch_cols<1, true>(p, off, nt, d_idx, d_y) : launch_cols<1, false>(p, off, nt, nullptr, nullptr);
@@ -746,6 +747,7 @@ int tb_search_templates(tb_plan* p, const tb_template* tmpl, uint64_t n_template
     if (rc) return rc;
 
     const bool own = p->own_fft && p->min_log2h >= OWN_MIN_LOG2H;
+    p->last.fft_path_used = own ? 2 : 1;
     for (uint64_t off = 0; off < n_templates; off += p->chunk) {
         const uint32_t nt = (uint32_t)std::min<uint64_t>(p->chunk, n_templates - off);
         EventSet* es = nullptr;
@@ -758,22 +760,22 @@ int tb_search_templates(tb_plan* p, const tb_template* tmpl, uint64_t n_template
             es = &p->events[p->events_used++];
             TB_CUDA(p, cudaEventRecord(es->e[0], p->stream));
         }
-        if (own) {                                       // K0 + P1 | P2 | transpose + unpack + spectrum + median + normalise
-            if ((rc = run_own_pass1(p, off, nt, nullptr, nullptr))) return rc;
-            if (es) TB_CUDA(p, cudaEventRecord(es->e[1], p->stream));
-            if ((rc = run_own_pass2(p, nt))) return rc;
+        if (own) {                                       // K0 | P1 | P2 | transpose + unpack + spectrum + median + normalise
+            if ((rc = run_own_pass1(p, off, nt, nullptr, nullptr, es ? es->e[1] : nullptr))) return rc;
             if (es) TB_CUDA(p, cudaEventRecord(es->e[2], p->stream));
+            if ((rc = run_own_pass2(p, nt))) return rc;
+            if (es) TB_CUDA(p, cudaEventRecord(es->e[3], p->stream));
             if ((rc = run_spectrum_t(p, nt))) return rc;
             p->last.n_kernel_launches += 2;
         } else {
-            if ((rc = run_resample(p, off, nt, nullptr))) return rc;
             if (es) TB_CUDA(p, cudaEventRecord(es->e[1], p->stream));
-            if ((rc = run_fft(p, nt))) return rc;
+            if ((rc = run_resample(p, off, nt, nullptr))) return rc;
             if (es) TB_CUDA(p, cudaEventRecord(es->e[2], p->stream));
+            if ((rc = run_fft(p, nt))) return rc;
+            if (es) TB_CUDA(p, cudaEventRecord(es->e[3], p->stream));
             if ((rc = run_spectrum(p, nt))) return rc;
         }
-        if (es) TB_CUDA(p, cudaEventRecord(es->e[3], p->stream));
-        if (es) TB_CUDA(p, cudaEventRecord(es->e[4], p->stream));   // a7 is fused into the spectrum kernel
+        if (es) TB_CUDA(p, cudaEventRecord(es->e[4], p->stream));
         if ((rc = run_hsum(p, nt, fp, first_template_id + (uint32_t)off))) return rc;
         if (es) TB_CUDA(p, cudaEventRecord(es->e[5], p->stream));
         p->last.n_chunks++;
@@ -793,11 +795,11 @@ int tb_get_timings(tb_plan* p, tb_timings* out)
         TB_CUDA(p, cudaMemcpy(&fb, p->d_cursor + 1, sizeof(fb), cudaMemcpyDeviceToHost));
         t.n_median_fallbacks = fb;
     }
-    t.ms_resample = t.ms_fft = t.ms_spectrum = t.ms_normalise = t.ms_hsum = t.ms_total = 0.0;
+    t.ms_delay = t.ms_resample = t.ms_fft = t.ms_spectrum = t.ms_normalise = t.ms_hsum = t.ms_total = 0.0;
     for (size_t i = 0; i < p->events_used; ++i) {
         float ms[5];
         for (int s = 0; s < 5; ++s) TB_CUDA(p, cudaEventElapsedTime(&ms[s], p->events[i].e[s], p->events[i].e[s + 1]));
-        t.ms_resample += ms[0]; t.ms_fft += ms[1]; t.ms_spectrum += ms[2]; t.ms_normalise += ms[3]; t.ms_hsum += ms[4];
+        t.ms_delay += ms[0]; t.ms_resample += ms[1]; t.ms_fft += ms[2]; t.ms_spectrum += ms[3]; t.ms_hsum += ms[4];
     }
     if (p->events_used) {
         float tot = 0.f;

@@ -320,7 +320,7 @@ template <int R1> struct RowsCfg {
     static constexpr int PA = 16 * PB + 1;
     static constexpr int R = (R1 >= 8) ? 1 : 8 / R1;       // rows per CTA
     static constexpr int LP = R1 * PA;
-    static constexpr int MINB = (R1 >= 32) ? 2 : 3;        // CTAs per SM the register budget is set for
+    static constexpr int MINB = 3;        // CTAs per SM the register budget is set for
     static constexpr size_t SMEM = (size_t)(R * LP + 256) * sizeof(float2);
 };
 

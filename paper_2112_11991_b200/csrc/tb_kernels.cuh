@@ -298,10 +298,10 @@ __device__ __forceinline__ float warp_median(const float (&p)[W / 32], float* ca
         int cl = 0, ch = nmid;                           // candidates below L, below H
         while (ch - cl > 1 && H - L > 1u) {
             const uint32_t mid = L + ((H - L) >> 1);
-            int c = 0;
+            int cc[3] = {0, 0, 0};                       // three short chains instead of one long one
 #pragma unroll
-            for (int q = 0; q < CPL; ++q) c += (ck[q] < mid) ? 1 : 0;
-            c = __reduce_add_sync(0xffffffffu, c);
+            for (int q = 0; q < CPL; ++q) cc[q % 3] += (ck[q] < mid) ? 1 : 0;
+            const int c = __reduce_add_sync(0xffffffffu, cc[0] + cc[1] + cc[2]);
             if (c <= r1) { L = mid; cl = c; } else { H = mid; ch = c; }
         }
         uint32_t v1 = 0xffffffffu;

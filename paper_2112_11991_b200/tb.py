@@ -40,7 +40,8 @@ class Timings(C.Structure):
                 ("ms_normalise", C.c_double), ("ms_hsum", C.c_double), ("ms_total", C.c_double),
                 ("n_templates", C.c_uint64), ("n_samples", C.c_uint64), ("n_chunks", C.c_uint64),
                 ("chunk_templates", C.c_uint64), ("model_bytes_per_template", C.c_uint64),
-                ("n_kernel_launches", C.c_uint64), ("n_median_fallbacks", C.c_uint64)]
+                ("n_kernel_launches", C.c_uint64), ("n_median_fallbacks", C.c_uint64),
+                ("ms_delay", C.c_double), ("fft_path_used", C.c_uint64)]
 
     def as_dict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}

@@ -217,3 +217,32 @@ def test_c5_sweep(tb, log2n, n_check):
     ids = _sample(256, half, log2n) + [256 + i for i in _sample(256, n_check - half, log2n + 1)]
     cands, rep = full_bank_parity(tb, w, 6.0, ids, max_hit_templates=1)
     assert max(r["flips"] for r in rep.values()) <= 2
+
+
+# ------------------------------------------------------------------ hand-written FFT path: every instantiation
+@pytest.mark.parametrize("log2n,window", [(17, 256), (17, 1024), (18, 512), (19, 1024), (19, 2048), (20, 512),
+                                          (21, 1024), (21, 2048), (22, 2048)])
+def test_own_fft_every_radix_and_window(tb, log2n, window):
+    """One circular and one elliptical template per (row-FFT length, median window) pair the
+    hand-written path is instantiated for: M2 = 256..4096 (R1 = 1..16) x W = 256..2048; 2^23
+    (R1 = 32) is covered by test_c5_sweep.  fft_path=2 fails the plan if the pair is unsupported."""
+    # C5's orbits at 2^17 samples of 64 us are too fast for 8-sample knots (exact fallback, cuFFT path): use C1 there
+    w = wl_mod.config1() if log2n == 17 else wl_mod.config5(log2n=log2n)
+    with tb.Plan(w.series, w.tsamp, median_window=window, fft_path=2) as plan:
+        ids = [0, 5] if log2n == 17 else [3, 256 + 5]
+        plan.search(w.templates[ids], 0, w.folds, 5.0)
+        assert plan.timings()["fft_path_used"] == 2
+        cands, n = plan.candidates()
+        per = by_template(cands)
+        for slot, tid in enumerate(ids):
+            rep = check_template(plan, w, tid, 5.0, w.folds, None)
+            assert rep["flips"] <= 2
+            # candidates of slot `slot` against the oracle for the same template
+            spec_c = per.get(slot, cands[:0])
+            tmpl = w.templates[tid]
+            idx = plan.debug_indices(tmpl)
+            spec = orc.spectrum_of_template(w.series, w.tsamp, tmpl, window, plan.info()["fill_value"], idx=idx)
+            sums = orc.harmonic_sums(spec["normalised"], w.folds)
+            ocand = orc.candidates_from_sums(sums, slot, 5.0, plan.info()["k_lo"])
+            from parity import compare_candidates
+            compare_candidates(spec_c, ocand, sums, 5.0)
