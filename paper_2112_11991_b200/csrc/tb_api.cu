@@ -9,6 +9,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <limits>
 #include <map>
@@ -68,6 +69,9 @@ struct tb_plan {
     float2 *d_tw1a = nullptr, *d_tw1b = nullptr, *d_tw2 = nullptr, *d_twn = nullptr, *d_twb = nullptr;
     float2 rot = {1.f, 0.f};                         // W_N^1
     int min_log2h = 0;                               // smallest knot spacing among the staged templates
+    int n_sm = 148;                                  // multiprocessors of the device
+    int pf_spec = 0;                                 // same for the spectrum former
+    int pf_rows = 0;                                 // L2 prefetch distance of pass 2, in CTAs (resident CTAs of the device)
 
     std::map<uint32_t, cufftHandle> fft_plans;       // by batch size, sharing one work area
     void* d_work = nullptr;
@@ -300,7 +304,7 @@ int launch_rows(tb_plan* p, uint32_t nt)
     if (!attr) { TB_CUDA(p, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM)); attr = true; }
     const unsigned grid = (unsigned)(((1u << p->log2m1) / Cfg::R) * nt);
     kern<<<grid, FFT_THREADS, Cfg::SMEM, p->stream>>>(reinterpret_cast<const float2*>(p->d_resampled), p->d_fft, p->log2m1,
-                                                     p->d_tw1b, p->d_tw2);
+                                                     p->d_tw1b, p->d_tw2, p->pf_rows);
     TB_CUDA(p, cudaGetLastError());
     return TB_OK;
 }
@@ -309,7 +313,7 @@ int launch_rows(tb_plan* p, uint32_t nt)
 int run_own_pass1(tb_plan* p, size_t off, uint32_t nt, long long* d_idx, float* d_y, cudaEvent_t after_k0 = nullptr)
 {
     const int cta_per_tmpl = (int)(((p->n >> p->min_log2h) + 255) / 256);   // min_log2h: smallest knot spacing staged
-    k_delay_segments<<<(unsigned)(cta_per_tmpl * nt), 256, 0, p->stream>>>(p->d_tmpl + off, (int)nt, (int)p->n, p->d_seg,
+    k_delay_segments<<<(unsigned)(cta_per_tmpl * nt), K0_THREADS, 0, p->stream>>>(p->d_tmpl + off, (int)nt, (int)p->n, p->d_seg,
                                                                            p->seg_stride, cta_per_tmpl);
     TB_CUDA(p, cudaGetLastError());
     if (after_k0) TB_CUDA(p, cudaEventRecord(after_k0, p->stream));
@@ -344,12 +348,12 @@ int launch_spectrum_t(tb_plan* p, uint32_t nt, float* d_raw)
         auto kern = k_spectrum_t<W, LOG2M1, true>;
         static bool attr = false;
         if (!attr) { TB_CUDA(p, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); attr = true; }
-        kern<<<grid, ST_THREADS, smem, p->stream>>>(p->d_fft, p->d_power, p->d_med, p->log2m2, (int)p->nblk, p->d_twn, p->d_twb, p->rot, fb, d_raw);
+        kern<<<grid, ST_THREADS, smem, p->stream>>>(p->d_fft, p->d_power, p->d_med, p->log2m2, (int)p->nblk, p->d_twn, p->d_twb, p->rot, fb, d_raw, p->pf_spec);
     } else {
         auto kern = k_spectrum_t<W, LOG2M1, false>;
         static bool attr = false;
         if (!attr) { TB_CUDA(p, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); attr = true; }
-        kern<<<grid, ST_THREADS, smem, p->stream>>>(p->d_fft, p->d_power, p->d_med, p->log2m2, (int)p->nblk, p->d_twn, p->d_twb, p->rot, fb, nullptr);
+        kern<<<grid, ST_THREADS, smem, p->stream>>>(p->d_fft, p->d_power, p->d_med, p->log2m2, (int)p->nblk, p->d_twn, p->d_twb, p->rot, fb, nullptr, p->pf_spec);
     }
     TB_CUDA(p, cudaGetLastError());
     return TB_OK;
@@ -669,6 +673,11 @@ int tb_plan_create(tb_plan** out, const float* series, uint64_t n_samples, doubl
         p->own_fft = fits && o.fft_path != 1;
     }
     if (p->own_fft) {
+        cudaDeviceGetAttribute(&p->n_sm, cudaDevAttrMultiProcessorCount, p->device);
+        const char* pf = getenv("TB_PF_ROWS");           // tuning knob: prefetch distance in CTAs (default: the resident CTAs, 3 per SM)
+        p->pf_rows = pf ? atoi(pf) : p->n_sm * 2;
+        const char* pfs = getenv("TB_PF_SPEC");
+        p->pf_spec = pfs ? atoi(pfs) : 32;
         p->seg_stride = (size_t)(p->n >> OWN_MIN_LOG2H);
         TB_TRY(cudaMalloc(&p->d_seg, (size_t)B * p->seg_stride * sizeof(SegRec)));
         int rc = make_twiddles(p);

@@ -154,10 +154,12 @@ __device__ __forceinline__ void fft_step2(float2* __restrict__ slot, int w, cons
 
 // ---------------------------------------------------------------------------------------------
 // K0  Hermite segment records of the delay for every template of the chunk.
-//   One CTA = 256 consecutive segments of one template (257 exact knots).  Output record s of
-//   template b at seg[b * seg_stride + s].  Same knots and fp64 coefficients as k_resample.
+//   One CTA = 256 consecutive segments of one template (257 exact knots, one per thread of its
+//   nine warps: the 257th knot must not double the fp64 latency chain of thread 0).  Output
+//   record s of template b at seg[b * seg_stride + s].  Same knots and fp64 coefficients as k_resample.
 // ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256)
+constexpr int K0_THREADS = 288;
+__global__ void __launch_bounds__(K0_THREADS)
 k_delay_segments(const TmplDev* __restrict__ tmpl, int n_tmpl, int n, SegRec* __restrict__ seg, size_t seg_stride,
                  int cta_per_tmpl)
 {
@@ -169,14 +171,15 @@ k_delay_segments(const TmplDev* __restrict__ tmpl, int n_tmpl, int n, SegRec* __
     const int nseg = n >> log2h;
     if (s0 >= nseg) return;
     const double h = (double)(1 << log2h);
-    for (int k = threadIdx.x; k <= 256; k += 256) {
+    if (threadIdx.x <= 256) {
+        const int k = threadIdx.x;
         double v, d;
         delay_knot(t, (s0 + k) << log2h, v, d);
         s_val[k] = v; s_slp[k] = d * h;
     }
     __syncthreads();
     const int s = s0 + threadIdx.x;
-    if (s >= nseg) return;
+    if (threadIdx.x >= 256 || s >= nseg) return;
     const double v0 = s_val[threadIdx.x], v1 = s_val[threadIdx.x + 1], g0 = s_slp[threadIdx.x], g1 = s_slp[threadIdx.x + 1];
     const double dv = v1 - v0;
     SegRec r;
@@ -245,28 +248,80 @@ k_fft_cols(const float* __restrict__ x, const SegRec* __restrict__ seg, size_t s
 
     tw2[threadIdx.x] = __ldg(tw2g + threadIdx.x);
 
-    // phase A: gather, radix-R1 over a, twiddle, to shared memory.  item i: col = i % C, w = i / C
+    // phase A0: source indices of every point of the tile, parked as an int2 in the point's own
+    // shared-memory slot (written and read back by the same thread: no barrier).  Splitting the
+    // index computation from the gather turns two dependent memory latencies per point
+    // (segment record -> series sample) into two loops of independent loads.
+    // Thread (col, w0) = (tid % C, tid / C) owns the points (a, w = w0 + 16 it), it < 16: row
+    // j1 = a 256 + w of the tile, samples nn, nn + 1 with nn = 2 (j1 M2 + c0 + col).
+    static_assert(C == 16 && FFT_THREADS == 256, "thread -> (col, w0) mapping");
+    const int col = threadIdx.x & (C - 1), w0 = threadIdx.x >> 4;
+    float2* __restrict__ myslot = fsm + col * LP + w0;                         // + a PA + it PB
+    const int nn0 = (int)((((size_t)w0 << log2m2) + c0 + col) << 1);
+    const int row_shift = log2m2 + 1;                                          // samples between rows j1, j1 + 1
+    if (!DEBUG && log2h >= 5) {
+        // h >= 32: the 32-sample run of a row lies inside one segment, the offset o of a sample in
+        // its segment is the same for every row of the thread, and the record index is linear in j1
+        const int o = nn0 & ((1 << log2h) - 1);
+        const float t0 = (float)o * inv_h, t1 = t0 + inv_h;
+        const char* __restrict__ rec0 = reinterpret_cast<const char*>(segs + (nn0 >> log2h));
+        const int rec_shift = row_shift - log2h + 6;                           // log2 bytes between the records of rows j1, j1 + 1
+#pragma unroll 4
+        for (int it = 0; it < 16; ++it) {
+#pragma unroll
+            for (int a = 0; a < R1; ++a) {
+                const int j1 = a * 256 + 16 * it;                              // row relative to w0
+                const char* r = rec0 + ((size_t)(unsigned)j1 << rec_shift);
+                const float4 f = __ldg(reinterpret_cast<const float4*>(r));
+                const int2 ie = __ldg(reinterpret_cast<const int2*>(r) + 2);
+                const int nn = nn0 + (j1 << row_shift);
+                const float y0 = fmaf(fmaf(fmaf(f.w, t0, f.z), t0, f.y), t0, f.x);
+                const float y1 = fmaf(fmaf(fmaf(f.w, t1, f.z), t1, f.y), t1, f.x);
+                const float z0 = y0 + 12582912.0f, z1 = y1 + 12582912.0f;      // 1.5 * 2^23: round to nearest integer
+                const int base = nn - ie.x + 0x4B400000;
+                int2 src = make_int2(base - __float_as_int(z0), base + 1 - __float_as_int(z1));
+                const float lim = 0.5f - __int_as_float(ie.y);
+                const bool tie0 = fabsf(y0 - (z0 - 12582912.0f)) > lim, tie1 = fabsf(y1 - (z1 - 12582912.0f)) > lim;
+                if (tie0 || tie1) {                                            // rare (about 2 eps per sample)
+                    const double2 c01 = __ldg(reinterpret_cast<const double2*>(r) + 2);
+                    const double2 c23 = __ldg(reinterpret_cast<const double2*>(r) + 3);
+                    const double ta = (double)o * (double)inv_h, tb = (double)(o + 1) * (double)inv_h;
+                    if (tie0) src.x = nn - floor_to_int(fma(fma(fma(c23.y, ta, c23.x), ta, c01.y), ta, c01.x));
+                    if (tie1) src.y = nn + 1 - floor_to_int(fma(fma(fma(c23.y, tb, c23.x), tb, c01.y), tb, c01.x));
+                }
+                *reinterpret_cast<int2*>(myslot + a * PA + it * PB) = src;
+            }
+        }
+    } else {
 #pragma unroll 2
-    for (int i = threadIdx.x; i < 256 * C; i += FFT_THREADS) {
-        const int col = i % C, w = i / C;
+        for (int it = 0; it < 16; ++it) {
+#pragma unroll
+            for (int a = 0; a < R1; ++a) {
+                const int nn = nn0 + ((a * 256 + 16 * it) << row_shift);
+                *reinterpret_cast<int2*>(myslot + a * PA + it * PB) = source_pair(segs, nn, log2h, inv_h);
+            }
+        }
+    }
+    // phase A1: gather (independent loads), radix-R1 over a, twiddle, back to the same slots
+#pragma unroll 4
+    for (int it = 0; it < 16; ++it) {
+        const int w = w0 + 16 * it;
+        float2* p = myslot + it * PB;
         float2 v[R1];
 #pragma unroll
         for (int a = 0; a < R1; ++a) {
-            const int j1 = a * 256 + w;
-            const int nn = (int)((((size_t)j1 << log2m2) + c0 + col) << 1);     // first of the two samples
-            const int2 sp = source_pair(segs, nn, log2h, inv_h);
-            const int s0 = sp.x, s1 = sp.y;
-            v[a].x = ((unsigned)s0 < (unsigned)n) ? __ldg(x + s0) : fill;
-            v[a].y = ((unsigned)s1 < (unsigned)n) ? __ldg(x + s1) : fill;
+            const int2 sp = *reinterpret_cast<const int2*>(p + a * PA);
+            v[a].x = ((unsigned)sp.x < (unsigned)n) ? __ldg(x + sp.x) : fill;
+            v[a].y = ((unsigned)sp.y < (unsigned)n) ? __ldg(x + sp.y) : fill;
             if (DEBUG) {
-                idx_out[(size_t)b * n + nn] = s0; idx_out[(size_t)b * n + nn + 1] = s1;
-                y_out[(size_t)b * n + nn] = v[a].x; y_out[(size_t)b * n + nn + 1] = v[a].y;
+                const size_t nn = (size_t)b * n + (size_t)(nn0 + ((a * 256 + 16 * it) << row_shift));
+                idx_out[nn] = sp.x; idx_out[nn + 1] = sp.y;
+                y_out[nn] = v[a].x; y_out[nn + 1] = v[a].y;
             }
         }
         fft_reg<R1>(v);
 #pragma unroll
         for (int ka = 1; ka < R1; ++ka) v[ka] = cmul(v[ka], __ldg(tw1 + ka * 256 + w));
-        float2* p = fsm + col * LP + (w >> 4) * PB + (w & 15);
 #pragma unroll
         for (int ka = 0; ka < R1; ++ka) p[ka * PA] = v[ka];
     }
@@ -327,7 +382,7 @@ template <int R1> struct RowsCfg {
 template <int R1>
 __global__ void __launch_bounds__(FFT_THREADS, RowsCfg<R1>::MINB)
 k_fft_rows_t(const float2* __restrict__ T, float2* __restrict__ Zt, int log2m1, const float2* __restrict__ tw1,
-             const float2* __restrict__ tw2g)
+             const float2* __restrict__ tw2g, int pf_dist)
 {
     using Cfg = RowsCfg<R1>;
     constexpr int PA = Cfg::PA, PB = Cfg::PB, R = Cfg::R, LP = Cfg::LP;
@@ -342,6 +397,13 @@ k_fft_rows_t(const float2* __restrict__ T, float2* __restrict__ Zt, int log2m1, 
     float2* __restrict__ Zb = Zt + off;
 
     tw2[threadIdx.x] = __ldg(tw2g + threadIdx.x);
+    // Pull the rows of the CTA that will take over this CTA's slot (pf_dist blocks ahead) into L2
+    // with one bulk prefetch, so that DRAM keeps streaming while the resident CTAs are in their
+    // compute phases (without it the reads come in bursts at CTA start and HBM idles in between).
+    if (threadIdx.x == 0 && pf_dist > 0 && blockIdx.x + pf_dist < gridDim.x) {
+        const float2* nxt = T + (size_t)(blockIdx.x + pf_dist) * (size_t)(R * L);
+        asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(nxt), "r"((unsigned)(R * L * sizeof(float2))) : "memory");
+    }
 
     {   // phase A: item (r, w) = (it, threadIdx.x); every global load of the thread is issued before
         // the first butterfly so that one memory round trip covers the whole tile

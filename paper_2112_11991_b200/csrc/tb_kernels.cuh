@@ -534,7 +534,7 @@ template <int W, int LOG2M1, bool RAW>
 __global__ void __launch_bounds__(ST_THREADS, (W <= 1024) ? 3 : 1)
 k_spectrum_t(const float2* __restrict__ Zt, float* __restrict__ P, float* __restrict__ med, int log2m2,
              int nblk, const float2* __restrict__ twa, const float2* __restrict__ twb, float2 rot,
-             unsigned long long* __restrict__ fallbacks, float* __restrict__ Praw)
+             unsigned long long* __restrict__ fallbacks, float* __restrict__ Praw, int pf_dist)
 {
     static_assert(W >= (1 << LOG2M1), "a median block is a whole number of columns");
     constexpr int M1 = 1 << LOG2M1;
@@ -553,6 +553,20 @@ k_spectrum_t(const float2* __restrict__ Zt, float* __restrict__ P, float* __rest
     const float2* __restrict__ Zr = Zt + (size_t)row * m;
     const int a = 8 * g * Q;                             // first column of the low tile
     const int wid = threadIdx.x >> 5, lane = threadIdx.x & 31;
+
+    // Pull the two tiles of the CTA that will take over this CTA's slot (pf_dist blocks ahead) into
+    // L2: one 128-byte line per row and side (the 16-byte tail of a run is the next group's line),
+    // so that DRAM keeps streaming while the resident CTAs select medians.
+    if (pf_dist > 0 && blockIdx.x + pf_dist < gridDim.x) {
+        const unsigned nb = blockIdx.x + pf_dist;
+        const float2* __restrict__ Zn = Zt + (size_t)(nb / groups) * m;
+        const int an = 8 * (int)(nb % groups) * Q;
+        const size_t m2n = (size_t)1 << log2m2;
+        for (int k1 = threadIdx.x; k1 < M1; k1 += ST_THREADS) {
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(Zn + (size_t)k1 * m2n + an));
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(Zn + (size_t)k1 * m2n + (m2n - an - 8 * Q)));
+        }
+    }
 
     {   // ---- phase 1: unpack + interbin, powers to shared memory in bin order ----
         const int k2off = threadIdx.x % NK2, k1s = (threadIdx.x / NK2) * LC;
@@ -659,16 +673,30 @@ k_spectrum_t(const float2* __restrict__ Zt, float* __restrict__ P, float* __rest
         for (int h = 0; h < 2; ++h) {
             if (!(h ? can_second : can_first)) continue;
             const float ma = h ? m_cur : m_prev, mb = h ? m_next : m_cur;
-            // baseline at bin offset eo: ma + ((eo -+ W/2) + 1/2)/W (mb - ma) = b0 + i * st32
-            const float st32 = 32.0f * INV_W * (mb - ma);
-            const float b0 = fmaf(((float)(lane + (h ? 0 : W / 2)) + 0.5f) * INV_W, mb - ma, ma);
+            // baseline at bin offset eo: ma + ((eo -+ W/2) + 1/2)/W (mb - ma) = b0 + i * st32; the
+            // factor 1/ln2 is folded into the baseline so that P^ = P * rcp(baseline / ln2)
+            constexpr float INV_LN2 = 1.0f / LN2;
+            const float st32 = (32.0f * INV_W * INV_LN2) * (mb - ma);
+            const float b0 = fmaf(((float)(lane + (h ? 0 : W / 2)) + 0.5f) * INV_W, mb - ma, ma) * INV_LN2;
+            if (fminf(ma, mb) > 0.f) {                   // the interpolated baseline lies between ma and mb: positive
 #pragma unroll
-            for (int ii = 0; ii < VPT / 2; ++ii) {
-                const int i = h * (VPT / 2) + ii;
-                const float bl = fmaf((float)ii, st32, b0);
-                float o = (bl > 0.f) ? __fdividef(p[i] * LN2, bl) : 0.f;
-                if (i == 0 && blk == 0 && lane == 0) o = 0.f;        // P^_0 = 0
-                Pr[32 * i] = o;
+                for (int ii = 0; ii < VPT / 2; ++ii) {
+                    const int i = h * (VPT / 2) + ii;
+                    float r;
+                    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(fmaf((float)ii, st32, b0)));
+                    float o = p[i] * r;
+                    if (i == 0 && blk == 0 && lane == 0) o = 0.f;    // P^_0 = 0
+                    Pr[32 * i] = o;
+                }
+            } else {
+#pragma unroll
+                for (int ii = 0; ii < VPT / 2; ++ii) {
+                    const int i = h * (VPT / 2) + ii;
+                    const float bl = fmaf((float)ii, st32, b0);
+                    float o = (bl > 0.f) ? __fdividef(p[i], bl) : 0.f;
+                    if (i == 0 && blk == 0 && lane == 0) o = 0.f;    // P^_0 = 0
+                    Pr[32 * i] = o;
+                }
             }
         }
     }
@@ -738,8 +766,8 @@ k_hsum_threshold(const float* __restrict__ Ph, int nb, int cta_per_row, FoldPara
 
 // ---------------------------------------------------------------------------------------------
 // K4t  tiled harmonic summer (a8 + a9) for Nb >= HS_T.  Same sums as k_hsum_threshold.
-//   One CTA = HS_T consecutive top-harmonic bins of one template; one thread = 16 consecutive
-//   bins k = k0 + 16 q + r.  For harmonic m/2^L (odd m) those 16 bins read the m*(16>>L)+1
+//   One CTA = HS_T consecutive top-harmonic bins of one template; a pair of threads = 16
+//   consecutive bins k = k0 + 16 q + r (one thread r < 8, the other r >= 8).  For harmonic m/2^L (odd m) those 16 bins read the m*(16>>L)+1
 //   consecutive values starting at (m k0 >> L) + m q (16>>L), and WHICH of them bin r takes,
 //   (m r + 2^(L-1)) >> L, is a compile-time constant: after unrolling there is no index
 //   arithmetic left, 9.4 loads per bin instead of 16, and every add is register-to-register.
@@ -751,7 +779,7 @@ k_hsum_threshold(const float* __restrict__ Ph, int nb, int cta_per_row, FoldPara
 //   while its 8.5 reads per bin are served (L2 -> SM traffic 17N bytes per template).
 // ---------------------------------------------------------------------------------------------
 constexpr int HS_T = 2048;
-constexpr int HS_THREADS = HS_T / 16;
+constexpr int HS_THREADS = HS_T / 8;
 
 __host__ __device__ constexpr int hs_len(int L, int m) { return m * (HS_T >> L) + 4; }
 __host__ __device__ constexpr int hs_off(int L, int m)
@@ -795,44 +823,44 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
                  : "memory");
 }
 
-// acc[r] += span[(M r + 2^(L-1)) >> L], span = the M*(16>>L)+1 staged values of this thread
-template <int L, int M>
-__device__ __forceinline__ void hs_accumulate(const float* __restrict__ sm, int q, float (&acc)[16])
+// One thread = 8 consecutive bins k = k0 + 16 q + 8 HALF + r, r < 8 (HALF is uniform per warp, so
+// a warp's lanes keep the conflict-free stride of m*(16>>L) words).  With r' = r + 8 HALF the
+// value bin r takes from the staged span of group q is (M r' + 2^(L-1)) >> L, a compile-time
+// constant; the thread loads only the NV values its 8 bins touch, starting OFF words into the span.
+template <int L, int M, int HALF>
+__device__ __forceinline__ void hs_accumulate(const float* __restrict__ sm, int q, float (&acc)[8])
 {
-    constexpr int STEP = M * (16 >> L);              // words between consecutive threads' spans
-    constexpr int NV = STEP + 1;
-    const float* sp = sm + hs_off(L, M) + q * STEP;
-    float v[NV];
-    if constexpr (L == 2) {                          // STEP multiple of 4: 128-bit loads
+    constexpr int STEP = M * (16 >> L);              // words between consecutive groups' spans
+    constexpr int RND = 1 << (L - 1);
+    constexpr bool VEC2 = (STEP % 2 == 0);           // even lane stride: 64-bit loads (32-bit ones would be 2-way bank conflicts)
+    constexpr int OFF0 = (M * 8 * HALF + RND) >> L;  // first value the 8 bins touch
+    constexpr int OFF = VEC2 ? (OFF0 & ~1) : OFF0;
+    constexpr int NV = ((M * (7 + 8 * HALF) + RND) >> L) - OFF + 1;
+    const float* sp = sm + hs_off(L, M) + q * STEP + OFF;
+    float v[NV + 1];
+    if constexpr (VEC2) {                            // the regions carry 4 floats of padding
 #pragma unroll
-        for (int i = 0; i < STEP; i += 4) {
-            const float4 t = *reinterpret_cast<const float4*>(sp + i);
-            v[i] = t.x; v[i + 1] = t.y; v[i + 2] = t.z; v[i + 3] = t.w;
-        }
-    } else if constexpr (L == 3) {                   // STEP multiple of 2: 64-bit loads
-#pragma unroll
-        for (int i = 0; i < STEP; i += 2) {
+        for (int i = 0; i < NV; i += 2) {
             const float2 t = *reinterpret_cast<const float2*>(sp + i);
             v[i] = t.x; v[i + 1] = t.y;
         }
     } else {
 #pragma unroll
-        for (int i = 0; i < STEP; ++i) v[i] = sp[i];
+        for (int i = 0; i < NV; ++i) v[i] = sp[i];
     }
-    v[STEP] = sp[STEP];
 #pragma unroll
-    for (int r = 0; r < 16; ++r) acc[r] += v[(M * r + (1 << (L - 1))) >> L];
+    for (int r = 0; r < 8; ++r) acc[r] += v[((M * (r + 8 * HALF) + RND) >> L) - OFF];
 }
 
 // rare path: emit the hits of one fold with a warp-aggregated atomic per bin offset
 template <int L>
-__device__ __forceinline__ void hs_emit(const float (&acc)[16], uint32_t kq, const FoldParams& fp, uint32_t tid,
+__device__ __forceinline__ void hs_emit(const float (&acc)[8], uint32_t kq, const FoldParams& fp, uint32_t tid,
                                         Candidate* __restrict__ out, unsigned long long* __restrict__ cursor,
                                         unsigned long long capacity)
 {
     const unsigned lane = threadIdx.x & 31;
 #pragma unroll
-    for (int r = 0; r < 16; ++r) {                   // unrolled: acc[] must stay in registers
+    for (int r = 0; r < 8; ++r) {                    // unrolled: acc[] must stay in registers
         const uint32_t k = kq + (uint32_t)r;
         const bool hit = (acc[r] >= fp.thr[L]) && (k >= (fp.k_lo << L));
         const unsigned mask = __ballot_sync(0xffffffffu, hit);
@@ -855,15 +883,13 @@ __device__ __forceinline__ void hs_emit(const float (&acc)[16], uint32_t kq, con
 }
 
 template <int L>
-__device__ __forceinline__ void hs_check(const float (&acc)[16], uint32_t kq, const FoldParams& fp, uint32_t tid,
+__device__ __forceinline__ void hs_check(const float (&acc)[8], uint32_t kq, const FoldParams& fp, uint32_t tid,
                                          Candidate* __restrict__ out, unsigned long long* __restrict__ cursor,
                                          unsigned long long capacity)
 {
-    bool any = false;
     const float thr = fp.thr[L];
-#pragma unroll
-    for (int r = 0; r < 16; ++r) any |= (acc[r] >= thr);
-    if (__any_sync(0xffffffffu, any)) hs_emit<L>(acc, kq, fp, tid, out, cursor, capacity);
+    const float mx = fmaxf(fmaxf(fmaxf(acc[0], acc[1]), fmaxf(acc[2], acc[3])), fmaxf(fmaxf(acc[4], acc[5]), fmaxf(acc[6], acc[7])));
+    if (__any_sync(0xffffffffu, mx >= thr)) hs_emit<L>(acc, kq, fp, tid, out, cursor, capacity);
 }
 
 // issue the 14 bulk copies of one tile's regions into `sm`, completion on `bar` (one thread)
@@ -877,27 +903,63 @@ __device__ __forceinline__ void hs_stage(float* sm, const float* __restrict__ p,
             bulk_g2s(sm + hs_off(L, m), p + (((size_t)m * (size_t)k0) >> L), (uint32_t)(hs_len(L, m) * sizeof(float)), bar);
 }
 
-struct HsDirect {                                    // folds 0 and 1 of one thread's 16 bins, from global memory
-    float4 a0, a1, a2, a3, h0, h1;
-    float  h2;
+struct HsDirect {                                    // folds 0 and 1 of one thread's 8 bins, from global memory
+    float4 a0, a1, h0;
+    float  h1;
 };
 __device__ __forceinline__ HsDirect hs_load_direct(const float* __restrict__ p, uint32_t kq)
 {
     HsDirect d;
     const float4* a = reinterpret_cast<const float4*>(p + kq);
-    d.a0 = __ldg(a); d.a1 = __ldg(a + 1); d.a2 = __ldg(a + 2); d.a3 = __ldg(a + 3);
-    const float* h = p + (kq >> 1);
+    d.a0 = __ldg(a); d.a1 = __ldg(a + 1);
+    const float* h = p + (kq >> 1);                  // kq is a multiple of 8
     d.h0 = __ldg(reinterpret_cast<const float4*>(h));
-    d.h1 = __ldg(reinterpret_cast<const float4*>(h) + 1);
-    d.h2 = __ldg(h + 8);
+    d.h1 = __ldg(h + 4);
     return d;
+}
+
+// sums + checks of one thread's 8 bins of the tile staged in `sm`
+template <int HALF>
+__device__ __forceinline__ void hs_tile_body(const float* __restrict__ sm, int q, const HsDirect& d, uint32_t kq,
+                                             uint64_t* bar, uint32_t parity, const FoldParams& fp, uint32_t tid,
+                                             Candidate* __restrict__ out, unsigned long long* __restrict__ cursor,
+                                             unsigned long long capacity)
+{
+    float acc[8] = {d.a0.x, d.a0.y, d.a0.z, d.a0.w, d.a1.x, d.a1.y, d.a1.z, d.a1.w};   // fold 0: the bin itself
+    hs_check<0>(acc, kq, fp, tid, out, cursor, capacity);
+    {                                                // fold 1: + P^[(k+1)>>1], 5 values from kq/2 on
+        const float v[5] = {d.h0.x, d.h0.y, d.h0.z, d.h0.w, d.h1};
+#pragma unroll
+        for (int r = 0; r < 8; ++r) acc[r] += v[(r + 1) >> 1];
+    }
+    hs_check<1>(acc, kq, fp, tid, out, cursor, capacity);
+
+    mbar_wait(bar, parity);
+    hs_accumulate<2, 1, HALF>(sm, q, acc);
+    hs_accumulate<2, 3, HALF>(sm, q, acc);
+    hs_check<2>(acc, kq, fp, tid, out, cursor, capacity);
+    hs_accumulate<3, 1, HALF>(sm, q, acc);
+    hs_accumulate<3, 3, HALF>(sm, q, acc);
+    hs_accumulate<3, 5, HALF>(sm, q, acc);
+    hs_accumulate<3, 7, HALF>(sm, q, acc);
+    hs_check<3>(acc, kq, fp, tid, out, cursor, capacity);
+    hs_accumulate<4, 1, HALF>(sm, q, acc);
+    hs_accumulate<4, 3, HALF>(sm, q, acc);
+    hs_accumulate<4, 5, HALF>(sm, q, acc);
+    hs_accumulate<4, 7, HALF>(sm, q, acc);
+    hs_accumulate<4, 9, HALF>(sm, q, acc);
+    hs_accumulate<4, 11, HALF>(sm, q, acc);
+    hs_accumulate<4, 13, HALF>(sm, q, acc);
+    hs_accumulate<4, 15, HALF>(sm, q, acc);
+    hs_check<4>(acc, kq, fp, tid, out, cursor, capacity);
 }
 
 // A CTA walks `tpc` consecutive tiles of one template with two staging buffers: while tile t is
 // summed out of one buffer the bulk copies of tile t+1 land in the other, and the fold-0/1
 // values of tile t+1 are already on their way to registers, so no warp waits on memory once the
-// first tile is in (the single-buffered version spent 2/3 of its issue slots waiting).
-__global__ void __launch_bounds__(HS_THREADS)
+// first tile is in.  Warps 0-3 take bins 0-7 of every group of 16, warps 4-7 bins 8-15: 16 warps
+// per SM instead of 8 on the same staged bytes (the staging, not the registers, limits residency).
+__global__ void __launch_bounds__(HS_THREADS, 2)
 k_hsum_tile(const float* __restrict__ Ph, int nb, int groups_per_row, int tpc, FoldParams fp, uint32_t first_id,
             Candidate* __restrict__ out, unsigned long long* __restrict__ cursor, unsigned long long capacity)
 {
@@ -907,50 +969,24 @@ k_hsum_tile(const float* __restrict__ Ph, int nb, int groups_per_row, int tpc, F
     const int tile0 = (blockIdx.x % groups_per_row) * tpc;
     const float* __restrict__ p = Ph + (size_t)row * (size_t)nb;
     const uint32_t tid = first_id + (uint32_t)row;
-    const int q = threadIdx.x;
+    const int q = threadIdx.x & (HS_T / 16 - 1), half = threadIdx.x / (HS_T / 16);
 
     if (threadIdx.x == 0) { mbar_init(&bar[0], 1); mbar_init(&bar[1], 1); }
     __syncthreads();
     if (threadIdx.x == 0) hs_stage(hs_sm, p, tile0 * HS_T, &bar[0]);
-    HsDirect nxt = hs_load_direct(p, (uint32_t)(tile0 * HS_T + 16 * q));
+    HsDirect nxt = hs_load_direct(p, (uint32_t)(tile0 * HS_T + 16 * q + 8 * half));
 
     for (int t = 0; t < tpc; ++t) {
         const int k0 = (tile0 + t) * HS_T;
-        const uint32_t kq = (uint32_t)(k0 + 16 * q);
+        const uint32_t kq = (uint32_t)(k0 + 16 * q + 8 * half);
         const float* sm = hs_sm + (t & 1) * HS_SMEM_FLOATS;
         if (t + 1 < tpc && threadIdx.x == 0)         // the other buffer was released by the barrier that ended tile t-1
             hs_stage(hs_sm + ((t + 1) & 1) * HS_SMEM_FLOATS, p, k0 + HS_T, &bar[(t + 1) & 1]);
         const HsDirect d = nxt;
         if (t + 1 < tpc) nxt = hs_load_direct(p, kq + HS_T);
-
-        float acc[16] = {d.a0.x, d.a0.y, d.a0.z, d.a0.w, d.a1.x, d.a1.y, d.a1.z, d.a1.w,
-                         d.a2.x, d.a2.y, d.a2.z, d.a2.w, d.a3.x, d.a3.y, d.a3.z, d.a3.w};   // fold 0: the bin itself
-        hs_check<0>(acc, kq, fp, tid, out, cursor, capacity);
-        {                                            // fold 1: + P^[(k+1)>>1], 9 values from 8 q'
-            const float v[9] = {d.h0.x, d.h0.y, d.h0.z, d.h0.w, d.h1.x, d.h1.y, d.h1.z, d.h1.w, d.h2};
-#pragma unroll
-            for (int r = 0; r < 16; ++r) acc[r] += v[(r + 1) >> 1];
-        }
-        hs_check<1>(acc, kq, fp, tid, out, cursor, capacity);
-
-        mbar_wait(&bar[t & 1], (uint32_t)((t >> 1) & 1));
-        hs_accumulate<2, 1>(sm, q, acc);
-        hs_accumulate<2, 3>(sm, q, acc);
-        hs_check<2>(acc, kq, fp, tid, out, cursor, capacity);
-        hs_accumulate<3, 1>(sm, q, acc);
-        hs_accumulate<3, 3>(sm, q, acc);
-        hs_accumulate<3, 5>(sm, q, acc);
-        hs_accumulate<3, 7>(sm, q, acc);
-        hs_check<3>(acc, kq, fp, tid, out, cursor, capacity);
-        hs_accumulate<4, 1>(sm, q, acc);
-        hs_accumulate<4, 3>(sm, q, acc);
-        hs_accumulate<4, 5>(sm, q, acc);
-        hs_accumulate<4, 7>(sm, q, acc);
-        hs_accumulate<4, 9>(sm, q, acc);
-        hs_accumulate<4, 11>(sm, q, acc);
-        hs_accumulate<4, 13>(sm, q, acc);
-        hs_accumulate<4, 15>(sm, q, acc);
-        hs_check<4>(acc, kq, fp, tid, out, cursor, capacity);
+        const uint32_t parity = (uint32_t)((t >> 1) & 1);
+        if (half) hs_tile_body<1>(sm, q, d, kq, &bar[t & 1], parity, fp, tid, out, cursor, capacity);
+        else      hs_tile_body<0>(sm, q, d, kq, &bar[t & 1], parity, fp, tid, out, cursor, capacity);
         __syncthreads();                             // every thread is done with buffer t&1: it may be refilled
     }
 }
