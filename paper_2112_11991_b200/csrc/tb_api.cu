@@ -70,6 +70,7 @@ struct tb_plan {
     float2 rot = {1.f, 0.f};                         // W_N^1
     int min_log2h = 0;                               // smallest knot spacing among the staged templates
     int n_sm = 148;                                  // multiprocessors of the device
+    int pf_cols = 0;                                 // same for pass 1 (segment records)
     int pf_spec = 0;                                 // same for the spectrum former
     int pf_rows = 0;                                 // L2 prefetch distance of pass 2, in CTAs (resident CTAs of the device)
 
@@ -290,7 +291,7 @@ int launch_cols(tb_plan* p, size_t off, uint32_t nt, long long* d_idx, float* d_
     const unsigned grid = (unsigned)(((1u << p->log2m2) / FFT_C) * nt);
     kern<<<grid, FFT_THREADS, cols_smem<R1>(), p->stream>>>(p->d_series, p->d_seg, p->seg_stride, p->d_tmpl + off, (int)nt,
                                                            (int)p->n, p->log2m2, p->fill, p->d_tw1a, p->d_tw2,
-                                                           reinterpret_cast<float2*>(p->d_resampled), d_idx, d_y);
+                                                           reinterpret_cast<float2*>(p->d_resampled), d_idx, d_y, p->pf_cols);
     TB_CUDA(p, cudaGetLastError());
     return TB_OK;
 }
@@ -676,6 +677,8 @@ int tb_plan_create(tb_plan** out, const float* series, uint64_t n_samples, doubl
         cudaDeviceGetAttribute(&p->n_sm, cudaDevAttrMultiProcessorCount, p->device);
         const char* pf = getenv("TB_PF_ROWS");           // tuning knob: prefetch distance in CTAs (default: the resident CTAs, 3 per SM)
         p->pf_rows = pf ? atoi(pf) : p->n_sm * 2;
+        const char* pfc = getenv("TB_PF_COLS");
+        p->pf_cols = pfc ? atoi(pfc) : 128;
         const char* pfs = getenv("TB_PF_SPEC");
         p->pf_spec = pfs ? atoi(pfs) : 32;
         p->seg_stride = (size_t)(p->n >> OWN_MIN_LOG2H);

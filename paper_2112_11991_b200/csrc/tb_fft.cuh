@@ -31,6 +31,13 @@
 
 namespace tb {
 
+#ifndef TB_A0_UNROLL
+#define TB_A0_UNROLL 4                 // rows per batch of independent segment-record loads (x R1 points)
+#endif
+#ifndef TB_A1_UNROLL
+#define TB_A1_UNROLL 4                 // rows per batch of independent gather loads
+#endif
+constexpr int A0_UNROLL = TB_A0_UNROLL, A1_UNROLL = TB_A1_UNROLL;
 constexpr int FFT_PB = 17;            // pitch of the b axis (16 + 1)
 constexpr int FFT_PA = 16 * FFT_PB;   // pitch of the a axis
 constexpr int FFT_THREADS = 256;
@@ -44,9 +51,39 @@ struct SegRec {                       // one Hermite segment of the delay, 64 by
 };
 static_assert(sizeof(SegRec) == 64, "segment record");
 
+// Complex arithmetic on the packed fp32x2 pipe of sm_100 (FADD2 / FFMA2: one issue slot per complex
+// add, three per complex multiply instead of two and four); the kernels are issue-bound, not FMA-bound.
+#ifndef TB_F32X2
+#define TB_F32X2 1
+#endif
+#if TB_F32X2
+__device__ __forceinline__ float2 cadd(float2 a, float2 b)
+{
+    float2 r;
+    asm("{ .reg .b64 ra, rb, rc; mov.b64 ra, {%2,%3}; mov.b64 rb, {%4,%5}; add.rn.f32x2 rc, ra, rb; mov.b64 {%0,%1}, rc; }"
+        : "=f"(r.x), "=f"(r.y) : "f"(a.x), "f"(a.y), "f"(b.x), "f"(b.y));
+    return r;
+}
+__device__ __forceinline__ float2 csub(float2 a, float2 b)
+{
+    float2 r;
+    asm("{ .reg .b64 ra, rb, rc; mov.b64 ra, {%2,%3}; mov.b64 rb, {%4,%5}; sub.rn.f32x2 rc, ra, rb; mov.b64 {%0,%1}, rc; }"
+        : "=f"(r.x), "=f"(r.y) : "f"(a.x), "f"(a.y), "f"(b.x), "f"(b.y));
+    return r;
+}
+__device__ __forceinline__ float2 cmul(float2 a, float2 w)      // (a.x, a.x) * w + (-a.y w.y, a.y w.x)
+{
+    float2 r;
+    const float cx = -a.y * w.y, cy = a.y * w.x;
+    asm("{ .reg .b64 ra, rb, rc, rd; mov.b64 ra, {%2,%2}; mov.b64 rb, {%3,%4}; mov.b64 rc, {%5,%6}; fma.rn.f32x2 rd, ra, rb, rc; mov.b64 {%0,%1}, rd; }"
+        : "=f"(r.x), "=f"(r.y) : "f"(a.x), "f"(w.x), "f"(w.y), "f"(cx), "f"(cy));
+    return r;
+}
+#else
 __device__ __forceinline__ float2 cmul(float2 a, float2 w) { return make_float2(a.x * w.x - a.y * w.y, a.x * w.y + a.y * w.x); }
 __device__ __forceinline__ float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
 __device__ __forceinline__ float2 csub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
+#endif
 __device__ __forceinline__ float2 mul_mi(float2 a) { return make_float2(a.y, -a.x); }   // a * (-i)
 
 // forward 4-point DFT of (x0,x1,x2,x3), natural order in and out
@@ -231,7 +268,7 @@ __global__ void __launch_bounds__(FFT_THREADS, 3)
 k_fft_cols(const float* __restrict__ x, const SegRec* __restrict__ seg, size_t seg_stride,
            const TmplDev* __restrict__ tmpl, int n_tmpl, int n, int log2m2, float fill,
            const float2* __restrict__ tw1, const float2* __restrict__ tw2g, float2* __restrict__ T,
-           long long* __restrict__ idx_out, float* __restrict__ y_out)
+           long long* __restrict__ idx_out, float* __restrict__ y_out, int pf_dist)
 {
     constexpr int PB = FFT_PB, PA = FFT_PA;
     constexpr int L = R1 * 256;                    // M1
@@ -247,6 +284,16 @@ k_fft_cols(const float* __restrict__ x, const SegRec* __restrict__ seg, size_t s
     float2* __restrict__ Tb = T + (size_t)b * m;
 
     tw2[threadIdx.x] = __ldg(tw2g + threadIdx.x);
+    // Pull the segment records of the CTA pf_dist blocks ahead (written by K0 just before, about
+    // half of them no longer in L2) into L2: one record per row of its tile.
+    if (!DEBUG && pf_dist > 0 && blockIdx.x + pf_dist < gridDim.x) {
+        const unsigned nb = blockIdx.x + pf_dist;
+        const int bn = nb % n_tmpl, cn = (nb / n_tmpl) * C;
+        const int lh = __ldg(&tmpl[bn].log2h);
+        const SegRec* __restrict__ sn = seg + (size_t)bn * seg_stride;
+        for (int j1 = threadIdx.x; j1 < L; j1 += FFT_THREADS)
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(sn + ((int)((((size_t)j1 << log2m2) + cn) << 1) >> lh)));
+    }
 
     // phase A0: source indices of every point of the tile, parked as an int2 in the point's own
     // shared-memory slot (written and read back by the same thread: no barrier).  Splitting the
@@ -266,12 +313,14 @@ k_fft_cols(const float* __restrict__ x, const SegRec* __restrict__ seg, size_t s
         const float t0 = (float)o * inv_h, t1 = t0 + inv_h;
         const char* __restrict__ rec0 = reinterpret_cast<const char*>(segs + (nn0 >> log2h));
         const int rec_shift = row_shift - log2h + 6;                           // log2 bytes between the records of rows j1, j1 + 1
-#pragma unroll 4
+        static_assert(16 * R1 <= 32, "one tie flag per point of the thread");
+        unsigned ties = 0;                                                     // points with a sample too close to a rounding tie for fp32
+#pragma unroll A0_UNROLL
         for (int it = 0; it < 16; ++it) {
 #pragma unroll
             for (int a = 0; a < R1; ++a) {
                 const int j1 = a * 256 + 16 * it;                              // row relative to w0
-                const char* r = rec0 + ((size_t)(unsigned)j1 << rec_shift);
+                const char* r = rec0 + ((unsigned)j1 << rec_shift);            // < 2^26 bytes
                 const float4 f = __ldg(reinterpret_cast<const float4*>(r));
                 const int2 ie = __ldg(reinterpret_cast<const int2*>(r) + 2);
                 const int nn = nn0 + (j1 << row_shift);
@@ -279,18 +328,26 @@ k_fft_cols(const float* __restrict__ x, const SegRec* __restrict__ seg, size_t s
                 const float y1 = fmaf(fmaf(fmaf(f.w, t1, f.z), t1, f.y), t1, f.x);
                 const float z0 = y0 + 12582912.0f, z1 = y1 + 12582912.0f;      // 1.5 * 2^23: round to nearest integer
                 const int base = nn - ie.x + 0x4B400000;
-                int2 src = make_int2(base - __float_as_int(z0), base + 1 - __float_as_int(z1));
                 const float lim = 0.5f - __int_as_float(ie.y);
-                const bool tie0 = fabsf(y0 - (z0 - 12582912.0f)) > lim, tie1 = fabsf(y1 - (z1 - 12582912.0f)) > lim;
-                if (tie0 || tie1) {                                            // rare (about 2 eps per sample)
-                    const double2 c01 = __ldg(reinterpret_cast<const double2*>(r) + 2);
-                    const double2 c23 = __ldg(reinterpret_cast<const double2*>(r) + 3);
-                    const double ta = (double)o * (double)inv_h, tb = (double)(o + 1) * (double)inv_h;
-                    if (tie0) src.x = nn - floor_to_int(fma(fma(fma(c23.y, ta, c23.x), ta, c01.y), ta, c01.x));
-                    if (tie1) src.y = nn + 1 - floor_to_int(fma(fma(fma(c23.y, tb, c23.x), tb, c01.y), tb, c01.x));
-                }
-                *reinterpret_cast<int2*>(myslot + a * PA + it * PB) = src;
+                const float res = fmaxf(fabsf(y0 - (z0 - 12582912.0f)), fabsf(y1 - (z1 - 12582912.0f)));
+                ties |= (res > lim ? 1u : 0u) << (it * R1 + a);
+                *reinterpret_cast<int2*>(myslot + a * PA + it * PB) =
+                    make_int2(base - __float_as_int(z0), base + 1 - __float_as_int(z1));
             }
+        }
+        while (ties) {                                                         // rare (about 2 eps per sample): decide in fp64
+            const int e = __ffs(ties) - 1;
+            ties &= ties - 1;
+            const int a = e % R1, it = e / R1;
+            const int j1 = a * 256 + 16 * it;
+            const char* r = rec0 + ((unsigned)j1 << rec_shift);
+            const int nn = nn0 + (j1 << row_shift);
+            const double2 c01 = __ldg(reinterpret_cast<const double2*>(r) + 2);
+            const double2 c23 = __ldg(reinterpret_cast<const double2*>(r) + 3);
+            const double ta = (double)o * (double)inv_h, tb = (double)(o + 1) * (double)inv_h;
+            *reinterpret_cast<int2*>(myslot + a * PA + it * PB) =
+                make_int2(nn - floor_to_int(fma(fma(fma(c23.y, ta, c23.x), ta, c01.y), ta, c01.x)),
+                          nn + 1 - floor_to_int(fma(fma(fma(c23.y, tb, c23.x), tb, c01.y), tb, c01.x)));
         }
     } else {
 #pragma unroll 2
@@ -303,7 +360,7 @@ k_fft_cols(const float* __restrict__ x, const SegRec* __restrict__ seg, size_t s
         }
     }
     // phase A1: gather (independent loads), radix-R1 over a, twiddle, back to the same slots
-#pragma unroll 4
+#pragma unroll A1_UNROLL
     for (int it = 0; it < 16; ++it) {
         const int w = w0 + 16 * it;
         float2* p = myslot + it * PB;
@@ -356,9 +413,9 @@ k_fft_cols(const float* __restrict__ x, const SegRec* __restrict__ seg, size_t s
 #pragma unroll
         for (int q = 0; q < 8; ++q) pw[8 + q] = cmul(pw[q], g8);
         float2* out = Tb + ((size_t)kbase << log2m2) + j2;
-        const size_t kstep = (size_t)(16 * R1) << log2m2;
+        const unsigned kstep = (unsigned)(16 * R1) << log2m2;                  // 15 kstep < M <= 2^27 elements
 #pragma unroll
-        for (int kc = 0; kc < 16; ++kc) __stcs(out + kc * kstep, cmul(v[kc], pw[kc]));   // streamed: read once by pass 2
+        for (int kc = 0; kc < 16; ++kc) __stcs(out + (unsigned)kc * kstep, cmul(v[kc], pw[kc]));   // streamed: read once by pass 2
     }
 }
 
