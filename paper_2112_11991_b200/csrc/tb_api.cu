@@ -6,6 +6,10 @@
 
 #include <cufft.h>
 
+#ifndef TB_HS_TPC
+#define TB_HS_TPC 16                   // tiles walked by one CTA of the harmonic summer
+#endif
+
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
@@ -462,7 +466,7 @@ int run_hsum(tb_plan* p, uint32_t nt, const FoldParams& fp, uint32_t first_id)
 {
     if (p->nb >= (uint64_t)HS_T) {
         const int tiles = (int)(p->nb / HS_T);
-        const int tpc = std::min(tiles, 8);                                  // tiles walked by one CTA (double-buffered)
+        const int tpc = std::min(tiles, TB_HS_TPC);                                  // tiles walked by one CTA (double-buffered)
         const size_t smem = 2 * HS_SMEM_FLOATS * sizeof(float);
         static bool attr_set = false;
         if (!attr_set) {

@@ -31,6 +31,12 @@
 
 namespace tb {
 
+#ifndef TB_COLS_MINB
+#define TB_COLS_MINB 3
+#endif
+#ifndef TB_ROWS_MINB
+#define TB_ROWS_MINB 2                  // CTAs per SM the pass-2 register budget is set for (2 measured faster than 3)
+#endif
 #ifndef TB_A0_UNROLL
 #define TB_A0_UNROLL 4                 // rows per batch of independent segment-record loads (x R1 points)
 #endif
@@ -264,7 +270,7 @@ __device__ __forceinline__ int2 source_pair(const SegRec* __restrict__ segs, int
 //   delay) and one segment record serve 16 threads.
 // ---------------------------------------------------------------------------------------------
 template <int R1, int C, bool DEBUG>
-__global__ void __launch_bounds__(FFT_THREADS, 3)
+__global__ void __launch_bounds__(FFT_THREADS, TB_COLS_MINB)
 k_fft_cols(const float* __restrict__ x, const SegRec* __restrict__ seg, size_t seg_stride,
            const TmplDev* __restrict__ tmpl, int n_tmpl, int n, int log2m2, float fill,
            const float2* __restrict__ tw1, const float2* __restrict__ tw2g, float2* __restrict__ T,
@@ -432,7 +438,7 @@ template <int R1> struct RowsCfg {
     static constexpr int PA = 16 * PB + 1;
     static constexpr int R = (R1 >= 8) ? 1 : 8 / R1;       // rows per CTA
     static constexpr int LP = R1 * PA;
-    static constexpr int MINB = 3;        // CTAs per SM the register budget is set for
+    static constexpr int MINB = TB_ROWS_MINB;        // CTAs per SM the register budget is set for
     static constexpr size_t SMEM = (size_t)(R * LP + 256) * sizeof(float2);
 };
 

@@ -254,71 +254,84 @@ __device__ __forceinline__ float2 r2c_unpack2(float2 zk, float2 zm, float2 w)   
 template <int W> __host__ __device__ constexpr int med_slots() { return (W / 32 >= 16) ? 12 : W / 32; }
 template <int W> __host__ __device__ constexpr int med_scratch_floats() { return 32 * med_slots<W>(); }
 
-template <int W>
+// the two middle values among the bracket candidates of a warp (lane l keeps `mine` <= CK of them
+// at cp[32 q]): bisection in key space (non-negative floats order like their bit patterns) on
+// [L, H) until exactly one candidate (or one key) is left around rank r1
+template <int CK>
+__device__ __forceinline__ void median_select(const float* __restrict__ cp, int mine, int r1, int nmid, uint32_t L,
+                                              uint32_t H, uint32_t& lower, uint32_t& upper)
+{
+    uint32_t ck[CK];
+#pragma unroll
+    for (int q = 0; q < CK; ++q) ck[q] = (q < mine) ? __float_as_uint(cp[32 * q]) : 0xffffffffu;
+    int cl = 0, ch = nmid;                               // candidates below L, below H
+    while (ch - cl > 1 && H - L > 1u) {
+        const uint32_t mid = L + ((H - L) >> 1);
+        int cc[3] = {0, 0, 0};                           // three short chains instead of one long one
+#pragma unroll
+        for (int q = 0; q < CK; ++q) cc[q % 3] += (ck[q] < mid) ? 1 : 0;
+        const int c = __reduce_add_sync(0xffffffffu, cc[0] + cc[1] + cc[2]);
+        if (c <= r1) { L = mid; cl = c; } else { H = mid; ch = c; }
+    }
+    uint32_t v1 = 0xffffffffu;
+#pragma unroll
+    for (int q = 0; q < CK; ++q) v1 = min(v1, ck[q] >= L ? ck[q] : 0xffffffffu);
+    v1 = __reduce_min_sync(0xffffffffu, v1);             // the candidate of rank r1
+    int le = 0;
+    uint32_t nxt = 0xffffffffu;
+#pragma unroll
+    for (int q = 0; q < CK; ++q) {
+        le += (ck[q] <= v1) ? 1 : 0;
+        nxt = min(nxt, ck[q] > v1 ? ck[q] : 0xffffffffu);
+    }
+    le  = __reduce_add_sync(0xffffffffu, le);
+    nxt = __reduce_min_sync(0xffffffffu, nxt);
+    lower = v1;
+    upper = (le >= r1 + 2) ? v1 : nxt;
+}
+
+// GUARD = false: the scratch holds W floats (a lane may keep all of its W/32 values), so the
+// bracket pass needs no capacity check.
+template <int W, bool GUARD = true>
 __device__ __forceinline__ float warp_median(const float (&p)[W / 32], float* cand, int lane,
                                              unsigned long long* __restrict__ fallbacks)
 {
     constexpr int VPT = W / 32;
     constexpr int K1 = W / 2 - 1;
-    constexpr int CPL = med_slots<W>();                  // bracket values a lane can keep
+    constexpr int CPL = med_slots<W>();                  // bracket values a lane can take into the selection
     // Fast path: the median of noise-like powers sits near 0.78 x the block mean, so count the
     // values below lo = 0.66 mean and keep those in [lo, hi = 0.90 mean) (about 13 % of the block,
     // 4 per lane) in a private per-lane list in shared memory (slot q of lane l at cand[l + 32 q]:
     // no scan, no compaction, no bank conflicts), then select among them.  If the two middle ranks
     // are not both inside the bracket, or a lane holds more than CPL bracket values, fall back to
-    // the bisection over all W values.
+    // the bisection over all W values.  The bracket test works on the bit patterns (one unsigned
+    // range check per value).
     float sum = 0.f;
 #pragma unroll
     for (int v = 0; v < VPT; ++v) sum += p[v];
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
     const float lo = sum * (0.66f / (float)W), hi = sum * (0.90f / (float)W);
-    int below = 0, mine = 0;
+    const uint32_t klo = __float_as_uint(lo), kspan = __float_as_uint(hi) - klo;
+    int below = 0;
     float* __restrict__ cp = cand + lane;
+    float* cw = cp;                                      // next free slot of this lane's list
 #pragma unroll
     for (int v = 0; v < VPT; ++v) {
-        const bool isb = p[v] < lo;
-        const bool ism = !isb && p[v] < hi;
-        below += isb ? 1 : 0;
-        if (ism && mine < CPL) cp[32 * mine] = p[v];
-        mine += ism ? 1 : 0;
+        const uint32_t k = __float_as_uint(p[v]);
+        below += (k < klo) ? 1 : 0;
+        if (k - klo < kspan && (!GUARD || cw < cp + 32 * CPL)) { *cw = p[v]; cw += 32; }
     }
+    const int mine = (int)(cw - cp) >> 5;
     below = __reduce_add_sync(0xffffffffu, below);
     const int nmid = __reduce_add_sync(0xffffffffu, mine);
     const int most = __reduce_max_sync(0xffffffffu, mine);
     uint32_t lower, upper;
-    if (below <= K1 && below + nmid >= K1 + 2 && most <= CPL) {
-        uint32_t ck[CPL];
-#pragma unroll
-        for (int q = 0; q < CPL; ++q) ck[q] = (q < mine) ? __float_as_uint(cp[32 * q]) : 0xffffffffu;
-        // bisection in key space (non-negative floats order like their bit patterns) on the
-        // bracket [L, H) until exactly one candidate (or one key) is left around rank r1
+    if (below <= K1 && below + nmid >= K1 + 2 && most <= ((GUARD && CPL < VPT) ? CPL - 1 : CPL)) {
+        __syncwarp();
         const int r1 = K1 - below;                       // rank among the candidates
-        uint32_t L = __float_as_uint(lo), H = __float_as_uint(hi);
-        int cl = 0, ch = nmid;                           // candidates below L, below H
-        while (ch - cl > 1 && H - L > 1u) {
-            const uint32_t mid = L + ((H - L) >> 1);
-            int cc[3] = {0, 0, 0};                       // three short chains instead of one long one
-#pragma unroll
-            for (int q = 0; q < CPL; ++q) cc[q % 3] += (ck[q] < mid) ? 1 : 0;
-            const int c = __reduce_add_sync(0xffffffffu, cc[0] + cc[1] + cc[2]);
-            if (c <= r1) { L = mid; cl = c; } else { H = mid; ch = c; }
-        }
-        uint32_t v1 = 0xffffffffu;
-#pragma unroll
-        for (int q = 0; q < CPL; ++q) v1 = min(v1, ck[q] >= L ? ck[q] : 0xffffffffu);
-        v1 = __reduce_min_sync(0xffffffffu, v1);         // the candidate of rank r1
-        int le = 0;
-        uint32_t nxt = 0xffffffffu;
-#pragma unroll
-        for (int q = 0; q < CPL; ++q) {
-            le += (ck[q] <= v1) ? 1 : 0;
-            nxt = min(nxt, ck[q] > v1 ? ck[q] : 0xffffffffu);
-        }
-        le  = __reduce_add_sync(0xffffffffu, le);
-        nxt = __reduce_min_sync(0xffffffffu, nxt);
-        lower = v1;
-        upper = (le >= r1 + 2) ? v1 : nxt;
+        if (CPL > 8 && most <= 8) median_select<(CPL > 8 ? 8 : CPL)>(cp, mine, r1, nmid, klo, klo + kspan, lower, upper);
+        else                      median_select<CPL>(cp, mine, r1, nmid, klo, klo + kspan, lower, upper);
         __syncwarp();
     } else {
         if (lane == 0 && fallbacks) atomicAdd(fallbacks, 1ull);
@@ -488,6 +501,12 @@ k_spectrum_median(const float2* __restrict__ X, size_t ld, float* __restrict__ P
 //   centres exactly like k_spectrum_median and writes 8 W bins with coalesced stores.
 //   Powers are carried as 4 P_k (the 1/2 of the unpack is skipped); the factor cancels in P^.
 // ---------------------------------------------------------------------------------------------
+#ifndef TB_ST_MINB
+#define TB_ST_MINB 3
+#endif
+#ifndef TB_ST_UN
+#define TB_ST_UN 8                     // row steps per load group of the spectrum former
+#endif
 constexpr int ST_WARPS = 9;
 constexpr int ST_THREADS = ST_WARPS * 32;
 
@@ -531,7 +550,7 @@ __device__ __forceinline__ float st_interbin(float2 x, float2 prev)
 }
 
 template <int W, int LOG2M1, bool RAW>
-__global__ void __launch_bounds__(ST_THREADS, (W <= 1024) ? 3 : 1)
+__global__ void __launch_bounds__(ST_THREADS, (W <= 1024) ? TB_ST_MINB : 1)
 k_spectrum_t(const float2* __restrict__ Zt, float* __restrict__ P, float* __restrict__ med, int log2m2,
              int nblk, const float2* __restrict__ twa, const float2* __restrict__ twb, float2 rot,
              unsigned long long* __restrict__ fallbacks, float* __restrict__ Praw, int pf_dist)
@@ -591,7 +610,7 @@ k_spectrum_t(const float2* __restrict__ Zt, float* __restrict__ P, float* __rest
         const float2* zkp = Zr + (size_t)k1s * m2 + k2;                                   // walks down the rows
         const float2* zmp = Zr + (size_t)(M1 - k1s) * m2 + (m2 - 1 - k2);                 // walks up; row M1 is never read (k1s = 0 below)
         const float2* __restrict__ wap = twa + k1s;
-        constexpr int UN = (LC % 8 == 0) ? 8 : 4;
+        constexpr int UN = (LC % TB_ST_UN == 0) ? TB_ST_UN : 4;
 #pragma unroll 1
         for (int i0 = 0; i0 < LC; i0 += UN) {
             float2 zk[UN], zm[UN];
@@ -653,7 +672,7 @@ k_spectrum_t(const float2* __restrict__ Zt, float* __restrict__ P, float* __rest
             for (int i = 0; i < VPT; ++i) Praw[(size_t)row * m + (size_t)blk * W + i * 32 + lane] = 0.25f * p[i];
         }
         // scratch for the bracket list: floats of this warp's own block (all of them are in registers now)
-        const float m_cur = warp_median<W>(p, (side ? s_hi - 3 : s_lo) + wid * (W + Q), lane, owner ? fallbacks : nullptr);
+        const float m_cur = warp_median<W, false>(p, (side ? s_hi - 3 : s_lo) + wid * (W + Q), lane, owner ? fallbacks : nullptr);
         if (lane == 0) {
             s_med[side][wid] = m_cur;
             if (owner) med[(size_t)row * nblk + blk] = 0.25f * m_cur;
