@@ -221,18 +221,27 @@ k_delay_segments(const TmplDev* __restrict__ tmpl, int n_tmpl, int n, SegRec* __
         s_val[k] = v; s_slp[k] = d * h;
     }
     __syncthreads();
-    const int s = s0 + threadIdx.x;
-    if (threadIdx.x >= 256 || s >= nseg) return;
-    const double v0 = s_val[threadIdx.x], v1 = s_val[threadIdx.x + 1], g0 = s_slp[threadIdx.x], g1 = s_slp[threadIdx.x + 1];
-    const double dv = v1 - v0;
-    SegRec r;
-    r.d0 = v0 + 0.5; r.d1 = g0; r.d2 = 3.0 * dv - (2.0 * g0 + g1); r.d3 = (g0 + g1) - 2.0 * dv;
-    const double i0 = rint(v0);
-    r.i0 = (int)i0;
-    r.f0 = (float)(v0 - i0); r.f1 = (float)r.d1; r.f2 = (float)r.d2; r.f3 = (float)r.d3;
-    r.eps = (float)((fabs(r.d1) + fabs(r.d2) + fabs(r.d3) + 2.0) * 1e-6);
-    r.pad0 = 0; r.pad1 = 0;
-    seg[(size_t)b * seg_stride + s] = r;
+    // records are staged piece-major in shared memory (4 pieces of 16 bytes, pitch 257) and written
+    // out as one contiguous, fully coalesced stretch: direct 64-byte-strided stores left the
+    // kernel waiting on the store queue (lg_throttle / drain in the ncu capture)
+    __shared__ float4 s_piece[4][257];
+    if (threadIdx.x < 256) {
+        const double v0 = s_val[threadIdx.x], v1 = s_val[threadIdx.x + 1], g0 = s_slp[threadIdx.x], g1 = s_slp[threadIdx.x + 1];
+        const double dv = v1 - v0;
+        const double d0 = v0 + 0.5, d1 = g0, d2 = 3.0 * dv - (2.0 * g0 + g1), d3 = (g0 + g1) - 2.0 * dv;
+        const double i0 = rint(v0);
+        const float eps = (float)((fabs(d1) + fabs(d2) + fabs(d3) + 2.0) * 1e-6);
+        s_piece[0][threadIdx.x] = make_float4((float)(v0 - i0), (float)d1, (float)d2, (float)d3);
+        s_piece[1][threadIdx.x] = make_float4(__int_as_float((int)i0), eps, 0.f, 0.f);
+        s_piece[2][threadIdx.x] = make_float4(__int_as_float(__double2loint(d0)), __int_as_float(__double2hiint(d0)),
+                                              __int_as_float(__double2loint(d1)), __int_as_float(__double2hiint(d1)));
+        s_piece[3][threadIdx.x] = make_float4(__int_as_float(__double2loint(d2)), __int_as_float(__double2hiint(d2)),
+                                              __int_as_float(__double2loint(d3)), __int_as_float(__double2hiint(d3)));
+    }
+    __syncthreads();
+    const int nrec = min(256, nseg - s0);
+    float4* __restrict__ out = reinterpret_cast<float4*>(seg + (size_t)b * seg_stride + s0);
+    for (int g = threadIdx.x; g < 4 * nrec; g += K0_THREADS) out[g] = s_piece[g & 3][g >> 2];
 }
 
 // source indices of the output sample pair (nn, nn+1), nn even (a3): fp32 cubic of the segment
