@@ -283,17 +283,17 @@ void launch_spectrum(tb_plan* p, uint32_t nt, float* d_raw)
 }
 
 // ---- hand-written FFT path -------------------------------------------------------------------
-constexpr int FFT_C = 16;                            // columns per CTA of pass 1 (runs of 32 samples / 128 bytes)
-template <int R1> constexpr size_t cols_smem() { return (size_t)(FFT_C * (R1 * FFT_PA + 16 / FFT_C) + 256) * sizeof(float2); }
+// columns per CTA of pass 1: 16 (runs of 32 samples / 128 bytes), 8 at M1 = 1024 where 16 would not fit in shared memory
+template <int R1, int C> constexpr size_t cols_smem() { return (size_t)(C * (R1 * FFT_PA + 16 / C) + 256) * sizeof(float2); }
 
-template <int R1, bool DEBUG>
+template <int R1, int FFT_C, bool DEBUG>
 int launch_cols(tb_plan* p, size_t off, uint32_t nt, long long* d_idx, float* d_y)
 {
     auto kern = k_fft_cols<R1, FFT_C, DEBUG>;
     static bool attr = false;
-    if (!attr) { TB_CUDA(p, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cols_smem<R1>())); attr = true; }
+    if (!attr) { TB_CUDA(p, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cols_smem<R1, FFT_C>())); attr = true; }
     const unsigned grid = (unsigned)(((1u << p->log2m2) / FFT_C) * nt);
-    kern<<<grid, FFT_THREADS, cols_smem<R1>(), p->stream>>>(p->d_series, p->d_seg, p->seg_stride, p->d_tmpl + off, (int)nt,
+    kern<<<grid, FFT_THREADS, cols_smem<R1, FFT_C>(), p->stream>>>(p->d_series, p->d_seg, p->seg_stride, p->d_tmpl + off, (int)nt,
                                                            (int)p->n, p->log2m2, p->fill, p->d_tw1a, p->d_tw2,
                                                            reinterpret_cast<float2*>(p->d_resampled), d_idx, d_y, p->pf_cols);
     TB_CUDA(p, cudaGetLastError());
@@ -324,8 +324,9 @@ int run_own_pass1(tb_plan* p, size_t off, uint32_t nt, long long* d_idx, float* 
     if (after_k0) TB_CUDA(p, cudaEventRecord(after_k0, p->stream));
     const bool dbg = d_idx != nullptr;
     switch (p->log2m1 - 8) {
-        case 0: return dbg ? launch_cols<1, true>(p, off, nt, d_idx, d_y) : launch_cols<1, false>(p, off, nt, nullptr, nullptr);
-        case 1: return dbg ? launch_cols<2, true>(p, off, nt, d_idx, d_y) : launch_cols<2, false>(p, off, nt, nullptr, nullptr);
+        case 0: return dbg ? launch_cols<1, 16, true>(p, off, nt, d_idx, d_y) : launch_cols<1, 16, false>(p, off, nt, nullptr, nullptr);
+        case 1: return dbg ? launch_cols<2, 16, true>(p, off, nt, d_idx, d_y) : launch_cols<2, 16, false>(p, off, nt, nullptr, nullptr);
+        case 2: return dbg ? launch_cols<4, 8, true>(p, off, nt, d_idx, d_y) : launch_cols<4, 8, false>(p, off, nt, nullptr, nullptr);
     }
     return fail(p, TB_ERR_INVALID_ARG, "unsupported M1");
 }
@@ -367,7 +368,8 @@ int launch_spectrum_t(tb_plan* p, uint32_t nt, float* d_raw)
 // (median window, log2 M1) pairs the transposing spectrum former is instantiated for
 bool spectrum_t_supported(uint32_t w, int log2m1)
 {
-    return (log2m1 == 8 && (w == 256 || w == 1024)) || (log2m1 == 9 && (w == 512 || w == 1024 || w == 2048));
+    return (log2m1 == 8 && (w == 256 || w == 1024)) || (log2m1 == 9 && (w == 512 || w == 1024 || w == 2048)) ||
+           (log2m1 == 10 && (w == 1024 || w == 2048));
 }
 
 int run_spectrum_t(tb_plan* p, uint32_t nt, float* d_raw = nullptr)
@@ -378,6 +380,8 @@ int run_spectrum_t(tb_plan* p, uint32_t nt, float* d_raw = nullptr)
         case 512 * 16 + 9: return launch_spectrum_t<512, 9>(p, nt, d_raw);
         case 1024 * 16 + 9: return launch_spectrum_t<1024, 9>(p, nt, d_raw);
         case 2048 * 16 + 9: return launch_spectrum_t<2048, 9>(p, nt, d_raw);
+        case 1024 * 16 + 10: return launch_spectrum_t<1024, 10>(p, nt, d_raw);
+        case 2048 * 16 + 10: return launch_spectrum_t<2048, 10>(p, nt, d_raw);
     }
     return fail(p, TB_ERR_INVALID_ARG, "median_window");
 }
@@ -667,11 +671,11 @@ int tb_plan_create(tb_plan** out, const float* series, uint64_t n_samples, doubl
     { int rc = load_series(p, series); if (rc) { destroy(p); return rc; } }
     pin_series_in_l2(p);
 
-    // FFT path: hand-written two-pass FFT (M = N/2 = M1 * M2, M1 = 512, or 256 at 2^17) when
-    // 2^17 <= N <= 2^23, W >= M1 and the median blocks pair up in groups of 16; batched cuFFT otherwise
+    // FFT path: hand-written two-pass FFT (M = N/2 = M1 * M2, M1 = 512, 256 at 2^17, 1024 at 2^24) when
+    // 2^17 <= N <= 2^24, W >= M1 and the median blocks pair up in groups of 16; batched cuFFT otherwise
     {
         const int lm = (int)ilog2(p->nb);
-        p->log2m1 = lm >= 17 ? 9 : 8;
+        p->log2m1 = lm >= 23 ? 10 : lm >= 17 ? 9 : 8;
         p->log2m2 = lm - p->log2m1;
         const bool fits = p->log2m2 >= 8 && p->log2m2 <= 13 && spectrum_t_supported(W, p->log2m1) && p->nblk >= 16 && p->nblk % 16 == 0;
         if (o.fft_path >= 2 && !fits) { destroy(p); return TB_ERR_INVALID_ARG; }

@@ -314,27 +314,31 @@ k_fft_cols(const float* __restrict__ x, const SegRec* __restrict__ seg, size_t s
     // shared-memory slot (written and read back by the same thread: no barrier).  Splitting the
     // index computation from the gather turns two dependent memory latencies per point
     // (segment record -> series sample) into two loops of independent loads.
-    // Thread (col, w0) = (tid % C, tid / C) owns the points (a, w = w0 + 16 it), it < 16: row
+    // Thread (col, w0) = (tid % C, tid / C) owns the points (a, w = w0 + NW0 it), it < NIT: row
     // j1 = a 256 + w of the tile, samples nn, nn + 1 with nn = 2 (j1 M2 + c0 + col).
-    static_assert(C == 16 && FFT_THREADS == 256, "thread -> (col, w0) mapping");
-    const int col = threadIdx.x & (C - 1), w0 = threadIdx.x >> 4;
-    float2* __restrict__ myslot = fsm + col * LP + w0;                         // + a PA + it PB
+    static_assert((C == 16 || C == 8) && FFT_THREADS == 256, "thread -> (col, w0) mapping");
+    constexpr int NW0 = FFT_THREADS / C, NIT = 256 / NW0;                      // w0 values, steps per thread
+    constexpr int UA0 = (A0_UNROLL * 2 / R1 > 0) ? A0_UNROLL * 2 / R1 : 1;      // 2 A0_UNROLL points per batch of loads
+    constexpr int UA1 = (A1_UNROLL * 2 / R1 > 0) ? A1_UNROLL * 2 / R1 : 1;
+    constexpr int ITP = (NW0 / 16) * PB;                                       // slot pitch of one step
+    const int col = threadIdx.x & (C - 1), w0 = threadIdx.x / C;
+    float2* __restrict__ myslot = fsm + col * LP + (w0 >> 4) * PB + (w0 & 15); // + a PA + it ITP
     const int nn0 = (int)((((size_t)w0 << log2m2) + c0 + col) << 1);
     const int row_shift = log2m2 + 1;                                          // samples between rows j1, j1 + 1
-    if (!DEBUG && log2h >= 5) {
-        // h >= 32: the 32-sample run of a row lies inside one segment, the offset o of a sample in
+    if (!DEBUG && (1 << log2h) >= 2 * C) {
+        // h >= 2C: the 2C-sample run of a row lies inside one segment, the offset o of a sample in
         // its segment is the same for every row of the thread, and the record index is linear in j1
         const int o = nn0 & ((1 << log2h) - 1);
         const float t0 = (float)o * inv_h, t1 = t0 + inv_h;
         const char* __restrict__ rec0 = reinterpret_cast<const char*>(segs + (nn0 >> log2h));
         const int rec_shift = row_shift - log2h + 6;                           // log2 bytes between the records of rows j1, j1 + 1
-        static_assert(16 * R1 <= 32, "one tie flag per point of the thread");
+        static_assert(NIT * R1 <= 32, "one tie flag per point of the thread");
         unsigned ties = 0;                                                     // points with a sample too close to a rounding tie for fp32
-#pragma unroll A0_UNROLL
-        for (int it = 0; it < 16; ++it) {
+#pragma unroll UA0
+        for (int it = 0; it < NIT; ++it) {
 #pragma unroll
             for (int a = 0; a < R1; ++a) {
-                const int j1 = a * 256 + 16 * it;                              // row relative to w0
+                const int j1 = a * 256 + NW0 * it;                             // row relative to w0
                 const char* r = rec0 + ((unsigned)j1 << rec_shift);            // < 2^26 bytes
                 const float4 f = __ldg(reinterpret_cast<const float4*>(r));
                 const int2 ie = __ldg(reinterpret_cast<const int2*>(r) + 2);
@@ -346,7 +350,7 @@ k_fft_cols(const float* __restrict__ x, const SegRec* __restrict__ seg, size_t s
                 const float lim = 0.5f - __int_as_float(ie.y);
                 const float res = fmaxf(fabsf(y0 - (z0 - 12582912.0f)), fabsf(y1 - (z1 - 12582912.0f)));
                 ties |= (res > lim ? 1u : 0u) << (it * R1 + a);
-                *reinterpret_cast<int2*>(myslot + a * PA + it * PB) =
+                *reinterpret_cast<int2*>(myslot + a * PA + it * ITP) =
                     make_int2(base - __float_as_int(z0), base + 1 - __float_as_int(z1));
             }
         }
@@ -354,31 +358,31 @@ k_fft_cols(const float* __restrict__ x, const SegRec* __restrict__ seg, size_t s
             const int e = __ffs(ties) - 1;
             ties &= ties - 1;
             const int a = e % R1, it = e / R1;
-            const int j1 = a * 256 + 16 * it;
+            const int j1 = a * 256 + NW0 * it;
             const char* r = rec0 + ((unsigned)j1 << rec_shift);
             const int nn = nn0 + (j1 << row_shift);
             const double2 c01 = __ldg(reinterpret_cast<const double2*>(r) + 2);
             const double2 c23 = __ldg(reinterpret_cast<const double2*>(r) + 3);
             const double ta = (double)o * (double)inv_h, tb = (double)(o + 1) * (double)inv_h;
-            *reinterpret_cast<int2*>(myslot + a * PA + it * PB) =
+            *reinterpret_cast<int2*>(myslot + a * PA + it * ITP) =
                 make_int2(nn - floor_to_int(fma(fma(fma(c23.y, ta, c23.x), ta, c01.y), ta, c01.x)),
                           nn + 1 - floor_to_int(fma(fma(fma(c23.y, tb, c23.x), tb, c01.y), tb, c01.x)));
         }
     } else {
 #pragma unroll 2
-        for (int it = 0; it < 16; ++it) {
+        for (int it = 0; it < NIT; ++it) {
 #pragma unroll
             for (int a = 0; a < R1; ++a) {
-                const int nn = nn0 + ((a * 256 + 16 * it) << row_shift);
-                *reinterpret_cast<int2*>(myslot + a * PA + it * PB) = source_pair(segs, nn, log2h, inv_h);
+                const int nn = nn0 + ((a * 256 + NW0 * it) << row_shift);
+                *reinterpret_cast<int2*>(myslot + a * PA + it * ITP) = source_pair(segs, nn, log2h, inv_h);
             }
         }
     }
     // phase A1: gather (independent loads), radix-R1 over a, twiddle, back to the same slots
-#pragma unroll A1_UNROLL
-    for (int it = 0; it < 16; ++it) {
-        const int w = w0 + 16 * it;
-        float2* p = myslot + it * PB;
+#pragma unroll UA1
+    for (int it = 0; it < NIT; ++it) {
+        const int w = w0 + NW0 * it;
+        float2* p = myslot + it * ITP;
         float2 v[R1];
 #pragma unroll
         for (int a = 0; a < R1; ++a) {
@@ -386,7 +390,7 @@ k_fft_cols(const float* __restrict__ x, const SegRec* __restrict__ seg, size_t s
             v[a].x = ((unsigned)sp.x < (unsigned)n) ? __ldg(x + sp.x) : fill;
             v[a].y = ((unsigned)sp.y < (unsigned)n) ? __ldg(x + sp.y) : fill;
             if (DEBUG) {
-                const size_t nn = (size_t)b * n + (size_t)(nn0 + ((a * 256 + 16 * it) << row_shift));
+                const size_t nn = (size_t)b * n + (size_t)(nn0 + ((a * 256 + NW0 * it) << row_shift));
                 idx_out[nn] = sp.x; idx_out[nn + 1] = sp.y;
                 y_out[nn] = v[a].x; y_out[nn + 1] = v[a].y;
             }
