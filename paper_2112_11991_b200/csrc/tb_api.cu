@@ -195,22 +195,19 @@ int load_series(tb_plan* p, const float* series)
         p->d_series = p->d_series_owned;
     }
     if (p->user_fill) return TB_OK;
-    if (!p->borrowed) {
-        double acc[16] = {0};                              // 16 fp64 partial sums (n is a multiple of 16)
-        for (uint64_t i = 0; i < p->n; i += 16)
-            for (int q = 0; q < 16; ++q) acc[q] += (double)series[i + q];
-        long double s = 0.0L;
-        for (int q = 0; q < 16; ++q) s += (long double)acc[q];
-        p->fill = (float)(double)(s / (long double)p->n);
-    } else {
-        double acc = 0.0;
-        if (!p->d_acc) TB_CUDA(p, cudaMalloc(&p->d_acc, sizeof(double)));
-        TB_CUDA(p, cudaMemsetAsync(p->d_acc, 0, sizeof(double), p->stream));
-        k_sum_f64<<<296, 256, 0, p->stream>>>(p->d_series, (size_t)p->n, p->d_acc);
-        TB_CUDA(p, cudaMemcpyAsync(&acc, p->d_acc, sizeof(double), cudaMemcpyDeviceToHost, p->stream));
-        TB_CUDA(p, cudaStreamSynchronize(p->stream));
-        p->fill = (float)(acc / (double)p->n);
-    }
+    // fill value (G8): fp64 mean of the series.  296 per-block partial sums on the device (each a
+    // fixed strided subset, summed in a fixed order), added up here in block order: deterministic,
+    // and the host never walks the series (that loop cost 4 ms of every end-to-end step at 2^23).
+    constexpr int SUM_BLOCKS = 296;
+    if (!p->d_acc) TB_CUDA(p, cudaMalloc(&p->d_acc, SUM_BLOCKS * sizeof(double)));
+    k_sum_f64<<<SUM_BLOCKS, 256, 0, p->stream>>>(p->d_series, (size_t)p->n, p->d_acc);
+    TB_CUDA(p, cudaGetLastError());
+    double part[SUM_BLOCKS];
+    TB_CUDA(p, cudaMemcpyAsync(part, p->d_acc, sizeof(part), cudaMemcpyDeviceToHost, p->stream));
+    TB_CUDA(p, cudaStreamSynchronize(p->stream));
+    long double acc = 0.0L;
+    for (int i = 0; i < SUM_BLOCKS; ++i) acc += (long double)part[i];
+    p->fill = (float)(double)(acc / (long double)p->n);
     return TB_OK;
 }
 

@@ -1010,14 +1010,22 @@ k_hsum_tile(const float* __restrict__ Ph, int nb, int groups_per_row, int tpc, F
     }
 }
 
-// fp64 sum of a device series (fill value when the series is borrowed device memory)
-__global__ void k_sum_f64(const float* __restrict__ x, size_t n, double* __restrict__ acc)
+// fp64 partial sums of the series (fill value): block b sums the elements b*256+t, stride
+// gridDim*256, per thread in index order, then the 256 threads in a fixed tree -> acc[b]
+__global__ void __launch_bounds__(256) k_sum_f64(const float* __restrict__ x, size_t n, double* __restrict__ acc)
 {
+    __shared__ double s_w[8];
     double s = 0.0;
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x)
         s += (double)x[i];
     for (int o = 16; o > 0; o >>= 1) s += __shfl_down_sync(0xffffffffu, s, o);
-    if ((threadIdx.x & 31) == 0) atomicAdd(acc, s);
+    if ((threadIdx.x & 31) == 0) s_w[threadIdx.x >> 5] = s;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double t = 0.0;
+        for (int w = 0; w < 8; ++w) t += s_w[w];
+        acc[blockIdx.x] = t;
+    }
 }
 
 }  // namespace tb
