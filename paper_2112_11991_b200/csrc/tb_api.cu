@@ -70,7 +70,8 @@ struct tb_plan {
     int log2m1 = 0, log2m2 = 0;
     SegRec* d_seg = nullptr;                         // [chunk][n >> MIN_LOG2H]
     size_t seg_stride = 0;
-    float2 *d_tw1a = nullptr, *d_tw1b = nullptr, *d_tw2 = nullptr, *d_twn = nullptr, *d_twb = nullptr;
+    float2 *d_tw1a = nullptr, *d_tw1b = nullptr, *d_tw2 = nullptr, *d_twn = nullptr, *d_twb = nullptr, *d_twc = nullptr;
+    bool cols32 = false;                             // pass 1 as 32 x 16 (M1 = 512)
     float2 rot = {1.f, 0.f};                         // W_N^1
     int min_log2h = 0;                               // smallest knot spacing among the staged templates
     int n_sm = 148;                                  // multiprocessors of the device
@@ -311,6 +312,20 @@ int launch_rows(tb_plan* p, uint32_t nt)
     return TB_OK;
 }
 
+template <bool DEBUG>
+int launch_cols32(tb_plan* p, size_t off, uint32_t nt, long long* d_idx, float* d_y)
+{
+    auto kern = k_fft_cols32<DEBUG>;
+    static bool attr = false;
+    if (!attr) { TB_CUDA(p, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C32_SMEM)); attr = true; }
+    const unsigned grid = (unsigned)(((1u << p->log2m2) / 16) * nt);
+    kern<<<grid, FFT_THREADS, C32_SMEM, p->stream>>>(p->d_series, p->d_seg, p->seg_stride, p->d_tmpl + off, (int)nt, (int)p->n,
+                                                    p->log2m2, p->fill, p->d_twc, reinterpret_cast<float2*>(p->d_resampled),
+                                                    d_idx, d_y, p->pf_cols);
+    TB_CUDA(p, cudaGetLastError());
+    return TB_OK;
+}
+
 // K0 + P1: delay segments, then gather + column FFTs into T (the buffer the legacy path uses for y)
 int run_own_pass1(tb_plan* p, size_t off, uint32_t nt, long long* d_idx, float* d_y, cudaEvent_t after_k0 = nullptr)
 {
@@ -320,6 +335,7 @@ int run_own_pass1(tb_plan* p, size_t off, uint32_t nt, long long* d_idx, float* 
     TB_CUDA(p, cudaGetLastError());
     if (after_k0) TB_CUDA(p, cudaEventRecord(after_k0, p->stream));
     const bool dbg = d_idx != nullptr;
+    if (p->cols32) return dbg ? launch_cols32<true>(p, off, nt, d_idx, d_y) : launch_cols32<false>(p, off, nt, nullptr, nullptr);
     switch (p->log2m1 - 8) {
         case 0: return dbg ? launch_cols<1, 16, true>(p, off, nt, d_idx, d_y) : launch_cols<1, 16, false>(p, off, nt, nullptr, nullptr);
         case 1: return dbg ? launch_cols<2, 16, true>(p, off, nt, d_idx, d_y) : launch_cols<2, 16, false>(p, off, nt, nullptr, nullptr);
@@ -418,6 +434,17 @@ int make_twiddles(tb_plan* p)
     for (size_t b = 0; b < hb.size(); ++b) {
         const long double a = -two_pi * (long double)((uint64_t)b << p->log2m1) / (long double)p->n;
         hb[b] = make_float2((float)cosl(a), (float)sinl(a));
+    }
+    if (p->log2m1 == 9) {                                // W_512^{c ka} of the 32 x 16 first pass
+        std::vector<float2> hc(512);
+        for (int ka = 0; ka < 32; ++ka)
+            for (int c = 0; c < 16; ++c) {
+                const long double a = -two_pi * (long double)(ka * c) / 512.0L;
+                hc[ka * 16 + c] = make_float2((float)cosl(a), (float)sinl(a));
+            }
+        if ((rc = upload(hc, &p->d_twc))) return rc;
+        const char* e = getenv("TB_COLS32");
+        p->cols32 = !(e && atoi(e) == 0);
     }
     p->rot = make_float2((float)cosl(two_pi / (long double)p->n), (float)-sinl(two_pi / (long double)p->n));
     if ((rc = upload(h2, &p->d_tw2))) return rc;
@@ -558,7 +585,7 @@ void destroy(tb_plan* p)
     for (auto& kv : p->fft_plans) cufftDestroy(kv.second);
     for (auto& es : p->events) for (auto& e : es.e) cudaEventDestroy(e);
     if (p->ev_staged) cudaEventDestroy(p->ev_staged);
-    cudaFree(p->d_seg); cudaFree(p->d_tw1a); cudaFree(p->d_tw1b); cudaFree(p->d_tw2); cudaFree(p->d_twn); cudaFree(p->d_twb);
+    cudaFree(p->d_seg); cudaFree(p->d_tw1a); cudaFree(p->d_tw1b); cudaFree(p->d_tw2); cudaFree(p->d_twn); cudaFree(p->d_twb); cudaFree(p->d_twc);
     cudaFree(p->d_work); cudaFree(p->d_acc); cudaFree(p->d_series_owned); cudaFree(p->d_resampled); cudaFree(p->d_fft);
     cudaFree(p->d_power); cudaFree(p->d_med); cudaFree(p->d_cand); cudaFree(p->d_cursor); cudaFree(p->d_tmpl);
     if (p->h_tmpl) cudaFreeHost(p->h_tmpl);

@@ -272,6 +272,72 @@ __device__ __forceinline__ int2 source_pair(const SegRec* __restrict__ segs, int
 }
 
 // ---------------------------------------------------------------------------------------------
+// phase A0 of pass 1: source indices of the thread's NIT * R1 points (rows j1 = a 256 + NW0 it
+// relative to the thread's first row, samples nn, nn + 1), parked as int2 at
+// myslot[a APITCH + it ITPITCH] (written and read back by the same thread: no barrier).
+// ---------------------------------------------------------------------------------------------
+template <int R1, int C, int APITCH, int ITPITCH>
+__device__ __forceinline__ void cols_park_indices(const SegRec* __restrict__ segs, int log2h, float inv_h,
+                                                  float2* __restrict__ myslot, int nn0, int row_shift)
+{
+    constexpr int NW0 = FFT_THREADS / C, NIT = 256 / NW0;
+    constexpr int UA0 = (A0_UNROLL * 2 / R1 > 0) ? A0_UNROLL * 2 / R1 : 1;      // 2 A0_UNROLL points per batch of loads
+    if ((1 << log2h) >= 2 * C) {
+        // h >= 2C: the 2C-sample run of a row lies inside one segment, the offset o of a sample in
+        // its segment is the same for every row of the thread, and the record index is linear in j1
+        const int o = nn0 & ((1 << log2h) - 1);
+        const float t0 = (float)o * inv_h, t1 = t0 + inv_h;
+        const char* __restrict__ rec0 = reinterpret_cast<const char*>(segs + (nn0 >> log2h));
+        const int rec_shift = row_shift - log2h + 6;                           // log2 bytes between the records of rows j1, j1 + 1
+        static_assert(NIT * R1 <= 32, "one tie flag per point of the thread");
+        unsigned ties = 0;                                                     // points with a sample too close to a rounding tie for fp32
+#pragma unroll UA0
+        for (int it = 0; it < NIT; ++it) {
+#pragma unroll
+            for (int a = 0; a < R1; ++a) {
+                const int j1 = a * 256 + NW0 * it;                             // row relative to w0
+                const char* r = rec0 + ((unsigned)j1 << rec_shift);            // < 2^26 bytes
+                const float4 f = __ldg(reinterpret_cast<const float4*>(r));
+                const int2 ie = __ldg(reinterpret_cast<const int2*>(r) + 2);
+                const int nn = nn0 + (j1 << row_shift);
+                const float y0 = fmaf(fmaf(fmaf(f.w, t0, f.z), t0, f.y), t0, f.x);
+                const float y1 = fmaf(fmaf(fmaf(f.w, t1, f.z), t1, f.y), t1, f.x);
+                const float z0 = y0 + 12582912.0f, z1 = y1 + 12582912.0f;      // 1.5 * 2^23: round to nearest integer
+                const int base = nn - ie.x + 0x4B400000;
+                const float lim = 0.5f - __int_as_float(ie.y);
+                const float res = fmaxf(fabsf(y0 - (z0 - 12582912.0f)), fabsf(y1 - (z1 - 12582912.0f)));
+                ties |= (res > lim ? 1u : 0u) << (it * R1 + a);
+                *reinterpret_cast<int2*>(myslot + a * APITCH + it * ITPITCH) =
+                    make_int2(base - __float_as_int(z0), base + 1 - __float_as_int(z1));
+            }
+        }
+        while (ties) {                                                         // rare (about 2 eps per sample): decide in fp64
+            const int e = __ffs(ties) - 1;
+            ties &= ties - 1;
+            const int a = e % R1, it = e / R1;
+            const int j1 = a * 256 + NW0 * it;
+            const char* r = rec0 + ((unsigned)j1 << rec_shift);
+            const int nn = nn0 + (j1 << row_shift);
+            const double2 c01 = __ldg(reinterpret_cast<const double2*>(r) + 2);
+            const double2 c23 = __ldg(reinterpret_cast<const double2*>(r) + 3);
+            const double ta = (double)o * (double)inv_h, tb = (double)(o + 1) * (double)inv_h;
+            *reinterpret_cast<int2*>(myslot + a * APITCH + it * ITPITCH) =
+                make_int2(nn - floor_to_int(fma(fma(fma(c23.y, ta, c23.x), ta, c01.y), ta, c01.x)),
+                          nn + 1 - floor_to_int(fma(fma(fma(c23.y, tb, c23.x), tb, c01.y), tb, c01.x)));
+        }
+    } else {
+#pragma unroll 2
+        for (int it = 0; it < NIT; ++it) {
+#pragma unroll
+            for (int a = 0; a < R1; ++a) {
+                const int nn = nn0 + ((a * 256 + NW0 * it) << row_shift);
+                *reinterpret_cast<int2*>(myslot + a * APITCH + it * ITPITCH) = source_pair(segs, nn, log2h, inv_h);
+            }
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
 // P1  gather + column FFTs.  CTA = C columns [c0, c0+C) of template b, all M1 = R1*256 rows.
 //   blockIdx.x = bundle * n_tmpl + b (template fastest: co-resident CTAs gather from the same
 //   stretch of the series, which stays in L2).  A row of the CTA's tile is a run of 2C
@@ -325,59 +391,7 @@ k_fft_cols(const float* __restrict__ x, const SegRec* __restrict__ seg, size_t s
     float2* __restrict__ myslot = fsm + col * LP + (w0 >> 4) * PB + (w0 & 15); // + a PA + it ITP
     const int nn0 = (int)((((size_t)w0 << log2m2) + c0 + col) << 1);
     const int row_shift = log2m2 + 1;                                          // samples between rows j1, j1 + 1
-    if (!DEBUG && (1 << log2h) >= 2 * C) {
-        // h >= 2C: the 2C-sample run of a row lies inside one segment, the offset o of a sample in
-        // its segment is the same for every row of the thread, and the record index is linear in j1
-        const int o = nn0 & ((1 << log2h) - 1);
-        const float t0 = (float)o * inv_h, t1 = t0 + inv_h;
-        const char* __restrict__ rec0 = reinterpret_cast<const char*>(segs + (nn0 >> log2h));
-        const int rec_shift = row_shift - log2h + 6;                           // log2 bytes between the records of rows j1, j1 + 1
-        static_assert(NIT * R1 <= 32, "one tie flag per point of the thread");
-        unsigned ties = 0;                                                     // points with a sample too close to a rounding tie for fp32
-#pragma unroll UA0
-        for (int it = 0; it < NIT; ++it) {
-#pragma unroll
-            for (int a = 0; a < R1; ++a) {
-                const int j1 = a * 256 + NW0 * it;                             // row relative to w0
-                const char* r = rec0 + ((unsigned)j1 << rec_shift);            // < 2^26 bytes
-                const float4 f = __ldg(reinterpret_cast<const float4*>(r));
-                const int2 ie = __ldg(reinterpret_cast<const int2*>(r) + 2);
-                const int nn = nn0 + (j1 << row_shift);
-                const float y0 = fmaf(fmaf(fmaf(f.w, t0, f.z), t0, f.y), t0, f.x);
-                const float y1 = fmaf(fmaf(fmaf(f.w, t1, f.z), t1, f.y), t1, f.x);
-                const float z0 = y0 + 12582912.0f, z1 = y1 + 12582912.0f;      // 1.5 * 2^23: round to nearest integer
-                const int base = nn - ie.x + 0x4B400000;
-                const float lim = 0.5f - __int_as_float(ie.y);
-                const float res = fmaxf(fabsf(y0 - (z0 - 12582912.0f)), fabsf(y1 - (z1 - 12582912.0f)));
-                ties |= (res > lim ? 1u : 0u) << (it * R1 + a);
-                *reinterpret_cast<int2*>(myslot + a * PA + it * ITP) =
-                    make_int2(base - __float_as_int(z0), base + 1 - __float_as_int(z1));
-            }
-        }
-        while (ties) {                                                         // rare (about 2 eps per sample): decide in fp64
-            const int e = __ffs(ties) - 1;
-            ties &= ties - 1;
-            const int a = e % R1, it = e / R1;
-            const int j1 = a * 256 + NW0 * it;
-            const char* r = rec0 + ((unsigned)j1 << rec_shift);
-            const int nn = nn0 + (j1 << row_shift);
-            const double2 c01 = __ldg(reinterpret_cast<const double2*>(r) + 2);
-            const double2 c23 = __ldg(reinterpret_cast<const double2*>(r) + 3);
-            const double ta = (double)o * (double)inv_h, tb = (double)(o + 1) * (double)inv_h;
-            *reinterpret_cast<int2*>(myslot + a * PA + it * ITP) =
-                make_int2(nn - floor_to_int(fma(fma(fma(c23.y, ta, c23.x), ta, c01.y), ta, c01.x)),
-                          nn + 1 - floor_to_int(fma(fma(fma(c23.y, tb, c23.x), tb, c01.y), tb, c01.x)));
-        }
-    } else {
-#pragma unroll 2
-        for (int it = 0; it < NIT; ++it) {
-#pragma unroll
-            for (int a = 0; a < R1; ++a) {
-                const int nn = nn0 + ((a * 256 + NW0 * it) << row_shift);
-                *reinterpret_cast<int2*>(myslot + a * PA + it * ITP) = source_pair(segs, nn, log2h, inv_h);
-            }
-        }
-    }
+    cols_park_indices<R1, C, PA, ITP>(segs, log2h, inv_h, myslot, nn0, row_shift);
     // phase A1: gather (independent loads), radix-R1 over a, twiddle, back to the same slots
 #pragma unroll UA1
     for (int it = 0; it < NIT; ++it) {
@@ -433,6 +447,98 @@ k_fft_cols(const float* __restrict__ x, const SegRec* __restrict__ seg, size_t s
         for (int q = 0; q < 8; ++q) pw[8 + q] = cmul(pw[q], g8);
         float2* out = Tb + ((size_t)kbase << log2m2) + j2;
         const unsigned kstep = (unsigned)(16 * R1) << log2m2;                  // 15 kstep < M <= 2^27 elements
+#pragma unroll
+        for (int kc = 0; kc < 16; ++kc) __stcs(out + (unsigned)kc * kstep, cmul(v[kc], pw[kc]));   // streamed: read once by pass 2
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// P1 for M1 = 512 = 32 x 16: two in-CTA steps instead of three.  Row j1 = 16 a + c (a < 32,
+// c < 16), output k1 = ka + 32 kc.  Thread (col, c) gathers its 32 rows a (the same rows, and
+// the same phase A0, as in k_fft_cols<2, 16>), does the radix-32 step in registers, multiplies
+// by W_512^{c ka} (table twc[ka 16 + c]) and writes slot[col][ka][c]; after ONE barrier the work
+// item (col, ka) does the radix-16 step over c, the four-step twiddle W_M^{j2 k1} and the
+// streaming stores of T[k1][j2].  One shared-memory round trip and one barrier less per point
+// than the 2 x 16 x 16 scheme, and a pitch of 513 keeps every access conflict free.
+// ---------------------------------------------------------------------------------------------
+constexpr int C32_PK = 16, C32_LP = 32 * C32_PK + 1;
+constexpr size_t C32_SMEM = (size_t)16 * C32_LP * sizeof(float2);
+
+template <bool DEBUG>
+__global__ void __launch_bounds__(FFT_THREADS, TB_COLS_MINB)
+k_fft_cols32(const float* __restrict__ x, const SegRec* __restrict__ seg, size_t seg_stride,
+             const TmplDev* __restrict__ tmpl, int n_tmpl, int n, int log2m2, float fill,
+             const float2* __restrict__ twc, float2* __restrict__ T,
+             long long* __restrict__ idx_out, float* __restrict__ y_out, int pf_dist)
+{
+    constexpr int C = 16, PK = C32_PK, LP = C32_LP, L = 512;
+    extern __shared__ __align__(16) float2 fsm[];
+    const int b  = blockIdx.x % n_tmpl;
+    const int c0 = (blockIdx.x / n_tmpl) * C;
+    const size_t m = (size_t)L << log2m2;          // M
+    const int log2h = tmpl[b].log2h;
+    const float inv_h = 1.0f / (float)(1 << log2h);
+    const SegRec* __restrict__ segs = seg + (size_t)b * seg_stride;
+    float2* __restrict__ Tb = T + (size_t)b * m;
+
+    if (!DEBUG && pf_dist > 0 && blockIdx.x + pf_dist < gridDim.x) {           // segment records of a later CTA -> L2
+        const unsigned nb = blockIdx.x + pf_dist;
+        const int bn = nb % n_tmpl, cn = (nb / n_tmpl) * C;
+        const int lh = __ldg(&tmpl[bn].log2h);
+        const SegRec* __restrict__ sn = seg + (size_t)bn * seg_stride;
+        for (int j1 = threadIdx.x; j1 < L; j1 += FFT_THREADS)
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(sn + ((int)((((size_t)j1 << log2m2) + cn) << 1) >> lh)));
+    }
+
+    const int col = threadIdx.x & 15, c = threadIdx.x >> 4;
+    float2* __restrict__ myslot = fsm + col * LP + c;                          // + a' PK, a' = 16 a + it
+    const int nn0 = (int)((((size_t)c << log2m2) + c0 + col) << 1);
+    const int row_shift = log2m2 + 1;
+    cols_park_indices<2, C, 16 * PK, PK>(segs, log2h, inv_h, myslot, nn0, row_shift);
+    {   // gather (64 independent loads), radix 32 over a', twiddle, back to the same slots
+        float2 v[32];
+#pragma unroll
+        for (int a = 0; a < 32; ++a) {
+            const int2 sp = *reinterpret_cast<const int2*>(myslot + a * PK);
+            v[a].x = ((unsigned)sp.x < (unsigned)n) ? __ldg(x + sp.x) : fill;
+            v[a].y = ((unsigned)sp.y < (unsigned)n) ? __ldg(x + sp.y) : fill;
+            if (DEBUG) {
+                const size_t nn = (size_t)b * n + (size_t)(nn0 + ((16 * a) << row_shift));
+                idx_out[nn] = sp.x; idx_out[nn + 1] = sp.y;
+                y_out[nn] = v[a].x; y_out[nn + 1] = v[a].y;
+            }
+        }
+        fft_reg<32>(v);
+        myslot[0] = v[0];
+#pragma unroll
+        for (int ka = 1; ka < 32; ++ka) myslot[ka * PK] = cmul(v[ka], __ldg(twc + ka * 16 + c));
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i < 16 * 32; i += FFT_THREADS) {                 // item (col, ka), col fastest
+        const int cl = i & 15, ka = i >> 4;
+        const float2* p = fsm + cl * LP + ka * PK;
+        float2 v[16];
+#pragma unroll
+        for (int cc = 0; cc < 16; ++cc) v[cc] = p[cc];
+        fft_reg<16>(v);
+        const int j2 = c0 + cl;
+        // W_M^{j2 k1} = W_M^{j2 ka} * g^kc, g = W_M^{32 j2}; both arguments are exact in fp32
+        const float inv_m = 1.0f / (float)m;
+        float sb, cb, sg, cg;
+        sincospif(-2.0f * (float)(j2 * ka) * inv_m, &sb, &cb);
+        sincospif(-2.0f * (float)(j2 * 32) * inv_m, &sg, &cg);
+        const float2 g1 = make_float2(cg, sg);
+        const float2 g2 = cmul(g1, g1), g4 = cmul(g2, g2), g8 = cmul(g4, g4);
+        float2 pw[16];
+        pw[0] = make_float2(cb, sb);
+        pw[1] = cmul(pw[0], g1);
+        pw[2] = cmul(pw[0], g2); pw[3] = cmul(pw[1], g2);
+#pragma unroll
+        for (int q = 0; q < 4; ++q) pw[4 + q] = cmul(pw[q], g4);
+#pragma unroll
+        for (int q = 0; q < 8; ++q) pw[8 + q] = cmul(pw[q], g8);
+        float2* out = Tb + ((size_t)ka << log2m2) + j2;
+        const unsigned kstep = 32u << log2m2;
 #pragma unroll
         for (int kc = 0; kc < 16; ++kc) __stcs(out + (unsigned)kc * kstep, cmul(v[kc], pw[kc]));   // streamed: read once by pass 2
     }
