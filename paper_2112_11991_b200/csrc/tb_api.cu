@@ -344,8 +344,30 @@ int run_own_pass1(tb_plan* p, size_t off, uint32_t nt, long long* d_idx, float* 
     return fail(p, TB_ERR_INVALID_ARG, "unsupported M1");
 }
 
+// three-pass FFT (N >= 2^25): rows of M2 = 2^16 = 256 x 256 points, in place over the slow index, then scattered rows
+int run_own_pass23(tb_plan* p, uint32_t nt)
+{
+    const unsigned rows = nt << p->log2m1;
+    {
+        auto kern = k_fft_cols<1, 16, false, true>;
+        static bool attr = false;
+        if (!attr) { TB_CUDA(p, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cols_smem<1, 16>())); attr = true; }
+        kern<<<rows * 16, FFT_THREADS, cols_smem<1, 16>(), p->stream>>>(nullptr, nullptr, 0, nullptr, (int)rows, 0, 8, 0.f, p->d_tw1b, p->d_tw2,
+                                                                       reinterpret_cast<float2*>(p->d_resampled), nullptr, nullptr, 0);
+        TB_CUDA(p, cudaGetLastError());
+    }
+    {
+        static bool attr = false;
+        if (!attr) { TB_CUDA(p, cudaFuncSetAttribute(k_fft_rows_scatter, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RS_SMEM)); attr = true; }
+        k_fft_rows_scatter<<<rows * 16, FFT_THREADS, RS_SMEM, p->stream>>>(reinterpret_cast<const float2*>(p->d_resampled), p->d_fft, p->d_tw2);
+        TB_CUDA(p, cudaGetLastError());
+    }
+    return TB_OK;
+}
+
 int run_own_pass2(tb_plan* p, uint32_t nt)
 {
+    if (p->log2m2 == 16) return run_own_pass23(p, nt);
     switch (p->log2m2 - 8) {
         case 0: return launch_rows<1>(p, nt);
         case 1: return launch_rows<2>(p, nt);
@@ -420,7 +442,7 @@ int make_twiddles(tb_plan* p)
     };
     int rc;
     if ((rc = tw1(p->log2m1, &p->d_tw1a))) return rc;
-    if ((rc = tw1(p->log2m2, &p->d_tw1b))) return rc;
+    if ((rc = tw1(p->log2m2 == 16 ? 8 : p->log2m2, &p->d_tw1b))) return rc;
     std::vector<float2> h2(256), hn((size_t)1 << p->log2m1), hb((size_t)1 << p->log2m2);
     for (int kb = 0; kb < 16; ++kb)
         for (int c = 0; c < 16; ++c) {
@@ -696,12 +718,12 @@ int tb_plan_create(tb_plan** out, const float* series, uint64_t n_samples, doubl
     pin_series_in_l2(p);
 
     // FFT path: hand-written two-pass FFT (M = N/2 = M1 * M2, M1 = 512, 256 at 2^17, 1024 at 2^24) when
-    // 2^17 <= N <= 2^24, W >= M1 and the median blocks pair up in groups of 16; batched cuFFT otherwise
+    // 2^17 <= N <= 2^26 (three passes with M2 = 256 x 256 at 2^25 and 2^26), W >= M1 and the median blocks pair up in groups of 16; batched cuFFT otherwise
     {
         const int lm = (int)ilog2(p->nb);
-        p->log2m1 = lm >= 23 ? 10 : lm >= 17 ? 9 : 8;
+        p->log2m1 = lm == 25 ? 9 : lm == 24 ? 8 : lm == 23 ? 10 : lm >= 17 ? 9 : 8;   // 2^25, 2^26: three passes, M2 = 2^16
         p->log2m2 = lm - p->log2m1;
-        const bool fits = p->log2m2 >= 8 && p->log2m2 <= 13 && spectrum_t_supported(W, p->log2m1) && p->nblk >= 16 && p->nblk % 16 == 0;
+        const bool fits = ((p->log2m2 >= 8 && p->log2m2 <= 13) || (p->log2m2 == 16 && lm >= 24)) && spectrum_t_supported(W, p->log2m1) && p->nblk >= 16 && p->nblk % 16 == 0;
         if (o.fft_path >= 2 && !fits) { destroy(p); return TB_ERR_INVALID_ARG; }
         p->own_fft = fits && o.fft_path != 1;
     }
@@ -810,7 +832,7 @@ int tb_search_templates(tb_plan* p, const tb_template* tmpl, uint64_t n_template
             if ((rc = run_own_pass2(p, nt))) return rc;
             if (es) TB_CUDA(p, cudaEventRecord(es->e[3], p->stream));
             if ((rc = run_spectrum_t(p, nt))) return rc;
-            p->last.n_kernel_launches += 2;
+            p->last.n_kernel_launches += (p->log2m2 == 16) ? 3 : 2;
         } else {
             if (es) TB_CUDA(p, cudaEventRecord(es->e[1], p->stream));
             if ((rc = run_resample(p, off, nt, nullptr))) return rc;

@@ -344,7 +344,10 @@ __device__ __forceinline__ void cols_park_indices(const SegRec* __restrict__ seg
 //   consecutive output samples: with C = 16 one 128-byte stretch of the series (shifted by the
 //   delay) and one segment record serve 16 threads.
 // ---------------------------------------------------------------------------------------------
-template <int R1, int C, bool DEBUG>
+//   DIRECT = true: no gather.  The kernel is the middle pass of the three-pass FFT (N >= 2^25):
+//   "template" b is one row of T seen as an [L][2^log2m2] matrix, transformed in place over its
+//   first index with the twiddle W_m^{j2 k1}, m = L 2^log2m2 (blockIdx.x = b * bundles + bundle).
+template <int R1, int C, bool DEBUG, bool DIRECT = false>
 __global__ void __launch_bounds__(FFT_THREADS, TB_COLS_MINB)
 k_fft_cols(const float* __restrict__ x, const SegRec* __restrict__ seg, size_t seg_stride,
            const TmplDev* __restrict__ tmpl, int n_tmpl, int n, int log2m2, float fill,
@@ -356,10 +359,11 @@ k_fft_cols(const float* __restrict__ x, const SegRec* __restrict__ seg, size_t s
     constexpr int LP = R1 * PA + 16 / C;           // slot pitch: 16/C mod 16 keeps the column-fastest accesses conflict free
     extern __shared__ __align__(16) float2 fsm[];
     float2* tw2 = fsm + C * LP;
-    const int b  = blockIdx.x % n_tmpl;
-    const int c0 = (blockIdx.x / n_tmpl) * C;
+    const int bundles = (1 << log2m2) / C;
+    const int b  = DIRECT ? blockIdx.x / bundles : blockIdx.x % n_tmpl;
+    const int c0 = (DIRECT ? blockIdx.x % bundles : blockIdx.x / n_tmpl) * C;
     const size_t m = (size_t)L << log2m2;          // M
-    const int log2h = tmpl[b].log2h;
+    const int log2h = DIRECT ? 0 : tmpl[b].log2h;
     const float inv_h = 1.0f / (float)(1 << log2h);
     const SegRec* __restrict__ segs = seg + (size_t)b * seg_stride;
     float2* __restrict__ Tb = T + (size_t)b * m;
@@ -367,7 +371,7 @@ k_fft_cols(const float* __restrict__ x, const SegRec* __restrict__ seg, size_t s
     tw2[threadIdx.x] = __ldg(tw2g + threadIdx.x);
     // Pull the segment records of the CTA pf_dist blocks ahead (written by K0 just before, about
     // half of them no longer in L2) into L2: one record per row of its tile.
-    if (!DEBUG && pf_dist > 0 && blockIdx.x + pf_dist < gridDim.x) {
+    if (!DEBUG && !DIRECT && pf_dist > 0 && blockIdx.x + pf_dist < gridDim.x) {
         const unsigned nb = blockIdx.x + pf_dist;
         const int bn = nb % n_tmpl, cn = (nb / n_tmpl) * C;
         const int lh = __ldg(&tmpl[bn].log2h);
@@ -384,14 +388,13 @@ k_fft_cols(const float* __restrict__ x, const SegRec* __restrict__ seg, size_t s
     // j1 = a 256 + w of the tile, samples nn, nn + 1 with nn = 2 (j1 M2 + c0 + col).
     static_assert((C == 16 || C == 8) && FFT_THREADS == 256, "thread -> (col, w0) mapping");
     constexpr int NW0 = FFT_THREADS / C, NIT = 256 / NW0;                      // w0 values, steps per thread
-    constexpr int UA0 = (A0_UNROLL * 2 / R1 > 0) ? A0_UNROLL * 2 / R1 : 1;      // 2 A0_UNROLL points per batch of loads
     constexpr int UA1 = (A1_UNROLL * 2 / R1 > 0) ? A1_UNROLL * 2 / R1 : 1;
     constexpr int ITP = (NW0 / 16) * PB;                                       // slot pitch of one step
     const int col = threadIdx.x & (C - 1), w0 = threadIdx.x / C;
     float2* __restrict__ myslot = fsm + col * LP + (w0 >> 4) * PB + (w0 & 15); // + a PA + it ITP
     const int nn0 = (int)((((size_t)w0 << log2m2) + c0 + col) << 1);
     const int row_shift = log2m2 + 1;                                          // samples between rows j1, j1 + 1
-    cols_park_indices<R1, C, PA, ITP>(segs, log2h, inv_h, myslot, nn0, row_shift);
+    if (!DIRECT) cols_park_indices<R1, C, PA, ITP>(segs, log2h, inv_h, myslot, nn0, row_shift);
     // phase A1: gather (independent loads), radix-R1 over a, twiddle, back to the same slots
 #pragma unroll UA1
     for (int it = 0; it < NIT; ++it) {
@@ -400,6 +403,10 @@ k_fft_cols(const float* __restrict__ x, const SegRec* __restrict__ seg, size_t s
         float2 v[R1];
 #pragma unroll
         for (int a = 0; a < R1; ++a) {
+            if (DIRECT) {
+                v[a] = __ldcs(Tb + ((size_t)(a * 256 + w) << log2m2) + c0 + col);
+                continue;
+            }
             const int2 sp = *reinterpret_cast<const int2*>(p + a * PA);
             v[a].x = ((unsigned)sp.x < (unsigned)n) ? __ldg(x + sp.x) : fill;
             v[a].y = ((unsigned)sp.y < (unsigned)n) ? __ldg(x + sp.y) : fill;
@@ -619,6 +626,50 @@ k_fft_rows_t(const float2* __restrict__ T, float2* __restrict__ Zt, int log2m1, 
         float2* out = Zb + (size_t)r * L + wp;     // k2 = wp + 16 R1 kc
 #pragma unroll
         for (int kc = 0; kc < 16; ++kc) __stcs(out + kc * (16 * R1), v[kc]);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Last pass of the three-pass FFT (N >= 2^25).  A row of M' = 256 * 256 points has been
+// transformed over its slow index by k_fft_cols<1, 16, false, true> (U[ka][jb], twiddled); this
+// kernel does the 256-point FFTs over jb for 16 consecutive ka and writes the row's spectrum in
+// natural order, Zt[row][ka + 256 kb], in 128-byte runs (16 consecutive ka per kb).
+//   blockIdx.x = row * 16 + group of 16 ka.
+// ---------------------------------------------------------------------------------------------
+constexpr int RS_ROWS = 16;
+constexpr size_t RS_SMEM = (size_t)(RS_ROWS * (16 * FFT_PB + 1) + 256) * sizeof(float2);
+
+__global__ void __launch_bounds__(FFT_THREADS, 3)
+k_fft_rows_scatter(const float2* __restrict__ U, float2* __restrict__ Zt, const float2* __restrict__ tw2g)
+{
+    constexpr int PB = FFT_PB, LP = 16 * FFT_PB + 1;
+    extern __shared__ __align__(16) float2 fsm[];
+    float2* tw2 = fsm + RS_ROWS * LP;
+    const size_t row = blockIdx.x >> 4;
+    const int ka0 = (blockIdx.x & 15) * RS_ROWS;
+    const float2* __restrict__ Ub = U + (row << 16) + (size_t)ka0 * 256;
+    float2* __restrict__ Zb = Zt + (row << 16) + ka0;
+    tw2[threadIdx.x] = __ldg(tw2g + threadIdx.x);
+    {
+        const int w = threadIdx.x;                   // jb = 16 b + c
+        float2 v[RS_ROWS];
+#pragma unroll
+        for (int r = 0; r < RS_ROWS; ++r) v[r] = __ldcs(Ub + r * 256 + w);
+#pragma unroll
+        for (int r = 0; r < RS_ROWS; ++r) fsm[r * LP + (w >> 4) * PB + (w & 15)] = v[r];
+    }
+    __syncthreads();
+    fft_step2<LP, PB>(fsm + (threadIdx.x >> 4) * LP, threadIdx.x & 15, tw2);   // item (r, c): radix 16 over b
+    __syncthreads();
+    {
+        const int r = threadIdx.x & 15, kb = threadIdx.x >> 4;                 // r fastest: 16 consecutive ka per store
+        const float2* p = fsm + r * LP + kb * PB;
+        float2 v[16];
+#pragma unroll
+        for (int c = 0; c < 16; ++c) v[c] = p[c];
+        fft_reg<16>(v);
+#pragma unroll
+        for (int kc = 0; kc < 16; ++kc) __stcs(Zb + (size_t)(kb + 16 * kc) * 256 + r, v[kc]);
     }
 }
 
