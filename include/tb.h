@@ -88,8 +88,10 @@ typedef struct {
     double   f_min_hz;            /* lowest searched fundamental frequency [0.1] (G20); <0 -> 0 */
     uint64_t max_candidates;      /* capacity of the device candidate buffer [1<<22] */
     uint32_t chunk_templates;     /* templates per launch group B; 0 -> chosen from free memory */
-    int32_t  series_is_device_ptr;/* 0: series is host memory and is copied; 1: series is device
-                                     memory on `device`, borrowed, must outlive the plan */
+    int32_t  series_is_device_ptr;/* 0: series is host memory; 1: series is device memory on
+                                     `device`.  Either way the plan copies it (on its stream);
+                                     the caller's buffer may be reused once the call returns and
+                                     the stream has been synchronised (tb_get_candidates does) */
     int32_t  has_fill;            /* 0: out-of-range samples take the fp64 mean of the series,
                                      rounded to fp32 (G8); 1: they take fill_value */
     float    fill_value;
@@ -121,7 +123,7 @@ typedef struct {
 
 /* Create a plan for one dedispersed time series S[i], i*tsamp.
  *   out        receives the plan (set to NULL on failure)
- *   series     float32[n_samples], host (copied) or device (borrowed) per opts
+ *   series     float32[n_samples], host or device memory per opts; copied into the plan
  *   n_samples  N, a power of two, 2*W <= N <= 2^28
  *   tsamp_s    sampling time in seconds, > 0
  *   opts       may be NULL (all defaults)
@@ -133,7 +135,8 @@ TB_API int tb_plan_create(tb_plan** out, const float* series, uint64_t n_samples
 /* Replace the plan's time series by another of the same length and sampling time (the next
  * DM trial / beam: PAPER.md L448, L660), reusing every buffer and FFT plan.  `series` is host
  * memory (copied on the plan's stream; pinned memory makes the copy asynchronous) unless the
- * plan was created with series_is_device_ptr, in which case it is a borrowed device pointer.
+ * plan was created with series_is_device_ptr, in which case it is device memory (copied device
+ * to device).
  * The fill value is recomputed unless the plan was created with has_fill. */
 TB_API int tb_plan_set_series(tb_plan* plan, const float* series);
 

@@ -48,6 +48,7 @@ struct tb_plan {
     bool timings = false;
     bool user_fill = false, borrowed = false, l2_pinned = false;
     float fill = 0.f;
+    float h_fillpad[4] = {0.f, 0.f, 0.f, 0.f};
     size_t ld = 0;                                   // complex row stride of the FFT output
 
     const float* d_series = nullptr;
@@ -155,6 +156,15 @@ int validate_template(const tb_template& t, double tsamp, std::string* why)
     return TB_OK;
 }
 
+// knot spacing of one template (the same expressions as make_tmpl, without the trigonometry)
+int tmpl_log2h(const tb_template& t, double tsamp)
+{
+    const long double two_pi = 8.0L * atanl(1.0L);
+    const long double c = (long double)tsamp / (long double)t.p_orb_s;
+    const long double g = (long double)t.tau_lts / (long double)tsamp;
+    return knot_log2((double)g, (double)(two_pi * c), t.ecc);
+}
+
 // step a1, in long double so that the constants are correctly rounded doubles
 void make_tmpl(const tb_template& t, double tsamp, TmplDev* o)
 {
@@ -185,17 +195,23 @@ void make_tmpl(const tb_template& t, double tsamp, TmplDev* o)
     o->log2h = knot_log2((double)g, o->w, t.ecc);
 }
 
-// copy (or borrow) the series and derive the fill value (G8)
+// the fill value also sits behind the series, x[N] (4 floats of padding): the fused path clamps an
+// out-of-range source index to N instead of testing it again at the gather
+int store_fill_pad(tb_plan* p)
+{
+    for (float& f : p->h_fillpad) f = p->fill;
+    TB_CUDA(p, cudaMemcpyAsync(p->d_series_owned + p->n, p->h_fillpad, sizeof(p->h_fillpad), cudaMemcpyHostToDevice, p->stream));
+    return TB_OK;
+}
+
+// copy the series (from host or device memory) and derive the fill value (G8)
 int load_series(tb_plan* p, const float* series)
 {
-    if (p->borrowed) {
-        p->d_series = series;
-    } else {
-        if (!p->d_series_owned) TB_CUDA(p, cudaMalloc(&p->d_series_owned, p->n * sizeof(float)));
-        TB_CUDA(p, cudaMemcpyAsync(p->d_series_owned, series, p->n * sizeof(float), cudaMemcpyHostToDevice, p->stream));
-        p->d_series = p->d_series_owned;
-    }
-    if (p->user_fill) return TB_OK;
+    if (!p->d_series_owned) TB_CUDA(p, cudaMalloc(&p->d_series_owned, (p->n + 4) * sizeof(float)));
+    TB_CUDA(p, cudaMemcpyAsync(p->d_series_owned, series, p->n * sizeof(float),
+                               p->borrowed ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, p->stream));
+    p->d_series = p->d_series_owned;
+    if (p->user_fill) return store_fill_pad(p);
     // fill value (G8): fp64 mean of the series.  296 per-block partial sums on the device (each a
     // fixed strided subset, summed in a fixed order), added up here in block order: deterministic,
     // and the host never walks the series (that loop cost 4 ms of every end-to-end step at 2^23).
@@ -209,7 +225,7 @@ int load_series(tb_plan* p, const float* series)
     long double acc = 0.0L;
     for (int i = 0; i < SUM_BLOCKS; ++i) acc += (long double)part[i];
     p->fill = (float)(double)(acc / (long double)p->n);
-    return TB_OK;
+    return store_fill_pad(p);
 }
 
 // Keep the series resident in L2 (persisting access-policy window on the plan's stream): every
@@ -560,14 +576,22 @@ int upload_templates(tb_plan* p, const tb_template* tmpl, uint64_t k)
         TB_CUDA(p, cudaMalloc(&p->d_tmpl, k * sizeof(TmplDev)));
         p->tmpl_cap = k;
     }
+    // knot spacings first (cheap): the smallest one selects the launch sequence and K0's grid;
+    // the constants themselves are made and uploaded chunk by chunk (stage_chunk), so that the
+    // host's extended-precision trigonometry overlaps the kernels of the previous chunk
     p->min_log2h = 7;
-    for (uint64_t i = 0; i < k; ++i) {
-        make_tmpl(tmpl[i], p->tsamp, &p->h_tmpl[i]);
-        p->min_log2h = std::min(p->min_log2h, (int)p->h_tmpl[i].log2h);
+    for (uint64_t i = 0; i < k; ++i) p->min_log2h = std::min(p->min_log2h, tmpl_log2h(tmpl[i], p->tsamp));
+    return TB_OK;
+}
+
+int stage_chunk(tb_plan* p, const tb_template* tmpl, uint64_t off, uint64_t nt, bool last)
+{
+    for (uint64_t i = off; i < off + nt; ++i) make_tmpl(tmpl[i], p->tsamp, &p->h_tmpl[i]);
+    TB_CUDA(p, cudaMemcpyAsync(p->d_tmpl + off, p->h_tmpl + off, nt * sizeof(TmplDev), cudaMemcpyHostToDevice, p->stream));
+    if (last) {
+        TB_CUDA(p, cudaEventRecord(p->ev_staged, p->stream));
+        p->staged_pending = true;
     }
-    TB_CUDA(p, cudaMemcpyAsync(p->d_tmpl, p->h_tmpl, k * sizeof(TmplDev), cudaMemcpyHostToDevice, p->stream));
-    TB_CUDA(p, cudaEventRecord(p->ev_staged, p->stream));
-    p->staged_pending = true;
     return TB_OK;
 }
 
@@ -619,7 +643,8 @@ int single_template_stage(tb_plan* p, const tb_template* tmpl)
 {
     if (!p || !tmpl) return fail(p, TB_ERR_INVALID_ARG, "null argument");
     TB_CUDA(p, cudaSetDevice(p->device));
-    return upload_templates(p, tmpl, 1);
+    const int rc = upload_templates(p, tmpl, 1);
+    return rc ? rc : stage_chunk(p, tmpl, 0, 1, true);
 }
 
 }  // namespace
@@ -761,7 +786,6 @@ int tb_plan_set_series(tb_plan* p, const float* series)
     if (!p || !series) return fail(p, TB_ERR_INVALID_ARG, "null argument");
     TB_CUDA(p, cudaSetDevice(p->device));
     const int rc = load_series(p, series);
-    if (!rc && p->borrowed) pin_series_in_l2(p);
     return rc;
 }
 
@@ -816,6 +840,7 @@ int tb_search_templates(tb_plan* p, const tb_template* tmpl, uint64_t n_template
     p->last.fft_path_used = own ? 2 : 1;
     for (uint64_t off = 0; off < n_templates; off += p->chunk) {
         const uint32_t nt = (uint32_t)std::min<uint64_t>(p->chunk, n_templates - off);
+        if ((rc = stage_chunk(p, tmpl, off, nt, off + nt == n_templates))) return rc;
         EventSet* es = nullptr;
         if (p->timings) {
             if (p->events_used == p->events.size()) {

@@ -276,9 +276,18 @@ __device__ __forceinline__ int2 source_pair(const SegRec* __restrict__ segs, int
 // relative to the thread's first row, samples nn, nn + 1), parked as int2 at
 // myslot[a APITCH + it ITPITCH] (written and read back by the same thread: no barrier).
 // ---------------------------------------------------------------------------------------------
-template <int R1, int C, int APITCH, int ITPITCH>
+// CLAMP: an out-of-range index is replaced by n, where the plan keeps the fill value (x[n]), so
+// that the gather needs no bounds test (the debug taps keep the raw index).
+template <bool CLAMP>
+__device__ __forceinline__ int2 clamp_pair(int2 s, int n)
+{
+    if (CLAMP) { s.x = (int)min((unsigned)s.x, (unsigned)n); s.y = (int)min((unsigned)s.y, (unsigned)n); }
+    return s;
+}
+
+template <int R1, int C, int APITCH, int ITPITCH, bool CLAMP>
 __device__ __forceinline__ void cols_park_indices(const SegRec* __restrict__ segs, int log2h, float inv_h,
-                                                  float2* __restrict__ myslot, int nn0, int row_shift)
+                                                  float2* __restrict__ myslot, int nn0, int row_shift, int n)
 {
     constexpr int NW0 = FFT_THREADS / C, NIT = 256 / NW0;
     constexpr int UA0 = (A0_UNROLL * 2 / R1 > 0) ? A0_UNROLL * 2 / R1 : 1;      // 2 A0_UNROLL points per batch of loads
@@ -308,7 +317,7 @@ __device__ __forceinline__ void cols_park_indices(const SegRec* __restrict__ seg
                 const float res = fmaxf(fabsf(y0 - (z0 - 12582912.0f)), fabsf(y1 - (z1 - 12582912.0f)));
                 ties |= (res > lim ? 1u : 0u) << (it * R1 + a);
                 *reinterpret_cast<int2*>(myslot + a * APITCH + it * ITPITCH) =
-                    make_int2(base - __float_as_int(z0), base + 1 - __float_as_int(z1));
+                    clamp_pair<CLAMP>(make_int2(base - __float_as_int(z0), base + 1 - __float_as_int(z1)), n);
             }
         }
         while (ties) {                                                         // rare (about 2 eps per sample): decide in fp64
@@ -322,8 +331,8 @@ __device__ __forceinline__ void cols_park_indices(const SegRec* __restrict__ seg
             const double2 c23 = __ldg(reinterpret_cast<const double2*>(r) + 3);
             const double ta = (double)o * (double)inv_h, tb = (double)(o + 1) * (double)inv_h;
             *reinterpret_cast<int2*>(myslot + a * APITCH + it * ITPITCH) =
-                make_int2(nn - floor_to_int(fma(fma(fma(c23.y, ta, c23.x), ta, c01.y), ta, c01.x)),
-                          nn + 1 - floor_to_int(fma(fma(fma(c23.y, tb, c23.x), tb, c01.y), tb, c01.x)));
+                clamp_pair<CLAMP>(make_int2(nn - floor_to_int(fma(fma(fma(c23.y, ta, c23.x), ta, c01.y), ta, c01.x)),
+                                            nn + 1 - floor_to_int(fma(fma(fma(c23.y, tb, c23.x), tb, c01.y), tb, c01.x))), n);
         }
     } else {
 #pragma unroll 2
@@ -331,7 +340,7 @@ __device__ __forceinline__ void cols_park_indices(const SegRec* __restrict__ seg
 #pragma unroll
             for (int a = 0; a < R1; ++a) {
                 const int nn = nn0 + ((a * 256 + NW0 * it) << row_shift);
-                *reinterpret_cast<int2*>(myslot + a * APITCH + it * ITPITCH) = source_pair(segs, nn, log2h, inv_h);
+                *reinterpret_cast<int2*>(myslot + a * APITCH + it * ITPITCH) = clamp_pair<CLAMP>(source_pair(segs, nn, log2h, inv_h), n);
             }
         }
     }
@@ -394,7 +403,7 @@ k_fft_cols(const float* __restrict__ x, const SegRec* __restrict__ seg, size_t s
     float2* __restrict__ myslot = fsm + col * LP + (w0 >> 4) * PB + (w0 & 15); // + a PA + it ITP
     const int nn0 = (int)((((size_t)w0 << log2m2) + c0 + col) << 1);
     const int row_shift = log2m2 + 1;                                          // samples between rows j1, j1 + 1
-    if (!DIRECT) cols_park_indices<R1, C, PA, ITP>(segs, log2h, inv_h, myslot, nn0, row_shift);
+    if (!DIRECT) cols_park_indices<R1, C, PA, ITP, !DEBUG>(segs, log2h, inv_h, myslot, nn0, row_shift, n);
     // phase A1: gather (independent loads), radix-R1 over a, twiddle, back to the same slots
 #pragma unroll UA1
     for (int it = 0; it < NIT; ++it) {
@@ -408,8 +417,13 @@ k_fft_cols(const float* __restrict__ x, const SegRec* __restrict__ seg, size_t s
                 continue;
             }
             const int2 sp = *reinterpret_cast<const int2*>(p + a * PA);
-            v[a].x = ((unsigned)sp.x < (unsigned)n) ? __ldg(x + sp.x) : fill;
-            v[a].y = ((unsigned)sp.y < (unsigned)n) ? __ldg(x + sp.y) : fill;
+            if (DEBUG) {                             // raw indices: test here; otherwise clamped to n, x[n] = fill
+                v[a].x = ((unsigned)sp.x < (unsigned)n) ? __ldg(x + sp.x) : fill;
+                v[a].y = ((unsigned)sp.y < (unsigned)n) ? __ldg(x + sp.y) : fill;
+            } else {
+                v[a].x = __ldg(x + sp.x);
+                v[a].y = __ldg(x + sp.y);
+            }
             if (DEBUG) {
                 const size_t nn = (size_t)b * n + (size_t)(nn0 + ((a * 256 + NW0 * it) << row_shift));
                 idx_out[nn] = sp.x; idx_out[nn + 1] = sp.y;
@@ -501,14 +515,19 @@ k_fft_cols32(const float* __restrict__ x, const SegRec* __restrict__ seg, size_t
     float2* __restrict__ myslot = fsm + col * LP + c;                          // + a' PK, a' = 16 a + it
     const int nn0 = (int)((((size_t)c << log2m2) + c0 + col) << 1);
     const int row_shift = log2m2 + 1;
-    cols_park_indices<2, C, 16 * PK, PK>(segs, log2h, inv_h, myslot, nn0, row_shift);
+    cols_park_indices<2, C, 16 * PK, PK, !DEBUG>(segs, log2h, inv_h, myslot, nn0, row_shift, n);
     {   // gather (64 independent loads), radix 32 over a', twiddle, back to the same slots
         float2 v[32];
 #pragma unroll
         for (int a = 0; a < 32; ++a) {
             const int2 sp = *reinterpret_cast<const int2*>(myslot + a * PK);
-            v[a].x = ((unsigned)sp.x < (unsigned)n) ? __ldg(x + sp.x) : fill;
-            v[a].y = ((unsigned)sp.y < (unsigned)n) ? __ldg(x + sp.y) : fill;
+            if (DEBUG) {                             // raw indices: test here; otherwise clamped to n, x[n] = fill
+                v[a].x = ((unsigned)sp.x < (unsigned)n) ? __ldg(x + sp.x) : fill;
+                v[a].y = ((unsigned)sp.y < (unsigned)n) ? __ldg(x + sp.y) : fill;
+            } else {
+                v[a].x = __ldg(x + sp.x);
+                v[a].y = __ldg(x + sp.y);
+            }
             if (DEBUG) {
                 const size_t nn = (size_t)b * n + (size_t)(nn0 + ((16 * a) << row_shift));
                 idx_out[nn] = sp.x; idx_out[nn + 1] = sp.y;
