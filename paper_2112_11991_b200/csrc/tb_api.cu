@@ -76,6 +76,7 @@ struct tb_plan {
     float2 rot = {1.f, 0.f};                         // W_N^1
     int min_log2h = 0;                               // smallest knot spacing among the staged templates
     int n_sm = 148;                                  // multiprocessors of the device
+    int pf_mid = 0, pf_scat = 0;                     // same for the two row passes of the three-pass FFT
     int pf_cols = 0;                                 // same for pass 1 (segment records)
     int pf_spec = 0;                                 // same for the spectrum former
     int pf_rows = 0;                                 // L2 prefetch distance of pass 2, in CTAs (resident CTAs of the device)
@@ -369,13 +370,13 @@ int run_own_pass23(tb_plan* p, uint32_t nt)
         static bool attr = false;
         if (!attr) { TB_CUDA(p, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cols_smem<1, 16>())); attr = true; }
         kern<<<rows * 16, FFT_THREADS, cols_smem<1, 16>(), p->stream>>>(nullptr, nullptr, 0, nullptr, (int)rows, 0, 8, 0.f, p->d_tw1b, p->d_tw2,
-                                                                       reinterpret_cast<float2*>(p->d_resampled), nullptr, nullptr, 0);
+                                                                       reinterpret_cast<float2*>(p->d_resampled), nullptr, nullptr, p->pf_mid);
         TB_CUDA(p, cudaGetLastError());
     }
     {
         static bool attr = false;
         if (!attr) { TB_CUDA(p, cudaFuncSetAttribute(k_fft_rows_scatter, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RS_SMEM)); attr = true; }
-        k_fft_rows_scatter<<<rows * 16, FFT_THREADS, RS_SMEM, p->stream>>>(reinterpret_cast<const float2*>(p->d_resampled), p->d_fft, p->d_tw2);
+        k_fft_rows_scatter<<<rows * 16, FFT_THREADS, RS_SMEM, p->stream>>>(reinterpret_cast<const float2*>(p->d_resampled), p->d_fft, p->d_tw2, p->pf_scat);
         TB_CUDA(p, cudaGetLastError());
     }
     return TB_OK;
@@ -758,6 +759,10 @@ int tb_plan_create(tb_plan** out, const float* series, uint64_t n_samples, doubl
         p->pf_rows = pf ? atoi(pf) : p->n_sm * 2;
         const char* pfc = getenv("TB_PF_COLS");
         p->pf_cols = pfc ? atoi(pfc) : 128;
+        const char* pfm = getenv("TB_PF_MID");
+        p->pf_mid = pfm ? atoi(pfm) : 1500;
+        const char* pfq = getenv("TB_PF_SCAT");
+        p->pf_scat = pfq ? atoi(pfq) : 1500;
         const char* pfs = getenv("TB_PF_SPEC");
         p->pf_spec = pfs ? atoi(pfs) : 32;
         p->seg_stride = (size_t)(p->n >> OWN_MIN_LOG2H);

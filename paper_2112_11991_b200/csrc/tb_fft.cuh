@@ -403,6 +403,11 @@ k_fft_cols(const float* __restrict__ x, const SegRec* __restrict__ seg, size_t s
     float2* __restrict__ myslot = fsm + col * LP + (w0 >> 4) * PB + (w0 & 15); // + a PA + it ITP
     const int nn0 = (int)((((size_t)w0 << log2m2) + c0 + col) << 1);
     const int row_shift = log2m2 + 1;                                          // samples between rows j1, j1 + 1
+    if (DIRECT && pf_dist > 0 && blockIdx.x + pf_dist < gridDim.x) {            // tile of a later CTA -> L2 (one line per row)
+        const unsigned nb = blockIdx.x + pf_dist;
+        const float2* __restrict__ Tn = T + (size_t)(nb / bundles) * m + (nb % bundles) * C;
+        for (int j1 = threadIdx.x; j1 < L; j1 += FFT_THREADS) asm volatile("prefetch.global.L2 [%0];" ::"l"(Tn + ((size_t)j1 << log2m2)));
+    }
     if (!DIRECT) cols_park_indices<R1, C, PA, ITP, !DEBUG>(segs, log2h, inv_h, myslot, nn0, row_shift, n);
     // phase A1: gather (independent loads), radix-R1 over a, twiddle, back to the same slots
 #pragma unroll UA1
@@ -659,7 +664,7 @@ constexpr int RS_ROWS = 16;
 constexpr size_t RS_SMEM = (size_t)(RS_ROWS * (16 * FFT_PB + 1) + 256) * sizeof(float2);
 
 __global__ void __launch_bounds__(FFT_THREADS, 3)
-k_fft_rows_scatter(const float2* __restrict__ U, float2* __restrict__ Zt, const float2* __restrict__ tw2g)
+k_fft_rows_scatter(const float2* __restrict__ U, float2* __restrict__ Zt, const float2* __restrict__ tw2g, int pf_dist)
 {
     constexpr int PB = FFT_PB, LP = 16 * FFT_PB + 1;
     extern __shared__ __align__(16) float2 fsm[];
@@ -669,6 +674,10 @@ k_fft_rows_scatter(const float2* __restrict__ U, float2* __restrict__ Zt, const 
     const float2* __restrict__ Ub = U + (row << 16) + (size_t)ka0 * 256;
     float2* __restrict__ Zb = Zt + (row << 16) + ka0;
     tw2[threadIdx.x] = __ldg(tw2g + threadIdx.x);
+    if (threadIdx.x == 0 && pf_dist > 0 && blockIdx.x + pf_dist < gridDim.x) {  // the 32 KB of a later CTA -> L2
+        const float2* nxt = U + (size_t)(blockIdx.x + pf_dist) * (RS_ROWS * 256);
+        asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(nxt), "r"((unsigned)(RS_ROWS * 256 * sizeof(float2))) : "memory");
+    }
     {
         const int w = threadIdx.x;                   // jb = 16 b + c
         float2 v[RS_ROWS];
