@@ -96,9 +96,10 @@ typedef struct {
                                      rounded to fp32 (G8); 1: they take fill_value */
     float    fill_value;
     int32_t  enable_timings;      /* 1: record CUDA events around every stage of every chunk */
-    int32_t  fft_path;            /* 0: automatic (hand-written two-pass FFT with fused gather where it
-                                     applies: 2^17 <= N <= 2^23, W in {512, 1024, 2048} (256 or 1024 at
-                                     2^17) and knot spacing >= 8; batched cuFFT otherwise); 1: always
+    int32_t  fft_path;            /* 0: automatic (hand-written FFT with fused gather where it applies:
+                                     2^17 <= N <= 2^26 (two passes up to 2^24, three above), W in
+                                     {512, 1024, 2048} (256 or 1024 at 2^17 and 2^25; 1024 or 2048 at
+                                     2^24) and knot spacing >= 8; batched cuFFT otherwise); 1: always
                                      cuFFT; 2: hand-written or TB_ERR_INVALID_ARG */
 } tb_plan_opts;
 
@@ -106,8 +107,10 @@ typedef struct {
  * summed over chunks; zero unless opts.enable_timings), and the byte model of DESIGN.md section 7.
  *   hand-written FFT path (fft_path_used = 2)        cuFFT path (fft_path_used = 1)
  *   ms_delay     K0 k_delay_segments (a2 knots)      0
- *   ms_resample  P1 k_fft_cols (a2+a3 + a4 pass 1)   k_resample (a2+a3)
- *   ms_fft       P2 k_fft_rows_t (a4 pass 2)         batched cuFFT R2C (a4)
+ *   ms_resample  P1 k_fft_cols32 / k_fft_cols        k_resample (a2+a3)
+ *                (a2+a3 + a4 pass 1)
+ *   ms_fft       P2 k_fft_rows_t (a4 pass 2; two     batched cuFFT R2C (a4)
+ *                kernels at N >= 2^25)
  *   ms_spectrum  k_spectrum_t (a4 unpack, a5-a7)     k_spectrum_median (a5-a7)
  *   ms_hsum      k_hsum_tile (a8+a9)                 same
  * ms_normalise is always 0 (a7 is fused into the spectrum kernels); kept for layout stability. */

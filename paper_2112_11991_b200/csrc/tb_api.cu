@@ -534,7 +534,7 @@ int run_hsum(tb_plan* p, uint32_t nt, const FoldParams& fp, uint32_t first_id)
     if (p->nb >= (uint64_t)HS_T) {
         const int tiles = (int)(p->nb / HS_T);
         const int tpc = std::min(tiles, TB_HS_TPC);                                  // tiles walked by one CTA (double-buffered)
-        const size_t smem = 2 * HS_SMEM_FLOATS * sizeof(float);
+        const size_t smem = HS_BUFS * HS_SMEM_FLOATS * sizeof(float);
         static bool attr_set = false;
         if (!attr_set) {
             TB_CUDA(p, cudaFuncSetAttribute(k_hsum_tile, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));

@@ -978,7 +978,11 @@ __device__ __forceinline__ void hs_tile_body(const float* __restrict__ sm, int q
 // values of tile t+1 are already on their way to registers, so no warp waits on memory once the
 // first tile is in.  Warps 0-3 take bins 0-7 of every group of 16, warps 4-7 bins 8-15: 16 warps
 // per SM instead of 8 on the same staged bytes (the staging, not the registers, limits residency).
-__global__ void __launch_bounds__(HS_THREADS, 2)
+#ifndef TB_HS_BUFS
+#define TB_HS_BUFS 2                    // staging buffers per CTA (1: three CTAs per SM, overlap across CTAs only)
+#endif
+constexpr int HS_BUFS = TB_HS_BUFS;
+__global__ void __launch_bounds__(HS_THREADS, HS_BUFS == 1 ? 3 : 2)
 k_hsum_tile(const float* __restrict__ Ph, int nb, int groups_per_row, int tpc, FoldParams fp, uint32_t first_id,
             Candidate* __restrict__ out, unsigned long long* __restrict__ cursor, unsigned long long capacity)
 {
@@ -998,15 +1002,16 @@ k_hsum_tile(const float* __restrict__ Ph, int nb, int groups_per_row, int tpc, F
     for (int t = 0; t < tpc; ++t) {
         const int k0 = (tile0 + t) * HS_T;
         const uint32_t kq = (uint32_t)(k0 + 16 * q + 8 * half);
-        const float* sm = hs_sm + (t & 1) * HS_SMEM_FLOATS;
-        if (t + 1 < tpc && threadIdx.x == 0)         // the other buffer was released by the barrier that ended tile t-1
+        const float* sm = hs_sm + (t % HS_BUFS) * HS_SMEM_FLOATS;
+        if (HS_BUFS == 2 && t + 1 < tpc && threadIdx.x == 0)   // the other buffer was released by the barrier that ended tile t-1
             hs_stage(hs_sm + ((t + 1) & 1) * HS_SMEM_FLOATS, p, k0 + HS_T, &bar[(t + 1) & 1]);
         const HsDirect d = nxt;
         if (t + 1 < tpc) nxt = hs_load_direct(p, kq + HS_T);
-        const uint32_t parity = (uint32_t)((t >> 1) & 1);
-        if (half) hs_tile_body<1>(sm, q, d, kq, &bar[t & 1], parity, fp, tid, out, cursor, capacity);
-        else      hs_tile_body<0>(sm, q, d, kq, &bar[t & 1], parity, fp, tid, out, cursor, capacity);
+        const uint32_t parity = (uint32_t)((t / HS_BUFS) & 1);
+        if (half) hs_tile_body<1>(sm, q, d, kq, &bar[t % HS_BUFS], parity, fp, tid, out, cursor, capacity);
+        else      hs_tile_body<0>(sm, q, d, kq, &bar[t % HS_BUFS], parity, fp, tid, out, cursor, capacity);
         __syncthreads();                             // every thread is done with buffer t&1: it may be refilled
+        if (HS_BUFS == 1 && t + 1 < tpc && threadIdx.x == 0) hs_stage(hs_sm, p, k0 + HS_T, &bar[0]);
     }
 }
 
