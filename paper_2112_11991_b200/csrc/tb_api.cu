@@ -18,6 +18,7 @@
 #include <limits>
 #include <map>
 #include <new>
+#include <set>
 #include <string>
 #include <vector>
 
@@ -90,6 +91,8 @@ struct tb_plan {
     size_t events_used = 0;
     tb_timings last = {};
 
+    std::set<const void*> smem_ok;                   // kernels whose dynamic shared-memory limit has been raised on this device
+
     std::string err;
 };
 
@@ -116,6 +119,15 @@ int fail(tb_plan* p, int code, const std::string& msg)
             return fail((p), r__ == CUFFT_ALLOC_FAILED ? TB_ERR_NOMEM : TB_ERR_CUFFT,                  \
                         std::string(#call) + ": cufft error " + std::to_string((int)r__));             \
     } while (0)
+
+// opt a kernel in to more than 48 KB of dynamic shared memory, once per plan (the attribute is per device)
+int allow_smem(tb_plan* p, const void* kern, size_t bytes)
+{
+    if (p->smem_ok.count(kern)) return TB_OK;
+    TB_CUDA(p, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
+    p->smem_ok.insert(kern);
+    return TB_OK;
+}
 
 bool is_pow2(uint64_t v) { return v && !(v & (v - 1)); }
 uint32_t ilog2(uint64_t v) { uint32_t l = 0; while ((1ull << (l + 1)) <= v) ++l; return l; }
@@ -305,8 +317,7 @@ template <int R1, int FFT_C, bool DEBUG>
 int launch_cols(tb_plan* p, size_t off, uint32_t nt, long long* d_idx, float* d_y)
 {
     auto kern = k_fft_cols<R1, FFT_C, DEBUG>;
-    static bool attr = false;
-    if (!attr) { TB_CUDA(p, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cols_smem<R1, FFT_C>())); attr = true; }
+    if (int rc_ = allow_smem(p, reinterpret_cast<const void*>(kern), (size_t)(cols_smem<R1, FFT_C>()))) return rc_;
     const unsigned grid = (unsigned)(((1u << p->log2m2) / FFT_C) * nt);
     kern<<<grid, FFT_THREADS, cols_smem<R1, FFT_C>(), p->stream>>>(p->d_series, p->d_seg, p->seg_stride, p->d_tmpl + off, (int)nt,
                                                            (int)p->n, p->log2m2, p->fill, p->d_tw1a, p->d_tw2,
@@ -320,8 +331,7 @@ int launch_rows(tb_plan* p, uint32_t nt)
 {
     using Cfg = RowsCfg<R1>;
     auto kern = k_fft_rows_t<R1>;
-    static bool attr = false;
-    if (!attr) { TB_CUDA(p, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM)); attr = true; }
+    if (int rc_ = allow_smem(p, reinterpret_cast<const void*>(kern), (size_t)(Cfg::SMEM))) return rc_;
     const unsigned grid = (unsigned)(((1u << p->log2m1) / Cfg::R) * nt);
     kern<<<grid, FFT_THREADS, Cfg::SMEM, p->stream>>>(reinterpret_cast<const float2*>(p->d_resampled), p->d_fft, p->log2m1,
                                                      p->d_tw1b, p->d_tw2, p->pf_rows);
@@ -333,8 +343,7 @@ template <bool DEBUG>
 int launch_cols32(tb_plan* p, size_t off, uint32_t nt, long long* d_idx, float* d_y)
 {
     auto kern = k_fft_cols32<DEBUG>;
-    static bool attr = false;
-    if (!attr) { TB_CUDA(p, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C32_SMEM)); attr = true; }
+    if (int rc_ = allow_smem(p, reinterpret_cast<const void*>(kern), (size_t)(C32_SMEM))) return rc_;
     const unsigned grid = (unsigned)(((1u << p->log2m2) / 16) * nt);
     kern<<<grid, FFT_THREADS, C32_SMEM, p->stream>>>(p->d_series, p->d_seg, p->seg_stride, p->d_tmpl + off, (int)nt, (int)p->n,
                                                     p->log2m2, p->fill, p->d_twc, reinterpret_cast<float2*>(p->d_resampled),
@@ -367,15 +376,13 @@ int run_own_pass23(tb_plan* p, uint32_t nt)
     const unsigned rows = nt << p->log2m1;
     {
         auto kern = k_fft_cols<1, 16, false, true>;
-        static bool attr = false;
-        if (!attr) { TB_CUDA(p, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cols_smem<1, 16>())); attr = true; }
+        if (int rc_ = allow_smem(p, reinterpret_cast<const void*>(kern), (size_t)(cols_smem<1, 16>()))) return rc_;
         kern<<<rows * 16, FFT_THREADS, cols_smem<1, 16>(), p->stream>>>(nullptr, nullptr, 0, nullptr, (int)rows, 0, 8, 0.f, p->d_tw1b, p->d_tw2,
                                                                        reinterpret_cast<float2*>(p->d_resampled), nullptr, nullptr, p->pf_mid);
         TB_CUDA(p, cudaGetLastError());
     }
     {
-        static bool attr = false;
-        if (!attr) { TB_CUDA(p, cudaFuncSetAttribute(k_fft_rows_scatter, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)RS_SMEM)); attr = true; }
+        if (int rc_ = allow_smem(p, reinterpret_cast<const void*>(k_fft_rows_scatter), (size_t)(RS_SMEM))) return rc_;
         k_fft_rows_scatter<<<rows * 16, FFT_THREADS, RS_SMEM, p->stream>>>(reinterpret_cast<const float2*>(p->d_resampled), p->d_fft, p->d_tw2, p->pf_scat);
         TB_CUDA(p, cudaGetLastError());
     }
@@ -404,13 +411,11 @@ int launch_spectrum_t(tb_plan* p, uint32_t nt, float* d_raw)
     unsigned long long* fb = p->d_cursor + 1;
     if (d_raw) {
         auto kern = k_spectrum_t<W, LOG2M1, true>;
-        static bool attr = false;
-        if (!attr) { TB_CUDA(p, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); attr = true; }
+        if (int rc_ = allow_smem(p, reinterpret_cast<const void*>(kern), (size_t)(smem))) return rc_;
         kern<<<grid, ST_THREADS, smem, p->stream>>>(p->d_fft, p->d_power, p->d_med, p->log2m2, (int)p->nblk, p->d_twn, p->d_twb, p->rot, fb, d_raw, p->pf_spec);
     } else {
         auto kern = k_spectrum_t<W, LOG2M1, false>;
-        static bool attr = false;
-        if (!attr) { TB_CUDA(p, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); attr = true; }
+        if (int rc_ = allow_smem(p, reinterpret_cast<const void*>(kern), (size_t)(smem))) return rc_;
         kern<<<grid, ST_THREADS, smem, p->stream>>>(p->d_fft, p->d_power, p->d_med, p->log2m2, (int)p->nblk, p->d_twn, p->d_twb, p->rot, fb, nullptr, p->pf_spec);
     }
     TB_CUDA(p, cudaGetLastError());
@@ -535,11 +540,7 @@ int run_hsum(tb_plan* p, uint32_t nt, const FoldParams& fp, uint32_t first_id)
         const int tiles = (int)(p->nb / HS_T);
         const int tpc = std::min(tiles, TB_HS_TPC);                                  // tiles walked by one CTA (double-buffered)
         const size_t smem = HS_BUFS * HS_SMEM_FLOATS * sizeof(float);
-        static bool attr_set = false;
-        if (!attr_set) {
-            TB_CUDA(p, cudaFuncSetAttribute(k_hsum_tile, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-            attr_set = true;
-        }
+        if (int rc_ = allow_smem(p, reinterpret_cast<const void*>(k_hsum_tile), smem)) return rc_;
         k_hsum_tile<<<(unsigned)((tiles / tpc) * nt), HS_THREADS, smem, p->stream>>>(p->d_power, (int)p->nb, tiles / tpc, tpc, fp,
                                                                                      first_id, p->d_cand, p->d_cursor,
                                                                                      (unsigned long long)p->max_cand);
