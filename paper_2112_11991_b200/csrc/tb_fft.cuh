@@ -34,6 +34,9 @@ namespace tb {
 #ifndef TB_COLS_MINB
 #define TB_COLS_MINB 3
 #endif
+#ifndef TB_ROWS_TW_TREE
+#define TB_ROWS_TW_TREE 1               // 8192-point rows: first-step twiddles from a product tree instead of 31 table loads
+#endif
 #ifndef TB_ROWS_MINB
 #define TB_ROWS_MINB 2                  // CTAs per SM the pass-2 register budget is set for (2 measured faster than 3)
 #endif
@@ -541,8 +544,27 @@ k_fft_cols32(const float* __restrict__ x, const SegRec* __restrict__ seg, size_t
         }
         fft_reg<32>(v);
         myslot[0] = v[0];
+#if TB_ROWS_TW_TREE
+        {   // W_512^{c ka} = q[ka >> 3] * t[ka & 7] from two table values (see fft_rows_body)
+            float2 t[8], q[4];
+            t[1] = __ldg(twc + 16 + c);
+            q[1] = __ldg(twc + 8 * 16 + c);
+            t[2] = cmul(t[1], t[1]); t[3] = cmul(t[2], t[1]); t[4] = cmul(t[2], t[2]);
+            t[5] = cmul(t[4], t[1]); t[6] = cmul(t[4], t[2]); t[7] = cmul(t[4], t[3]);
+            q[2] = cmul(q[1], q[1]); q[3] = cmul(q[2], q[1]);
+#pragma unroll
+            for (int ka = 1; ka < 8; ++ka) myslot[ka * PK] = cmul(v[ka], t[ka]);
+#pragma unroll
+            for (int h = 1; h < 4; ++h) {
+                myslot[8 * h * PK] = cmul(v[8 * h], q[h]);
+#pragma unroll
+                for (int l = 1; l < 8; ++l) myslot[(8 * h + l) * PK] = cmul(v[8 * h + l], cmul(q[h], t[l]));
+            }
+        }
+#else
 #pragma unroll
         for (int ka = 1; ka < 32; ++ka) myslot[ka * PK] = cmul(v[ka], __ldg(twc + ka * 16 + c));
+#endif
     }
     __syncthreads();
     for (int i = threadIdx.x; i < 16 * 32; i += FFT_THREADS) {                 // item (col, ka), col fastest
@@ -632,6 +654,27 @@ k_fft_rows_t(const float2* __restrict__ T, float2* __restrict__ Zt, int log2m1, 
             fft_reg<R1>(v[r]);
             float2* p = fsm + r * LP + (w >> 4) * PB + (w & 15);
             p[0] = v[r][0];
+#if TB_ROWS_TW_TREE
+            if constexpr (R1 == 32) {
+                // W_L^{w ka} = q[ka >> 3] * t[ka & 7] from two table values (ka = 1 and 8): 29 complex
+                // products on the FMA pipe instead of 29 more loads on the LSU/MIO path this kernel
+                // throttles on; at most four roundings deep
+                float2 t[8], q[4];
+                t[1] = __ldg(tw1 + 256 + w);
+                q[1] = __ldg(tw1 + 8 * 256 + w);
+                t[2] = cmul(t[1], t[1]); t[3] = cmul(t[2], t[1]); t[4] = cmul(t[2], t[2]);
+                t[5] = cmul(t[4], t[1]); t[6] = cmul(t[4], t[2]); t[7] = cmul(t[4], t[3]);
+                q[2] = cmul(q[1], q[1]); q[3] = cmul(q[2], q[1]);
+#pragma unroll
+                for (int ka = 1; ka < 8; ++ka) p[ka * PA] = cmul(v[r][ka], t[ka]);
+#pragma unroll
+                for (int h = 1; h < 4; ++h) {
+                    p[8 * h * PA] = cmul(v[r][8 * h], q[h]);
+#pragma unroll
+                    for (int l = 1; l < 8; ++l) p[(8 * h + l) * PA] = cmul(v[r][8 * h + l], cmul(q[h], t[l]));
+                }
+            } else
+#endif
 #pragma unroll
             for (int ka = 1; ka < R1; ++ka) p[ka * PA] = cmul(v[r][ka], __ldg(tw1 + ka * 256 + w));
         }
