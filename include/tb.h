@@ -27,6 +27,9 @@
  *     tb_search_templates returns once the work is queued (host template staging is complete);
  *     tb_get_candidates / tb_get_timings / tb_debug_* synchronise that stream.
  *   - No global state; plans are independent; one plan must not be used from two threads at once.
+ *     (tb_plan_create reads the tuning-only environment variables TB_PF_ROWS, TB_PF_COLS, TB_PF_SPEC,
+ *     TB_PF_MID, TB_PF_SCAT (L2 prefetch distances, in CTAs) and TB_COLS32 (0: older first-pass
+ *     kernel); they change launch parameters, never results.)
  */
 #ifndef TB_H_
 #define TB_H_

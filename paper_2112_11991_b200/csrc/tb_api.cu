@@ -756,7 +756,7 @@ int tb_plan_create(tb_plan** out, const float* series, uint64_t n_samples, doubl
     }
     if (p->own_fft) {
         cudaDeviceGetAttribute(&p->n_sm, cudaDevAttrMultiProcessorCount, p->device);
-        const char* pf = getenv("TB_PF_ROWS");           // tuning knob: prefetch distance in CTAs (default: the resident CTAs, 3 per SM)
+        const char* pf = getenv("TB_PF_ROWS");           // tuning knob: prefetch distance in CTAs (default: two per SM)
         p->pf_rows = pf ? atoi(pf) : p->n_sm * 2;
         const char* pfc = getenv("TB_PF_COLS");
         p->pf_cols = pfc ? atoi(pfc) : 128;
