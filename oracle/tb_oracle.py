@@ -18,8 +18,16 @@ better than the 1e-9-sample tie window the north_star allows.
 
 Parity pins (tests/test_oracle_pins.py, ``-m "not gpu"``):
   kepler_solve ............ T4  residual <= 1e-12 and the printed App. B series
-  roemer_delay ............ T2  e=0 Kepler path == circular closed form; T1 tau=0 -> identity
-  resample_indices ........ T1, T3 (idx_0 = 0), T11 (monotone map, out-of-range bound)
+  roemer_delay ............ T2  e=0 Kepler path == circular closed form; T1 tau=0 -> identity;
+                            e>0: eq A1 assembled from the PRINTED e-series (eqs 15-16, App. B) to
+                            2 e^7 tau, and the hand-solvable points M = 0, pi, pi/2 - e
+  resample_indices ........ T1, T3 (idx_0 = 0), T11 (monotone map, out-of-range bound); the
+                            extended-precision re-decision: samples built 2e-11..3e-8 from a
+                            rounding tie against a 50-digit mpmath evaluation (both sides)
+  sign convention (G2-G4) . a series synthesised from eq A2 read literally (t' = t - Delta_R(t),
+                            no inverse map) is found at phi0 + pi and not at phi0: the paper is
+                            at odds with itself about this sign (eq 2/4 vs A2 vs Alg. 1), so
+                            the reading is pinned only up to that phase flip (both are searched)
   rfft_forward ............ T5 Parseval, T6 brute-force O(N^2) DFT at N=1024
   interbin_power .......... T7 closed forms for an integer-bin and a half-bin tone
   block_medians / baseline  hand-sorted toy input; T8 median = ln2 * mean for exponential noise

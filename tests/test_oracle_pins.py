@@ -298,3 +298,128 @@ def test_tie_distance_arbiter():
     d64 = orc.shift_in_samples(np.arange(5000), 1e-3, (60.0, 0.5, 1.0, 0.0, 0.0))
     dl = orc.tie_distance(np.arange(5000), 1e-3, (60.0, 0.5, 1.0, 0.0, 0.0))
     assert np.max(np.abs(np.abs((d64 - np.floor(d64)) - 0.5) - dl)) < 1e-9
+
+
+# ------------------------------------------------------------------ eq A1 at e > 0: the assembly of roemer_delay
+def test_roemer_delay_elliptical_against_the_printed_series():
+    """Delta = tau[(sum_k C_k cos kM - e) sin(omega) + (sum_k S_k sin kM) cos(omega)]: eq A1
+    with cos E and sqrt(1-e^2) sin E replaced by the PRINTED e-series (eqs 15-16, App. B
+    L719-747; the S-series already carries the sqrt(1-e^2) factor).  Truncated after e^6, so the
+    two agree to ~1.2 e^7 per unit tau; a dropped sqrt(1-e^2), a swapped sin/cos(omega) or a
+    missing -e moves the delay by >= e^2/2 tau."""
+    C, S = _load_series()
+    tsamp, p_orb, tau, phi0 = 1e-3, 37.0, 2.5, 0.4
+    j = np.arange(0, 40000, 7)
+    M = 2 * np.pi / p_orb * (j * tsamp) + phi0
+    for e in (0.01, 0.05, 0.1):
+        cosE = sum(sum(float(c) * e**p for p, c in terms) * np.cos(k * M) for k, terms in C.items())
+        qsinE = sum(sum(float(c) * e**p for p, c in terms) * np.sin(k * M) for k, terms in S.items())
+        for om in (0.3, 1.2, 4.0):
+            series = tau * ((cosE - e) * math.sin(om) + qsinE * math.cos(om))
+            got = orc.roemer_delay(j, tsamp, (p_orb, tau, phi0, e, om))
+            assert np.max(np.abs(got - series)) < (2.0 * e**7 * (abs(math.sin(om)) + abs(math.cos(om))) + 1e-14) * tau
+
+
+def test_roemer_delay_elliptical_closed_form_points():
+    """Points of eq A1 where Kepler's equation (eq 3) solves by hand:
+    M = 0 -> E = 0; M = pi -> E = pi; M = pi/2 - e -> E = pi/2."""
+    tau, tsamp = 3.0, 1e-3
+    j0 = np.zeros(1, dtype=np.int64)
+    for e in (0.05, 0.3, 0.7):
+        q = math.sqrt(1 - e * e)
+        for om in (0.3, 1.2, 4.0):
+            d = orc.roemer_delay(j0, tsamp, (50.0, tau, 0.0, e, om))[0]
+            assert abs(d - tau * (1 - e) * math.sin(om)) < 1e-14 * tau
+            d = orc.roemer_delay(j0, tsamp, (50.0, tau, math.pi, e, om))[0]
+            assert abs(d + tau * (1 + e) * math.sin(om)) < 1e-14 * tau
+            d = orc.roemer_delay(j0, tsamp, (50.0, tau, math.pi / 2 - e, e, om))[0]
+            assert abs(d - tau * (-e * math.sin(om) + q * math.cos(om))) < 1e-14 * tau
+            # a quarter of a period later in TIME (not at j = 0): t = P/4, phi0 = pi/2 - e - pi/2
+            p = 40.96
+            d = orc.roemer_delay(np.array([10240]), tsamp, (p, tau, -e, e, om))[0]
+            assert abs(d - tau * (-e * math.sin(om) + q * math.cos(om))) < 1e-12 * tau
+
+
+# ------------------------------------------------------------------ G10: the extended-precision tie decision
+def _exact_shift(j, tsamp, tmpl, digits=50):
+    """delta_j of eqs 3 / A1 / Alg. 1 L682-702 evaluated with mpmath at `digits` decimal digits on
+    the exact values of the double-precision inputs (independent of the oracle: own formulas)."""
+    import mpmath as mp
+    with mp.workdps(digits):
+        p_orb, tau, phi0, e, om = (mp.mpf(float(v)) for v in tmpl)
+        ts = mp.mpf(float(tsamp))
+
+        def delay(t):
+            M = 2 * mp.pi / p_orb * t + phi0
+            E = mp.findroot(lambda x: x - e * mp.sin(x) - M, M) if e != 0 else M
+            return tau * ((mp.cos(E) - e) * mp.sin(om) + mp.sqrt(1 - e * e) * mp.sin(E) * mp.cos(om))
+
+        return (delay(mp.mpf(int(j)) * ts) - delay(mp.mpf(0))) / ts
+
+
+def _tau_for_shift(j, tsamp, tmpl_unit_tau, target):
+    """tau (double) for which delta_j = target, from the exact shift per unit tau."""
+    import mpmath as mp
+    with mp.workdps(50):
+        return float(mp.mpf(target) / _exact_shift(j, tsamp, tmpl_unit_tau))
+
+
+@pytest.mark.parametrize("p_orb,phi0,e,om,j,n_int,off", [
+    (60.0, 1.0, 0.0, 0.0, 20011, 250, 3e-8),         # circular, moderate: fp64 would also get this right
+    (60.0, 1.0, 0.0, 0.0, 20011, 250, 2e-10),        # inside the north_star tie window's decade
+    (55.0, 2.2, 0.08, 1.2, 31337, 400, 3e-8),        # elliptical
+    (107.3, 0.7, 0.0, 0.0, 8000011, -60000, 2e-9),   # C4-like extreme (tau/tsamp ~ 5e4, j ~ 2^23)
+    # 2e-11 from the tie: plain fp64 (phase error ~1e-10 samples here) decides these WRONGLY on one
+    # side; only the extended-precision re-decision gets both sides right
+    (107.3, 0.7, 0.0, 0.0, 8001020, -60000, 2e-11),
+    (95.1, 2.9, 0.07, 2.2, 8000011, 110000, 2e-11),
+    (95.1, 2.9, 0.07, 2.2, 8001020, 110000, 2e-11),
+])
+def test_tie_branch_decides_like_the_exact_formula(p_orb, phi0, e, om, j, n_int, off):
+    """A sample constructed to sit `off` below / above a rounding tie (delta_j = n + 1/2 -+ off):
+    resample_indices must take floor(delta + 1/2) of the EXACT delta (50-digit mpmath), i.e. the
+    re-decision of lines "near" in resample_indices is what fixes the integer (reading G10)."""
+    import mpmath as mp
+    tsamp = 64e-6 if j > 1000000 else 1e-3
+    for side in (-1, +1):
+        tau = _tau_for_shift(j, tsamp, (p_orb, 1.0, phi0, e, om), mp.mpf(n_int) + mp.mpf(1) / 2 + side * mp.mpf(off))
+        tmpl = (p_orb, tau, phi0, e, om)
+        exact = _exact_shift(j, tsamp, tmpl)
+        with mp.workdps(50):
+            frac_off = float(exact - mp.floor(exact) - mp.mpf(1) / 2)
+            want = int(j) - int(mp.floor(exact + mp.mpf(1) / 2))
+        assert 0.3 * off < abs(frac_off) < 1.7 * off and np.sign(frac_off) == side     # the construction holds (tau is rounded to a double)
+        assert want == int(j) - (n_int + (1 if side > 0 else 0))
+        # the oracle's own fp64 shift is inside TIE_GUARD, so the extended-precision branch decides
+        d64 = orc.shift_in_samples(np.array([j]), tsamp, tmpl)[0]
+        assert abs((d64 - math.floor(d64)) - 0.5) < orc.TIE_GUARD
+        n = j + 1
+        idx = orc.resample_indices(n, tsamp, tmpl)
+        assert idx[j] == want
+        assert abs(orc.tie_distance(np.array([j]), tsamp, tmpl)[0] - abs(frac_off)) < 0.1 * off
+
+
+# ------------------------------------------------------------------ G2-G4: the sign convention against eq A2 taken literally
+def test_sign_convention_against_literal_eq_a2():
+    """Eq A2 read literally, with NO inverse-map construction: the pulsar-frame
+    time of the sample observed at t is t' = t - Delta_R(t).  Alg. 1 L702 gathers S[j - Delta_j/tsamp]
+    (reading G3), which is the map t = t' - Delta_R(t'), i.e. the opposite sign (G4: the paper is
+    at odds with itself: eq 2/4 vs A2 vs Alg. 1).  A sign flip of Delta_R is phi0 -> phi0 + pi for
+    a circular orbit, and the two maps then differ only by the second-order term
+    tau^2 Omega cos(.) sin(.) (0.4 ms here, against a 1 ms pulse).  So a series synthesised from
+    literal A2 must be found by the oracle with the template at phi0 + pi and NOT at phi0."""
+    n, tsamp, p_spin, p_orb, tau, phi0 = 1 << 16, 1e-3, 0.020, 40.0, 0.05, 0.9
+    rng = np.random.default_rng(4242)
+    t = np.arange(n) * tsamp
+    t_psr = t - tau * np.sin(2 * np.pi / p_orb * t + phi0)             # eq A2 with eq A1 at e = 0
+    ph = t_psr / p_spin
+    d = ph - np.rint(ph)
+    sig = 0.05 / (2.0 * math.sqrt(2.0 * math.log(2.0)))
+    x = (rng.standard_normal(n) + 0.45 * np.exp(-0.5 * (d / sig) ** 2)).astype(np.float32)
+    found = orc.search_template(x, tsamp, (p_orb, tau, phi0 + np.pi, 0.0, 0.0), 0)
+    assert found, "literal-A2 signal not recovered at phi0 + pi"
+    best = max(found, key=lambda c: c[4])
+    assert abs(best[2] / ((1 << best[1]) * n * tsamp) - 1.0 / p_spin) < 1.0 / (n * tsamp)
+    assert best[4] > 10.0
+    assert orc.search_template(x, tsamp, (p_orb, tau, phi0, 0.0, 0.0), 0) == []
+    assert orc.search_template(x, tsamp, (p_orb, 0.0, phi0, 0.0, 0.0), 0) == []      # and not without resampling
