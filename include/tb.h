@@ -26,10 +26,13 @@
  *   - Work is queued on the plan's stream (opts.stream, or a stream the plan creates).
  *     tb_search_templates returns once the work is queued (host template staging is complete);
  *     tb_get_candidates / tb_get_timings / tb_debug_* synchronise that stream.
- *   - No global state; plans are independent; one plan must not be used from two threads at once.
- *     (tb_plan_create reads the tuning-only environment variables TB_PF_ROWS, TB_PF_COLS, TB_PF_SPEC,
- *     TB_PF_MID, TB_PF_SCAT (L2 prefetch distances, in CTAs) and TB_COLS32 (0: older first-pass
- *     kernel); they change launch parameters, never results.)
+ *   - No global state in the library and no environment variables; plans are independent; one
+ *     plan must not be used from two threads at once.  Two device-wide side effects, both of
+ *     performance only: tb_plan_create RAISES cudaLimitPersistingL2CacheSize to the size of the
+ *     series if it is smaller (it is never lowered or reset, so other plans keep their L2 set-aside),
+ *     and it sets a persisting access-policy window for the series on the plan's stream; on a
+ *     caller-owned stream (opts.stream) the window that stream had before is restored by
+ *     tb_plan_destroy.
  */
 #ifndef TB_H_
 #define TB_H_
@@ -64,8 +67,9 @@ typedef struct tb_plan tb_plan;   /* opaque */
  *   phi0_rad  initial orbital phase alpha (mean anomaly at t = 0), radians, finite
  *   ecc       eccentricity e, 0 <= e < 1
  *   omega_rad longitude of periastron psi, radians, finite
- * ecc == 0 && omega_rad == 0 selects the circular closed form Delta = tau sin(Omega t + phi0)
- * (eq 4 L49 / eq A1 at e = 0); anything else the Kepler solve of eq 3 + eq A1. */
+ * ecc == 0 takes E = M without a Kepler solve: Delta = tau sin(Omega t + phi0 + omega_rad), which for
+ * omega_rad == 0 is the circular closed form (eq 4 L49 / eq A1 at e = 0, G6); ecc > 0 takes the
+ * Kepler solve of eq 3 + eq A1. */
 typedef struct {
     double p_orb_s, tau_lts, phi0_rad, ecc, omega_rad;
 } tb_template;                    /* 40 bytes */
@@ -124,7 +128,10 @@ typedef struct {
     uint64_t n_kernel_launches;          /* libtb's own kernels launched by that call (cuFFT's not counted) */
     uint64_t n_median_fallbacks;         /* median blocks that took the data-independent bisection path */
     double   ms_delay;
-    uint64_t fft_path_used;              /* 1: batched cuFFT, 2: hand-written two-pass FFT with fused gather */
+    uint64_t fft_path_used;              /* bit 0: some templates went through k_resample + batched cuFFT; bit 1: some
+                                            through the hand-written FFT with fused gather (a bank is split per template:
+                                            knot spacing >= 8 samples -> fused path); 3 = both, and then the per-stage
+                                            times above are sums over both kinds of chunk */
 } tb_timings;
 
 /* Create a plan for one dedispersed time series S[i], i*tsamp.
@@ -151,6 +158,8 @@ TB_API int tb_plan_set_series(tb_plan* plan, const float* series);
  *   folds / n_folds   the harmonic folds to threshold: distinct values from {0,1,2,3,4}
  *   sigma_threshold   candidates have sigma_L >= sigma_threshold (finite)
  * Invalid templates make the whole call fail with TB_ERR_INVALID_ARG before any work is queued.
+ * If a later step fails (TB_ERR_CUDA / TB_ERR_CUFFT / TB_ERR_NOMEM) the candidates of the chunks
+ * that had already been queued REMAIN in the buffer; call tb_clear_candidates before retrying.
  * n_templates == 0 is valid and does nothing. */
 TB_API int tb_search_templates(tb_plan* plan, const tb_template* tmpl, uint64_t n_templates,
                         uint32_t first_template_id, const uint32_t* folds, uint32_t n_folds,
@@ -185,6 +194,11 @@ TB_API int tb_debug_spectrum(tb_plan* plan, const tb_template* tmpl, float* p_in
 
 /* Resampled series y_j of one template (a3): host float32[N]. */
 TB_API int tb_debug_resampled(tb_plan* plan, const tb_template* tmpl, float* y_out);
+
+/* Harmonic sums of one template (a8; eq 9, G16) through the production summing kernel with its
+ * tap enabled and every threshold at +infinity: sums_out[L * (N/2) + k] = S_L[k], L = 0..4,
+ * k = 0..N/2-1; host float32[5 * N/2].  Emits no candidates. */
+TB_API int tb_debug_hsums(tb_plan* plan, const tb_template* tmpl, float* sums_out);
 
 /* Host fp64: the summed power at which sigma_L equals `sigma` (G17).  fold 0..4. */
 TB_API int tb_sigma_to_power(uint32_t fold, double sigma, double* power_out);

@@ -6,9 +6,7 @@
 
 #include <cufft.h>
 
-#ifndef TB_HS_TPC
-#define TB_HS_TPC 16                   // tiles walked by one CTA of the harmonic summer
-#endif
+constexpr int HS_TPC = 16;             // tiles walked by one CTA of the harmonic summer
 
 #include <algorithm>
 #include <cmath>
@@ -48,6 +46,7 @@ struct tb_plan {
     uint32_t chunk = 0;
     bool timings = false;
     bool user_fill = false, borrowed = false, l2_pinned = false;
+    cudaStreamAttrValue l2_prev = {};                // access-policy window a caller-owned stream had before the plan set its own
     float fill = 0.f;
     float h_fillpad[4] = {0.f, 0.f, 0.f, 0.f};
     size_t ld = 0;                                   // complex row stride of the FFT output
@@ -70,17 +69,20 @@ struct tb_plan {
     // hand-written FFT path (tb_fft.cuh): M = N/2 = M1 * M2
     bool own_fft = false;
     int log2m1 = 0, log2m2 = 0;
-    SegRec* d_seg = nullptr;                         // [chunk][n >> MIN_LOG2H]
-    size_t seg_stride = 0;
+    SegRec* d_seg = nullptr;                         // [chunk][seg_stride], grown on demand (seg_stride = n >> smallest knot spacing staged)
+    size_t seg_stride = 0, seg_cap = 0;              // records per template, records allocated
     float2 *d_tw1a = nullptr, *d_tw1b = nullptr, *d_tw2 = nullptr, *d_twn = nullptr, *d_twb = nullptr, *d_twc = nullptr;
     bool cols32 = false;                             // pass 1 as 32 x 16 (M1 = 512)
     float2 rot = {1.f, 0.f};                         // W_N^1
-    int min_log2h = 0;                               // smallest knot spacing among the staged templates
+    int chunk_log2h = 0;                             // smallest knot spacing among the templates of the chunk being launched
     int n_sm = 148;                                  // multiprocessors of the device
-    int pf_mid = 0, pf_scat = 0;                     // same for the two row passes of the three-pass FFT
-    int pf_cols = 0;                                 // same for pass 1 (segment records)
-    int pf_spec = 0;                                 // same for the spectrum former
-    int pf_rows = 0;                                 // L2 prefetch distance of pass 2, in CTAs (resident CTAs of the device)
+    // L2 prefetch distances in CTAs (measured on B200, profiles/r01_v3.md)
+    int pf_rows = 0;                                 // pass 2: two CTAs per SM ahead
+    int pf_cols = 128;                               // pass 1 (segment records)
+    int pf_mid = 1500, pf_scat = 1500;               // the two row passes of the three-pass FFT
+    int pf_spec = 32;                                // spectrum former
+    std::vector<uint32_t> order;                     // staging order of the current call: fused-path templates first
+    size_t n_own = 0;                                // how many of them take the fused path
 
     std::map<uint32_t, cufftHandle> fft_plans;       // by batch size, sharing one work area
     void* d_work = nullptr;
@@ -243,12 +245,20 @@ int load_series(tb_plan* p, const float* series)
 
 // Keep the series resident in L2 (persisting access-policy window on the plan's stream): every
 // template gathers from the same 4N bytes while tens of GB of scratch stream through the cache.
+// Device-wide side effect (documented in tb.h): cudaLimitPersistingL2CacheSize is RAISED to the
+// series size if it is smaller, never lowered, and never reset (other plans' windows stay valid).
+// On a caller-owned stream the previous window is saved here and restored by destroy().
 void pin_series_in_l2(tb_plan* p)
 {
     cudaDeviceProp prop;
     if (cudaGetDeviceProperties(&prop, p->device) != cudaSuccess || prop.persistingL2CacheMaxSize <= 0) return;
     const size_t bytes = std::min<size_t>(p->n * sizeof(float), (size_t)prop.accessPolicyMaxWindowSize);
-    cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, std::min<size_t>(bytes, (size_t)prop.persistingL2CacheMaxSize));
+    const size_t want = std::min<size_t>(bytes, (size_t)prop.persistingL2CacheMaxSize);
+    size_t have = 0;
+    if (cudaDeviceGetLimit(&have, cudaLimitPersistingL2CacheSize) != cudaSuccess) have = 0;
+    if (have < want) cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, want);
+    if (!p->own_stream && cudaStreamGetAttribute(p->stream, cudaStreamAttributeAccessPolicyWindow, &p->l2_prev) != cudaSuccess)
+        std::memset(&p->l2_prev, 0, sizeof(p->l2_prev));
     cudaStreamAttrValue attr;
     std::memset(&attr, 0, sizeof(attr));
     attr.accessPolicyWindow.base_ptr = const_cast<float*>(p->d_series);
@@ -355,7 +365,7 @@ int launch_cols32(tb_plan* p, size_t off, uint32_t nt, long long* d_idx, float* 
 // K0 + P1: delay segments, then gather + column FFTs into T (the buffer the legacy path uses for y)
 int run_own_pass1(tb_plan* p, size_t off, uint32_t nt, long long* d_idx, float* d_y, cudaEvent_t after_k0 = nullptr)
 {
-    const int cta_per_tmpl = (int)(((p->n >> p->min_log2h) + 255) / 256);   // min_log2h: smallest knot spacing staged
+    const int cta_per_tmpl = (int)(((p->n >> p->chunk_log2h) + 255) / 256);   // chunk_log2h: smallest knot spacing in this chunk
     k_delay_segments<<<(unsigned)(cta_per_tmpl * nt), K0_THREADS, 0, p->stream>>>(p->d_tmpl + off, (int)nt, (int)p->n, p->d_seg,
                                                                            p->seg_stride, cta_per_tmpl);
     TB_CUDA(p, cudaGetLastError());
@@ -487,8 +497,7 @@ int make_twiddles(tb_plan* p)
                 hc[ka * 16 + c] = make_float2((float)cosl(a), (float)sinl(a));
             }
         if ((rc = upload(hc, &p->d_twc))) return rc;
-        const char* e = getenv("TB_COLS32");
-        p->cols32 = !(e && atoi(e) == 0);
+        p->cols32 = true;
     }
     p->rot = make_float2((float)cosl(two_pi / (long double)p->n), (float)-sinl(two_pi / (long double)p->n));
     if ((rc = upload(h2, &p->d_tw2))) return rc;
@@ -534,27 +543,43 @@ int run_spectrum(tb_plan* p, uint32_t nt, float* d_raw = nullptr)
     return TB_OK;
 }
 
-int run_hsum(tb_plan* p, uint32_t nt, const FoldParams& fp, uint32_t first_id)
+// a8 + a9 for the nt templates at d_tmpl + off (their ids come from TmplDev::id); tap: parity tap [5][nb] or null
+int run_hsum(tb_plan* p, size_t off, uint32_t nt, const FoldParams& fp, float* tap = nullptr)
 {
+    const TmplDev* tm = p->d_tmpl + off;
     if (p->nb >= (uint64_t)HS_T) {
         const int tiles = (int)(p->nb / HS_T);
-        const int tpc = std::min(tiles, TB_HS_TPC);                                  // tiles walked by one CTA (double-buffered)
+        const int tpc = std::min(tiles, HS_TPC);                                     // tiles walked by one CTA (double-buffered)
         const size_t smem = HS_BUFS * HS_SMEM_FLOATS * sizeof(float);
-        if (int rc_ = allow_smem(p, reinterpret_cast<const void*>(k_hsum_tile), smem)) return rc_;
-        k_hsum_tile<<<(unsigned)((tiles / tpc) * nt), HS_THREADS, smem, p->stream>>>(p->d_power, (int)p->nb, tiles / tpc, tpc, fp,
-                                                                                     first_id, p->d_cand, p->d_cursor,
-                                                                                     (unsigned long long)p->max_cand);
+        const unsigned grid = (unsigned)((tiles / tpc) * nt);
+        if (tap) {
+            if (int rc_ = allow_smem(p, reinterpret_cast<const void*>(k_hsum_tile<true>), smem)) return rc_;
+            k_hsum_tile<true><<<grid, HS_THREADS, smem, p->stream>>>(p->d_power, (int)p->nb, tiles / tpc, tpc, fp, tm, p->d_cand, p->d_cursor,
+                                                                    (unsigned long long)p->max_cand, tap);
+        } else {
+            if (int rc_ = allow_smem(p, reinterpret_cast<const void*>(k_hsum_tile<false>), smem)) return rc_;
+            k_hsum_tile<false><<<grid, HS_THREADS, smem, p->stream>>>(p->d_power, (int)p->nb, tiles / tpc, tpc, fp, tm, p->d_cand, p->d_cursor,
+                                                                     (unsigned long long)p->max_cand, nullptr);
+        }
         TB_CUDA(p, cudaGetLastError());
         return TB_OK;
     }
     const int cta_per_row = (int)((p->nb + 255) / 256);
-    k_hsum_threshold<<<(unsigned)(cta_per_row * nt), 256, 0, p->stream>>>(p->d_power, (int)p->nb, cta_per_row, fp,
-                                                                          first_id, p->d_cand, p->d_cursor,
-                                                                          (unsigned long long)p->max_cand);
+    if (tap) k_hsum_threshold<true><<<(unsigned)(cta_per_row * nt), 256, 0, p->stream>>>(p->d_power, (int)p->nb, cta_per_row, fp, tm, p->d_cand,
+                                                                                     p->d_cursor, (unsigned long long)p->max_cand, tap);
+    else     k_hsum_threshold<false><<<(unsigned)(cta_per_row * nt), 256, 0, p->stream>>>(p->d_power, (int)p->nb, cta_per_row, fp, tm, p->d_cand,
+                                                                                      p->d_cursor, (unsigned long long)p->max_cand, nullptr);
     TB_CUDA(p, cudaGetLastError());
     return TB_OK;
 }
 
+// the fused path needs records of >= 8 samples; the rest of a bank goes through k_resample + cuFFT
+bool takes_own_path(const tb_plan* p, const tb_template& t) { return p->own_fft && tmpl_log2h(t, p->tsamp) >= OWN_MIN_LOG2H; }
+
+// Validate the bank, size the staging buffers, and split it by launch sequence (stable partition:
+// templates the fused path can take first, the others after them), so that one fast-orbit template
+// does not send the whole bank through the library-FFT path.  p->order[pos] = index in the caller's
+// array of the template staged at position pos; the candidates carry first_id + that index.
 int upload_templates(tb_plan* p, const tb_template* tmpl, uint64_t k)
 {
     for (uint64_t i = 0; i < k; ++i) {
@@ -578,22 +603,50 @@ int upload_templates(tb_plan* p, const tb_template* tmpl, uint64_t k)
         TB_CUDA(p, cudaMalloc(&p->d_tmpl, k * sizeof(TmplDev)));
         p->tmpl_cap = k;
     }
-    // knot spacings first (cheap): the smallest one selects the launch sequence and K0's grid;
-    // the constants themselves are made and uploaded chunk by chunk (stage_chunk), so that the
-    // host's extended-precision trigonometry overlaps the kernels of the previous chunk
-    p->min_log2h = 7;
-    for (uint64_t i = 0; i < k; ++i) p->min_log2h = std::min(p->min_log2h, tmpl_log2h(tmpl[i], p->tsamp));
+    // knot spacings first (cheap): they select the launch sequence of every template and the size of
+    // the segment table; the constants themselves are made and uploaded chunk by chunk (stage_chunk),
+    // so that the host's extended-precision trigonometry overlaps the kernels of the previous chunk
+    p->order.resize(k);
+    std::vector<uint32_t> rest;
+    size_t n_own = 0;
+    int min_own = 7;
+    for (uint64_t i = 0; i < k; ++i) {
+        const int l = p->own_fft ? tmpl_log2h(tmpl[i], p->tsamp) : 0;
+        if (p->own_fft && l >= OWN_MIN_LOG2H) { p->order[n_own++] = (uint32_t)i; min_own = std::min(min_own, l); }
+        else rest.push_back((uint32_t)i);
+    }
+    std::copy(rest.begin(), rest.end(), p->order.begin() + n_own);
+    p->n_own = n_own;
+    if (n_own) {                                         // segment table: chunk x (n >> smallest spacing) records
+        p->seg_stride = (size_t)(p->n >> min_own);
+        const size_t need = (size_t)std::min<uint64_t>(p->chunk, n_own) * p->seg_stride;
+        if (need > p->seg_cap) {
+            TB_CUDA(p, cudaStreamSynchronize(p->stream));
+            if (p->d_seg) cudaFree(p->d_seg);
+            p->d_seg = nullptr; p->seg_cap = 0;
+            TB_CUDA(p, cudaMalloc(&p->d_seg, need * sizeof(SegRec)));
+            p->seg_cap = need;
+        }
+    }
     return TB_OK;
 }
 
-int stage_chunk(tb_plan* p, const tb_template* tmpl, uint64_t off, uint64_t nt, bool last)
+// constants of the templates staged at positions [off, off + nt), uploaded on the plan's stream
+int stage_chunk(tb_plan* p, const tb_template* tmpl, uint64_t off, uint64_t nt, uint32_t first_id)
 {
-    for (uint64_t i = off; i < off + nt; ++i) make_tmpl(tmpl[i], p->tsamp, &p->h_tmpl[i]);
-    TB_CUDA(p, cudaMemcpyAsync(p->d_tmpl + off, p->h_tmpl + off, nt * sizeof(TmplDev), cudaMemcpyHostToDevice, p->stream));
-    if (last) {
-        TB_CUDA(p, cudaEventRecord(p->ev_staged, p->stream));
-        p->staged_pending = true;
+    int lmin = 7;
+    for (uint64_t i = off; i < off + nt; ++i) {
+        make_tmpl(tmpl[p->order[i]], p->tsamp, &p->h_tmpl[i]);
+        p->h_tmpl[i].id = first_id + p->order[i];
+        p->h_tmpl[i].pad = 0;
+        lmin = std::min(lmin, p->h_tmpl[i].log2h);
     }
+    p->chunk_log2h = lmin;
+    TB_CUDA(p, cudaMemcpyAsync(p->d_tmpl + off, p->h_tmpl + off, nt * sizeof(TmplDev), cudaMemcpyHostToDevice, p->stream));
+    // recorded after EVERY chunk: whatever way the call ends, the next one waits for the last copy
+    // out of the pinned staging buffer before it rewrites it
+    TB_CUDA(p, cudaEventRecord(p->ev_staged, p->stream));
+    p->staged_pending = true;
     return TB_OK;
 }
 
@@ -615,7 +668,7 @@ int make_fold_params(tb_plan* p, const uint32_t* folds, uint32_t n_folds, double
         const double root = mu + sigma * s;
         fp->thr[L] = seen[L] ? (root <= 0 ? 0.f : (float)(root * root)) : std::numeric_limits<float>::infinity();
     }
-    fp->k_lo = p->k_lo;
+    for (uint32_t L = 0; L < 5; ++L) fp->lo[L] = (uint32_t)std::min<uint64_t>((uint64_t)p->k_lo << L, p->nb);
     return TB_OK;
 }
 
@@ -624,12 +677,8 @@ void destroy(tb_plan* p)
     if (!p) return;
     cudaSetDevice(p->device);
     if (p->stream) cudaStreamSynchronize(p->stream);
-    if (p->l2_pinned) {
-        cudaStreamAttrValue attr;
-        std::memset(&attr, 0, sizeof(attr));
-        cudaStreamSetAttribute(p->stream, cudaStreamAttributeAccessPolicyWindow, &attr);
-        cudaCtxResetPersistingL2Cache();
-    }
+    if (p->l2_pinned && !p->own_stream)              // give a caller-owned stream its previous window back
+        cudaStreamSetAttribute(p->stream, cudaStreamAttributeAccessPolicyWindow, &p->l2_prev);
     for (auto& kv : p->fft_plans) cufftDestroy(kv.second);
     for (auto& es : p->events) for (auto& e : es.e) cudaEventDestroy(e);
     if (p->ev_staged) cudaEventDestroy(p->ev_staged);
@@ -646,7 +695,7 @@ int single_template_stage(tb_plan* p, const tb_template* tmpl)
     if (!p || !tmpl) return fail(p, TB_ERR_INVALID_ARG, "null argument");
     TB_CUDA(p, cudaSetDevice(p->device));
     const int rc = upload_templates(p, tmpl, 1);
-    return rc ? rc : stage_chunk(p, tmpl, 0, 1, true);
+    return rc ? rc : stage_chunk(p, tmpl, 0, 1, 0);
 }
 
 }  // namespace
@@ -756,18 +805,7 @@ int tb_plan_create(tb_plan** out, const float* series, uint64_t n_samples, doubl
     }
     if (p->own_fft) {
         cudaDeviceGetAttribute(&p->n_sm, cudaDevAttrMultiProcessorCount, p->device);
-        const char* pf = getenv("TB_PF_ROWS");           // tuning knob: prefetch distance in CTAs (default: two per SM)
-        p->pf_rows = pf ? atoi(pf) : p->n_sm * 2;
-        const char* pfc = getenv("TB_PF_COLS");
-        p->pf_cols = pfc ? atoi(pfc) : 128;
-        const char* pfm = getenv("TB_PF_MID");
-        p->pf_mid = pfm ? atoi(pfm) : 1500;
-        const char* pfq = getenv("TB_PF_SCAT");
-        p->pf_scat = pfq ? atoi(pfq) : 1500;
-        const char* pfs = getenv("TB_PF_SPEC");
-        p->pf_spec = pfs ? atoi(pfs) : 32;
-        p->seg_stride = (size_t)(p->n >> OWN_MIN_LOG2H);
-        TB_TRY(cudaMalloc(&p->d_seg, (size_t)B * p->seg_stride * sizeof(SegRec)));
+        p->pf_rows = p->n_sm * 2;
         int rc = make_twiddles(p);
         if (rc) { destroy(p); return rc; }
     }
@@ -842,41 +880,46 @@ int tb_search_templates(tb_plan* p, const tb_template* tmpl, uint64_t n_template
     rc = upload_templates(p, tmpl, n_templates);
     if (rc) return rc;
 
-    const bool own = p->own_fft && p->min_log2h >= OWN_MIN_LOG2H;
-    p->last.fft_path_used = own ? 2 : 1;
-    for (uint64_t off = 0; off < n_templates; off += p->chunk) {
-        const uint32_t nt = (uint32_t)std::min<uint64_t>(p->chunk, n_templates - off);
-        if ((rc = stage_chunk(p, tmpl, off, nt, off + nt == n_templates))) return rc;
-        EventSet* es = nullptr;
-        if (p->timings) {
-            if (p->events_used == p->events.size()) {
-                EventSet ne;
-                for (auto& e : ne.e) TB_CUDA(p, cudaEventCreate(&e));
-                p->events.push_back(ne);
+    // two runs of chunks: the templates the fused path takes (positions [0, n_own) of the staging
+    // order), then the rest through k_resample + cuFFT; fft_path_used is the OR of the two
+    p->last.fft_path_used = (p->n_own ? 2u : 0u) | (p->n_own < n_templates ? 1u : 0u);
+    for (int part = 0; part < 2; ++part) {
+        const bool own = part == 0;
+        const uint64_t lo = own ? 0 : p->n_own, hi = own ? p->n_own : n_templates;
+        for (uint64_t off = lo; off < hi; off += p->chunk) {
+            const uint32_t nt = (uint32_t)std::min<uint64_t>(p->chunk, hi - off);
+            if ((rc = stage_chunk(p, tmpl, off, nt, first_template_id))) return rc;
+            EventSet* es = nullptr;
+            if (p->timings) {
+                if (p->events_used == p->events.size()) {
+                    EventSet ne;
+                    for (auto& e : ne.e) TB_CUDA(p, cudaEventCreate(&e));
+                    p->events.push_back(ne);
+                }
+                es = &p->events[p->events_used++];
+                TB_CUDA(p, cudaEventRecord(es->e[0], p->stream));
             }
-            es = &p->events[p->events_used++];
-            TB_CUDA(p, cudaEventRecord(es->e[0], p->stream));
+            if (own) {                                   // K0 | P1 | P2 | transpose + unpack + spectrum + median + normalise
+                if ((rc = run_own_pass1(p, off, nt, nullptr, nullptr, es ? es->e[1] : nullptr))) return rc;
+                if (es) TB_CUDA(p, cudaEventRecord(es->e[2], p->stream));
+                if ((rc = run_own_pass2(p, nt))) return rc;
+                if (es) TB_CUDA(p, cudaEventRecord(es->e[3], p->stream));
+                if ((rc = run_spectrum_t(p, nt))) return rc;
+                p->last.n_kernel_launches += (p->log2m2 == 16) ? 3 : 2;
+            } else {
+                if (es) TB_CUDA(p, cudaEventRecord(es->e[1], p->stream));
+                if ((rc = run_resample(p, off, nt, nullptr))) return rc;
+                if (es) TB_CUDA(p, cudaEventRecord(es->e[2], p->stream));
+                if ((rc = run_fft(p, nt))) return rc;
+                if (es) TB_CUDA(p, cudaEventRecord(es->e[3], p->stream));
+                if ((rc = run_spectrum(p, nt))) return rc;
+            }
+            if (es) TB_CUDA(p, cudaEventRecord(es->e[4], p->stream));
+            if ((rc = run_hsum(p, off, nt, fp))) return rc;
+            if (es) TB_CUDA(p, cudaEventRecord(es->e[5], p->stream));
+            p->last.n_chunks++;
+            p->last.n_kernel_launches += 3;
         }
-        if (own) {                                       // K0 | P1 | P2 | transpose + unpack + spectrum + median + normalise
-            if ((rc = run_own_pass1(p, off, nt, nullptr, nullptr, es ? es->e[1] : nullptr))) return rc;
-            if (es) TB_CUDA(p, cudaEventRecord(es->e[2], p->stream));
-            if ((rc = run_own_pass2(p, nt))) return rc;
-            if (es) TB_CUDA(p, cudaEventRecord(es->e[3], p->stream));
-            if ((rc = run_spectrum_t(p, nt))) return rc;
-            p->last.n_kernel_launches += (p->log2m2 == 16) ? 3 : 2;
-        } else {
-            if (es) TB_CUDA(p, cudaEventRecord(es->e[1], p->stream));
-            if ((rc = run_resample(p, off, nt, nullptr))) return rc;
-            if (es) TB_CUDA(p, cudaEventRecord(es->e[2], p->stream));
-            if ((rc = run_fft(p, nt))) return rc;
-            if (es) TB_CUDA(p, cudaEventRecord(es->e[3], p->stream));
-            if ((rc = run_spectrum(p, nt))) return rc;
-        }
-        if (es) TB_CUDA(p, cudaEventRecord(es->e[4], p->stream));
-        if ((rc = run_hsum(p, nt, fp, first_template_id + (uint32_t)off))) return rc;
-        if (es) TB_CUDA(p, cudaEventRecord(es->e[5], p->stream));
-        p->last.n_chunks++;
-        p->last.n_kernel_launches += 3;
     }
     return TB_OK;
 }
@@ -946,7 +989,7 @@ int tb_debug_resample_indices(tb_plan* p, const tb_template* tmpl, int64_t* idx_
     if (rc) return rc;
     long long* d_idx = nullptr;
     TB_CUDA(p, cudaMalloc(&d_idx, p->n * sizeof(long long)));
-    if (p->own_fft && p->min_log2h >= OWN_MIN_LOG2H) {
+    if (p->n_own) {
         float* d_y = nullptr;
         cudaError_t e = cudaMalloc(&d_y, p->n * sizeof(float));
         if (e != cudaSuccess) { cudaFree(d_idx); return fail(p, TB_ERR_NOMEM, "debug buffer"); }
@@ -969,7 +1012,7 @@ int tb_debug_resampled(tb_plan* p, const tb_template* tmpl, float* y_out)
     if (!y_out) return fail(p, TB_ERR_INVALID_ARG, "null argument");
     int rc = single_template_stage(p, tmpl);
     if (rc) return rc;
-    if (p->own_fft && p->min_log2h >= OWN_MIN_LOG2H) {
+    if (p->n_own) {
         long long* d_idx = nullptr;
         float* d_y = nullptr;
         TB_CUDA(p, cudaMalloc(&d_idx, p->n * sizeof(long long)));
@@ -995,7 +1038,7 @@ int tb_debug_spectrum(tb_plan* p, const tb_template* tmpl, float* p_interbinned,
 {
     int rc = single_template_stage(p, tmpl);
     if (rc) return rc;
-    const bool own = p->own_fft && p->min_log2h >= OWN_MIN_LOG2H;
+    const bool own = p->n_own != 0;
     if (own) {
         if ((rc = run_own_pass1(p, 0, 1, nullptr, nullptr))) return rc;
         if ((rc = run_own_pass2(p, 1))) return rc;
@@ -1014,6 +1057,35 @@ int tb_debug_spectrum(tb_plan* p, const tb_template* tmpl, float* p_interbinned,
         e = cudaMemcpyAsync(p_normalised, p->d_power, p->nb * sizeof(float), cudaMemcpyDeviceToHost, p->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(p->stream);
     cudaFree(d_raw);
+    if (rc) return rc;
+    if (e != cudaSuccess) return fail(p, TB_ERR_CUDA, cudaGetErrorString(e));
+    return TB_OK;
+}
+
+int tb_debug_hsums(tb_plan* p, const tb_template* tmpl, float* sums_out)
+{
+    if (!sums_out) return fail(p, TB_ERR_INVALID_ARG, "null argument");
+    int rc = single_template_stage(p, tmpl);
+    if (rc) return rc;
+    if (p->n_own) {
+        if ((rc = run_own_pass1(p, 0, 1, nullptr, nullptr))) return rc;
+        if ((rc = run_own_pass2(p, 1))) return rc;
+        if ((rc = run_spectrum_t(p, 1))) return rc;
+    } else {
+        if ((rc = run_resample(p, 0, 1, nullptr))) return rc;
+        if ((rc = run_fft(p, 1))) return rc;
+        if ((rc = run_spectrum(p, 1))) return rc;
+    }
+    // the production harmonic summer with its tap on and thresholds at +inf (no candidate is emitted)
+    FoldParams fp;
+    for (int L = 0; L < 5; ++L) { fp.thr[L] = std::numeric_limits<float>::infinity(); fp.mu[L] = 0.f; fp.inv_s[L] = 0.f; fp.lo[L] = 0; }
+    float* d_tap = nullptr;
+    TB_CUDA(p, cudaMalloc(&d_tap, 5 * p->nb * sizeof(float)));
+    rc = run_hsum(p, 0, 1, fp, d_tap);
+    cudaError_t e = cudaSuccess;
+    if (!rc) e = cudaMemcpyAsync(sums_out, d_tap, 5 * p->nb * sizeof(float), cudaMemcpyDeviceToHost, p->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(p->stream);
+    cudaFree(d_tap);
     if (rc) return rc;
     if (e != cudaSuccess) return fail(p, TB_ERR_CUDA, cudaGetErrorString(e));
     return TB_OK;

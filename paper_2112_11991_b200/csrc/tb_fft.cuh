@@ -31,22 +31,10 @@
 
 namespace tb {
 
-#ifndef TB_COLS_MINB
-#define TB_COLS_MINB 3
-#endif
-#ifndef TB_ROWS_TW_TREE
-#define TB_ROWS_TW_TREE 1               // 8192-point rows: first-step twiddles from a product tree instead of 31 table loads
-#endif
-#ifndef TB_ROWS_MINB
-#define TB_ROWS_MINB 2                  // CTAs per SM the pass-2 register budget is set for (2 measured faster than 3)
-#endif
-#ifndef TB_A0_UNROLL
-#define TB_A0_UNROLL 4                 // rows per batch of independent segment-record loads (x R1 points)
-#endif
-#ifndef TB_A1_UNROLL
-#define TB_A1_UNROLL 4                 // rows per batch of independent gather loads
-#endif
-constexpr int A0_UNROLL = TB_A0_UNROLL, A1_UNROLL = TB_A1_UNROLL;
+constexpr int COLS_MINB = 3;            // CTAs per SM the pass-1 register budget is set for
+constexpr int ROWS_MINB = 2;            // CTAs per SM the pass-2 register budget is set for (2 measured faster than 3)
+constexpr int A0_UNROLL = 4;            // rows per batch of independent segment-record loads (x R1 points)
+constexpr int A1_UNROLL = 4;            // rows per batch of independent gather loads
 constexpr int FFT_PB = 17;            // pitch of the b axis (16 + 1)
 constexpr int FFT_PA = 16 * FFT_PB;   // pitch of the a axis
 constexpr int FFT_THREADS = 256;
@@ -62,10 +50,6 @@ static_assert(sizeof(SegRec) == 64, "segment record");
 
 // Complex arithmetic on the packed fp32x2 pipe of sm_100 (FADD2 / FFMA2: one issue slot per complex
 // add, three per complex multiply instead of two and four); the kernels are issue-bound, not FMA-bound.
-#ifndef TB_F32X2
-#define TB_F32X2 1
-#endif
-#if TB_F32X2
 __device__ __forceinline__ float2 cadd(float2 a, float2 b)
 {
     float2 r;
@@ -88,11 +72,6 @@ __device__ __forceinline__ float2 cmul(float2 a, float2 w)      // (a.x, a.x) * 
         : "=f"(r.x), "=f"(r.y) : "f"(a.x), "f"(w.x), "f"(w.y), "f"(cx), "f"(cy));
     return r;
 }
-#else
-__device__ __forceinline__ float2 cmul(float2 a, float2 w) { return make_float2(a.x * w.x - a.y * w.y, a.x * w.y + a.y * w.x); }
-__device__ __forceinline__ float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
-__device__ __forceinline__ float2 csub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
-#endif
 __device__ __forceinline__ float2 mul_mi(float2 a) { return make_float2(a.y, -a.x); }   // a * (-i)
 
 // forward 4-point DFT of (x0,x1,x2,x3), natural order in and out
@@ -360,7 +339,7 @@ __device__ __forceinline__ void cols_park_indices(const SegRec* __restrict__ seg
 //   "template" b is one row of T seen as an [L][2^log2m2] matrix, transformed in place over its
 //   first index with the twiddle W_m^{j2 k1}, m = L 2^log2m2 (blockIdx.x = b * bundles + bundle).
 template <int R1, int C, bool DEBUG, bool DIRECT = false>
-__global__ void __launch_bounds__(FFT_THREADS, TB_COLS_MINB)
+__global__ void __launch_bounds__(FFT_THREADS, COLS_MINB)
 k_fft_cols(const float* __restrict__ x, const SegRec* __restrict__ seg, size_t seg_stride,
            const TmplDev* __restrict__ tmpl, int n_tmpl, int n, int log2m2, float fill,
            const float2* __restrict__ tw1, const float2* __restrict__ tw2g, float2* __restrict__ T,
@@ -494,7 +473,7 @@ constexpr int C32_PK = 16, C32_LP = 32 * C32_PK + 1;
 constexpr size_t C32_SMEM = (size_t)16 * C32_LP * sizeof(float2);
 
 template <bool DEBUG>
-__global__ void __launch_bounds__(FFT_THREADS, TB_COLS_MINB)
+__global__ void __launch_bounds__(FFT_THREADS, COLS_MINB)
 k_fft_cols32(const float* __restrict__ x, const SegRec* __restrict__ seg, size_t seg_stride,
              const TmplDev* __restrict__ tmpl, int n_tmpl, int n, int log2m2, float fill,
              const float2* __restrict__ twc, float2* __restrict__ T,
@@ -544,7 +523,6 @@ k_fft_cols32(const float* __restrict__ x, const SegRec* __restrict__ seg, size_t
         }
         fft_reg<32>(v);
         myslot[0] = v[0];
-#if TB_ROWS_TW_TREE
         {   // W_512^{c ka} = q[ka >> 3] * t[ka & 7] from two table values (see fft_rows_body)
             float2 t[8], q[4];
             t[1] = __ldg(twc + 16 + c);
@@ -561,10 +539,6 @@ k_fft_cols32(const float* __restrict__ x, const SegRec* __restrict__ seg, size_t
                 for (int l = 1; l < 8; ++l) myslot[(8 * h + l) * PK] = cmul(v[8 * h + l], cmul(q[h], t[l]));
             }
         }
-#else
-#pragma unroll
-        for (int ka = 1; ka < 32; ++ka) myslot[ka * PK] = cmul(v[ka], __ldg(twc + ka * 16 + c));
-#endif
     }
     __syncthreads();
     for (int i = threadIdx.x; i < 16 * 32; i += FFT_THREADS) {                 // item (col, ka), col fastest
@@ -610,7 +584,7 @@ template <int R1> struct RowsCfg {
     static constexpr int PA = 16 * PB + 1;
     static constexpr int R = (R1 >= 8) ? 1 : 8 / R1;       // rows per CTA
     static constexpr int LP = R1 * PA;
-    static constexpr int MINB = TB_ROWS_MINB;        // CTAs per SM the register budget is set for
+    static constexpr int MINB = ROWS_MINB;        // CTAs per SM the register budget is set for
     static constexpr size_t SMEM = (size_t)(R * LP + 256) * sizeof(float2);
 };
 
@@ -654,7 +628,6 @@ k_fft_rows_t(const float2* __restrict__ T, float2* __restrict__ Zt, int log2m1, 
             fft_reg<R1>(v[r]);
             float2* p = fsm + r * LP + (w >> 4) * PB + (w & 15);
             p[0] = v[r][0];
-#if TB_ROWS_TW_TREE
             if constexpr (R1 == 32) {
                 // W_L^{w ka} = q[ka >> 3] * t[ka & 7] from two table values (ka = 1 and 8): 29 complex
                 // products on the FMA pipe instead of 29 more loads on the LSU/MIO path this kernel
@@ -674,7 +647,6 @@ k_fft_rows_t(const float2* __restrict__ T, float2* __restrict__ Zt, int log2m1, 
                     for (int l = 1; l < 8; ++l) p[(8 * h + l) * PA] = cmul(v[r][8 * h + l], cmul(q[h], t[l]));
                 }
             } else
-#endif
 #pragma unroll
             for (int ka = 1; ka < R1; ++ka) p[ka * PA] = cmul(v[r][ka], __ldg(tw1 + ka * 256 + w));
         }

@@ -22,13 +22,15 @@ struct TmplDev {
     double d0;           // zero offset in samples: A cos E0 + B sin E0 at M = phi0      (L675, L682-692)
     int32_t log2h;       // Hermite knot spacing h = 2^log2h samples (0: every sample is a knot)
     int32_t circular;    // 1: e == 0, E = M (no Kepler solve)
+    uint32_t id;         // template id reported in the candidates (first_template_id + index in the caller's array)
+    uint32_t pad;
 };
 
 struct FoldParams {
     float    thr[5];     // power threshold T_L per fold, +inf for folds not requested
     float    mu[5];      // mu_n, n = 2^L
     float    inv_s[5];   // 1/s_n
-    uint32_t k_lo;       // lowest fundamental bin (G20); fold L starts at k_lo << L
+    uint32_t lo[5];      // lowest bin of fold L: min(k_lo 2^L, Nb), made on the host in 64 bits (G20)
 };
 
 struct Candidate {       // == tb_candidate
@@ -501,12 +503,8 @@ k_spectrum_median(const float2* __restrict__ X, size_t ld, float* __restrict__ P
 //   centres exactly like k_spectrum_median and writes 8 W bins with coalesced stores.
 //   Powers are carried as 4 P_k (the 1/2 of the unpack is skipped); the factor cancels in P^.
 // ---------------------------------------------------------------------------------------------
-#ifndef TB_ST_MINB
-#define TB_ST_MINB 3
-#endif
-#ifndef TB_ST_UN
-#define TB_ST_UN 8                     // row steps per load group of the spectrum former
-#endif
+constexpr int ST_MINB = 3;             // CTAs per SM the spectrum former's register budget is set for (W <= 1024)
+constexpr int ST_UN = 8;               // row steps per load group of the spectrum former
 constexpr int ST_WARPS = 9;
 constexpr int ST_THREADS = ST_WARPS * 32;
 
@@ -550,7 +548,7 @@ __device__ __forceinline__ float st_interbin(float2 x, float2 prev)
 }
 
 template <int W, int LOG2M1, bool RAW>
-__global__ void __launch_bounds__(ST_THREADS, (W <= 1024) ? TB_ST_MINB : 1)
+__global__ void __launch_bounds__(ST_THREADS, (W <= 1024) ? ST_MINB : 1)
 k_spectrum_t(const float2* __restrict__ Zt, float* __restrict__ P, float* __restrict__ med, int log2m2,
              int nblk, const float2* __restrict__ twa, const float2* __restrict__ twb, float2 rot,
              unsigned long long* __restrict__ fallbacks, float* __restrict__ Praw, int pf_dist)
@@ -610,7 +608,7 @@ k_spectrum_t(const float2* __restrict__ Zt, float* __restrict__ P, float* __rest
         const float2* zkp = Zr + (size_t)k1s * m2 + k2;                                   // walks down the rows
         const float2* zmp = Zr + (size_t)(M1 - k1s) * m2 + (m2 - 1 - k2);                 // walks up; row M1 is never read (k1s = 0 below)
         const float2* __restrict__ wap = twa + k1s;
-        constexpr int UN = (LC % TB_ST_UN == 0) ? TB_ST_UN : 4;
+        constexpr int UN = (LC % ST_UN == 0) ? ST_UN : 4;
 #pragma unroll 1
         for (int i0 = 0; i0 < LC; i0 += UN) {
             float2 zk[UN], zm[UN];
@@ -728,10 +726,12 @@ k_spectrum_t(const float2* __restrict__ Zt, float* __restrict__ P, float* __rest
 //   ballots its hits and takes one atomic per warp on the device cursor (L660 "peak detection",
 //   G19).  The cursor keeps counting past the capacity so that overflow is reported, not hidden.
 // ---------------------------------------------------------------------------------------------
+//   TAP = true (parity tap tb_debug_hsums): every S_L[k] is also written to tap[L * nb + k].
+template <bool TAP>
 __global__ void __launch_bounds__(256)
-k_hsum_threshold(const float* __restrict__ Ph, int nb, int cta_per_row, FoldParams fp, uint32_t first_id,
+k_hsum_threshold(const float* __restrict__ Ph, int nb, int cta_per_row, FoldParams fp, const TmplDev* __restrict__ tmpl,
                  Candidate* __restrict__ out, unsigned long long* __restrict__ cursor,
-                 unsigned long long capacity)
+                 unsigned long long capacity, float* __restrict__ tap)
 {
     const int row = blockIdx.x / cta_per_row;
     const int k   = (blockIdx.x % cta_per_row) * 256 + threadIdx.x;
@@ -752,16 +752,20 @@ k_hsum_threshold(const float* __restrict__ Ph, int nb, int cta_per_row, FoldPara
 #pragma unroll
         for (uint32_t m = 1; m < 16; m += 2) s += __ldg(p + ((m * uk + 8u) >> 4));
         S[4] = s;
+        if (TAP) {
+#pragma unroll
+            for (int L = 0; L < 5; ++L) tap[(size_t)L * nb + k] = S[L];
+        }
     }
     bool any = false;
     if (live) {
 #pragma unroll
-        for (int L = 0; L < 5; ++L) any |= (S[L] >= fp.thr[L]) && ((uint32_t)k >= (fp.k_lo << L));
+        for (int L = 0; L < 5; ++L) any |= (S[L] >= fp.thr[L]) && ((uint32_t)k >= fp.lo[L]);
     }
     if (__ballot_sync(0xffffffffu, any) == 0u) return;
 #pragma unroll
     for (int L = 0; L < 5; ++L) {
-        const bool hit = live && (S[L] >= fp.thr[L]) && ((uint32_t)k >= (fp.k_lo << L));
+        const bool hit = live && (S[L] >= fp.thr[L]) && ((uint32_t)k >= fp.lo[L]);
         const unsigned mask = __ballot_sync(0xffffffffu, hit);
         if (mask == 0u) continue;
         unsigned long long basepos = 0;
@@ -771,7 +775,7 @@ k_hsum_threshold(const float* __restrict__ Ph, int nb, int cta_per_row, FoldPara
             const unsigned long long pos = basepos + (unsigned long long)__popc(mask & ((1u << lane) - 1u));
             if (pos < capacity) {
                 Candidate c;
-                c.template_id = first_id + (uint32_t)row;
+                c.template_id = __ldg(&tmpl[row].id);
                 c.fold = (uint32_t)L;
                 c.bin = (uint32_t)k;
                 c.power = S[L];
@@ -881,7 +885,7 @@ __device__ __forceinline__ void hs_emit(const float (&acc)[8], uint32_t kq, cons
 #pragma unroll
     for (int r = 0; r < 8; ++r) {                    // unrolled: acc[] must stay in registers
         const uint32_t k = kq + (uint32_t)r;
-        const bool hit = (acc[r] >= fp.thr[L]) && (k >= (fp.k_lo << L));
+        const bool hit = (acc[r] >= fp.thr[L]) && (k >= fp.lo[L]);
         const unsigned mask = __ballot_sync(0xffffffffu, hit);
         if (mask == 0u) continue;
         const int leader = __ffs(mask) - 1;
@@ -938,29 +942,42 @@ __device__ __forceinline__ HsDirect hs_load_direct(const float* __restrict__ p, 
 }
 
 // sums + checks of one thread's 8 bins of the tile staged in `sm`
-template <int HALF>
+template <bool TAP>
+__device__ __forceinline__ void hs_tap(const float (&acc)[8], float* __restrict__ tap)
+{
+    if (TAP) {
+        *reinterpret_cast<float4*>(tap) = make_float4(acc[0], acc[1], acc[2], acc[3]);
+        *reinterpret_cast<float4*>(tap + 4) = make_float4(acc[4], acc[5], acc[6], acc[7]);
+    }
+}
+
+template <int HALF, bool TAP>
 __device__ __forceinline__ void hs_tile_body(const float* __restrict__ sm, int q, const HsDirect& d, uint32_t kq,
                                              uint64_t* bar, uint32_t parity, const FoldParams& fp, uint32_t tid,
                                              Candidate* __restrict__ out, unsigned long long* __restrict__ cursor,
-                                             unsigned long long capacity)
+                                             unsigned long long capacity, float* __restrict__ tap, size_t nb)
 {
     float acc[8] = {d.a0.x, d.a0.y, d.a0.z, d.a0.w, d.a1.x, d.a1.y, d.a1.z, d.a1.w};   // fold 0: the bin itself
+    hs_tap<TAP>(acc, tap + kq);
     hs_check<0>(acc, kq, fp, tid, out, cursor, capacity);
     {                                                // fold 1: + P^[(k+1)>>1], 5 values from kq/2 on
         const float v[5] = {d.h0.x, d.h0.y, d.h0.z, d.h0.w, d.h1};
 #pragma unroll
         for (int r = 0; r < 8; ++r) acc[r] += v[(r + 1) >> 1];
     }
+    hs_tap<TAP>(acc, tap + nb + kq);
     hs_check<1>(acc, kq, fp, tid, out, cursor, capacity);
 
     mbar_wait(bar, parity);
     hs_accumulate<2, 1, HALF>(sm, q, acc);
     hs_accumulate<2, 3, HALF>(sm, q, acc);
+    hs_tap<TAP>(acc, tap + 2 * nb + kq);
     hs_check<2>(acc, kq, fp, tid, out, cursor, capacity);
     hs_accumulate<3, 1, HALF>(sm, q, acc);
     hs_accumulate<3, 3, HALF>(sm, q, acc);
     hs_accumulate<3, 5, HALF>(sm, q, acc);
     hs_accumulate<3, 7, HALF>(sm, q, acc);
+    hs_tap<TAP>(acc, tap + 3 * nb + kq);
     hs_check<3>(acc, kq, fp, tid, out, cursor, capacity);
     hs_accumulate<4, 1, HALF>(sm, q, acc);
     hs_accumulate<4, 3, HALF>(sm, q, acc);
@@ -970,6 +987,7 @@ __device__ __forceinline__ void hs_tile_body(const float* __restrict__ sm, int q
     hs_accumulate<4, 11, HALF>(sm, q, acc);
     hs_accumulate<4, 13, HALF>(sm, q, acc);
     hs_accumulate<4, 15, HALF>(sm, q, acc);
+    hs_tap<TAP>(acc, tap + 4 * nb + kq);
     hs_check<4>(acc, kq, fp, tid, out, cursor, capacity);
 }
 
@@ -978,20 +996,20 @@ __device__ __forceinline__ void hs_tile_body(const float* __restrict__ sm, int q
 // values of tile t+1 are already on their way to registers, so no warp waits on memory once the
 // first tile is in.  Warps 0-3 take bins 0-7 of every group of 16, warps 4-7 bins 8-15: 16 warps
 // per SM instead of 8 on the same staged bytes (the staging, not the registers, limits residency).
-#ifndef TB_HS_BUFS
-#define TB_HS_BUFS 2                    // staging buffers per CTA (1: three CTAs per SM, overlap across CTAs only)
-#endif
-constexpr int HS_BUFS = TB_HS_BUFS;
-__global__ void __launch_bounds__(HS_THREADS, HS_BUFS == 1 ? 3 : 2)
-k_hsum_tile(const float* __restrict__ Ph, int nb, int groups_per_row, int tpc, FoldParams fp, uint32_t first_id,
-            Candidate* __restrict__ out, unsigned long long* __restrict__ cursor, unsigned long long capacity)
+//   TAP = true (parity tap tb_debug_hsums): every S_L[k] is also written to tap[L * nb + k].
+constexpr int HS_BUFS = 2;
+template <bool TAP>
+__global__ void __launch_bounds__(HS_THREADS, 2)
+k_hsum_tile(const float* __restrict__ Ph, int nb, int groups_per_row, int tpc, FoldParams fp, const TmplDev* __restrict__ tmpl,
+            Candidate* __restrict__ out, unsigned long long* __restrict__ cursor, unsigned long long capacity,
+            float* __restrict__ tap)
 {
     extern __shared__ __align__(16) float hs_sm[];   // two buffers of HS_SMEM_FLOATS
     __shared__ __align__(8) uint64_t bar[2];
     const int row   = blockIdx.x / groups_per_row;
     const int tile0 = (blockIdx.x % groups_per_row) * tpc;
     const float* __restrict__ p = Ph + (size_t)row * (size_t)nb;
-    const uint32_t tid = first_id + (uint32_t)row;
+    const uint32_t tid = __ldg(&tmpl[row].id);
     const int q = threadIdx.x & (HS_T / 16 - 1), half = threadIdx.x / (HS_T / 16);
 
     if (threadIdx.x == 0) { mbar_init(&bar[0], 1); mbar_init(&bar[1], 1); }
@@ -1002,16 +1020,15 @@ k_hsum_tile(const float* __restrict__ Ph, int nb, int groups_per_row, int tpc, F
     for (int t = 0; t < tpc; ++t) {
         const int k0 = (tile0 + t) * HS_T;
         const uint32_t kq = (uint32_t)(k0 + 16 * q + 8 * half);
-        const float* sm = hs_sm + (t % HS_BUFS) * HS_SMEM_FLOATS;
-        if (HS_BUFS == 2 && t + 1 < tpc && threadIdx.x == 0)   // the other buffer was released by the barrier that ended tile t-1
+        const float* sm = hs_sm + (t & 1) * HS_SMEM_FLOATS;
+        if (t + 1 < tpc && threadIdx.x == 0)         // the other buffer was released by the barrier that ended tile t-1
             hs_stage(hs_sm + ((t + 1) & 1) * HS_SMEM_FLOATS, p, k0 + HS_T, &bar[(t + 1) & 1]);
         const HsDirect d = nxt;
         if (t + 1 < tpc) nxt = hs_load_direct(p, kq + HS_T);
-        const uint32_t parity = (uint32_t)((t / HS_BUFS) & 1);
-        if (half) hs_tile_body<1>(sm, q, d, kq, &bar[t % HS_BUFS], parity, fp, tid, out, cursor, capacity);
-        else      hs_tile_body<0>(sm, q, d, kq, &bar[t % HS_BUFS], parity, fp, tid, out, cursor, capacity);
+        const uint32_t parity = (uint32_t)((t >> 1) & 1);
+        if (half) hs_tile_body<1, TAP>(sm, q, d, kq, &bar[t & 1], parity, fp, tid, out, cursor, capacity, tap, (size_t)nb);
+        else      hs_tile_body<0, TAP>(sm, q, d, kq, &bar[t & 1], parity, fp, tid, out, cursor, capacity, tap, (size_t)nb);
         __syncthreads();                             // every thread is done with buffer t&1: it may be refilled
-        if (HS_BUFS == 1 && t + 1 < tpc && threadIdx.x == 0) hs_stage(hs_sm, p, k0 + HS_T, &bar[0]);
     }
 }
 

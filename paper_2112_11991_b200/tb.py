@@ -49,7 +49,7 @@ class Timings(C.Structure):
 
 EXPORTS = ["tb_plan_create", "tb_plan_set_series", "tb_search_templates", "tb_get_candidates", "tb_clear_candidates", "tb_plan_destroy",
            "tb_strerror", "tb_last_error", "tb_get_timings", "tb_debug_resample_indices", "tb_debug_spectrum",
-           "tb_debug_resampled", "tb_sigma_to_power", "tb_plan_info", "tb_template_knot_log2"]
+           "tb_debug_resampled", "tb_debug_hsums", "tb_sigma_to_power", "tb_plan_info", "tb_template_knot_log2"]
 
 _vp, _u64, _u32 = C.c_void_p, C.c_uint64, C.c_uint32
 lib.tb_plan_create.argtypes = [C.POINTER(_vp), _vp, _u64, C.c_double, C.POINTER(PlanOpts)]
@@ -66,6 +66,7 @@ lib.tb_get_timings.argtypes = [_vp, C.POINTER(Timings)]
 lib.tb_debug_resample_indices.argtypes = [_vp, _vp, _vp]
 lib.tb_debug_spectrum.argtypes = [_vp, _vp, _vp, _vp, _vp]
 lib.tb_debug_resampled.argtypes = [_vp, _vp, _vp]
+lib.tb_debug_hsums.argtypes = [_vp, _vp, _vp]
 lib.tb_sigma_to_power.argtypes = [_u32, C.c_double, C.POINTER(C.c_double)]
 lib.tb_plan_info.argtypes = [_vp, C.POINTER(C.c_float), C.POINTER(_u32), C.POINTER(_u32)]
 lib.tb_template_knot_log2.argtypes = [_vp, _vp, C.POINTER(C.c_int32)]
@@ -197,6 +198,14 @@ def tb_debug_resampled(plan, template, n_samples) -> np.ndarray:
     return out
 
 
+def tb_debug_hsums(plan, template, n_samples) -> np.ndarray:
+    """float32[5, N/2]: S_L[k] of every fold and bin through the production harmonic summer."""
+    t = as_templates(template)
+    out = np.empty((5, int(n_samples) // 2), dtype=np.float32)
+    _check(lib.tb_debug_hsums(plan, t.ctypes.data, out.ctypes.data), plan)
+    return out
+
+
 def tb_debug_spectrum(plan, template, n_samples, median_window=1024):
     t = as_templates(template)
     nb = int(n_samples) // 2
@@ -250,6 +259,9 @@ class Plan:
 
     def debug_resampled(self, template):
         return tb_debug_resampled(self.handle, template, self.n_samples)
+
+    def debug_hsums(self, template):
+        return tb_debug_hsums(self.handle, template, self.n_samples)
 
     def debug_spectrum(self, template):
         return tb_debug_spectrum(self.handle, template, self.n_samples, self.median_window)

@@ -16,3 +16,15 @@ def pytest_configure(config):
 def c1():
     from paper_2112_11991_b200 import workloads
     return workloads.config1()
+
+
+def pytest_terminal_summary(terminalreporter):
+    """What the full-size parity tests actually compared (SURVEY 8(d) protocol), also under -q."""
+    try:
+        from parity import SUMMARY
+    except ImportError:
+        return
+    if SUMMARY:
+        terminalreporter.section("parity sample")
+        for line in SUMMARY:
+            terminalreporter.write_line(line)
