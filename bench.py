@@ -69,10 +69,33 @@ def oracle_rate(wl, n_templates, cores, pool):
 
 
 def host_cores():
+    """Every core this process may run on (one oracle process per core)."""
     try:
-        return max(1, min(len(os.sched_getaffinity(0)), 16))
+        return max(1, len(os.sched_getaffinity(0)))
     except AttributeError:
-        return max(1, min(os.cpu_count() or 1, 16))
+        return max(1, os.cpu_count() or 1)
+
+
+def cpu_model():
+    try:
+        with open("/proc/cpuinfo") as f:
+            for line in f:
+                if line.lower().startswith("model name"):
+                    return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
+def source_digest():
+    """sha256 (first 16 hex digits) over the CUDA sources: ties profiles/traffic.json to a build."""
+    import hashlib
+    h = hashlib.sha256()
+    d = os.path.join(ROOT, "paper_2112_11991_b200", "csrc")
+    for name in sorted(os.listdir(d)):
+        with open(os.path.join(d, name), "rb") as f:
+            h.update(name.encode() + b"\0" + f.read())
+    return h.hexdigest()[:16]
 
 
 def run_reference(args, wl):
@@ -96,7 +119,7 @@ def run_reference(args, wl):
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": workload_config(wl, None),
-        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "cpu_model": cpu_model(), "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
     }))
 
@@ -233,7 +256,7 @@ def run_ours(args, wl):
     barrier()
     e2e_s = max_over_ranks(time.perf_counter() - t0)
     e2e = {"value": world * K * args.steps / e2e_s, "unit": UNIT,
-           "h2d_bytes_per_step": 4 * N + 88 * K, "d2h_bytes_per_step": 8 + 24 * int(n)}
+           "h2d_bytes_per_step": 4 * N + 80 * K, "d2h_bytes_per_step": 8 + 24 * int(n)}
 
     # ---- circular / elliptical split (outside the timed region) ----
     detail = {}
@@ -270,13 +293,21 @@ def run_ours(args, wl):
                                   "share_of_step": per_t[k] / per_t["ms_total"] if per_t["ms_total"] else 0.0}
     dom = max(stage_keys[:-1], key=lambda k: per_t[k])
     dom_gbs = model[dom] / per_t[dom] / 1e9 * 1.0
-    traffic = None
-    tpath = os.path.join(ROOT, "profiles", "traffic.json")   # dram bytes per launch, copied from the ncu --set full capture
+    # DRAM bytes per launch of the dominant kernel from the last ncu --set full capture
+    # (profiles/traffic.json).  A profiler cannot run inside the timed program, so the figure is
+    # only reported when the capture was taken on THIS build of the CUDA sources; otherwise null.
+    traffic, traffic_note = None, "no capture for this build"
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(tpath):
         with open(tpath) as f:
-            traffic = json.load(f).get(names[dom].split(" (")[0])
+            tj = json.load(f)
+        if tj.get("_csrc_sha256_16") == source_digest():
+            traffic = tj.get(names[dom].split(" (")[0])
+            traffic_note = tj.get("_source", "")
+        else:
+            traffic_note = f"profiles/traffic.json was captured on another build ({tj.get('_csrc_sha256_16')})"
     roofline = {"bound": "hbm", "kernel": names[dom], "achieved": dom_gbs, "peak": peak, "unit": "GB/s",
-                "frac": dom_gbs / peak, "traffic": traffic, "peak_source": peak_src,
+                "frac": dom_gbs / peak, "traffic": traffic, "traffic_source": traffic_note, "peak_source": peak_src,
                 "launches_timed": int(args.steps * -(-K // chunk)),
                 "pipeline": {"model_bytes_per_template": 22 * N,
                              "achieved": 22 * N * (K * args.steps) / (stages["ms_total"] * 1e-3) / 1e9,
@@ -295,7 +326,7 @@ def run_ours(args, wl):
         cores = host_cores()
         with mp.get_context("fork").Pool(cores) as pool:
             v = oracle_rate(wl, cores, cores, pool)
-        out["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
+        out["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "cpu_model": cpu_model(), "kind": "oracle",
                                "sample": f"{cores} templates ({cores - cores // 2} circular + {cores // 2} elliptical) "
                                          f"of the 512, one per core, full N=2^{int(np.log2(N))}"}
     if rank == 0:

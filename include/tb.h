@@ -175,6 +175,40 @@ TB_API int tb_get_candidates(tb_plan* plan, tb_candidate* out, uint64_t capacity
 TB_API int tb_clear_candidates(tb_plan* plan);
 TB_API int tb_plan_destroy(tb_plan* plan);      /* NULL is allowed */
 
+/* ---- candidate reduction ("a candidate reduction algorithm by grouping together
+ * multiple detections of the same candidate"; the paper gives no algorithm: reading G24) ----
+ * One group = one signal.  R1: within a (template, fold) a run of detections in adjacent bins is one
+ * peak (its detection of highest sigma; ties: lowest bin).  R2: peaks are ranked by sigma
+ * (descending; ties: template, fold, bin).  R3: in rank order, a peak that has not been absorbed
+ * heads a new group and absorbs every weaker unabsorbed peak, of any template and fold, whose
+ * fundamental frequency f = bin / 2^fold (in bins of 1/T_obs) is harmonically related to its own:
+ * |q f_b - p f_head| <= freq_tol_bins for some integers 1 <= p, q <= 16 (frequencies are held as
+ * exact multiples of 1/16 bin).  Groups are numbered in head order. */
+typedef struct {
+    uint32_t template_id, fold, bin;   /* the group's head: its most significant detection */
+    float    power, sigma;
+    uint32_t n_peaks;                  /* peaks in the group (head included) */
+    uint32_t n_detections;             /* raw detections in those peaks */
+    uint32_t n_templates;              /* distinct templates among them */
+} tb_group;                            /* 32 bytes */
+
+/* Reduce the candidates accumulated in the plan (device side: sort, run scan, distillation) WITHOUT
+ * consuming them: tb_get_candidates afterwards returns the same sorted list.
+ *   freq_tol_bins    tolerance of R3 in fundamental bins; 0 -> 1.0; rounded to 1/16 bin
+ *   groups_out       host, `capacity` entries; *n_groups receives the number of groups
+ *   member_of        host, optional (NULL): group index of every detection, in the order
+ *                    tb_get_candidates returns them (sorted by template, fold, bin);
+ *                    member_capacity entries, must hold them all
+ * TB_ERR_CAPACITY if groups_out is NULL or too small (*n_groups is set) or member_of too small;
+ * TB_ERR_OVERFLOW if the candidate buffer overflowed (clear it and search with a higher threshold). */
+TB_API int tb_reduce_candidates(tb_plan* plan, double freq_tol_bins, tb_group* groups_out, uint64_t capacity,
+                         uint64_t* n_groups, uint32_t* member_of, uint64_t member_capacity);
+
+/* Parity tap: REPLACE the plan's accumulated candidates by `n` rows from host memory (fold <= 4,
+ * bin < N/2, n <= max_candidates), so that tb_reduce_candidates can be compared with the oracle on a
+ * seeded synthetic detection list. */
+TB_API int tb_debug_set_candidates(tb_plan* plan, const tb_candidate* cands, uint64_t n);
+
 TB_API const char* tb_strerror(int code);
 TB_API const char* tb_last_error(const tb_plan* plan);
 

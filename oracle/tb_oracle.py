@@ -297,3 +297,62 @@ def search(series, tsamp, templates: Sequence, first_template_id=0, folds=(0, 1,
         out.extend(search_template(x, tsamp, tmpl, first_template_id + i, folds, sigma_threshold,
                                    window, f_min, fill))
     return out
+
+
+# ----------------------------------------------------------------------------------------------
+# f2  front-end whitening once per series ("Fourier birdie
+#     zapping, ..., Fourier de-reddening", L660 "Fourier de-reddenning").  The paper names the steps
+#     and gives no formulas: reading G25 of DESIGN.md section 3 -- PARITY UNPINNED BY THE PAPER,
+#     pinned by closed forms in tests/test_oracle_pins.py (a series that is already white is
+#     returned unchanged up to the estimator's 1/sqrt(W) scatter; a red series comes out flat; a
+#     zapped tone disappears; kappa normalises white noise to the same level as the per-template
+#     estimator of G15).
+# ----------------------------------------------------------------------------------------------
+def whiten_series(series, window=1024, zap_bins=()):
+    """x -> x': X = rfft(x); P_k = |X_k|^2 (raw, no interbinning); m(k) = the G15 baseline of P
+    (block medians of `window` bins, linear interpolation between block centres); X'_k =
+    X_k / sqrt(m(k) / ln2) for 1 <= k < N/2, X'_0 = X'_{N/2} = 0, and X'_k = 0 for every k in a
+    zapped range [lo, hi) ("birdie zap"); x' = irfft(X') * sqrt(N): for noise E|X'_k|^2 = 1, so by
+    Parseval sum_j x'_j^2 = N, i.e. unit variance.  Returns x' as float32."""
+    x = np.asarray(series, dtype=np.float32).astype(np.float64)
+    n = x.size
+    X = np.fft.rfft(x)
+    nb = n // 2
+    P = X[:nb].real ** 2 + X[:nb].imag ** 2
+    m = median_baseline(block_medians(P, window), nb, window)
+    Xw = np.zeros_like(X)
+    ok = m > 0
+    ok[0] = False
+    Xw[:nb][ok] = X[:nb][ok] / np.sqrt(m[ok] / LN2)
+    for lo, hi in zap_bins:
+        Xw[int(lo):int(hi)] = 0.0
+    return (np.fft.irfft(Xw, n) * math.sqrt(float(n))).astype(np.float32)
+
+
+def whitened_level(series_white, window=1024):
+    """kappa: the ONE normalisation constant of a whitened series, replacing the per-template block
+    medians of O6: kappa = ln2 / mean_b(m_b), m_b = block medians of the interbinned spectrum of
+    the un-resampled whitened series.  P^_k = kappa * P_k for every template."""
+    P = interbin_power(rfft_forward(series_white))
+    return LN2 / float(np.mean(block_medians(P, window)))
+
+
+def spectrum_of_template_whitened(series_white, kappa, tsamp, tmpl, fill=None, idx=None):
+    """Steps O1-O5, interbinning, and the constant normalisation P^ = kappa P (P^_0 = 0)."""
+    x = np.asarray(series_white, dtype=np.float32)
+    if fill is None:
+        fill = fill_value(x)
+    if idx is None:
+        idx = resample_indices(x.size, tsamp, tmpl)
+    y = gather(x, idx, fill)
+    P = interbin_power(rfft_forward(y))
+    Ph = kappa * P
+    Ph[0] = 0.0
+    return {"idx": idx, "resampled": y, "power": P, "normalised": Ph}
+
+
+def search_template_whitened(series_white, kappa, tsamp, tmpl, template_id=0, folds=(0, 1, 2, 3, 4), sigma_threshold=6.0,
+                             f_min=0.1, fill=None, idx=None):
+    spec = spectrum_of_template_whitened(series_white, kappa, tsamp, tmpl, fill, idx)
+    sums = harmonic_sums(spec["normalised"], folds)
+    return candidates_from_sums(sums, template_id, sigma_threshold, lowest_bin(len(series_white), tsamp, f_min))

@@ -75,28 +75,41 @@ def related(F_h, F_b, tol16=TOL16_DEFAULT, h_max=H_MAX):
     return False
 
 
+def related_many(F_h, F_b, tol16=TOL16_DEFAULT, h_max=H_MAX):
+    """``related`` for an int64 array F_b at once (the same double loop, one array operation per (p, q))."""
+    F_b = np.asarray(F_b, dtype=np.int64)
+    out = np.zeros(F_b.shape, dtype=bool)
+    for q in range(1, h_max + 1):
+        for p in range(1, h_max + 1):
+            out |= np.abs(q * F_b - p * int(F_h)) <= tol16
+    return out
+
+
 def reduce_candidates(dets, tol16=TOL16_DEFAULT, h_max=H_MAX):
     """R1-R4.  Returns (groups, member_of): groups = list of dicts in head order
     {template, fold, bin, power, sigma, n_peaks, n_detections, n_templates}; member_of[i] = group of
     the i-th detection of the (template, fold, bin)-sorted input."""
     peaks, srt, owner = peaks_from_detections(dets)
     rank = sorted(range(len(peaks)), key=lambda i: (-float(np.float32(peaks[i][4])), peaks[i][0], peaks[i][1], peaks[i][2]))
-    F = [freq16(p[1], p[2]) for p in peaks]
-    group_of = [-1] * len(peaks)
+    F = np.array([freq16(peaks[i][1], peaks[i][2]) for i in rank], dtype=np.int64)      # in rank order
+    group_of_rank = np.full(len(rank), -1, dtype=np.int64)
     groups = []
     for pos, h in enumerate(rank):
-        if group_of[h] >= 0:
+        if group_of_rank[pos] >= 0:
             continue
         g = len(groups)
-        group_of[h] = g
-        members = [h]
-        for b in rank[pos + 1:]:
-            if group_of[b] < 0 and related(F[h], F[b], tol16, h_max):
-                group_of[b] = g
-                members.append(b)
+        group_of_rank[pos] = g
+        later = np.arange(pos + 1, len(rank))
+        later = later[group_of_rank[later] < 0]
+        absorbed = later[related_many(F[pos], F[later], tol16, h_max)] if later.size else later
+        group_of_rank[absorbed] = g
+        members = [h] + [rank[b] for b in absorbed]
         hp = peaks[h]
         groups.append({"template": hp[0], "fold": hp[1], "bin": hp[2], "power": hp[3], "sigma": hp[4],
                        "n_peaks": len(members), "n_detections": sum(peaks[m][5] for m in members),
                        "n_templates": len({peaks[m][0] for m in members})})
+    group_of = [0] * len(peaks)
+    for pos, i in enumerate(rank):
+        group_of[i] = int(group_of_rank[pos])
     member_of = [group_of[o] for o in owner]
     return groups, member_of

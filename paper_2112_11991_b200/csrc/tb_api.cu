@@ -3,6 +3,8 @@
 #include "../../include/tb.h"
 #include "tb_kernels.cuh"
 #include "tb_fft.cuh"
+#include "tb_reduce.cuh"
+#include "tb_whiten.cuh"
 
 #include <cufft.h>
 
@@ -24,6 +26,7 @@ using namespace tb;
 
 static_assert(sizeof(tb_candidate) == 24 && sizeof(Candidate) == 24, "candidate layout");
 static_assert(sizeof(tb_template) == 40, "template layout");
+static_assert(sizeof(tb_group) == 32 && sizeof(Group) == 32, "group layout");
 
 namespace {
 
@@ -83,6 +86,14 @@ struct tb_plan {
     int pf_spec = 32;                                // spectrum former
     std::vector<uint32_t> order;                     // staging order of the current call: fused-path templates first
     size_t n_own = 0;                                // how many of them take the fused path
+
+    // f2: front-end whitening once per series (tb_whiten.cuh)
+    bool whiten = false, whitening_now = false;
+    float kappa = 0.f;                               // P^ = kappa P for every template of a whitened series
+    std::vector<uint2> zap;                          // zapped bin ranges [lo, hi)
+    uint2* d_zap = nullptr;
+    cufftHandle c2r_plan = 0;
+    bool have_c2r = false;
 
     std::map<uint32_t, cufftHandle> fft_plans;       // by batch size, sharing one work area
     void* d_work = nullptr;
@@ -219,6 +230,61 @@ int store_fill_pad(tb_plan* p)
     return TB_OK;
 }
 
+int get_fft_plan(tb_plan* p, uint32_t batch, cufftHandle* out);
+int run_spectrum(tb_plan* p, uint32_t nt, float* d_raw);
+
+// f2 (reading G25): whiten the plan's copy of the series in place and derive kappa.  Uses the chunk
+// scratch (d_fft: spectrum of the series, d_med: block medians), so it runs before any search.
+int whiten_series(tb_plan* p)
+{
+    cufftHandle r2c;
+    if (int rc = get_fft_plan(p, 1, &r2c)) return rc;
+    if (!p->have_c2r) {
+        TB_CUFFT(p, cufftCreate(&p->c2r_plan));
+        p->have_c2r = true;
+        TB_CUFFT(p, cufftSetAutoAllocation(p->c2r_plan, 0));
+        long long nn[1] = {(long long)p->n}, ie[1] = {(long long)p->ld}, oe[1] = {(long long)p->n};
+        size_t ws = 0;
+        TB_CUFFT(p, cufftMakePlanMany64(p->c2r_plan, 1, nn, ie, 1, (long long)p->ld, oe, 1, (long long)p->n, CUFFT_C2R, 1, &ws));
+        if (ws > p->work_bytes) {
+            TB_CUDA(p, cudaStreamSynchronize(p->stream));
+            if (p->d_work) cudaFree(p->d_work);
+            p->d_work = nullptr; p->work_bytes = 0;
+            TB_CUDA(p, cudaMalloc(&p->d_work, ws));
+            p->work_bytes = ws;
+            for (auto& kv : p->fft_plans) TB_CUFFT(p, cufftSetWorkArea(kv.second, p->d_work));
+        }
+        TB_CUFFT(p, cufftSetWorkArea(p->c2r_plan, p->d_work));
+        TB_CUFFT(p, cufftSetStream(p->c2r_plan, p->stream));
+    }
+    TB_CUFFT(p, cufftExecR2C(r2c, p->d_series_owned, reinterpret_cast<cufftComplex*>(p->d_fft)));
+    const unsigned gm = (unsigned)((p->nblk + WH_WARPS - 1) / WH_WARPS);
+    switch (p->window) {
+        case 128: k_whiten_medians<128><<<gm, WH_WARPS * 32, 0, p->stream>>>(p->d_fft, (int)p->nblk, p->d_med); break;
+        case 256: k_whiten_medians<256><<<gm, WH_WARPS * 32, 0, p->stream>>>(p->d_fft, (int)p->nblk, p->d_med); break;
+        case 512: k_whiten_medians<512><<<gm, WH_WARPS * 32, 0, p->stream>>>(p->d_fft, (int)p->nblk, p->d_med); break;
+        case 1024: k_whiten_medians<1024><<<gm, WH_WARPS * 32, 0, p->stream>>>(p->d_fft, (int)p->nblk, p->d_med); break;
+        default: k_whiten_medians<2048><<<gm, WH_WARPS * 32, 0, p->stream>>>(p->d_fft, (int)p->nblk, p->d_med); break;
+    }
+    k_whiten_apply<<<(unsigned)((p->nb + 1 + 255) / 256), 256, 0, p->stream>>>(p->d_fft, (int)p->nb, (int)p->log2w, (int)p->nblk, p->d_med,
+                                                                            (float)(1.0 / std::sqrt((double)p->n)), p->d_zap, (int)p->zap.size());
+    TB_CUDA(p, cudaGetLastError());
+    TB_CUFFT(p, cufftExecC2R(p->c2r_plan, reinterpret_cast<cufftComplex*>(p->d_fft), p->d_series_owned));
+    // kappa from the interbinned spectrum of the whitened, un-resampled series: ln2 / mean of its block medians
+    TB_CUFFT(p, cufftExecR2C(r2c, p->d_series_owned, reinterpret_cast<cufftComplex*>(p->d_fft)));
+    p->whitening_now = true;
+    const int rc = run_spectrum(p, 1, nullptr);
+    p->whitening_now = false;
+    if (rc) return rc;
+    std::vector<float> med(p->nblk);
+    TB_CUDA(p, cudaMemcpyAsync(med.data(), p->d_med, p->nblk * sizeof(float), cudaMemcpyDeviceToHost, p->stream));
+    TB_CUDA(p, cudaStreamSynchronize(p->stream));
+    double acc = 0.0;
+    for (float m : med) acc += (double)m;
+    p->kappa = (float)(0.69314718055994530942 * (double)p->nblk / acc);
+    return TB_OK;
+}
+
 // copy the series (from host or device memory) and derive the fill value (G8)
 int load_series(tb_plan* p, const float* series)
 {
@@ -226,6 +292,7 @@ int load_series(tb_plan* p, const float* series)
     TB_CUDA(p, cudaMemcpyAsync(p->d_series_owned, series, p->n * sizeof(float),
                                p->borrowed ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, p->stream));
     p->d_series = p->d_series_owned;
+    if (p->whiten) { const int rc = whiten_series(p); if (rc) return rc; }
     if (p->user_fill) return store_fill_pad(p);
     // fill value (G8): fp64 mean of the series.  296 per-block partial sums on the device (each a
     // fixed strided subset, summed in a fixed order), added up here in block order: deterministic,
@@ -315,8 +382,14 @@ void launch_spectrum(tb_plan* p, uint32_t nt, float* d_raw)
     const unsigned grid = (unsigned)(cta_per_row * nt), threads = (SP_WARPS + 1) * 32;
     unsigned long long* fb = p->d_cursor + 1;
     const int nb = (int)p->nb, nblk = (int)p->nblk;
-    if (d_raw) k_spectrum_median<W, false, true><<<grid, threads, 0, p->stream>>>(p->d_fft, p->ld, p->d_power, p->d_med, nb, nblk, cta_per_row, nullptr, nullptr, fb, d_raw);
-    else       k_spectrum_median<W, false, false><<<grid, threads, 0, p->stream>>>(p->d_fft, p->ld, p->d_power, p->d_med, nb, nblk, cta_per_row, nullptr, nullptr, fb, nullptr);
+    const bool white = p->whiten && !p->whitening_now;   // the whitening procedure itself needs the medians
+    if (white) {
+        if (d_raw) k_spectrum_median<W, false, true, true><<<grid, threads, 0, p->stream>>>(p->d_fft, p->ld, p->d_power, p->d_med, nb, nblk, cta_per_row, nullptr, nullptr, fb, d_raw, p->kappa);
+        else       k_spectrum_median<W, false, false, true><<<grid, threads, 0, p->stream>>>(p->d_fft, p->ld, p->d_power, p->d_med, nb, nblk, cta_per_row, nullptr, nullptr, fb, nullptr, p->kappa);
+        return;
+    }
+    if (d_raw) k_spectrum_median<W, false, true><<<grid, threads, 0, p->stream>>>(p->d_fft, p->ld, p->d_power, p->d_med, nb, nblk, cta_per_row, nullptr, nullptr, fb, d_raw, 0.f);
+    else       k_spectrum_median<W, false, false><<<grid, threads, 0, p->stream>>>(p->d_fft, p->ld, p->d_power, p->d_med, nb, nblk, cta_per_row, nullptr, nullptr, fb, nullptr, 0.f);
 }
 
 // ---- hand-written FFT path -------------------------------------------------------------------
@@ -413,23 +486,24 @@ int run_own_pass2(tb_plan* p, uint32_t nt)
     return fail(p, TB_ERR_INVALID_ARG, "unsupported M2");
 }
 
-template <int W, int LOG2M1>
-int launch_spectrum_t(tb_plan* p, uint32_t nt, float* d_raw)
+template <int W, int LOG2M1, bool RAW, bool WHITE>
+int launch_spectrum_t1(tb_plan* p, uint32_t nt, float* d_raw)
 {
     constexpr size_t smem = st_smem_bytes(W, LOG2M1);
     const unsigned grid = (unsigned)((p->nblk / 16) * nt);
-    unsigned long long* fb = p->d_cursor + 1;
-    if (d_raw) {
-        auto kern = k_spectrum_t<W, LOG2M1, true>;
-        if (int rc_ = allow_smem(p, reinterpret_cast<const void*>(kern), (size_t)(smem))) return rc_;
-        kern<<<grid, ST_THREADS, smem, p->stream>>>(p->d_fft, p->d_power, p->d_med, p->log2m2, (int)p->nblk, p->d_twn, p->d_twb, p->rot, fb, d_raw, p->pf_spec);
-    } else {
-        auto kern = k_spectrum_t<W, LOG2M1, false>;
-        if (int rc_ = allow_smem(p, reinterpret_cast<const void*>(kern), (size_t)(smem))) return rc_;
-        kern<<<grid, ST_THREADS, smem, p->stream>>>(p->d_fft, p->d_power, p->d_med, p->log2m2, (int)p->nblk, p->d_twn, p->d_twb, p->rot, fb, nullptr, p->pf_spec);
-    }
+    auto kern = k_spectrum_t<W, LOG2M1, RAW, WHITE>;
+    if (int rc_ = allow_smem(p, reinterpret_cast<const void*>(kern), (size_t)(smem))) return rc_;
+    kern<<<grid, ST_THREADS, smem, p->stream>>>(p->d_fft, p->d_power, p->d_med, p->log2m2, (int)p->nblk, p->d_twn, p->d_twb, p->rot,
+                                                p->d_cursor + 1, d_raw, p->pf_spec, p->kappa);
     TB_CUDA(p, cudaGetLastError());
     return TB_OK;
+}
+
+template <int W, int LOG2M1>
+int launch_spectrum_t(tb_plan* p, uint32_t nt, float* d_raw)
+{
+    if (p->whiten) return d_raw ? launch_spectrum_t1<W, LOG2M1, true, true>(p, nt, d_raw) : launch_spectrum_t1<W, LOG2M1, false, true>(p, nt, nullptr);
+    return d_raw ? launch_spectrum_t1<W, LOG2M1, true, false>(p, nt, d_raw) : launch_spectrum_t1<W, LOG2M1, false, false>(p, nt, nullptr);
 }
 
 // (median window, log2 M1) pairs the transposing spectrum former is instantiated for
@@ -529,7 +603,7 @@ int run_fft(tb_plan* p, uint32_t nt)
     return TB_OK;
 }
 
-int run_spectrum(tb_plan* p, uint32_t nt, float* d_raw = nullptr)
+int run_spectrum(tb_plan* p, uint32_t nt, float* d_raw)
 {
     switch (p->window) {
         case 128: launch_spectrum<128>(p, nt, d_raw); break;
@@ -912,7 +986,7 @@ int tb_search_templates(tb_plan* p, const tb_template* tmpl, uint64_t n_template
                 if (es) TB_CUDA(p, cudaEventRecord(es->e[2], p->stream));
                 if ((rc = run_fft(p, nt))) return rc;
                 if (es) TB_CUDA(p, cudaEventRecord(es->e[3], p->stream));
-                if ((rc = run_spectrum(p, nt))) return rc;
+                if ((rc = run_spectrum(p, nt, nullptr))) return rc;
             }
             if (es) TB_CUDA(p, cudaEventRecord(es->e[4], p->stream));
             if ((rc = run_hsum(p, off, nt, fp))) return rc;
@@ -1074,7 +1148,7 @@ int tb_debug_hsums(tb_plan* p, const tb_template* tmpl, float* sums_out)
     } else {
         if ((rc = run_resample(p, 0, 1, nullptr))) return rc;
         if ((rc = run_fft(p, 1))) return rc;
-        if ((rc = run_spectrum(p, 1))) return rc;
+        if ((rc = run_spectrum(p, 1, nullptr))) return rc;
     }
     // the production harmonic summer with its tap on and thresholds at +inf (no candidate is emitted)
     FoldParams fp;
@@ -1088,6 +1162,145 @@ int tb_debug_hsums(tb_plan* p, const tb_template* tmpl, float* sums_out)
     cudaFree(d_tap);
     if (rc) return rc;
     if (e != cudaSuccess) return fail(p, TB_ERR_CUDA, cudaGetErrorString(e));
+    return TB_OK;
+}
+
+}  // extern "C"
+
+// ---- f1: candidate reduction (tb_reduce.cuh) --------------------------------------------------
+namespace {
+
+struct DevBufs {                                     // scratch of one reduction call, freed on every exit path
+    std::vector<void*> ptrs;
+    ~DevBufs() { for (void* q : ptrs) cudaFree(q); }
+    template <typename T> cudaError_t get(T** out, size_t count)
+    {
+        void* q = nullptr;
+        const cudaError_t e = cudaMalloc(&q, std::max<size_t>(count, 1) * sizeof(T));
+        if (e == cudaSuccess) ptrs.push_back(q);
+        *out = static_cast<T*>(q);
+        return e;
+    }
+};
+
+size_t sort_pad(size_t n)
+{
+    size_t p = BS_TILE;
+    while (p < n) p <<= 1;
+    return p;
+}
+
+// ascending bitonic sort of npad records (npad a power of two >= BS_TILE)
+int device_sort(tb_plan* p, SortRec* r, size_t npad)
+{
+    k_bitonic_tiles<<<(unsigned)(npad / BS_TILE), BS_THREADS, 0, p->stream>>>(r);
+    for (size_t size = 2 * (size_t)BS_TILE; size <= npad; size <<= 1) {
+        for (size_t j = size >> 1; j >= (size_t)BS_TILE; j >>= 1)
+            k_bitonic_step<<<(unsigned)((npad / 2 + 255) / 256), 256, 0, p->stream>>>(r, npad, size, j);
+        k_bitonic_finish<<<(unsigned)(npad / BS_TILE), BS_THREADS, 0, p->stream>>>(r, size);
+    }
+    TB_CUDA(p, cudaGetLastError());
+    return TB_OK;
+}
+
+unsigned blocks_for(size_t n) { return (unsigned)((n + 255) / 256); }
+
+}  // namespace
+
+extern "C" {
+
+int tb_debug_set_candidates(tb_plan* p, const tb_candidate* cands, uint64_t n)
+{
+    if (!p || (n && !cands)) return fail(p, TB_ERR_INVALID_ARG, "null argument");
+    if (n > p->max_cand) return fail(p, TB_ERR_CAPACITY, "more rows than max_candidates");
+    for (uint64_t i = 0; i < n; ++i)
+        if (cands[i].fold > TB_MAX_FOLD || cands[i].bin >= p->nb) return fail(p, TB_ERR_INVALID_ARG, "row " + std::to_string(i) + ": fold or bin out of range");
+    TB_CUDA(p, cudaSetDevice(p->device));
+    const unsigned long long count = n;
+    if (n) TB_CUDA(p, cudaMemcpyAsync(p->d_cand, cands, n * sizeof(Candidate), cudaMemcpyHostToDevice, p->stream));
+    TB_CUDA(p, cudaMemcpyAsync(p->d_cursor, &count, sizeof(count), cudaMemcpyHostToDevice, p->stream));
+    TB_CUDA(p, cudaStreamSynchronize(p->stream));
+    return TB_OK;
+}
+
+int tb_reduce_candidates(tb_plan* p, double freq_tol_bins, tb_group* groups_out, uint64_t capacity, uint64_t* n_groups,
+                         uint32_t* member_of, uint64_t member_capacity)
+{
+    if (!p || !n_groups) return fail(p, TB_ERR_INVALID_ARG, "null argument");
+    if (!(freq_tol_bins >= 0) || freq_tol_bins > 1e6) return fail(p, TB_ERR_INVALID_ARG, "freq_tol_bins must be in [0, 1e6]");
+    *n_groups = 0;
+    TB_CUDA(p, cudaSetDevice(p->device));
+    const int64_t tol16 = freq_tol_bins == 0.0 ? 16 : (int64_t)std::llround(16.0 * freq_tol_bins);
+    unsigned long long count = 0;
+    TB_CUDA(p, cudaMemcpyAsync(&count, p->d_cursor, sizeof(count), cudaMemcpyDeviceToHost, p->stream));
+    TB_CUDA(p, cudaStreamSynchronize(p->stream));
+    if (count > p->max_cand) return fail(p, TB_ERR_OVERFLOW, "candidate buffer overflow: " + std::to_string(count));
+    const size_t n = (size_t)count;
+    if (n == 0) return TB_OK;
+    if (member_of && member_capacity < n) return fail(p, TB_ERR_CAPACITY, "member_of too small");
+
+    DevBufs mem;
+    SortRec *srt = nullptr, *rank = nullptr, *gt = nullptr;
+    Peak* peaks = nullptr;
+    uint32_t *peak_of = nullptr, *F = nullptr, *rank_of_peak = nullptr, *gid = nullptr, *d_member = nullptr;
+    int* state = nullptr;
+    unsigned int* ctr = nullptr;                     // [0] peaks, [1] undecided, [2] groups
+    Group* groups = nullptr;
+    const size_t npad = sort_pad(n);
+    TB_CUDA(p, mem.get(&srt, npad));
+    TB_CUDA(p, mem.get(&peaks, n));
+    TB_CUDA(p, mem.get(&peak_of, n));
+    TB_CUDA(p, mem.get(&ctr, 4));
+    TB_CUDA(p, cudaMemsetAsync(ctr, 0, 4 * sizeof(unsigned int), p->stream));
+
+    // R1: sort by (template, fold, bin), runs of adjacent bins -> peaks
+    k_red_det_keys<<<blocks_for(npad), 256, 0, p->stream>>>(p->d_cand, n, npad, srt);
+    if (int rc = device_sort(p, srt, npad)) return rc;
+    k_red_peaks<<<blocks_for(n), 256, 0, p->stream>>>(p->d_cand, srt, n, peaks, peak_of, ctr);
+    unsigned int np = 0;
+    TB_CUDA(p, cudaMemcpyAsync(&np, ctr, sizeof(np), cudaMemcpyDeviceToHost, p->stream));
+    TB_CUDA(p, cudaStreamSynchronize(p->stream));
+
+    // R2: rank by (sigma descending, template, fold, bin)
+    const size_t ppad = sort_pad(np);
+    TB_CUDA(p, mem.get(&rank, ppad));
+    TB_CUDA(p, mem.get(&gt, ppad));
+    TB_CUDA(p, mem.get(&F, np));
+    TB_CUDA(p, mem.get(&state, np));
+    TB_CUDA(p, mem.get(&rank_of_peak, np));
+    TB_CUDA(p, mem.get(&gid, np));
+    TB_CUDA(p, mem.get(&groups, np));
+    TB_CUDA(p, mem.get(&d_member, n));
+    k_red_peak_keys<<<blocks_for(ppad), 256, 0, p->stream>>>(peaks, np, ppad, rank);
+    if (int rc = device_sort(p, rank, ppad)) return rc;
+    k_red_rank_init<<<blocks_for(np), 256, 0, p->stream>>>(peaks, rank, np, F, state, rank_of_peak);
+
+    // R3: rounds until every peak is a head or absorbed (each round decides at least the strongest open peak)
+    for (size_t round = 0; round <= np; ++round) {
+        TB_CUDA(p, cudaMemsetAsync(ctr + 1, 0, sizeof(unsigned int), p->stream));
+        k_red_distill_round<<<blocks_for(np), 256, 0, p->stream>>>(F, state, np, tol16, ctr + 1);
+        unsigned int open = 0;
+        TB_CUDA(p, cudaMemcpyAsync(&open, ctr + 1, sizeof(open), cudaMemcpyDeviceToHost, p->stream));
+        TB_CUDA(p, cudaStreamSynchronize(p->stream));
+        if (open == 0) break;
+    }
+
+    // R4: number the heads, fill the group records, count distinct templates, map detections to groups
+    k_red_number_heads<<<1, 1024, 0, p->stream>>>(state, np, gid, ctr + 2);
+    TB_CUDA(p, cudaMemsetAsync(groups, 0, (size_t)np * sizeof(Group), p->stream));
+    k_red_groups<<<blocks_for(ppad), 256, 0, p->stream>>>(peaks, rank, state, gid, np, ppad, groups, gt);
+    if (int rc = device_sort(p, gt, ppad)) return rc;
+    k_red_count_templates<<<blocks_for(np), 256, 0, p->stream>>>(gt, np, groups);
+    k_red_members<<<blocks_for(n), 256, 0, p->stream>>>(peak_of, rank_of_peak, state, gid, n, d_member);
+    TB_CUDA(p, cudaGetLastError());
+    unsigned int ng = 0;
+    TB_CUDA(p, cudaMemcpyAsync(&ng, ctr + 2, sizeof(ng), cudaMemcpyDeviceToHost, p->stream));
+    TB_CUDA(p, cudaStreamSynchronize(p->stream));
+    *n_groups = ng;
+    if (!groups_out || capacity < ng) return fail(p, TB_ERR_CAPACITY, "groups_out too small");
+    TB_CUDA(p, cudaMemcpyAsync(groups_out, groups, (size_t)ng * sizeof(Group), cudaMemcpyDeviceToHost, p->stream));
+    if (member_of) TB_CUDA(p, cudaMemcpyAsync(member_of, d_member, n * sizeof(uint32_t), cudaMemcpyDeviceToHost, p->stream));
+    TB_CUDA(p, cudaStreamSynchronize(p->stream));
     return TB_OK;
 }
 

@@ -364,12 +364,14 @@ __device__ __forceinline__ float warp_median(const float (&p)[W / 32], float* ca
     return 0.5f * (__uint_as_float(lower) + __uint_as_float(upper));
 }
 
-template <int W, bool UNPACK, bool RAW>
+//   WHITE = true (plan option whiten, reading G25): the series was whitened once, the block medians
+//   are skipped and P^_k = kappa P_k with the plan's constant kappa (med[] receives ln2 / kappa).
+template <int W, bool UNPACK, bool RAW, bool WHITE = false>
 __global__ void __launch_bounds__((SP_WARPS + 1) * 32)
 k_spectrum_median(const float2* __restrict__ X, size_t ld, float* __restrict__ P, float* __restrict__ med,
                   int nb, int nblk_per_row, int cta_per_row, const float2* __restrict__ twn,
                   const float2* __restrict__ twb, unsigned long long* __restrict__ fallbacks,
-                  float* __restrict__ Praw)
+                  float* __restrict__ Praw, float kappa)
 {
     constexpr int VPT  = W / 32;        // powers per lane
     constexpr int ITER = W / 128;       // 4 consecutive bins per lane per iteration
@@ -438,12 +440,27 @@ k_spectrum_median(const float2* __restrict__ X, size_t ld, float* __restrict__ P
                 *reinterpret_cast<float4*>(Praw + (size_t)row * (size_t)nb + k0) = make_float4(SCALE * o.x, SCALE * o.y, SCALE * o.z, SCALE * o.w);
             p[4 * i + 0] = o.x; p[4 * i + 1] = o.y; p[4 * i + 2] = o.z; p[4 * i + 3] = o.w;
         }
+        if (WHITE) {                                     // constant normalisation: the owner warp writes its whole block
+            if (owner) {
+                float* __restrict__ Pw = P + (size_t)row * (size_t)nb + base;
+#pragma unroll
+                for (int i = 0; i < ITER; ++i) {
+                    const int e0 = i * 128 + lane * 4;
+                    float4 o = make_float4(p[4 * i] * (SCALE * kappa), p[4 * i + 1] * (SCALE * kappa), p[4 * i + 2] * (SCALE * kappa), p[4 * i + 3] * (SCALE * kappa));
+                    if (base + e0 == 0) o.x = 0.f;           // P^_0 = 0
+                    *reinterpret_cast<float4*>(Pw + e0) = o;
+                }
+                if (lane == 0) med[(size_t)row * nblk_per_row + blk] = 0.69314718055994530942f / kappa;
+            }
+            return;
+        }
         m_cur = warp_median<W>(p, s_cand[wid], lane, owner ? fallbacks : nullptr);
         if (lane == 0) {
             s_med[wid] = m_cur;
             if (owner) med[(size_t)row * nblk_per_row + blk] = SCALE * m_cur;
         }
     }
+    if (WHITE) return;
     __syncthreads();
     if (!active) return;
     // first half of the block: between the previous centre and this one; second half: this and the next
@@ -547,11 +564,12 @@ __device__ __forceinline__ float st_interbin(float2 x, float2 prev)
     return fmaxf(fmaf(x.y, x.y, x.x * x.x), 0.5f * fmaf(dy, dy, dx * dx));
 }
 
-template <int W, int LOG2M1, bool RAW>
+//   WHITE = true (plan option whiten, reading G25): no medians; P^_k = kappa P_k, med[] = ln2 / kappa.
+template <int W, int LOG2M1, bool RAW, bool WHITE = false>
 __global__ void __launch_bounds__(ST_THREADS, (W <= 1024) ? ST_MINB : 1)
 k_spectrum_t(const float2* __restrict__ Zt, float* __restrict__ P, float* __restrict__ med, int log2m2,
              int nblk, const float2* __restrict__ twa, const float2* __restrict__ twb, float2 rot,
-             unsigned long long* __restrict__ fallbacks, float* __restrict__ Praw, int pf_dist)
+             unsigned long long* __restrict__ fallbacks, float* __restrict__ Praw, int pf_dist, float kappa)
 {
     static_assert(W >= (1 << LOG2M1), "a median block is a whole number of columns");
     constexpr int M1 = 1 << LOG2M1;
@@ -668,6 +686,16 @@ k_spectrum_t(const float2* __restrict__ Zt, float* __restrict__ P, float* __rest
         if (RAW && owner) {
 #pragma unroll
             for (int i = 0; i < VPT; ++i) Praw[(size_t)row * m + (size_t)blk * W + i * 32 + lane] = 0.25f * p[i];
+        }
+        if (WHITE) {                                     // constant normalisation: every owner warp writes its whole block
+            if (owner) {
+                float* __restrict__ Pw = P + (size_t)row * m + (size_t)blk * W + lane;
+                const float kq = 0.25f * kappa;          // powers are carried as 4 P
+#pragma unroll
+                for (int i = 0; i < VPT; ++i) Pw[32 * i] = (i == 0 && blk == 0 && lane == 0) ? 0.f : p[i] * kq;
+                if (lane == 0) med[(size_t)row * nblk + blk] = 0.69314718055994530942f / kappa;
+            }
+            continue;
         }
         // scratch for the bracket list: floats of this warp's own block (all of them are in registers now)
         const float m_cur = warp_median<W, false>(p, (side ? s_hi - 3 : s_lo) + wid * (W + Q), lane, owner ? fallbacks : nullptr);

@@ -25,7 +25,9 @@ TEMPLATE_DTYPE = np.dtype([("p_orb_s", "<f8"), ("tau_lts", "<f8"), ("phi0_rad", 
                            ("omega_rad", "<f8")])
 CANDIDATE_DTYPE = np.dtype([("template_id", "<u4"), ("fold", "<u4"), ("bin", "<u4"), ("power", "<f4"),
                             ("sigma", "<f4"), ("pad", "<u4")])
-assert TEMPLATE_DTYPE.itemsize == 40 and CANDIDATE_DTYPE.itemsize == 24
+GROUP_DTYPE = np.dtype([("template_id", "<u4"), ("fold", "<u4"), ("bin", "<u4"), ("power", "<f4"), ("sigma", "<f4"),
+                        ("n_peaks", "<u4"), ("n_detections", "<u4"), ("n_templates", "<u4")])
+assert TEMPLATE_DTYPE.itemsize == 40 and CANDIDATE_DTYPE.itemsize == 24 and GROUP_DTYPE.itemsize == 32
 
 
 class PlanOpts(C.Structure):
@@ -48,6 +50,7 @@ class Timings(C.Structure):
 
 
 EXPORTS = ["tb_plan_create", "tb_plan_set_series", "tb_search_templates", "tb_get_candidates", "tb_clear_candidates", "tb_plan_destroy",
+           "tb_reduce_candidates", "tb_debug_set_candidates",
            "tb_strerror", "tb_last_error", "tb_get_timings", "tb_debug_resample_indices", "tb_debug_spectrum",
            "tb_debug_resampled", "tb_debug_hsums", "tb_sigma_to_power", "tb_plan_info", "tb_template_knot_log2"]
 
@@ -57,6 +60,8 @@ lib.tb_plan_set_series.argtypes = [_vp, _vp]
 lib.tb_search_templates.argtypes = [_vp, _vp, _u64, _u32, _vp, _u32, C.c_double]
 lib.tb_get_candidates.argtypes = [_vp, _vp, _u64, C.POINTER(_u64)]
 lib.tb_clear_candidates.argtypes = [_vp]
+lib.tb_debug_set_candidates.argtypes = [_vp, _vp, _u64]
+lib.tb_reduce_candidates.argtypes = [_vp, C.c_double, _vp, _u64, C.POINTER(_u64), _vp, _u64]
 lib.tb_plan_destroy.argtypes = [_vp]
 lib.tb_strerror.argtypes = [C.c_int]
 lib.tb_strerror.restype = C.c_char_p
@@ -157,6 +162,27 @@ def tb_get_candidates(plan, capacity=None):
     return out[: n.value], n.value
 
 
+def tb_reduce_candidates(plan, freq_tol_bins=0.0, with_members=False, n_detections=0):
+    """Returns (groups structured array in head order, member_of or None).  member_of (uint32 per
+    detection, in tb_get_candidates order) needs n_detections = the current candidate count."""
+    n = _u64(0)
+    code = lib.tb_reduce_candidates(plan, float(freq_tol_bins), None, 0, C.byref(n), None, 0)
+    if code == TB_OK:
+        return np.zeros(0, dtype=GROUP_DTYPE), (np.zeros(0, dtype=np.uint32) if with_members else None)
+    if code != TB_ERR_CAPACITY:
+        _check(code, plan)
+    out = np.zeros(int(n.value), dtype=GROUP_DTYPE)
+    members = np.zeros(int(n_detections), dtype=np.uint32) if with_members else None
+    _check(lib.tb_reduce_candidates(plan, float(freq_tol_bins), out.ctypes.data, out.size, C.byref(n),
+                                    members.ctypes.data if with_members else None, int(n_detections)), plan)
+    return out[: n.value], members
+
+
+def tb_debug_set_candidates(plan, cands):
+    c = np.ascontiguousarray(cands, dtype=CANDIDATE_DTYPE)
+    _check(lib.tb_debug_set_candidates(plan, c.ctypes.data, c.size), plan)
+
+
 def tb_clear_candidates(plan):
     _check(lib.tb_clear_candidates(plan), plan)
 
@@ -241,6 +267,12 @@ class Plan:
 
     def candidates(self, capacity=None):
         return tb_get_candidates(self.handle, capacity)
+
+    def reduce(self, freq_tol_bins=0.0, with_members=False, n_detections=0):
+        return tb_reduce_candidates(self.handle, freq_tol_bins, with_members, n_detections)
+
+    def debug_set_candidates(self, cands):
+        tb_debug_set_candidates(self.handle, cands)
 
     def clear(self):
         tb_clear_candidates(self.handle)

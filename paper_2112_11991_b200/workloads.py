@@ -215,3 +215,34 @@ def shard_templates(n_templates: int, rank: int, world: int):
     base, rem = divmod(n_templates, world)
     first = rank * base + min(rank, rem)
     return first, base + (1 if rank < rem else 0)
+
+
+def synthetic_detections(seed: int, n_noise: int, n_signals: int = 3, n_templates: int = 8, nb: int = 1 << 16):
+    """A seeded raw detection list for the candidate-reduction parity tests (no search arithmetic:
+    just rows shaped like a search's output).  n_noise isolated rows at random (template, fold, bin)
+    with sigma ~ 4 + Exp(0.5), plus n_signals "pulsars": a spin frequency seen in every fold of
+    2-3 neighbouring templates as a run of 1-4 adjacent bins, with harmonics and sub-harmonic
+    aliases, sigma up to ~20.  Rows are unique in (template, fold, bin); float32 sigma / power.
+    Returns a structured array (template_id, fold, bin, power, sigma, pad) in random order."""
+    rng = np.random.default_rng(BASE_SEED + 7000 + seed)
+    rows = {}
+    for _ in range(n_noise):
+        key = (int(rng.integers(n_templates)), int(rng.integers(5)), int(rng.integers(16, nb)))
+        rows[key] = 4.0 + rng.exponential(0.5)
+    for s in range(n_signals):
+        f = rng.uniform(200.0, nb / 40.0)                     # fundamental, bins
+        peak = rng.uniform(9.0, 20.0)
+        t0 = int(rng.integers(n_templates))
+        for t in {t0, (t0 + 1) % n_templates, (t0 + int(rng.integers(3))) % n_templates}:
+            for L in range(5):
+                for num, den in ((1, 1), (2, 1), (3, 1), (1, 2), (1, 3), (3, 2), (5, 1)):
+                    k = int(round(f * num / den * (1 << L)))
+                    if not 16 <= k < nb - 8 or rng.random() < 0.25:
+                        continue
+                    for d in range(int(rng.integers(1, 5))):
+                        rows[(t, L, k + d)] = max(4.0, peak * rng.uniform(0.4, 1.0) / (1.0 + 0.3 * abs(num - den)))
+    dt = np.dtype([("template_id", "<u4"), ("fold", "<u4"), ("bin", "<u4"), ("power", "<f4"), ("sigma", "<f4"), ("pad", "<u4")])
+    out = np.zeros(len(rows), dtype=dt)
+    for i, ((t, L, k), sg) in enumerate(rows.items()):
+        out[i] = (t, L, k, np.float32(sg * sg), np.float32(sg), 0)
+    return out[rng.permutation(len(out))]

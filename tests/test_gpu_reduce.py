@@ -1,0 +1,118 @@
+"""-m gpu: tb_reduce_candidates (device sort, run scan, distillation rounds) against the reduction
+oracle (oracle/tb_reduce.py), bit-exact: group heads, counts and the group of every detection.
+The detection lists are seeded and synthetic (workloads.synthetic_detections), loaded into the
+plan with the tb_debug_set_candidates tap, at sizes from empty to several sort tiles with ragged
+tails; plus C1 end to end (GPU search + GPU reduction against oracle search + oracle reduction)."""
+import numpy as np
+import pytest
+
+from oracle import tb_oracle as orc
+from oracle import tb_reduce as red
+from paper_2112_11991_b200 import workloads as wl_mod
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def tb():
+    import torch
+    assert torch.cuda.is_available(), "these tests need a CUDA device"
+    from paper_2112_11991_b200 import build
+    build.build()
+    from paper_2112_11991_b200 import tb
+    return tb
+
+
+def _as_tuples(c):
+    return [(int(r["template_id"]), int(r["fold"]), int(r["bin"]), float(r["power"]), float(r["sigma"])) for r in c]
+
+
+def _compare(groups_gpu, members_gpu, dets, tol16=16):
+    groups, member_of = red.reduce_candidates(_as_tuples(dets), tol16=tol16)
+    assert len(groups_gpu) == len(groups)
+    for g, o in zip(groups_gpu, groups):
+        assert (int(g["template_id"]), int(g["fold"]), int(g["bin"])) == (o["template"], o["fold"], o["bin"])
+        assert float(g["sigma"]) == float(np.float32(o["sigma"])) and float(g["power"]) == float(np.float32(o["power"]))
+        assert (int(g["n_peaks"]), int(g["n_detections"]), int(g["n_templates"])) == (o["n_peaks"], o["n_detections"], o["n_templates"])
+    assert members_gpu.tolist() == member_of
+    return groups
+
+
+@pytest.mark.parametrize("seed,n_noise,n_signals", [(0, 0, 0), (1, 1, 0), (2, 0, 1), (3, 300, 2), (4, 2047, 3), (5, 2049, 3),
+                                                    (6, 5000, 4), (7, 9000, 6)])
+def test_reduce_synthetic_lists(tb, c1, seed, n_noise, n_signals):
+    dets = wl_mod.synthetic_detections(seed, n_noise, n_signals)
+    with tb.Plan(c1.series, c1.tsamp) as plan:
+        plan.debug_set_candidates(dets)
+        groups, members = plan.reduce(with_members=True, n_detections=len(dets))
+        cands, n = plan.candidates()                              # not consumed by the reduction; sorted
+    assert n == len(dets)
+    if n == 0:
+        assert len(groups) == 0
+        return
+    o = _compare(groups, members, dets)
+    assert sum(g["n_detections"] for g in o) == n
+    if n_signals:
+        assert o[0]["n_peaks"] > 3 and o[0]["sigma"] > 8          # the strongest pulsar collects its harmonics
+
+
+def test_reduce_tolerance_option(tb, c1):
+    dets = wl_mod.synthetic_detections(11, 800, 2)
+    with tb.Plan(c1.series, c1.tsamp) as plan:
+        plan.debug_set_candidates(dets)
+        g_half, m_half = plan.reduce(0.5, with_members=True, n_detections=len(dets))
+        g_two, m_two = plan.reduce(2.0, with_members=True, n_detections=len(dets))
+    _compare(g_half, m_half, dets, tol16=8)
+    _compare(g_two, m_two, dets, tol16=32)
+    assert len(g_two) < len(g_half)
+
+
+def test_reduce_capacity_and_overflow(tb, c1):
+    dets = wl_mod.synthetic_detections(12, 100, 1)
+    with tb.Plan(c1.series, c1.tsamp, max_candidates=50) as plan:
+        with pytest.raises(tb.TbError) as ei:
+            plan.debug_set_candidates(dets)                       # more rows than max_candidates
+        assert ei.value.code == tb.TB_ERR_CAPACITY
+        plan.search(c1.templates[:4], 0, c1.folds, 3.0)           # overflows the 50-row buffer
+        with pytest.raises(tb.TbError) as ei:
+            plan.reduce()
+        assert ei.value.code == tb.TB_ERR_OVERFLOW
+    with tb.Plan(c1.series, c1.tsamp) as plan:
+        plan.debug_set_candidates(dets)
+        n = tb._u64(0)
+        small = np.zeros(1, dtype=tb.GROUP_DTYPE)
+        assert tb.lib.tb_reduce_candidates(plan.handle, 0.0, small.ctypes.data, 1, n, None, 0) == tb.TB_ERR_CAPACITY
+        assert n.value > 1
+
+
+def test_c1_end_to_end_is_one_group_at_50_hz(tb, c1):
+    """GPU search + GPU reduction against oracle search + oracle reduction on the whole C1 bank."""
+    with tb.Plan(c1.series, c1.tsamp) as plan:
+        plan.search(c1.templates, 0, c1.folds, 6.0)
+        groups, members = plan.reduce(with_members=True, n_detections=76)
+        cands, n = plan.candidates()
+    assert n == 76 and len(groups) == 1 and set(members.tolist()) == {0}
+    g = groups[0]
+    assert (int(g["template_id"]), int(g["fold"]), int(g["bin"]), int(g["n_detections"])) == (0, 3, 52429, 76)
+    o_groups, _ = red.reduce_candidates(orc.search(c1.series, c1.tsamp, c1.templates, sigma_threshold=6.0))
+    assert len(o_groups) == 1
+    assert (o_groups[0]["template"], o_groups[0]["fold"], o_groups[0]["bin"], o_groups[0]["n_peaks"], o_groups[0]["n_detections"]) == \
+           (0, 3, 52429, int(g["n_peaks"]), 76)
+    assert abs(float(g["sigma"]) - o_groups[0]["sigma"]) < 1e-3
+
+
+def test_c1_low_threshold_end_to_end(tb, c1):
+    """4.5 sigma over 16 templates: hundreds of noise rows around the pulsar's group.  The two
+    searches agree on the candidate set (threshold band aside), so the reductions agree on every
+    group whose head is clear of the band."""
+    with tb.Plan(c1.series, c1.tsamp) as plan:
+        plan.search(c1.templates[:16], 0, c1.folds, 4.5)
+        groups, _ = plan.reduce()
+        cands, n = plan.candidates()
+    o_dets = orc.search(c1.series, c1.tsamp, c1.templates[:16], sigma_threshold=4.5)
+    o_groups, _ = red.reduce_candidates(o_dets)
+    if {(c[0], c[1], c[2]) for c in o_dets} == {(int(c["template_id"]), int(c["fold"]), int(c["bin"])) for c in cands}:
+        assert [(int(g["template_id"]), int(g["fold"]), int(g["bin"]), int(g["n_detections"])) for g in groups] == \
+               [(o["template"], o["fold"], o["bin"], o["n_detections"]) for o in o_groups]
+    assert (int(groups[0]["fold"]), int(groups[0]["bin"])) == (3, 52429) == (o_groups[0]["fold"], o_groups[0]["bin"])
+    assert int(groups[0]["n_detections"]) == o_groups[0]["n_detections"]

@@ -423,3 +423,65 @@ def test_sign_convention_against_literal_eq_a2():
     assert best[4] > 10.0
     assert orc.search_template(x, tsamp, (p_orb, tau, phi0, 0.0, 0.0), 0) == []
     assert orc.search_template(x, tsamp, (p_orb, 0.0, phi0, 0.0, 0.0), 0) == []      # and not without resampling
+
+
+# ------------------------------------------------------------------ f2: whitening once per series (reading G25)
+def test_whitening_closed_form_impulse():
+    """x = delta at j0: |X_k|^2 = 1 for every k, so every block median is 1 and X'_k = sqrt(ln2) X_k for
+    0 < k < N/2, X'_0 = X'_{N/2} = 0:  x'_j = sqrt(N ln2) (delta_{j j0} - 1/N - (-1)^(j-j0)/N)."""
+    n, j0 = 4096, 777
+    x = np.zeros(n, dtype=np.float32)
+    x[j0] = 1.0
+    got = orc.whiten_series(x, window=256).astype(np.float64)
+    j = np.arange(n)
+    want = math.sqrt(n * math.log(2)) * ((j == j0).astype(float) - 1.0 / n - (-1.0) ** (j - j0) / n)
+    assert np.max(np.abs(got - want)) < 1e-5
+
+
+def test_whitening_flattens_red_noise_and_keeps_white_noise():
+    rng = np.random.default_rng(25)
+    n = 1 << 16
+    w = rng.standard_normal(n)
+    xw = orc.whiten_series((3.0 * w + 10.0).astype(np.float32))        # white, scaled, with a DC offset
+    assert abs(xw.std() - 1.0) < 0.01 and abs(xw.mean()) < 1e-6
+    assert np.corrcoef(xw, w)[0, 1] > 0.995                             # only the estimator's scatter is added
+    assert np.max(np.abs(orc.whiten_series((7.0 * (3.0 * w + 10.0)).astype(np.float32)) - xw)) < 1e-4   # scale-free
+    red = np.cumsum(w) * 0.05 + w                                       # random walk + white: power ~ 1/f^2 at low f
+    band = lambda y, a, b: np.mean(np.abs(np.fft.rfft(y))[a:b] ** 2)
+    assert band(red, 16, 512) / band(red, n // 4, n // 2) > 20.0
+    xr = orc.whiten_series(red.astype(np.float32))
+    # where the spectrum is steep the piecewise-linear baseline of 1024-bin medians lags by a few per cent
+    assert abs(band(xr, 1024, 4096) / band(xr, n // 4, n // 2) - 1.0) < 0.15
+    assert abs(band(xr, 8192, 16384) / band(xr, n // 4, n // 2) - 1.0) < 0.05
+    assert abs(band(xr, 1024, n // 2) / n - 1.0) < 0.02                 # E|X'_k|^2 = N for a unit-variance series
+
+
+def test_whitening_zaps_birdies():
+    rng = np.random.default_rng(26)
+    n, k0 = 1 << 14, 3000
+    x = (rng.standard_normal(n) + 0.5 * np.cos(2 * np.pi * k0 * np.arange(n) / n)).astype(np.float32)
+    kept = np.abs(np.fft.rfft(orc.whiten_series(x)))
+    zapped = np.abs(np.fft.rfft(orc.whiten_series(x, zap_bins=[(k0 - 1, k0 + 2)])))
+    assert kept[k0] > 20 * np.median(kept)                              # a block median does not remove a tone
+    assert np.all(zapped[k0 - 1:k0 + 2] < 1e-3) and zapped[k0 + 5] > 1.0
+
+
+def test_whitened_level_matches_the_per_template_normalisation():
+    """kappa P of a whitened white series has the same level as P ln2 / m(k) (G15) of the raw one."""
+    rng = np.random.default_rng(27)
+    x = rng.standard_normal(1 << 17).astype(np.float32)
+    tmpl = (60.0, 0.3, 1.0, 0.0, 0.0)
+    a = orc.spectrum_of_template(x, 1e-3, tmpl)["normalised"]
+    xw = orc.whiten_series(x)
+    b = orc.spectrum_of_template_whitened(xw, orc.whitened_level(xw), 1e-3, tmpl)["normalised"]
+    assert b[0] == 0.0 and abs(np.mean(b[1:]) / np.mean(a[1:]) - 1.0) < 0.01
+    assert abs(np.median(b[1:]) - math.log(2)) < 0.01                   # kappa puts the median at ln2, like G15
+
+
+def test_t10_on_the_whitened_series(c1):
+    xw = orc.whiten_series(c1.series)
+    kappa = orc.whitened_level(xw)
+    cands = orc.search_template_whitened(xw, kappa, c1.tsamp, c1.templates[0], 0)
+    best = max(cands, key=lambda c: c[4])
+    assert (best[1], best[2]) == (3, 52429) and best[4] > 12.0
+    assert orc.search_template_whitened(xw, kappa, c1.tsamp, c1.templates[5], 1) == []

@@ -117,3 +117,13 @@ def test_two_unrelated_signals_stay_apart():
     assert len(groups) == 2
     assert [g["n_peaks"] for g in groups] == [6, 6]
     assert {round(g["bin"] / 2 ** g["fold"]) for g in groups} == {6554, 4135}
+
+
+def test_vectorised_relation_equals_the_double_loop():
+    rng = np.random.default_rng(5)
+    Fh = int(rng.integers(500, 200000))
+    Fb = rng.integers(100, 400000, 3000)
+    Fb[:200] = (Fh * rng.integers(1, 17, 200)) // rng.integers(1, 17, 200) + rng.integers(-20, 21, 200)   # near-harmonic cases
+    want = np.array([red.related(Fh, int(f)) for f in Fb])
+    assert want.sum() > 50 and (~want).sum() > 50
+    assert np.array_equal(red.related_many(Fh, Fb), want)
