@@ -108,6 +108,15 @@ typedef struct {
                                      {512, 1024, 2048} (256 or 1024 at 2^17 and 2^25; 1024 or 2048 at
                                      2^24) and knot spacing >= 8; batched cuFFT otherwise); 1: always
                                      cuFFT; 2: hand-written or TB_ERR_INVALID_ARG */
+    int32_t  whiten;              /* 1: front-end whitening once per series ("Fourier
+                                     de-reddening", "birdie zapping"; reading G25): tb_plan_create and
+                                     tb_plan_set_series replace the series by x' = C2R(X_k / sqrt(m(k)/ln2)) / sqrt(N)
+                                     (m(k): the G15 baseline of the raw powers |X_k|^2, X'_0 = X'_{N/2} = 0, zapped
+                                     ranges = 0; unit variance for noise), and every template is then normalised by
+                                     ONE constant, P^_k = kappa P_k, kappa = ln2 / mean of the block medians of the
+                                     interbinned spectrum of x' -- step a6 leaves the per-template loop */
+    uint32_t n_zap_ranges;        /* number of zapped bin ranges (used only when whiten is set) */
+    const uint32_t* zap_ranges;   /* host, 2 * n_zap_ranges values: [lo, hi) pairs, lo < hi <= N/2; copied */
 } tb_plan_opts;
 
 /* Per-stage device time of the last tb_search_templates call (CUDA events on the plan's stream,
@@ -228,6 +237,10 @@ TB_API int tb_debug_spectrum(tb_plan* plan, const tb_template* tmpl, float* p_in
 
 /* Resampled series y_j of one template (a3): host float32[N]. */
 TB_API int tb_debug_resampled(tb_plan* plan, const tb_template* tmpl, float* y_out);
+
+/* The plan's working copy of the series (host float32[N]; the whitened series when opts.whiten is
+ * set) and the normalisation constant kappa of a whitened plan (0 otherwise).  Either may be NULL. */
+TB_API int tb_debug_series(tb_plan* plan, float* x_out, double* kappa_out);
 
 /* Harmonic sums of one template (a8; eq 9, G16) through the production summing kernel with its
  * tap enabled and every threshold at +infinity: sums_out[L * (N/2) + k] = S_L[k], L = 0..4,

@@ -92,7 +92,7 @@ struct tb_plan {
     float kappa = 0.f;                               // P^ = kappa P for every template of a whitened series
     std::vector<uint2> zap;                          // zapped bin ranges [lo, hi)
     uint2* d_zap = nullptr;
-    cufftHandle c2r_plan = 0;
+    cufftHandle c2r_plan = 0, d2z_plan = 0;      // Z2D and D2Z of the whitening step
     bool have_c2r = false;
 
     std::map<uint32_t, cufftHandle> fft_plans;       // by batch size, sharing one work area
@@ -230,6 +230,19 @@ int store_fill_pad(tb_plan* p)
     return TB_OK;
 }
 
+struct DevBufs {                                     // scratch of one reduction call, freed on every exit path
+    std::vector<void*> ptrs;
+    ~DevBufs() { for (void* q : ptrs) cudaFree(q); }
+    template <typename T> cudaError_t get(T** out, size_t count)
+    {
+        void* q = nullptr;
+        const cudaError_t e = cudaMalloc(&q, std::max<size_t>(count, 1) * sizeof(T));
+        if (e == cudaSuccess) ptrs.push_back(q);
+        *out = static_cast<T*>(q);
+        return e;
+    }
+};
+
 int get_fft_plan(tb_plan* p, uint32_t batch, cufftHandle* out);
 int run_spectrum(tb_plan* p, uint32_t nt, float* d_raw);
 
@@ -237,40 +250,39 @@ int run_spectrum(tb_plan* p, uint32_t nt, float* d_raw);
 // scratch (d_fft: spectrum of the series, d_med: block medians), so it runs before any search.
 int whiten_series(tb_plan* p)
 {
-    cufftHandle r2c;
-    if (int rc = get_fft_plan(p, 1, &r2c)) return rc;
+    // double-precision transforms, once per series (see tb_whiten.cuh); the plans are cached
     if (!p->have_c2r) {
-        TB_CUFFT(p, cufftCreate(&p->c2r_plan));
+        TB_CUFFT(p, cufftPlan1d(&p->d2z_plan, (int)p->n, CUFFT_D2Z, 1));
+        cufftResult r = cufftPlan1d(&p->c2r_plan, (int)p->n, CUFFT_Z2D, 1);
+        if (r != CUFFT_SUCCESS) { cufftDestroy(p->d2z_plan); return fail(p, r == CUFFT_ALLOC_FAILED ? TB_ERR_NOMEM : TB_ERR_CUFFT, "cufftPlan1d(Z2D)"); }
         p->have_c2r = true;
-        TB_CUFFT(p, cufftSetAutoAllocation(p->c2r_plan, 0));
-        long long nn[1] = {(long long)p->n}, ie[1] = {(long long)p->ld}, oe[1] = {(long long)p->n};
-        size_t ws = 0;
-        TB_CUFFT(p, cufftMakePlanMany64(p->c2r_plan, 1, nn, ie, 1, (long long)p->ld, oe, 1, (long long)p->n, CUFFT_C2R, 1, &ws));
-        if (ws > p->work_bytes) {
-            TB_CUDA(p, cudaStreamSynchronize(p->stream));
-            if (p->d_work) cudaFree(p->d_work);
-            p->d_work = nullptr; p->work_bytes = 0;
-            TB_CUDA(p, cudaMalloc(&p->d_work, ws));
-            p->work_bytes = ws;
-            for (auto& kv : p->fft_plans) TB_CUFFT(p, cufftSetWorkArea(kv.second, p->d_work));
-        }
-        TB_CUFFT(p, cufftSetWorkArea(p->c2r_plan, p->d_work));
+        TB_CUFFT(p, cufftSetStream(p->d2z_plan, p->stream));
         TB_CUFFT(p, cufftSetStream(p->c2r_plan, p->stream));
     }
-    TB_CUFFT(p, cufftExecR2C(r2c, p->d_series_owned, reinterpret_cast<cufftComplex*>(p->d_fft)));
+    DevBufs mem;
+    double* dx = nullptr;
+    double2* dX = nullptr;
+    TB_CUDA(p, mem.get(&dx, p->n));
+    TB_CUDA(p, mem.get(&dX, p->nb + 1));
+    k_f32_to_f64<<<1184, 256, 0, p->stream>>>(p->d_series_owned, dx, (size_t)p->n);
+    TB_CUFFT(p, cufftExecD2Z(p->d2z_plan, dx, reinterpret_cast<cufftDoubleComplex*>(dX)));
     const unsigned gm = (unsigned)((p->nblk + WH_WARPS - 1) / WH_WARPS);
     switch (p->window) {
-        case 128: k_whiten_medians<128><<<gm, WH_WARPS * 32, 0, p->stream>>>(p->d_fft, (int)p->nblk, p->d_med); break;
-        case 256: k_whiten_medians<256><<<gm, WH_WARPS * 32, 0, p->stream>>>(p->d_fft, (int)p->nblk, p->d_med); break;
-        case 512: k_whiten_medians<512><<<gm, WH_WARPS * 32, 0, p->stream>>>(p->d_fft, (int)p->nblk, p->d_med); break;
-        case 1024: k_whiten_medians<1024><<<gm, WH_WARPS * 32, 0, p->stream>>>(p->d_fft, (int)p->nblk, p->d_med); break;
-        default: k_whiten_medians<2048><<<gm, WH_WARPS * 32, 0, p->stream>>>(p->d_fft, (int)p->nblk, p->d_med); break;
+        case 128: k_whiten_medians<128><<<gm, WH_WARPS * 32, 0, p->stream>>>(dX, (int)p->nblk, p->d_med); break;
+        case 256: k_whiten_medians<256><<<gm, WH_WARPS * 32, 0, p->stream>>>(dX, (int)p->nblk, p->d_med); break;
+        case 512: k_whiten_medians<512><<<gm, WH_WARPS * 32, 0, p->stream>>>(dX, (int)p->nblk, p->d_med); break;
+        case 1024: k_whiten_medians<1024><<<gm, WH_WARPS * 32, 0, p->stream>>>(dX, (int)p->nblk, p->d_med); break;
+        default: k_whiten_medians<2048><<<gm, WH_WARPS * 32, 0, p->stream>>>(dX, (int)p->nblk, p->d_med); break;
     }
-    k_whiten_apply<<<(unsigned)((p->nb + 1 + 255) / 256), 256, 0, p->stream>>>(p->d_fft, (int)p->nb, (int)p->log2w, (int)p->nblk, p->d_med,
-                                                                            (float)(1.0 / std::sqrt((double)p->n)), p->d_zap, (int)p->zap.size());
+    k_whiten_apply<<<(unsigned)((p->nb + 1 + 255) / 256), 256, 0, p->stream>>>(dX, (int)p->nb, (int)p->log2w, (int)p->nblk, p->d_med,
+                                                                            1.0 / std::sqrt((double)p->n), p->d_zap, (int)p->zap.size());
     TB_CUDA(p, cudaGetLastError());
-    TB_CUFFT(p, cufftExecC2R(p->c2r_plan, reinterpret_cast<cufftComplex*>(p->d_fft), p->d_series_owned));
-    // kappa from the interbinned spectrum of the whitened, un-resampled series: ln2 / mean of its block medians
+    TB_CUFFT(p, cufftExecZ2D(p->c2r_plan, reinterpret_cast<cufftDoubleComplex*>(dX), dx));
+    k_f64_to_f32<<<1184, 256, 0, p->stream>>>(dx, p->d_series_owned, (size_t)p->n);
+    // kappa from the interbinned spectrum of the whitened, un-resampled series (the production
+    // single-precision path: batched R2C + k_spectrum_median): ln2 / mean of its block medians
+    cufftHandle r2c;
+    if (int rc = get_fft_plan(p, 1, &r2c)) return rc;
     TB_CUFFT(p, cufftExecR2C(r2c, p->d_series_owned, reinterpret_cast<cufftComplex*>(p->d_fft)));
     p->whitening_now = true;
     const int rc = run_spectrum(p, 1, nullptr);
@@ -278,7 +290,7 @@ int whiten_series(tb_plan* p)
     if (rc) return rc;
     std::vector<float> med(p->nblk);
     TB_CUDA(p, cudaMemcpyAsync(med.data(), p->d_med, p->nblk * sizeof(float), cudaMemcpyDeviceToHost, p->stream));
-    TB_CUDA(p, cudaStreamSynchronize(p->stream));
+    TB_CUDA(p, cudaStreamSynchronize(p->stream));                // also fences the scratch freed by ~DevBufs
     double acc = 0.0;
     for (float m : med) acc += (double)m;
     p->kappa = (float)(0.69314718055994530942 * (double)p->nblk / acc);
@@ -754,6 +766,8 @@ void destroy(tb_plan* p)
     if (p->l2_pinned && !p->own_stream)              // give a caller-owned stream its previous window back
         cudaStreamSetAttribute(p->stream, cudaStreamAttributeAccessPolicyWindow, &p->l2_prev);
     for (auto& kv : p->fft_plans) cufftDestroy(kv.second);
+    if (p->have_c2r) { cufftDestroy(p->c2r_plan); cufftDestroy(p->d2z_plan); }
+    cudaFree(p->d_zap);
     for (auto& es : p->events) for (auto& e : es.e) cudaEventDestroy(e);
     if (p->ev_staged) cudaEventDestroy(p->ev_staged);
     cudaFree(p->d_seg); cudaFree(p->d_tw1a); cudaFree(p->d_tw1b); cudaFree(p->d_tw2); cudaFree(p->d_twn); cudaFree(p->d_twb); cudaFree(p->d_twc);
@@ -833,6 +847,15 @@ int tb_plan_create(tb_plan** out, const float* series, uint64_t n_samples, doubl
     p->k_lo = (uint32_t)std::min<double>(std::ceil(p->f_min * ((double)n_samples * tsamp_s)), 4294967295.0);
     p->max_cand = o.max_candidates ? o.max_candidates : (1ull << 22);
     p->timings = o.enable_timings != 0;
+    p->whiten = o.whiten != 0;
+    if (o.n_zap_ranges) {
+        if (!o.zap_ranges) { delete p; return TB_ERR_INVALID_ARG; }
+        for (uint32_t z = 0; z < o.n_zap_ranges; ++z) {
+            const uint32_t lo = o.zap_ranges[2 * z], hi = o.zap_ranges[2 * z + 1];
+            if (lo >= hi || hi > n_samples / 2) { delete p; return TB_ERR_INVALID_ARG; }
+            p->zap.push_back(make_uint2(lo, hi));
+        }
+    }
     p->ld = p->nb + 4;                                // N/2+1 bins padded to a multiple of 4 complex (32 B)
 
     auto bail = [&](int code, const std::string& m) { (void)m; destroy(p); return code; };
@@ -860,12 +883,9 @@ int tb_plan_create(tb_plan** out, const float* series, uint64_t n_samples, doubl
     }
     p->chunk = B;
 
-    // series + fill value
     p->borrowed = o.series_is_device_ptr != 0;
     p->user_fill = o.has_fill != 0;
     p->fill = o.fill_value;
-    { int rc = load_series(p, series); if (rc) { destroy(p); return rc; } }
-    pin_series_in_l2(p);
 
     // FFT path: hand-written two-pass FFT (M = N/2 = M1 * M2, M1 = 512, 256 at 2^17, 1024 at 2^24) when
     // 2^17 <= N <= 2^26 (three passes with M2 = 256 x 256 at 2^25 and 2^26), W >= M1 and the median blocks pair up in groups of 16; batched cuFFT otherwise
@@ -890,10 +910,18 @@ int tb_plan_create(tb_plan** out, const float* series, uint64_t n_samples, doubl
     TB_TRY(cudaMalloc(&p->d_cand, p->max_cand * sizeof(Candidate)));
     TB_TRY(cudaMalloc(&p->d_cursor, 2 * sizeof(unsigned long long)));   // [0] candidate cursor, [1] median fallbacks
     TB_TRY(cudaMemsetAsync(p->d_cursor, 0, 2 * sizeof(unsigned long long), p->stream));
+    if (!p->zap.empty()) {
+        TB_TRY(cudaMalloc(&p->d_zap, p->zap.size() * sizeof(uint2)));
+        TB_TRY(cudaMemcpy(p->d_zap, p->zap.data(), p->zap.size() * sizeof(uint2), cudaMemcpyHostToDevice));
+    }
 #undef TB_TRY
     cufftHandle h;
     int rc = get_fft_plan(p, B, &h);
     if (rc) { destroy(p); return rc; }
+    // series + fill value (+ whitening, which uses the chunk scratch allocated above)
+    rc = load_series(p, series);
+    if (rc) { destroy(p); return rc; }
+    pin_series_in_l2(p);
     if (cudaStreamSynchronize(p->stream) != cudaSuccess) { destroy(p); return TB_ERR_CUDA; }
     *out = p;
     return TB_OK;
@@ -1136,6 +1164,16 @@ int tb_debug_spectrum(tb_plan* p, const tb_template* tmpl, float* p_interbinned,
     return TB_OK;
 }
 
+int tb_debug_series(tb_plan* p, float* x_out, double* kappa_out)
+{
+    if (!p) return TB_ERR_INVALID_ARG;
+    TB_CUDA(p, cudaSetDevice(p->device));
+    if (x_out) TB_CUDA(p, cudaMemcpyAsync(x_out, p->d_series, p->n * sizeof(float), cudaMemcpyDeviceToHost, p->stream));
+    TB_CUDA(p, cudaStreamSynchronize(p->stream));
+    if (kappa_out) *kappa_out = p->whiten ? (double)p->kappa : 0.0;
+    return TB_OK;
+}
+
 int tb_debug_hsums(tb_plan* p, const tb_template* tmpl, float* sums_out)
 {
     if (!sums_out) return fail(p, TB_ERR_INVALID_ARG, "null argument");
@@ -1169,19 +1207,6 @@ int tb_debug_hsums(tb_plan* p, const tb_template* tmpl, float* sums_out)
 
 // ---- f1: candidate reduction (tb_reduce.cuh) --------------------------------------------------
 namespace {
-
-struct DevBufs {                                     // scratch of one reduction call, freed on every exit path
-    std::vector<void*> ptrs;
-    ~DevBufs() { for (void* q : ptrs) cudaFree(q); }
-    template <typename T> cudaError_t get(T** out, size_t count)
-    {
-        void* q = nullptr;
-        const cudaError_t e = cudaMalloc(&q, std::max<size_t>(count, 1) * sizeof(T));
-        if (e == cudaSuccess) ptrs.push_back(q);
-        *out = static_cast<T*>(q);
-        return e;
-    }
-};
 
 size_t sort_pad(size_t n)
 {

@@ -34,7 +34,8 @@ class PlanOpts(C.Structure):
     _fields_ = [("struct_size", C.c_uint32), ("device", C.c_int32), ("stream", C.c_void_p),
                 ("median_window", C.c_uint32), ("f_min_hz", C.c_double), ("max_candidates", C.c_uint64),
                 ("chunk_templates", C.c_uint32), ("series_is_device_ptr", C.c_int32), ("has_fill", C.c_int32),
-                ("fill_value", C.c_float), ("enable_timings", C.c_int32), ("fft_path", C.c_int32)]
+                ("fill_value", C.c_float), ("enable_timings", C.c_int32), ("fft_path", C.c_int32),
+                ("whiten", C.c_int32), ("n_zap_ranges", C.c_uint32), ("zap_ranges", C.c_void_p)]
 
 
 class Timings(C.Structure):
@@ -52,7 +53,7 @@ class Timings(C.Structure):
 EXPORTS = ["tb_plan_create", "tb_plan_set_series", "tb_search_templates", "tb_get_candidates", "tb_clear_candidates", "tb_plan_destroy",
            "tb_reduce_candidates", "tb_debug_set_candidates",
            "tb_strerror", "tb_last_error", "tb_get_timings", "tb_debug_resample_indices", "tb_debug_spectrum",
-           "tb_debug_resampled", "tb_debug_hsums", "tb_sigma_to_power", "tb_plan_info", "tb_template_knot_log2"]
+           "tb_debug_resampled", "tb_debug_hsums", "tb_debug_series", "tb_sigma_to_power", "tb_plan_info", "tb_template_knot_log2"]
 
 _vp, _u64, _u32 = C.c_void_p, C.c_uint64, C.c_uint32
 lib.tb_plan_create.argtypes = [C.POINTER(_vp), _vp, _u64, C.c_double, C.POINTER(PlanOpts)]
@@ -72,6 +73,7 @@ lib.tb_debug_resample_indices.argtypes = [_vp, _vp, _vp]
 lib.tb_debug_spectrum.argtypes = [_vp, _vp, _vp, _vp, _vp]
 lib.tb_debug_resampled.argtypes = [_vp, _vp, _vp]
 lib.tb_debug_hsums.argtypes = [_vp, _vp, _vp]
+lib.tb_debug_series.argtypes = [_vp, _vp, C.POINTER(C.c_double)]
 lib.tb_sigma_to_power.argtypes = [_u32, C.c_double, C.POINTER(C.c_double)]
 lib.tb_plan_info.argtypes = [_vp, C.POINTER(C.c_float), C.POINTER(_u32), C.POINTER(_u32)]
 lib.tb_template_knot_log2.argtypes = [_vp, _vp, C.POINTER(C.c_int32)]
@@ -103,7 +105,7 @@ def as_templates(templates) -> np.ndarray:
 
 def tb_plan_create(series, n_samples, tsamp_s, *, device=0, stream=None, median_window=0, f_min_hz=0.0,
                    max_candidates=0, chunk_templates=0, series_is_device_ptr=False, fill_value=None,
-                   enable_timings=False, fft_path=0):
+                   enable_timings=False, fft_path=0, whiten=False, zap_ranges=()):
     """series: numpy float32[N] (host) or an integer device address when series_is_device_ptr."""
     o = PlanOpts()
     o.struct_size = C.sizeof(PlanOpts)
@@ -113,6 +115,9 @@ def tb_plan_create(series, n_samples, tsamp_s, *, device=0, stream=None, median_
     o.has_fill, o.fill_value = (0, 0.0) if fill_value is None else (1, float(fill_value))
     o.enable_timings = int(bool(enable_timings))
     o.fft_path = int(fft_path)
+    o.whiten = int(bool(whiten))
+    zap = np.ascontiguousarray(np.asarray(zap_ranges, dtype=np.uint32).reshape(-1, 2))
+    o.n_zap_ranges, o.zap_ranges = len(zap), (zap.ctypes.data if len(zap) else None)
     if series_is_device_ptr:
         ptr = int(series)
     else:
@@ -224,6 +229,14 @@ def tb_debug_resampled(plan, template, n_samples) -> np.ndarray:
     return out
 
 
+def tb_debug_series(plan, n_samples):
+    """(the plan's working series float32[N] -- whitened if the plan whitens --, kappa)."""
+    x = np.empty(int(n_samples), dtype=np.float32)
+    k = C.c_double()
+    _check(lib.tb_debug_series(plan, x.ctypes.data, C.byref(k)), plan)
+    return x, k.value
+
+
 def tb_debug_hsums(plan, template, n_samples) -> np.ndarray:
     """float32[5, N/2]: S_L[k] of every fold and bin through the production harmonic summer."""
     t = as_templates(template)
@@ -291,6 +304,9 @@ class Plan:
 
     def debug_resampled(self, template):
         return tb_debug_resampled(self.handle, template, self.n_samples)
+
+    def debug_series(self):
+        return tb_debug_series(self.handle, self.n_samples)
 
     def debug_hsums(self, template):
         return tb_debug_hsums(self.handle, template, self.n_samples)

@@ -47,18 +47,31 @@ def check_indices(plan, wl, tmpl):
     return idx_gpu, compare_indices(idx_gpu, wl.n_samples, wl.tsamp, tmpl)
 
 
-def compare_template(series, tsamp, tmpl, tid, W, fill, k_lo, f_min, gpu, sigma_threshold, folds, gpu_cands):
+WHITE_ATOL = 3e-5                           # |x'_gpu - x'_oracle| of a whitened (unit-variance) series: two fp32 FFTs of length N
+
+
+def compare_template(series, tsamp, tmpl, tid, W, fill, k_lo, f_min, gpu, sigma_threshold, folds, gpu_cands, kappa=None):
     """All comparisons for one template.  gpu: dict with idx, y, P, Ph, med and optionally S
-    (float32[5, Nb]).  Returns a small report dict; raises AssertionError on a parity failure."""
+    (float32[5, Nb]).  Returns a small report dict; raises AssertionError on a parity failure.
+    kappa: None for the default path (per-template block medians, G15); for a whitened plan (reading
+    G25) `series` is the ORACLE's whitened series and kappa the oracle's constant: the gathered
+    series may then differ from the GPU's by the rounding of the whitening FFTs (WHITE_ATOL)."""
     n = len(series)
     n_flips = compare_indices(gpu["idx"], n, tsamp, tmpl)
-    spec = orc.spectrum_of_template(series, tsamp, tmpl, W, fill, idx=gpu["idx"])
-    assert np.array_equal(gpu["y"], spec["resampled"]), "resampled series differs"
     nb = n // 2
-    base = orc.median_baseline(spec["medians"], nb, W)
+    if kappa is None:
+        spec = orc.spectrum_of_template(series, tsamp, tmpl, W, fill, idx=gpu["idx"])
+        assert np.array_equal(gpu["y"], spec["resampled"]), "resampled series differs"
+        base = orc.median_baseline(spec["medians"], nb, W)
+        eM = np.abs(gpu["med"].astype(np.float64) - spec["medians"]) / spec["medians"]
+    else:
+        spec = orc.spectrum_of_template_whitened(series, kappa, tsamp, tmpl, fill, idx=gpu["idx"])
+        dy = np.abs(gpu["y"].astype(np.float64) - spec["resampled"])
+        assert dy.max() <= WHITE_ATOL, f"resampled whitened series differs by {dy.max():.3g}"
+        base = np.full(nb, orc.LN2 / kappa)
+        eM = np.abs(gpu["med"].astype(np.float64) - orc.LN2 / kappa) / (orc.LN2 / kappa)     # the tap reports ln2 / kappa
     eP = np.abs(gpu["P"].astype(np.float64) - spec["power"]) / np.maximum(spec["power"], base)
     eH = np.abs(gpu["Ph"].astype(np.float64) - spec["normalised"]) / np.maximum(spec["normalised"], 1.0)
-    eM = np.abs(gpu["med"].astype(np.float64) - spec["medians"]) / spec["medians"]
     assert eP.max() <= REL_TOL, f"interbinned spectrum off by {eP.max():.3g} at bin {eP.argmax()}"
     assert eM.max() <= REL_TOL, f"block median off by {eM.max():.3g} at block {eM.argmax()}"
     assert eH.max() <= REL_TOL, f"normalised spectrum off by {eH.max():.3g} at bin {eH.argmax()}"
@@ -90,14 +103,17 @@ def gpu_outputs(plan, tmpl, hsums=False):
     return out
 
 
-def check_template(plan, wl, tid, sigma_threshold=None, folds=None, gpu_cands=None, hsums=False):
-    """Full per-template parity in this process; returns a small report dict."""
+def check_template(plan, wl, tid, sigma_threshold=None, folds=None, gpu_cands=None, hsums=False, white=None):
+    """Full per-template parity in this process; returns a small report dict.
+    white: (oracle's whitened series, oracle's kappa) for a plan created with whiten=True."""
     tmpl = wl.templates[tid]
     folds = wl.folds if folds is None else folds
     sigma_threshold = wl.sigma_threshold if sigma_threshold is None else sigma_threshold
     info = plan.info()
-    return compare_template(wl.series, wl.tsamp, tmpl, tid, plan.median_window, info["fill_value"], info["k_lo"], wl.f_min,
-                            gpu_outputs(plan, tmpl, hsums), sigma_threshold, folds, gpu_cands)
+    series, kappa = (wl.series, None) if white is None else white
+    fill = info["fill_value"] if white is None else orc.fill_value(series)
+    return compare_template(series, wl.tsamp, tmpl, tid, plan.median_window, fill, info["k_lo"], wl.f_min,
+                            gpu_outputs(plan, tmpl, hsums), sigma_threshold, folds, gpu_cands, kappa)
 
 
 def compare_candidates(gpu_cands, ocand, sums, sigma_threshold):
@@ -143,7 +159,7 @@ def _pool_job(job):
             gpu["S"] = np.load(os.path.join(path, "S.npy"))
         cands = np.load(os.path.join(path, "cands.npy")) if os.path.exists(os.path.join(path, "cands.npy")) else None
         rep = compare_template(c["series"], c["tsamp"], c["templates"][tid], slot, c["W"], c["fill"], c["k_lo"], c["f_min"],
-                               gpu, c["sigma"], c["folds"], cands)
+                               gpu, c["sigma"], c["folds"], cands, c["kappa"])
         return tid, rep, None
     except AssertionError as e:
         return tid, None, f"template {tid}: {e}"
@@ -164,7 +180,7 @@ def default_workers(n_samples):
     return int(max(1, min(cores, 32, 0.6 * avail_gb / max(per_worker_gb, 1e-3))))
 
 
-def pooled_parity(plan, wl, ids, sigma_threshold, folds, per_cands, hsums_ids=(), slots=None, workers=None):
+def pooled_parity(plan, wl, ids, sigma_threshold, folds, per_cands, hsums_ids=(), slots=None, workers=None, white=None):
     """check_template for many templates with the oracle in a pool of forked workers.
     ids: template indices into wl.templates; per_cands: {slot id -> candidate rows} of the GPU (a
     template without an entry is compared against an empty list); slots: the template_id each of
@@ -173,7 +189,9 @@ def pooled_parity(plan, wl, ids, sigma_threshold, folds, per_cands, hsums_ids=()
     slots = dict(zip(ids, ids if slots is None else slots))
     info = plan.info()
     _CTX.clear()
-    _CTX.update(series=wl.series, tsamp=wl.tsamp, templates=wl.templates, W=plan.median_window, fill=info["fill_value"],
+    series, kappa = (wl.series, None) if white is None else white
+    _CTX.update(series=series, tsamp=wl.tsamp, templates=wl.templates, W=plan.median_window,
+                fill=info["fill_value"] if white is None else orc.fill_value(series), kappa=kappa,
                 k_lo=info["k_lo"], f_min=wl.f_min, sigma=sigma_threshold, folds=tuple(folds))
     workers = workers or default_workers(wl.n_samples)
     shm = "/dev/shm" if os.path.isdir("/dev/shm") else None
