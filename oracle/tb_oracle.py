@@ -84,7 +84,52 @@ def is_circular(tmpl) -> bool:
     return float(tmpl[3]) == 0.0 and float(tmpl[4]) == 0.0
 
 
-def roemer_delay(j, tsamp, tmpl, dtype=np.float64, force_kepler=False):
+# Appendix B of the paper: coefficients of the e-series of eqs 15-16 (L106-111),
+#   cos E = sum_k C_k(e) cos kM,   sqrt(1 - e^2) sin E = sum_k S_k(e) sin kM,
+# as {k: ((power of e, numerator, denominator), ...)}, "up-to the 7th power in e" = terms through e^6
+# of the ELL7 model (L668).  tests/test_oracle_pins.py checks this table against the same numbers
+# typed independently into tests/golden/appendix_b_series.txt.
+ELL_C = {0: ((1, -1, 2),),
+         1: ((0, 1, 1), (2, -3, 8), (4, 5, 192), (6, -7, 9216)),
+         2: ((1, 1, 2), (3, -1, 3), (5, 1, 16)),
+         3: ((2, 3, 8), (4, -45, 128), (6, 567, 5120)),
+         4: ((3, 1, 3), (5, -2, 5)),
+         5: ((4, 125, 384), (6, -4375, 9216)),
+         6: ((5, 27, 80),),
+         7: ((6, 16807, 46080),)}
+ELL_S = {1: ((0, 1, 1), (2, -5, 8), (4, -11, 192), (6, -457, 9216)),
+         2: ((1, 1, 2), (3, -5, 12), (5, 1, 24)),
+         3: ((2, 3, 8), (4, -51, 128), (6, 543, 5120)),
+         4: ((3, 1, 3), (5, -13, 30)),
+         5: ((4, 125, 384), (6, -4625, 9216)),
+         6: ((5, 27, 80),),
+         7: ((6, 16807, 46080),)}
+
+
+def ell_coefficients(ecc, dtype=np.float64):
+    """(C_k(e), k = 0..7), (S_k(e), k = 1..7) of Appendix B as arrays of `dtype`."""
+    e = dtype(float(ecc))
+    C = [sum(dtype(num) / dtype(den) * e ** pw for pw, num, den in ELL_C[k]) for k in range(8)]
+    S = [sum(dtype(num) / dtype(den) * e ** pw for pw, num, den in ELL_S[k]) for k in range(1, 8)]
+    return C, S
+
+
+def roemer_delay_ell(j, tsamp, tmpl, dtype=np.float64):
+    """SURVEY 8(f) row f4, reading G26: the ELL7 approximate-orbit delay.  Eq A1 with
+    cos E and sqrt(1-e^2) sin E replaced by the printed series of eqs 15-16 (L106-111, L668: "The
+    alternative is to expand cos E and sin E as a power series ... ELL1 ... ELL2 and so on"):
+        Delta = tau[(sum_{k=0}^{7} C_k cos kM - e) sin(omega) + (sum_{k=1}^{7} S_k sin kM) cos(omega)],
+    M = Omega t + phi0.  No Kepler solve.  Differs from the BT delay by about 1.2 e^7 tau."""
+    p_orb, tau, phi0, ecc, omega = (dtype(float(v)) for v in tmpl)
+    t = np.asarray(j).astype(dtype) * dtype(float(tsamp))
+    M = (_two_pi(dtype) / p_orb) * t + phi0
+    C, S = ell_coefficients(float(tmpl[3]), dtype)
+    cosE = sum(C[k] * np.cos(dtype(k) * M) for k in range(8))
+    qsinE = sum(S[k - 1] * np.sin(dtype(k) * M) for k in range(1, 8))
+    return tau * ((cosE - ecc) * np.sin(omega) + qsinE * np.cos(omega))
+
+
+def roemer_delay(j, tsamp, tmpl, dtype=np.float64, force_kepler=False, model="bt"):
     """Roemer delay Delta_R(t = j*tsamp) in seconds.
 
     tmpl = (P_orb [s], tau = a sin(i)/c [lt-s], phi0 [rad], e, omega [rad]); the paper's
@@ -92,7 +137,10 @@ def roemer_delay(j, tsamp, tmpl, dtype=np.float64, force_kepler=False):
       M   = Omega t + phi0,  Omega = 2 pi / P_orb            (eq 3; Alg. 1, reading G1)
       circular:   Delta = tau sin(M)                         (eq A1 L666 at e = 0, psi = 0; G6)
       elliptical: Delta = tau[(cos E - e) sin(omega) + sqrt(1-e^2) sin E cos(omega)]   (eq A1)
+    model = "bt" (the paper's resampler, L668: "we implemented the BT model") or "ell" (roemer_delay_ell).
     """
+    if model == "ell":
+        return roemer_delay_ell(j, tsamp, tmpl, dtype)
     p_orb, tau, phi0, ecc, omega = (dtype(float(v)) for v in tmpl)
     t = np.asarray(j).astype(dtype) * dtype(float(tsamp))
     M = (_two_pi(dtype) / p_orb) * t + phi0
@@ -102,30 +150,30 @@ def roemer_delay(j, tsamp, tmpl, dtype=np.float64, force_kepler=False):
     return tau * ((np.cos(E) - ecc) * np.sin(omega) + np.sqrt(1 - ecc * ecc) * np.sin(E) * np.cos(omega))
 
 
-def shift_in_samples(j, tsamp, tmpl, dtype=np.float64, force_kepler=False):
+def shift_in_samples(j, tsamp, tmpl, dtype=np.float64, force_kepler=False, model="bt"):
     """delta_j = (Delta_R(j tsamp) - Delta_R(0)) / tsamp  (zero offset t0: PAPER.md:L675,
     Alg. 1; sign reading G2: the offset is subtracted from the delay so delta_0 = 0)."""
-    d = roemer_delay(j, tsamp, tmpl, dtype, force_kepler)
-    d0 = roemer_delay(np.zeros(1, dtype=np.int64), tsamp, tmpl, dtype, force_kepler)[0]
+    d = roemer_delay(j, tsamp, tmpl, dtype, force_kepler, model)
+    d0 = roemer_delay(np.zeros(1, dtype=np.int64), tsamp, tmpl, dtype, force_kepler, model)[0]
     return (d - d0) / dtype(float(tsamp))
 
 
-def tie_distance(j, tsamp, tmpl):
+def tie_distance(j, tsamp, tmpl, model="bt"):
     """Arbiter: |frac(delta_j) - 1/2| evaluated in extended precision for the sample numbers j."""
-    d = shift_in_samples(np.asarray(j, dtype=np.int64), tsamp, tmpl, np.longdouble)
+    d = shift_in_samples(np.asarray(j, dtype=np.int64), tsamp, tmpl, np.longdouble, model=model)
     return np.abs((d - np.floor(d)) - np.longdouble(0.5)).astype(np.float64)
 
 
-def resample_indices(n_samples, tsamp, tmpl, force_kepler=False):
+def resample_indices(n_samples, tsamp, tmpl, force_kepler=False, model="bt"):
     """idx_j = j - floor(delta_j + 1/2), j = 0..N-1  (Alg. 1 "[.]_int", prose L675
     "nearest integer"; readings G3 = gather evaluated at the output index, G7 = round delta,
     never j - delta).  Returns int64[N]; entries may lie outside [0, N)."""
     j = np.arange(int(n_samples), dtype=np.int64)
-    d = shift_in_samples(j, tsamp, tmpl, np.float64, force_kepler)
+    d = shift_in_samples(j, tsamp, tmpl, np.float64, force_kepler, model)
     s = np.floor(d + 0.5).astype(np.int64)
     near = np.abs((d - np.floor(d)) - 0.5) < TIE_GUARD
     if near.any():
-        dl = shift_in_samples(j[near], tsamp, tmpl, np.longdouble, force_kepler)
+        dl = shift_in_samples(j[near], tsamp, tmpl, np.longdouble, force_kepler, model)
         s[near] = np.floor(dl + np.longdouble(0.5)).astype(np.int64)
     return j - s
 

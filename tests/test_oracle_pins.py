@@ -485,3 +485,42 @@ def test_t10_on_the_whitened_series(c1):
     best = max(cands, key=lambda c: c[4])
     assert (best[1], best[2]) == (3, 52429) and best[4] > 12.0
     assert orc.search_template_whitened(xw, kappa, c1.tsamp, c1.templates[5], 1) == []
+
+
+# ------------------------------------------------------------------ f4: the ELL7 approximate-orbit delay (reading G26)
+def test_ell_table_is_the_printed_appendix_b():
+    """The oracle's coefficient table against the numbers typed independently into the golden file
+    from PAPER.md:L719-747."""
+    C, S = _load_series()
+    assert {k: sorted((pw, fr.numerator, fr.denominator) for pw, fr in v) for k, v in C.items()} == \
+           {k: sorted(tuple(t) for t in v) for k, v in orc.ELL_C.items()}
+    assert {k: sorted((pw, fr.numerator, fr.denominator) for pw, fr in v) for k, v in S.items()} == \
+           {k: sorted(tuple(t) for t in v) for k, v in orc.ELL_S.items()}
+
+
+def test_ell_delay_against_the_kepler_solve_and_closed_forms():
+    tsamp, p_orb, tau, phi0 = 1e-3, 41.0, 3.0, 0.9
+    j = np.arange(0, 60000, 11)
+    for e in (0.0, 0.02, 0.1):
+        for om in (0.0, 0.7, 2.9, 5.1):
+            tm = (p_orb, tau, phi0, e, om)
+            ell = orc.roemer_delay(j, tsamp, tm, model="ell")
+            bt = orc.roemer_delay(j, tsamp, tm, force_kepler=True)
+            assert np.max(np.abs(ell - bt)) < (2.0 * e**7 * (abs(math.sin(om)) + abs(math.cos(om))) + 2e-15) * tau
+    # e = 0: C_1 = S_1 = 1, everything else 0: tau sin(M + omega) exactly (eq A1 at e = 0)
+    M = 2 * np.pi / p_orb * (j * tsamp) + phi0
+    assert np.max(np.abs(orc.roemer_delay(j, tsamp, (p_orb, tau, phi0, 0.0, 1.3), model="ell") - tau * np.sin(M + 1.3))) < 1e-14 * tau
+    # first order in e by hand: cos E = cos M + e (cos 2M - 1)/2 + O(e^2), sqrt(1-e^2) sin E = sin M + e sin 2M / 2 + O(e^2)
+    e = 1e-4
+    d = orc.roemer_delay(j, tsamp, (p_orb, tau, phi0, e, 0.4), model="ell")
+    first = tau * ((np.cos(M) + e * (np.cos(2 * M) - 1) / 2 - e) * math.sin(0.4) + (np.sin(M) + e * np.sin(2 * M) / 2) * math.cos(0.4))
+    assert np.max(np.abs(d - first)) < 2.0 * e * e * tau
+    # and the index map: identical to BT's except where the 1.2 e^7 tau / tsamp difference crosses a rounding tie
+    tm = (p_orb, 0.5, phi0, 0.05, 0.7)
+    a = orc.resample_indices(1 << 15, tsamp, tm, model="ell")
+    b = orc.resample_indices(1 << 15, tsamp, tm)
+    assert a[0] == 0 and np.count_nonzero(a != b) <= 2 and np.max(np.abs(a - b)) <= 1
+    tm = (400.0, 20.0, phi0, 0.3, 0.7)                      # e = 0.3: the truncation, 1.2 e^7 tau / tsamp = 5 samples, is visible
+    a = orc.resample_indices(1 << 18, tsamp, tm, model="ell")
+    b = orc.resample_indices(1 << 18, tsamp, tm)
+    assert np.count_nonzero(a != b) > 1000 and 2 <= np.max(np.abs(a - b)) <= 8
