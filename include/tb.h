@@ -117,6 +117,11 @@ typedef struct {
                                      interbinned spectrum of x' -- step a6 leaves the per-template loop */
     uint32_t n_zap_ranges;        /* number of zapped bin ranges (used only when whiten is set) */
     const uint32_t* zap_ranges;   /* host, 2 * n_zap_ranges values: [lo, hi) pairs, lo < hi <= N/2; copied */
+    int32_t  delay_model;         /* 0: the paper's resampler, eq A1 with the Kepler solve ("BT model", L668);
+                                     1: the ELL7 approximate orbit (eqs 15-16, App. B; reading
+                                     G26): cos E and sqrt(1-e^2) sin E from the printed series through e^6, no Kepler
+                                     solve; differs from 0 by about 1.2 e^7 tau (0.015 samples at e = 0.1, tau/tsamp =
+                                     1.25e5), so a mode of its own with its own oracle, not bit-compatible with 0 */
 } tb_plan_opts;
 
 /* Per-stage device time of the last tb_search_templates call (CUDA events on the plan's stream,

@@ -66,6 +66,9 @@ struct tb_plan {
     size_t tmpl_cap = 0;
     TmplDev* h_tmpl = nullptr;                       // pinned staging
     size_t h_tmpl_cap = 0;
+    bool ell = false;                                // delay_model 1: ELL7 series instead of the Kepler solve (f4)
+    EllCoef* d_ell = nullptr;                        // [tmpl_cap], staged with the templates
+    EllCoef* h_ell = nullptr;
     cudaEvent_t ev_staged = nullptr;                 // the last template upload has been consumed
     bool staged_pending = false;
 
@@ -159,10 +162,32 @@ void sigma_constants(uint32_t fold, double* mu, double* s)
 // h = 2^l <= 128 with  (h w)^4 / 384 * (tau/tsamp) * K(e) <= 2e-11 samples, where
 // K(e) = R^4 + 11 e R^5 + 25 e^2 R^6 + 15 e^3 R^7, R = 1/(1-e), bounds the 4th derivative of
 // A cos E + B sin E with respect to the mean anomaly.
-int knot_log2(double tau_over_tsamp, double w, double e)
+// Appendix B of the paper: {power of e, numerator, denominator} of C_k, S_k, k = 1..7
+struct EllTerm { int k, pw; double num, den; };
+const EllTerm ELL_C_TERMS[] = {{1, 0, 1, 1}, {1, 2, -3, 8}, {1, 4, 5, 192}, {1, 6, -7, 9216}, {2, 1, 1, 2}, {2, 3, -1, 3}, {2, 5, 1, 16},
+                               {3, 2, 3, 8}, {3, 4, -45, 128}, {3, 6, 567, 5120}, {4, 3, 1, 3}, {4, 5, -2, 5}, {5, 4, 125, 384},
+                               {5, 6, -4375, 9216}, {6, 5, 27, 80}, {7, 6, 16807, 46080}};
+const EllTerm ELL_S_TERMS[] = {{1, 0, 1, 1}, {1, 2, -5, 8}, {1, 4, -11, 192}, {1, 6, -457, 9216}, {2, 1, 1, 2}, {2, 3, -5, 12}, {2, 5, 1, 24},
+                               {3, 2, 3, 8}, {3, 4, -51, 128}, {3, 6, 543, 5120}, {4, 3, 1, 3}, {4, 5, -13, 30}, {5, 4, 125, 384},
+                               {5, 6, -4625, 9216}, {6, 5, 27, 80}, {7, 6, 16807, 46080}};
+
+void ell_coefficients(double ecc, long double (&C)[8], long double (&S)[8])      // C[k], S[k], k = 1..7
+{
+    for (int k = 0; k < 8; ++k) C[k] = S[k] = 0.0L;
+    for (const EllTerm& t : ELL_C_TERMS) C[t.k] += (long double)t.num / (long double)t.den * powl((long double)ecc, t.pw);
+    for (const EllTerm& t : ELL_S_TERMS) S[t.k] += (long double)t.num / (long double)t.den * powl((long double)ecc, t.pw);
+}
+
+int knot_log2(double tau_over_tsamp, double w, double e, bool ell = false)
 {
     const double R = 1.0 / (1.0 - e);
-    const double K = std::pow(R, 4) + 11 * e * std::pow(R, 5) + 25 * e * e * std::pow(R, 6) + 15 * e * e * e * std::pow(R, 7);
+    double K = std::pow(R, 4) + 11 * e * std::pow(R, 5) + 25 * e * e * std::pow(R, 6) + 15 * e * e * e * std::pow(R, 7);
+    if (ell) {                                       // 4th derivative of the series: sum k^4 (|C_k| + |S_k|)
+        long double C[8], S[8];
+        ell_coefficients(e, C, S);
+        K = 0.0;
+        for (int k = 1; k <= 7; ++k) K += std::pow((double)k, 4) * (double)(fabsl(C[k]) + fabsl(S[k]));
+    }
     int l = 7;
     for (; l > 0; --l) {
         const double hw = std::ldexp(w, l);
@@ -183,16 +208,16 @@ int validate_template(const tb_template& t, double tsamp, std::string* why)
 }
 
 // knot spacing of one template (the same expressions as make_tmpl, without the trigonometry)
-int tmpl_log2h(const tb_template& t, double tsamp)
+int tmpl_log2h(const tb_template& t, double tsamp, bool ell)
 {
     const long double two_pi = 8.0L * atanl(1.0L);
     const long double c = (long double)tsamp / (long double)t.p_orb_s;
     const long double g = (long double)t.tau_lts / (long double)tsamp;
-    return knot_log2((double)g, (double)(two_pi * c), t.ecc);
+    return knot_log2((double)g, (double)(two_pi * c), t.ecc, ell);
 }
 
 // step a1, in long double so that the constants are correctly rounded doubles
-void make_tmpl(const tb_template& t, double tsamp, TmplDev* o)
+void make_tmpl(const tb_template& t, double tsamp, TmplDev* o, EllCoef* ell = nullptr)
 {
     const long double two_pi = 8.0L * atanl(1.0L);
     const long double c = (long double)tsamp / (long double)t.p_orb_s;
@@ -219,6 +244,21 @@ void make_tmpl(const tb_template& t, double tsamp, TmplDev* o)
     }
     o->d0 = (double)((long double)o->A * cosl(E) + (long double)o->B * sinl(E));
     o->log2h = knot_log2((double)g, o->w, t.ecc);
+    if (ell) {                                       // ELL7 mode: the S-series carries sqrt(1-e^2); zero offset from the series itself
+        long double C[8], S[8];
+        ell_coefficients(t.ecc, C, S);
+        o->B = (double)(g * cosl((long double)t.omega_rad));
+        long double sc = 0.0L, ss = 0.0L;
+        for (int k = 1; k <= 7; ++k) {
+            ell->c[k - 1] = (double)C[k]; ell->s[k - 1] = (double)S[k];
+            sc += (long double)ell->c[k - 1] * cosl((long double)k * M);
+            ss += (long double)ell->s[k - 1] * sinl((long double)k * M);
+        }
+        ell->c[7] = ell->s[7] = 0.0;
+        o->d0 = (double)((long double)o->A * sc + (long double)o->B * ss);
+        o->circular = 0;
+        o->log2h = knot_log2((double)g, o->w, t.ecc, true);
+    }
 }
 
 // the fill value also sits behind the series, x[N] (4 floats of padding): the fused path clamps an
@@ -452,7 +492,7 @@ int run_own_pass1(tb_plan* p, size_t off, uint32_t nt, long long* d_idx, float* 
 {
     const int cta_per_tmpl = (int)(((p->n >> p->chunk_log2h) + 255) / 256);   // chunk_log2h: smallest knot spacing in this chunk
     k_delay_segments<<<(unsigned)(cta_per_tmpl * nt), K0_THREADS, 0, p->stream>>>(p->d_tmpl + off, (int)nt, (int)p->n, p->d_seg,
-                                                                           p->seg_stride, cta_per_tmpl);
+                                                                           p->seg_stride, cta_per_tmpl, p->ell ? p->d_ell + off : nullptr);
     TB_CUDA(p, cudaGetLastError());
     if (after_k0) TB_CUDA(p, cudaEventRecord(after_k0, p->stream));
     const bool dbg = d_idx != nullptr;
@@ -598,10 +638,10 @@ int run_resample(tb_plan* p, size_t off, uint32_t nt, long long* d_idx)
     const unsigned grid = (unsigned)((p->n / tile) * nt);
     if (d_idx)
         k_resample<true><<<grid, RS_THREADS, 0, p->stream>>>(p->d_series, p->d_resampled, p->d_tmpl + off, (int)nt,
-                                                             (int)p->n, tile, p->fill, d_idx);
+                                                             (int)p->n, tile, p->fill, d_idx, p->ell ? p->d_ell + off : nullptr);
     else
         k_resample<false><<<grid, RS_THREADS, 0, p->stream>>>(p->d_series, p->d_resampled, p->d_tmpl + off, (int)nt,
-                                                              (int)p->n, tile, p->fill, nullptr);
+                                                              (int)p->n, tile, p->fill, nullptr, p->ell ? p->d_ell + off : nullptr);
     TB_CUDA(p, cudaGetLastError());
     return TB_OK;
 }
@@ -660,7 +700,6 @@ int run_hsum(tb_plan* p, size_t off, uint32_t nt, const FoldParams& fp, float* t
 }
 
 // the fused path needs records of >= 8 samples; the rest of a bank goes through k_resample + cuFFT
-bool takes_own_path(const tb_plan* p, const tb_template& t) { return p->own_fft && tmpl_log2h(t, p->tsamp) >= OWN_MIN_LOG2H; }
 
 // Validate the bank, size the staging buffers, and split it by launch sequence (stable partition:
 // templates the fused path can take first, the others after them), so that one fast-orbit template
@@ -680,6 +719,11 @@ int upload_templates(tb_plan* p, const tb_template* tmpl, uint64_t k)
         if (p->h_tmpl) cudaFreeHost(p->h_tmpl);
         p->h_tmpl = nullptr; p->h_tmpl_cap = 0;
         TB_CUDA(p, cudaMallocHost(&p->h_tmpl, k * sizeof(TmplDev)));
+        if (p->ell) {
+            if (p->h_ell) cudaFreeHost(p->h_ell);
+            p->h_ell = nullptr;
+            TB_CUDA(p, cudaMallocHost(&p->h_ell, k * sizeof(EllCoef)));
+        }
         p->h_tmpl_cap = k;
     }
     if (k > p->tmpl_cap) {
@@ -687,6 +731,11 @@ int upload_templates(tb_plan* p, const tb_template* tmpl, uint64_t k)
         if (p->d_tmpl) cudaFree(p->d_tmpl);
         p->d_tmpl = nullptr; p->tmpl_cap = 0;
         TB_CUDA(p, cudaMalloc(&p->d_tmpl, k * sizeof(TmplDev)));
+        if (p->ell) {
+            if (p->d_ell) cudaFree(p->d_ell);
+            p->d_ell = nullptr;
+            TB_CUDA(p, cudaMalloc(&p->d_ell, k * sizeof(EllCoef)));
+        }
         p->tmpl_cap = k;
     }
     // knot spacings first (cheap): they select the launch sequence of every template and the size of
@@ -697,7 +746,7 @@ int upload_templates(tb_plan* p, const tb_template* tmpl, uint64_t k)
     size_t n_own = 0;
     int min_own = 7;
     for (uint64_t i = 0; i < k; ++i) {
-        const int l = p->own_fft ? tmpl_log2h(tmpl[i], p->tsamp) : 0;
+        const int l = p->own_fft ? tmpl_log2h(tmpl[i], p->tsamp, p->ell) : 0;
         if (p->own_fft && l >= OWN_MIN_LOG2H) { p->order[n_own++] = (uint32_t)i; min_own = std::min(min_own, l); }
         else rest.push_back((uint32_t)i);
     }
@@ -722,13 +771,14 @@ int stage_chunk(tb_plan* p, const tb_template* tmpl, uint64_t off, uint64_t nt, 
 {
     int lmin = 7;
     for (uint64_t i = off; i < off + nt; ++i) {
-        make_tmpl(tmpl[p->order[i]], p->tsamp, &p->h_tmpl[i]);
+        make_tmpl(tmpl[p->order[i]], p->tsamp, &p->h_tmpl[i], p->ell ? &p->h_ell[i] : nullptr);
         p->h_tmpl[i].id = first_id + p->order[i];
         p->h_tmpl[i].pad = 0;
         lmin = std::min(lmin, p->h_tmpl[i].log2h);
     }
     p->chunk_log2h = lmin;
     TB_CUDA(p, cudaMemcpyAsync(p->d_tmpl + off, p->h_tmpl + off, nt * sizeof(TmplDev), cudaMemcpyHostToDevice, p->stream));
+    if (p->ell) TB_CUDA(p, cudaMemcpyAsync(p->d_ell + off, p->h_ell + off, nt * sizeof(EllCoef), cudaMemcpyHostToDevice, p->stream));
     // recorded after EVERY chunk: whatever way the call ends, the next one waits for the last copy
     // out of the pinned staging buffer before it rewrites it
     TB_CUDA(p, cudaEventRecord(p->ev_staged, p->stream));
@@ -774,6 +824,8 @@ void destroy(tb_plan* p)
     cudaFree(p->d_work); cudaFree(p->d_acc); cudaFree(p->d_series_owned); cudaFree(p->d_resampled); cudaFree(p->d_fft);
     cudaFree(p->d_power); cudaFree(p->d_med); cudaFree(p->d_cand); cudaFree(p->d_cursor); cudaFree(p->d_tmpl);
     if (p->h_tmpl) cudaFreeHost(p->h_tmpl);
+    if (p->h_ell) cudaFreeHost(p->h_ell);
+    cudaFree(p->d_ell);
     if (p->own_stream && p->stream) cudaStreamDestroy(p->stream);
     delete p;
 }
@@ -848,6 +900,8 @@ int tb_plan_create(tb_plan** out, const float* series, uint64_t n_samples, doubl
     p->max_cand = o.max_candidates ? o.max_candidates : (1ull << 22);
     p->timings = o.enable_timings != 0;
     p->whiten = o.whiten != 0;
+    if (o.delay_model != 0 && o.delay_model != 1) { delete p; return TB_ERR_INVALID_ARG; }
+    p->ell = o.delay_model == 1;
     if (o.n_zap_ranges) {
         if (!o.zap_ranges) { delete p; return TB_ERR_INVALID_ARG; }
         for (uint32_t z = 0; z < o.n_zap_ranges; ++z) {
@@ -956,7 +1010,8 @@ int tb_template_knot_log2(const tb_plan* plan, const tb_template* tmpl, int32_t*
     std::string why;
     if (validate_template(*tmpl, plan->tsamp, &why)) return TB_ERR_INVALID_ARG;
     TmplDev d;
-    make_tmpl(*tmpl, plan->tsamp, &d);
+    EllCoef ec;
+    make_tmpl(*tmpl, plan->tsamp, &d, plan->ell ? &ec : nullptr);
     *log2_h = d.log2h;
     return TB_OK;
 }

@@ -186,7 +186,7 @@ __device__ __forceinline__ void fft_step2(float2* __restrict__ slot, int w, cons
 constexpr int K0_THREADS = 288;
 __global__ void __launch_bounds__(K0_THREADS)
 k_delay_segments(const TmplDev* __restrict__ tmpl, int n_tmpl, int n, SegRec* __restrict__ seg, size_t seg_stride,
-                 int cta_per_tmpl)
+                 int cta_per_tmpl, const EllCoef* __restrict__ ell)
 {
     __shared__ double s_val[257], s_slp[257];
     const int b = blockIdx.x % n_tmpl;
@@ -199,7 +199,7 @@ k_delay_segments(const TmplDev* __restrict__ tmpl, int n_tmpl, int n, SegRec* __
     if (threadIdx.x <= 256) {
         const int k = threadIdx.x;
         double v, d;
-        delay_knot(t, (s0 + k) << log2h, v, d);
+        delay_knot(t, (s0 + k) << log2h, v, d, ell ? ell + b : nullptr);
         s_val[k] = v; s_slp[k] = d * h;
     }
     __syncthreads();

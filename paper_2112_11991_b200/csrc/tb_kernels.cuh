@@ -26,6 +26,14 @@ struct TmplDev {
     uint32_t pad;
 };
 
+// ELL7 approximate-orbit mode (reading G26; eqs 15-16,
+// App. B): cos E = sum C_k(e) cos kM, sqrt(1-e^2) sin E = sum S_k(e) sin kM, k = 1..7
+// (C_0 and the -e of eq A1 are constants and cancel against the zero offset).
+struct EllCoef {
+    double c[8];         // c[k-1] = C_k(e), k = 1..7 (c[7] unused)
+    double s[8];         // s[k-1] = S_k(e)
+};
+
 struct FoldParams {
     float    thr[5];     // power threshold T_L per fold, +inf for folds not requested
     float    mu[5];      // mu_n, n = 2^L
@@ -51,7 +59,10 @@ constexpr int SP_WARPS   = 8;        // spectrum/median CTA = 8 warps, one media
 //   section 6.1: index parity error budget).  E from Newton's method on E - e sin E = M
 //   (eq 3; Alg. 1; G9), delay from eq A1 (L666).
 // ---------------------------------------------------------------------------------------------
-__device__ __forceinline__ void delay_knot(const TmplDev& t, int j, double& val, double& slope)
+//   ell != nullptr: the ELL7 series instead of the Kepler solve (then t.A = (tau/tsamp) sin(omega),
+//   t.B = (tau/tsamp) cos(omega): the S-series carries the sqrt(1-e^2)); cos kM, sin kM by the
+//   Chebyshev recurrence from one sincos.
+__device__ __forceinline__ void delay_knot(const TmplDev& t, int j, double& val, double& slope, const EllCoef* __restrict__ ell = nullptr)
 {
     const double TWO_PI_HI = 6.283185307179586232;      // fl(2 pi)
     const double TWO_PI_LO = 2.449293598294706414e-16;  // 2 pi - fl(2 pi)
@@ -68,6 +79,26 @@ __device__ __forceinline__ void delay_knot(const TmplDev& t, int j, double& val,
     const double bb  = M - m;
     const double Mlo = ((m - (M - bb)) + (t.phi0 - bb)) + me;
 
+    if (ell) {
+        double s1, c1;
+        sincos(M, &s1, &c1);
+        const double two_c = 2.0 * c1;
+        double cp = 1.0, sp = 0.0, ck = c1, sk = s1;                     // (cos, sin) of (k-1) M and k M
+        double sumC = ell->c[0] * c1, sumS = ell->s[0] * s1;             // sum C_k cos kM, sum S_k sin kM
+        double dC = -ell->c[0] * s1, dS = ell->s[0] * c1;                // their derivatives with respect to M
+#pragma unroll
+        for (int k = 2; k <= 7; ++k) {
+            const double cn = fma(two_c, ck, -cp), sn = fma(two_c, sk, -sp);
+            cp = ck; sp = sk; ck = cn; sk = sn;
+            const double Ck = ell->c[k - 1], Sk = ell->s[k - 1];
+            sumC = fma(Ck, cn, sumC); sumS = fma(Sk, sn, sumS);
+            dC = fma(-(double)k * Ck, sn, dC); dS = fma((double)k * Sk, cn, dS);
+        }
+        const double dv = fma(t.A, dC, t.B * dS);                        // d(delay)/dM
+        val   = fma(dv, Mlo, fma(t.A, sumC, fma(t.B, sumS, -t.d0)));
+        slope = dv * t.w;
+        return;
+    }
     double sE, cE, r;
     if (t.circular) {
         sincos(M, &sE, &cE);
@@ -122,7 +153,7 @@ __device__ __forceinline__ int floor_to_int(double x)
 template <bool DEBUG_IDX>
 __global__ void __launch_bounds__(RS_THREADS)
 k_resample(const float* __restrict__ x, float* __restrict__ y, const TmplDev* __restrict__ tmpl,
-           int n_tmpl, int n, int tile, float fill, long long* __restrict__ idx_out)
+           int n_tmpl, int n, int tile, float fill, long long* __restrict__ idx_out, const EllCoef* __restrict__ ell)
 {
     __shared__ double s_val[RS_MAXSEG + 1];
     __shared__ double s_slp[RS_MAXSEG + 1];
@@ -144,7 +175,7 @@ k_resample(const float* __restrict__ x, float* __restrict__ y, const TmplDev* __
         if (jsub != tbase) __syncthreads();
         for (int k = threadIdx.x; k <= nseg; k += RS_THREADS) {
             double v, d;
-            delay_knot(t, jsub + (k << log2h), v, d);
+            delay_knot(t, jsub + (k << log2h), v, d, ell ? ell + b : nullptr);
             s_val[k] = v;
             s_slp[k] = d * (double)h;
         }

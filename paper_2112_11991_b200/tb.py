@@ -35,7 +35,8 @@ class PlanOpts(C.Structure):
                 ("median_window", C.c_uint32), ("f_min_hz", C.c_double), ("max_candidates", C.c_uint64),
                 ("chunk_templates", C.c_uint32), ("series_is_device_ptr", C.c_int32), ("has_fill", C.c_int32),
                 ("fill_value", C.c_float), ("enable_timings", C.c_int32), ("fft_path", C.c_int32),
-                ("whiten", C.c_int32), ("n_zap_ranges", C.c_uint32), ("zap_ranges", C.c_void_p)]
+                ("whiten", C.c_int32), ("n_zap_ranges", C.c_uint32), ("zap_ranges", C.c_void_p),
+                ("delay_model", C.c_int32)]
 
 
 class Timings(C.Structure):
@@ -105,7 +106,7 @@ def as_templates(templates) -> np.ndarray:
 
 def tb_plan_create(series, n_samples, tsamp_s, *, device=0, stream=None, median_window=0, f_min_hz=0.0,
                    max_candidates=0, chunk_templates=0, series_is_device_ptr=False, fill_value=None,
-                   enable_timings=False, fft_path=0, whiten=False, zap_ranges=()):
+                   enable_timings=False, fft_path=0, whiten=False, zap_ranges=(), delay_model=0):
     """series: numpy float32[N] (host) or an integer device address when series_is_device_ptr."""
     o = PlanOpts()
     o.struct_size = C.sizeof(PlanOpts)
@@ -116,6 +117,7 @@ def tb_plan_create(series, n_samples, tsamp_s, *, device=0, stream=None, median_
     o.enable_timings = int(bool(enable_timings))
     o.fft_path = int(fft_path)
     o.whiten = int(bool(whiten))
+    o.delay_model = int(delay_model)
     zap = np.ascontiguousarray(np.asarray(zap_ranges, dtype=np.uint32).reshape(-1, 2))
     o.n_zap_ranges, o.zap_ranges = len(zap), (zap.ctypes.data if len(zap) else None)
     if series_is_device_ptr:

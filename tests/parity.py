@@ -31,33 +31,33 @@ SIGMA_BAND = 1e-3
 SUMMARY = []                                # one line per full-size comparison, printed by conftest at the end of the run
 
 
-def compare_indices(idx_gpu, n_samples, tsamp, tmpl):
-    idx_orc = orc.resample_indices(n_samples, tsamp, tmpl)
+def compare_indices(idx_gpu, n_samples, tsamp, tmpl, model="bt"):
+    idx_orc = orc.resample_indices(n_samples, tsamp, tmpl, model=model)
     mism = np.nonzero(idx_gpu != idx_orc)[0]
     if mism.size:
         assert mism.size <= 8, f"{mism.size} index mismatches (first at j={mism[0]})"
         assert np.all(np.abs(idx_gpu[mism] - idx_orc[mism]) == 1)
-        dist = orc.tie_distance(mism, tsamp, tmpl)
+        dist = orc.tie_distance(mism, tsamp, tmpl, model)
         assert np.all(dist < TIE_WINDOW), f"index mismatch outside the tie window: j={mism}, dist={dist}"
     return int(mism.size)
 
 
-def check_indices(plan, wl, tmpl):
+def check_indices(plan, wl, tmpl, model="bt"):
     idx_gpu = plan.debug_indices(tmpl)
-    return idx_gpu, compare_indices(idx_gpu, wl.n_samples, wl.tsamp, tmpl)
+    return idx_gpu, compare_indices(idx_gpu, wl.n_samples, wl.tsamp, tmpl, model)
 
 
 WHITE_ATOL = 3e-5                           # |x'_gpu - x'_oracle| of a whitened (unit-variance) series: two fp32 FFTs of length N
 
 
-def compare_template(series, tsamp, tmpl, tid, W, fill, k_lo, f_min, gpu, sigma_threshold, folds, gpu_cands, kappa=None):
+def compare_template(series, tsamp, tmpl, tid, W, fill, k_lo, f_min, gpu, sigma_threshold, folds, gpu_cands, kappa=None, model="bt"):
     """All comparisons for one template.  gpu: dict with idx, y, P, Ph, med and optionally S
     (float32[5, Nb]).  Returns a small report dict; raises AssertionError on a parity failure.
     kappa: None for the default path (per-template block medians, G15); for a whitened plan (reading
     G25) `series` is the ORACLE's whitened series and kappa the oracle's constant: the gathered
     series may then differ from the GPU's by the rounding of the whitening FFTs (WHITE_ATOL)."""
     n = len(series)
-    n_flips = compare_indices(gpu["idx"], n, tsamp, tmpl)
+    n_flips = compare_indices(gpu["idx"], n, tsamp, tmpl, model)           # model: "bt" (Kepler solve) or "ell" (plan delay_model=1)
     nb = n // 2
     if kappa is None:
         spec = orc.spectrum_of_template(series, tsamp, tmpl, W, fill, idx=gpu["idx"])
@@ -103,7 +103,7 @@ def gpu_outputs(plan, tmpl, hsums=False):
     return out
 
 
-def check_template(plan, wl, tid, sigma_threshold=None, folds=None, gpu_cands=None, hsums=False, white=None):
+def check_template(plan, wl, tid, sigma_threshold=None, folds=None, gpu_cands=None, hsums=False, white=None, model="bt"):
     """Full per-template parity in this process; returns a small report dict.
     white: (oracle's whitened series, oracle's kappa) for a plan created with whiten=True."""
     tmpl = wl.templates[tid]
@@ -113,7 +113,7 @@ def check_template(plan, wl, tid, sigma_threshold=None, folds=None, gpu_cands=No
     series, kappa = (wl.series, None) if white is None else white
     fill = info["fill_value"] if white is None else orc.fill_value(series)
     return compare_template(series, wl.tsamp, tmpl, tid, plan.median_window, fill, info["k_lo"], wl.f_min,
-                            gpu_outputs(plan, tmpl, hsums), sigma_threshold, folds, gpu_cands, kappa)
+                            gpu_outputs(plan, tmpl, hsums), sigma_threshold, folds, gpu_cands, kappa, model)
 
 
 def compare_candidates(gpu_cands, ocand, sums, sigma_threshold):
@@ -159,7 +159,7 @@ def _pool_job(job):
             gpu["S"] = np.load(os.path.join(path, "S.npy"))
         cands = np.load(os.path.join(path, "cands.npy")) if os.path.exists(os.path.join(path, "cands.npy")) else None
         rep = compare_template(c["series"], c["tsamp"], c["templates"][tid], slot, c["W"], c["fill"], c["k_lo"], c["f_min"],
-                               gpu, c["sigma"], c["folds"], cands, c["kappa"])
+                               gpu, c["sigma"], c["folds"], cands, c["kappa"], c["model"])
         return tid, rep, None
     except AssertionError as e:
         return tid, None, f"template {tid}: {e}"
@@ -180,7 +180,7 @@ def default_workers(n_samples):
     return int(max(1, min(cores, 32, 0.6 * avail_gb / max(per_worker_gb, 1e-3))))
 
 
-def pooled_parity(plan, wl, ids, sigma_threshold, folds, per_cands, hsums_ids=(), slots=None, workers=None, white=None):
+def pooled_parity(plan, wl, ids, sigma_threshold, folds, per_cands, hsums_ids=(), slots=None, workers=None, white=None, model="bt"):
     """check_template for many templates with the oracle in a pool of forked workers.
     ids: template indices into wl.templates; per_cands: {slot id -> candidate rows} of the GPU (a
     template without an entry is compared against an empty list); slots: the template_id each of
@@ -191,7 +191,7 @@ def pooled_parity(plan, wl, ids, sigma_threshold, folds, per_cands, hsums_ids=()
     _CTX.clear()
     series, kappa = (wl.series, None) if white is None else white
     _CTX.update(series=series, tsamp=wl.tsamp, templates=wl.templates, W=plan.median_window,
-                fill=info["fill_value"] if white is None else orc.fill_value(series), kappa=kappa,
+                fill=info["fill_value"] if white is None else orc.fill_value(series), kappa=kappa, model=model,
                 k_lo=info["k_lo"], f_min=wl.f_min, sigma=sigma_threshold, folds=tuple(folds))
     workers = workers or default_workers(wl.n_samples)
     shm = "/dev/shm" if os.path.isdir("/dev/shm") else None

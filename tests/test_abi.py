@@ -28,7 +28,7 @@ def test_every_declared_symbol_is_exported(tb):
 
 
 def test_struct_layouts_match_header(tb):
-    assert ctypes.sizeof(tb.PlanOpts) == 80                      # + whiten, n_zap_ranges, zap_ranges
+    assert ctypes.sizeof(tb.PlanOpts) == 88                      # + whiten, n_zap_ranges, zap_ranges, delay_model
     assert ctypes.sizeof(tb.Timings) == 6 * 8 + 7 * 8 + 2 * 8      # + ms_delay, fft_path_used
     assert tb.TEMPLATE_DTYPE.itemsize == 40 and tb.CANDIDATE_DTYPE.itemsize == 24
 
