@@ -1,0 +1,280 @@
+"""Pins for oracle/tb_bank.py (metric, density, prior box, random placement).
+
+What the paper and the mathematics fix, none of it through the CUDA path.  Citations are
+PAPER.md line numbers.  Each pin is an independent route to the quantity (finite differences of the
+exact Kepler phase, the mismatch from its definition, closed forms, 50-digit arithmetic), chosen so
+that a dropped term, a wrong sign or a transposed index in the oracle fails at least one of them.
+"""
+import math
+
+import numpy as np
+import pytest
+
+from oracle import tb_bank as bank
+from oracle import tb_oracle as orc
+
+T_OBS, F0 = 537.0, 25.0
+LAM_E = [1.3, 2 * math.pi / (0.21 * T_OBS), 0.9, 2.2, 0.05]      # tau, Omega, alpha, psi, e: 4.8 orbits
+LAM_C = LAM_E[:3]
+
+
+def exact_phase(t, f0, lam, elliptical=True):
+    """eq 1-2 (L35-41) with E from the Kepler solve of the search oracle (no e-series)."""
+    t = np.asarray(t, np.longdouble)
+    tau, om, al = (np.longdouble(v) for v in lam[:3])
+    M = om * t + al
+    if not elliptical:
+        return 2 * np.pi * np.longdouble(f0) * (t + tau * np.sin(M))
+    psi, e = np.longdouble(lam[3]), np.longdouble(lam[4])
+    E = orc.kepler_solve(M, float(lam[4]), tol=1e-18)
+    X = np.sin(psi) * np.cos(E) + np.cos(psi) * np.sqrt(1 - e * e) * np.sin(E)
+    return 8 * np.arctan(np.longdouble(1)) * np.longdouble(f0) * (t + tau * X)
+
+
+def test_series_phase_is_the_kepler_phase_to_e7():
+    t = np.linspace(0, T_OBS, 257)
+    d = np.abs(bank.phase(t, F0, LAM_E, True) - exact_phase(t, F0, LAM_E))
+    assert float(d.max()) < 2 * math.pi * F0 * LAM_E[0] * 2 * LAM_E[4] ** 7     # 2 e^7 tau (T4 of the search oracle)
+
+
+def test_derivatives_against_finite_differences_of_the_exact_phase():
+    """Every column of phase_derivatives (f0, tau, Omega, alpha, psi, e) against central differences of
+    the Kepler-solved phase; the series truncation (~e^6 in d/de) bounds the agreement."""
+    t = np.linspace(0, T_OBS, 129)
+    D = bank.phase_derivatives(t, F0, LAM_E, True).astype(np.float64)
+    steps = [1e-4, 1e-5, 1e-9, 1e-5, 1e-5, 1e-5]
+    for a in range(6):
+        def ph(s):
+            f0, lam = F0, list(LAM_E)
+            if a == 0:
+                f0 = F0 + s
+            else:
+                lam[a - 1] += s
+            return exact_phase(t, f0, lam)
+        fd = ((ph(steps[a]) - ph(-steps[a])) / (2 * steps[a])).astype(np.float64)
+        scale = np.abs(D[a]).max()
+        assert np.abs(fd - D[a]).max() < 2e-5 * scale, f"column {a}"
+    Dc = bank.phase_derivatives(t, F0, LAM_C, False).astype(np.float64)
+    M = LAM_C[1] * t + LAM_C[2]
+    assert np.allclose(Dc[1], 2 * math.pi * F0 * np.sin(M), rtol=1e-14, atol=1e-10)            # eq 4
+    assert np.allclose(Dc[2], 2 * math.pi * F0 * LAM_C[0] * t * np.cos(M), rtol=1e-14, atol=1e-8)
+
+
+def test_circular_metric_closed_forms_over_whole_orbits():
+    """Omega T = 2 pi n: <sin^2 M> = <cos^2 M> = 1/2, <sin M> = <cos M> = <sin M cos M> = 0,
+    <t sin M> = -cos(alpha)/Omega, <t^2> - <t>^2 = T^2/12  (eq 13, eq 14 L101 by hand)."""
+    n_orb, tau, al = 3, 0.7, 0.4
+    om = 2 * math.pi * n_orb / T_OBS
+    g = bank.metric(F0, [tau, om, al], T_OBS, False).astype(np.float64)
+    k = 2 * math.pi
+    assert g[1, 1] == pytest.approx((k * F0) ** 2 / 2, rel=1e-12)                               # tau tau
+    assert g[3, 3] == pytest.approx((k * F0 * tau) ** 2 / 2, rel=1e-12)                         # alpha alpha
+    assert abs(g[1, 3]) < 1e-9 * g[1, 1]                                                        # tau alpha
+    assert g[0, 1] == pytest.approx(k * k * F0 * (-math.cos(al) / om + tau / 2), rel=1e-11)     # f tau
+    assert g[0, 0] == pytest.approx(k * k * (T_OBS ** 2 / 12 + tau * tau / 2 - 2 * tau * math.cos(al) / om), rel=1e-11)
+    assert np.allclose(g, g.T, rtol=1e-13)
+
+
+def test_metric_is_the_quadratic_form_of_the_mismatch():
+    """eq 12 (L92): m(L, L + dL) = g_ab dL^a dL^b + O(dL^3), the mismatch taken from its definition on
+    the EXACT phase; single axes and axis pairs, so every element and its sign is reached."""
+    g = bank.metric(F0, LAM_E, T_OBS, True).astype(np.float64)
+    target = 2e-5                                               # small enough for the cubic term, large enough for rounding
+    unit = [math.sqrt(target / g[a, a]) for a in range(6)]
+    base = lambda t: exact_phase(t, F0, LAM_E)
+    for a in range(6):
+        for b in range(a, 6):
+            d = np.zeros(6)
+            d[a] += unit[a]
+            d[b] += unit[b] * (1.0 if a != b else 0.0)
+            shifted = lambda t, d=d: exact_phase(t, F0 + d[0], [LAM_E[i] + d[i + 1] for i in range(5)])
+            m = bank.mismatch_direct(T_OBS, base, shifted)
+            q = float(d @ g @ d)
+            assert m == pytest.approx(q, rel=3e-2, abs=2e-8), f"axes {a},{b}: mismatch {m}, metric {q}"
+
+
+def test_projection_is_the_minimum_over_frequency():
+    """eq 22 (L142): gamma_ab dl^a dl^b is the mismatch left after the spin frequency is re-fitted
+    (the FFT searches it, L140): minimise the direct mismatch over a frequency offset numerically."""
+    from scipy.optimize import minimize_scalar
+    g = bank.metric(F0, LAM_E, T_OBS, True).astype(np.float64)
+    gam = bank.projected_metric(g)
+    rng = np.random.default_rng(5)
+    base = lambda t: exact_phase(t, F0, LAM_E)
+    for _ in range(3):
+        d = rng.standard_normal(5)
+        d *= math.sqrt(2e-5 / float(d @ gam @ d))
+        df0 = -float(g[0, 1:] @ d) / g[0, 0]
+        f = lambda df: bank.mismatch_direct(T_OBS, base, lambda t: exact_phase(t, F0 + df, [LAM_E[i] + d[i] for i in range(5)]), 256)
+        w = 3 * math.sqrt(2e-5 / g[0, 0])
+        res = minimize_scalar(f, bounds=(df0 - w, df0 + w), method="bounded", options={"xatol": 1e-12})
+        assert res.fun == pytest.approx(2e-5, rel=3e-2)
+        assert res.x == pytest.approx(df0, abs=0.05 * w)
+    assert np.allclose(gam, gam.T, rtol=1e-12) and np.all(np.linalg.eigvalsh(gam / np.sqrt(np.outer(np.diag(gam), np.diag(gam)))) > 0)
+
+
+def test_density_against_50_digit_arithmetic():
+    """The density (eq 13 + eq 22 + determinant) evaluated with mpmath at 50 digits: composite
+    Gauss-Legendre with mpmath's own nodes, the e-series retyped from tests/golden/appendix_b_series.txt.
+    One several-orbit point (well conditioned) and one P_orb = 8 h point in a 1.2 h observation
+    (Table 1: cond ~ 1e11, the regime of reading G29)."""
+    import os
+    import mpmath as mp
+    mp.mp.dps = 50
+    C = {k: [] for k in range(8)}
+    S = {k: [] for k in range(8)}
+    with open(os.path.join(os.path.dirname(__file__), "golden", "appendix_b_series.txt")) as fh:
+        for line in fh:
+            if line[0] in "CS":
+                which, k, pw, num, den = line.split()
+                (C if which == "C" else S)[int(k)].append((int(pw), mp.mpf(int(num)) / int(den)))
+
+    def density_mp(f0, lam, t_obs, panels):
+        tau, om, al, psi, e = (mp.mpf(v) for v in lam)
+        f0, t_obs = mp.mpf(f0), mp.mpf(t_obs)
+        c = [sum(q * e ** p for p, q in C[k]) for k in range(8)]
+        s = [sum(q * e ** p for p, q in S[k]) for k in range(8)]
+        dc = [sum(p * q * e ** (p - 1) for p, q in C[k] if p) for k in range(8)]
+        ds = [sum(p * q * e ** (p - 1) for p, q in S[k] if p) for k in range(8)]
+        sp, cp, k2 = mp.sin(psi), mp.cos(psi), 2 * mp.pi
+
+        def D(t):
+            M = om * t + al
+            co = [mp.cos(k * M) for k in range(8)]
+            si = [mp.sin(k * M) for k in range(8)]
+            X = sp * sum(c[k] * co[k] for k in range(8)) + cp * sum(s[k] * si[k] for k in range(8))
+            XM = sp * sum(-k * c[k] * si[k] for k in range(8)) + cp * sum(k * s[k] * co[k] for k in range(8))
+            Xp = cp * sum(c[k] * co[k] for k in range(8)) - sp * sum(s[k] * si[k] for k in range(8))
+            Xe = sp * sum(dc[k] * co[k] for k in range(8)) + cp * sum(ds[k] * si[k] for k in range(8))
+            return [k2 * (t + tau * X), k2 * f0 * X, k2 * f0 * tau * t * XM, k2 * f0 * tau * XM, k2 * f0 * tau * Xp, k2 * f0 * tau * Xe]
+
+        nodes = mp.calculus.quadrature.GaussLegendre(mp.mp).calc_nodes(5, mp.mp.prec)     # 48 nodes per panel
+        mean = [mp.mpf(0)] * 6
+        mom = [[mp.mpf(0)] * 6 for _ in range(6)]
+        for p in range(panels):
+            a, b = t_obs * p / panels, t_obs * (p + 1) / panels
+            for x, w in nodes:
+                d = D((a + b) / 2 + (b - a) / 2 * x)
+                ww = w / (2 * panels)
+                for i in range(6):
+                    mean[i] += ww * d[i]
+                    for j in range(i, 6):
+                        mom[i][j] += ww * d[i] * d[j]
+        g = mp.matrix(6, 6)
+        for i in range(6):
+            for j in range(6):
+                g[i, j] = mom[min(i, j)][max(i, j)] - mean[i] * mean[j]
+        gam = mp.matrix(5, 5)
+        for i in range(5):
+            for j in range(5):
+                gam[i, j] = g[i + 1, j + 1] - g[0, i + 1] * g[0, j + 1] / g[0, 0]
+        return mp.sqrt(abs(mp.det(gam)))
+
+    assert bank.density(F0, LAM_E, T_OBS, True, 512) == pytest.approx(float(density_mp(F0, LAM_E, T_OBS, 8)), rel=1e-10)
+    slow = [3.0, 2 * math.pi / (8 * 3600.0), 1.0, 0.7, 0.05]
+    assert bank.density(66.67, slow, 4320.0, True, 128) == pytest.approx(float(density_mp(66.67, slow, 4320.0, 2)), rel=1e-5)
+
+
+def test_density_is_a_density_under_change_of_coordinates():
+    """sqrt(det gamma) d^n lambda is the invariant volume element (eq 17): in the coordinates
+    (X, Y) = (tau sin psi, tau cos psi) of eq 29 (L176-186) the density is the (tau, psi) one divided by
+    the Jacobian tau.  The metric in (X, Y) is built here from finite differences of the oracle's phase."""
+    lam = list(LAM_E)
+    tau, psi = lam[0], lam[3]
+    t, w = bank.quadrature(T_OBS, 512)
+    D = bank.phase_derivatives(t, F0, lam, True)
+    # chain rule: d/dX = sin(psi) d/dtau + cos(psi)/tau d/dpsi,  d/dY = cos(psi) d/dtau - sin(psi)/tau d/dpsi
+    DX = math.sin(psi) * D[1] + math.cos(psi) / tau * D[4]
+    DY = math.cos(psi) * D[1] - math.sin(psi) / tau * D[4]
+    D2 = np.stack([D[0], DX, D[2], D[3], DY, D[5]])
+    mean = D2 @ w
+    g2 = (D2 * w) @ D2.T - np.outer(mean, mean)
+    rho_xy = float(np.sqrt(abs(bank.determinant(bank.projected_metric(g2)))))
+    assert rho_xy * tau == pytest.approx(bank.density(F0, lam, T_OBS, True, 512), rel=1e-9)
+    # and the chain-rule columns are the derivatives of the phase written in (X, Y): finite differences
+    def ph_xy(X, Y, tt):
+        return bank.phase(tt, F0, [math.hypot(X, Y), lam[1], lam[2], math.atan2(X, Y), lam[4]], True)
+    X0, Y0, h = tau * math.sin(psi), tau * math.cos(psi), 1e-6
+    fd = ((ph_xy(X0 + h, Y0, t) - ph_xy(X0 - h, Y0, t)) / (2 * h)).astype(np.float64)
+    assert np.abs(fd - DX.astype(np.float64)).max() < 1e-6 * np.abs(fd).max()
+
+
+def test_tau_max_is_keplers_third_law():
+    """eq 31 (L248): a_p sin(i)/c with a^3 = G (m_p + m_c) P^2 / (4 pi^2), a_p = a m_c / (m_p + m_c), in SI."""
+    G, c, msun = 6.67430e-11, 299792458.0, 1.98841e30
+    for p_orb, mp_, mc in [(21600.0, 1.4, 8.0), (43200.0, 1.4, 8.0), (7200.0, 1.2, 0.3)]:
+        a = (G * (mp_ + mc) * msun * p_orb ** 2 / (4 * math.pi ** 2)) ** (1.0 / 3.0)
+        expect = a * mc / (mp_ + mc) / c
+        assert bank.tau_max(2 * math.pi / p_orb, mp_, mc) == pytest.approx(expect, rel=2e-4)       # G M_sun known to 1e-4 via G
+        assert bank.tau_max(2 * math.pi / p_orb, mp_, mc, 0.5) == pytest.approx(0.5 * expect, rel=2e-4)
+    assert bank.tau_max(2 * math.pi / 21600.0, 1.4, 8.0) == pytest.approx(6.96, abs=0.01)          # by hand, Table 1's box
+
+
+def test_ball_volume_and_template_count():
+    assert bank.ball_volume(1) == pytest.approx(2.0)
+    assert bank.ball_volume(2) == pytest.approx(math.pi)
+    assert bank.ball_volume(3) == pytest.approx(4 * math.pi / 3)
+    assert bank.ball_volume(5) == pytest.approx(8 * math.pi ** 2 / 15)
+    # eq 20 (L131) inverted: N templates, each covering a fraction x of the volume, leave (1 - x)^N uncovered
+    vol, m_star, n = 5000.0, 0.2, 3
+    x = m_star ** (n / 2) * bank.ball_volume(n) / vol
+    N = bank.n_templates(0.9, m_star, n, vol)
+    assert 1 - (1 - x) ** N == pytest.approx(0.9, rel=1e-12)
+    # eq 21 (L136) is the limit of eq 20 for x << 1 and always a little larger
+    assert bank.n_templates(0.9, m_star, n, vol, exact=False) == pytest.approx(N, rel=2 * x)
+    assert bank.n_templates(0.9, m_star, n, vol, exact=False) > N
+    assert bank.n_templates(0.9, m_star, 5, 1e9, exact=False) == pytest.approx(math.log(10) * 1e9 / (0.2 ** 2.5 * 8 * math.pi ** 2 / 15))
+
+
+SPACE_C = dict(t_obs=537.0, f_max=25.0, p_orb_min=0.1 * 537.0, p_orb_max=0.35 * 537.0, m_pulsar_min=1.4, m_comp_max=8.0,
+               theta=1e-3, e_max=0.1, elliptical=False)
+
+
+def test_proposal_box_and_pdf():
+    rng = np.random.default_rng(9)
+    sp = dict(SPACE_C, elliptical=True)
+    for u in rng.random((50, 6)):
+        lam = bank.proposal(u, sp)
+        p = 2 * math.pi / lam[1]
+        assert sp["p_orb_min"] <= p <= sp["p_orb_max"]
+        assert 0 <= lam[0] <= bank.tau_max(lam[1], 1.4, 8.0, 1e-3) and 0 <= lam[4] <= 0.1
+        assert 0 <= lam[2] < 2 * math.pi and 0 <= lam[3] < 2 * math.pi
+        tmpl = bank.template_of(lam, True)
+        assert tmpl == (p, lam[0], lam[2], lam[4], lam[3])
+    # the pdf integrates to one over the box; q * tau_max does not depend on tau, alpha, psi, e: integrate over Omega
+    om_lo, om_hi = 2 * math.pi / sp["p_orb_max"], 2 * math.pi / sp["p_orb_min"]
+    om = np.linspace(om_lo, om_hi, 20001)
+    f = np.array([bank.proposal_pdf([0.0, o, 0.0, 0.0, 0.0], sp) * bank.tau_max(o, 1.4, 8.0, 1e-3) for o in om])
+    integral = float(np.sum((f[1:] + f[:-1]) / 2 * np.diff(om))) * (2 * math.pi) ** 2 * 0.1
+    assert integral == pytest.approx(1.0, rel=1e-7)
+
+
+def test_rejection_placement_by_brute_force():
+    """generate(): accept iff u5 rho_max < rho (G28); the accepted templates are the proposals in order;
+    the volume estimate is the mean of rho / q (eq 17).  Then a statistical check that accepted
+    points follow the density: in a 1-D slice (only tau varies) the accepted fraction per tau bin is
+    proportional to the bin-averaged density."""
+    rng = np.random.default_rng(12)
+    u = rng.random((40, 6))
+    rho_all = np.array([bank.density(SPACE_C["f_max"], bank.proposal(x, SPACE_C), SPACE_C["t_obs"], False) for x in u])
+    rho_max = float(np.quantile(rho_all, 0.8))                  # some proposals exceed it: always accepted
+    out, rho, mask, vol = bank.generate(u, SPACE_C, rho_max)
+    assert np.array_equal(rho, rho_all)
+    assert np.array_equal(mask, u[:, 5] * rho_max < rho_all) and 5 < mask.sum() < 40
+    expect = np.array([bank.template_of(bank.proposal(x, SPACE_C), False) for x in u[mask]])
+    assert np.array_equal(out, expect) and np.all(out[:, 3:] == 0)
+    q = np.array([bank.proposal_pdf(bank.proposal(x, SPACE_C), SPACE_C) for x in u])
+    assert vol == pytest.approx(float(np.mean(rho_all / q)), rel=1e-12)
+    # circular density grows like tau^2 (two of the three orbital derivatives carry a factor tau)
+    lam = bank.proposal([0.3, 0.5, 0.2], SPACE_C)
+    r1 = bank.density(25.0, lam, 537.0, False)
+    r2 = bank.density(25.0, [2 * lam[0], lam[1], lam[2]], 537.0, False)
+    assert r2 / r1 == pytest.approx(4.0, rel=1e-6)          # not exact: d Phi / d f0 carries tau X (reading G27)
+    assert bank.density(25.0, [0.0, lam[1], lam[2]], 537.0, False) == 0.0
+    # accepted tau values in a fixed-(Omega, alpha) slice: pdf ~ tau^2 on [0, tmax] -> the mean of tau/tmax is 3/4
+    n = 1500
+    us = np.column_stack([np.full(n, 0.3), rng.random(n), np.full(n, 0.2), np.zeros(n), np.zeros(n), rng.random(n)])
+    top = bank.density(25.0, [bank.tau_max(lam[1], 1.4, 8.0, 1e-3), lam[1], lam[2]], 537.0, False)
+    _, _, acc, _ = bank.generate(us, SPACE_C, top, n_quad=64)
+    assert 400 < acc.sum() < 600                                # acceptance rate 1/3
+    assert abs(us[acc, 1].mean() - 0.75) < 4 * math.sqrt(3.0 / 80.0 / acc.sum())
