@@ -260,6 +260,51 @@ TB_API int tb_sigma_to_power(uint32_t fold, double sigma, double* power_out);
 TB_API int tb_plan_info(const tb_plan* plan, float* fill_value, uint32_t* chunk_templates, uint32_t* k_lo);
 TB_API int tb_template_knot_log2(const tb_plan* plan, const tb_template* tmpl, int32_t* log2_h);
 
+/* ---- random template bank (PAPER.md sections 2.2-2.7; readings G27-G29) ----
+ * Plan-free: these calls own their device memory for the duration of the call, run on the default
+ * stream of `device` and synchronise before returning.
+ *
+ * The density of templates is rho(lambda) = sqrt|det gamma_ab| (L115, L263), gamma the frequency-
+ * projected metric (eq 22) of g_ab = <d_a Phi d_b Phi>_T - <d_a Phi>_T <d_b Phi>_T (eq 13,
+ * time averages over [0, t_obs_s], eq 14) for the phase Phi = 2 pi f0 [t + tau X(t)] of eq 1-2
+ * (L35-41), X = sin(psi) cos E + cos(psi) sqrt(1-e^2) sin E with the e-series of eqs 15-16 (L106-111,
+ * App. B), or X = sin(Omega t + alpha) (eq 4) when elliptical == 0.  Coordinates
+ * lambda = (tau [lt-s], Omega [rad/s], alpha [rad], psi [rad], e) (reading G27); f0 = f_max_hz (eq 30).
+ * Time averages: composite 32-point Gauss-Legendre, 1024 nodes (4096 when the shortest orbit makes
+ * more than 7 revolutions in t_obs_s; more than 28 revolutions -> TB_ERR_INVALID_ARG). */
+typedef struct {
+    uint32_t struct_size;         /* sizeof(tb_bank_space) */
+    int32_t  device;              /* CUDA device ordinal */
+    double   t_obs_s;             /* T of eq 14 */
+    double   f_max_hz;            /* spin frequency the bank is built for (L140, eq 30) */
+    double   p_orb_min_s, p_orb_max_s;        /* P_orb ~ U(min, max)              (Table 1) */
+    double   m_pulsar_min, m_comp_max, theta; /* eq 31 (L248), solar masses; 0 < theta <= 1:
+                                                 tau ~ U(0, theta (G M_sun)^(1/3) Omega^(-2/3) m_c / (c (m_p + m_c)^(2/3))) */
+    double   e_max;               /* e ~ U(0, e_max), 0 < e_max <= 0.3 (used when elliptical)   */
+    int32_t  elliptical;          /* 0: three orbital parameters (tau, Omega, alpha); 1: five (+ psi, e) */
+    int32_t  pad;
+} tb_bank_space;
+
+/* rho at n given points.  lam: host double[n][5] = (tau, Omega, alpha, psi, e) per point (psi, e
+ * ignored when elliptical == 0; tau >= 0, Omega > 0, 0 <= e <= 0.3); rho_out: host double[n].
+ * Only t_obs_s, f_max_hz, elliptical and device of `space` are used. */
+TB_API int tb_bank_density(const tb_bank_space* space, const double* lam, uint64_t n, double* rho_out);
+
+/* Rejection placement (L263; reading G28).  uniforms: host double[n][6], every value in [0, 1); proposal i
+ * is P_orb = min + u0 (max - min), tau = u1 tau_max(Omega), alpha = 2 pi u2, psi = 2 pi u3, e = u4 e_max
+ * and is accepted iff u5 * rho_max < rho.  Accepted proposals are written to `out` (host, capacity
+ * entries) as templates (P_orb, tau, phi0 = alpha, e, omega = psi) IN PROPOSAL ORDER.
+ *   n_accepted   receives the number accepted (also when it exceeds capacity -> TB_ERR_CAPACITY)
+ *   rho_out      optional (NULL), host double[n]: the density of every proposal
+ *   volume_out   optional (NULL): Monte-Carlo estimate of the proper volume V = int rho d lambda
+ *                (eq 17) over the box, mean of rho / q with q the pdf of the proposal */
+TB_API int tb_bank_generate(const tb_bank_space* space, const double* uniforms, uint64_t n, double rho_max,
+                     tb_template* out, uint64_t capacity, uint64_t* n_accepted, double* rho_out, double* volume_out);
+
+/* Host fp64: number of random templates for coverage eta at nominal mismatch m_star in n_dim
+ * dimensions and proper volume `volume`: eq 20 (L131; exact != 0) or eq 21 (L136), C_n of eq 18 (L123). */
+TB_API int tb_bank_n_templates(double eta, double m_star, uint32_t n_dim, double volume, int32_t exact, double* n_out);
+
 #ifdef __cplusplus
 }
 #endif

@@ -27,13 +27,14 @@ Readings:
        as printed (L45-47); derivatives are those of eq 1-2 exactly (d/df includes the tau X term
        that eq 28's dimensionless form drops), so that eq 12's mismatch holds to O(Delta^3).
   G28  rejection sampling instead of emcee (above).
-  G29  arithmetic: the time averages are Gauss-Legendre sums (numpy leggauss, N_QUAD nodes: exact
-       to rounding for these band-limited integrands) and everything from the derivatives to the
-       determinant runs in x87 extended precision (numpy.longdouble): for P_orb >> T the metric is
-       ill conditioned (cond ~ 1e12) and a plain fp64 evaluation of eq 13 / eq 22 / det loses most
-       digits; the longdouble evaluation of the SAME formulas is accurate to about 2e-6 there
-       (pinned against a 50-digit mpmath evaluation) and to 1e-12 for the several-orbit banks of
-       BASELINE.json's configs.
+  G29  arithmetic: the time averages are Gauss-Legendre sums (exact to rounding for these band-
+       limited integrands).  For P_orb >> T the metric is ill conditioned (cond 1e11 for typical
+       points of the paper's box, 1e15 and more where e -> 0 makes psi and alpha degenerate), and
+       the literal chain eq 13 -> eq 22 -> det loses cond * epsilon: fp64 is useless there and even
+       x87 extended precision is off by 3e-5 typically and by a factor 4 at the degenerate points.
+       So `density` evaluates the SAME formulas either in numpy.longdouble (fast; accurate to 1e-12
+       for the several-orbit banks of BASELINE.json's configs, cond ~ 1e4) or, with digits=D, in
+       D-digit mpmath arithmetic (density_mp), which is what the paper's box is compared in.
 
 Parity pins (tests/test_bank_pins.py, -m "not gpu"):
   phase_derivatives ... every column against central finite differences of the EXACT phase (Kepler
@@ -136,22 +137,28 @@ def phase_derivatives(t, f0, lam, elliptical):
 # ----------------------------------------------------------------------------------------------
 # eq 13, 14, 22: metric, projected metric, density
 # ----------------------------------------------------------------------------------------------
+_GL_CACHE = {}
+
+
 def quadrature(t_obs, n_quad=N_QUAD):
     """Nodes in [0, T] and weights summing to 1: <G>_T = sum_i w_i G(t_i)  (eq 14).
     Gauss-Legendre: numpy's fp64 nodes refined to longdouble by Newton steps on P_n (with fp64 nodes
-    the ill-conditioned metrics of G29 come out 50 times less accurate)."""
-    x = np.asarray(np.polynomial.legendre.leggauss(n_quad)[0], LD)
+    the ill-conditioned metrics of G29 come out 50 times less accurate).  The rule is cached per
+    n_quad (numpy's leggauss is an eigenvalue problem: slow when many worker processes call it)."""
+    if n_quad not in _GL_CACHE:
+        x = np.asarray(np.polynomial.legendre.leggauss(n_quad)[0], LD)
 
-    def p_and_dp(x):
-        p0, p1 = np.ones_like(x), x.copy()
-        for k in range(2, n_quad + 1):
-            p0, p1 = p1, ((2 * k - 1) * x * p1 - (k - 1) * p0) / LD(k)
-        return p1, n_quad * (x * p1 - p0) / (x * x - 1)
+        def p_and_dp(x):
+            p0, p1 = np.ones_like(x), x.copy()
+            for k in range(2, n_quad + 1):
+                p0, p1 = p1, ((2 * k - 1) * x * p1 - (k - 1) * p0) / LD(k)
+            return p1, n_quad * (x * p1 - p0) / (x * x - 1)
 
-    for _ in range(3):
-        p, dp = p_and_dp(x)
-        x = x - p / dp
-    w = 2 / ((1 - x * x) * p_and_dp(x)[1] ** 2)
+        for _ in range(3):
+            p, dp = p_and_dp(x)
+            x = x - p / dp
+        _GL_CACHE[n_quad] = (x, 2 / ((1 - x * x) * p_and_dp(x)[1] ** 2))
+    x, w = _GL_CACHE[n_quad]
     return (LD(t_obs) / 2) * (x + 1), w / 2
 
 
@@ -186,9 +193,69 @@ def determinant(a):
     return det
 
 
-def density(f0, lam, t_obs, elliptical, n_quad=N_QUAD):
-    """sqrt|det gamma| at lam = (tau, Omega, alpha[, psi, e])  (L115, L263)."""
+def density(f0, lam, t_obs, elliptical, n_quad=N_QUAD, digits=None):
+    """sqrt|det gamma| at lam = (tau, Omega, alpha[, psi, e])  (L115, L263).
+    digits=None: longdouble (error ~ cond * 1e-19: fine for several-orbit banks, cond ~ 1e4);
+    digits=D: the same formulas in D-digit mpmath arithmetic (density_mp), for the paper's own box
+    where the condition number reaches 1e11..1e16 (psi and alpha degenerate as e -> 0)."""
+    if digits:
+        return density_mp(f0, lam, t_obs, elliptical, n_quad, digits)
     return float(np.sqrt(np.abs(determinant(projected_metric(metric(f0, lam, t_obs, elliptical, n_quad))))))
+
+
+def density_mp(f0, lam, t_obs, elliptical, n_quad=N_QUAD, digits=50):
+    """eq 13 -> eq 22 -> determinant, literally, in mpmath arithmetic of `digits` digits (reading G29).
+    Time averages: composite Gauss-Legendre with mpmath's own 96-point rule on ceil(n_quad / 96) panels."""
+    import mpmath as mp
+    with mp.workdps(digits):
+        tau, om, al = (mp.mpf(float(v)) for v in lam[:3])
+        f0, t_obs = mp.mpf(float(f0)), mp.mpf(float(t_obs))
+        k2 = 2 * mp.pi
+        if elliptical:
+            psi, e = mp.mpf(float(lam[3])), mp.mpf(float(lam[4]))
+            C = [sum(mp.mpf(num) / den * e ** pw for pw, num, den in ELL_C[k]) for k in range(8)]
+            S = [mp.mpf(0)] + [sum(mp.mpf(num) / den * e ** pw for pw, num, den in ELL_S[k]) for k in range(1, 8)]
+            dC = [sum(pw * mp.mpf(num) / den * e ** (pw - 1) for pw, num, den in ELL_C[k] if pw) for k in range(8)]
+            dS = [mp.mpf(0)] + [sum(pw * mp.mpf(num) / den * e ** (pw - 1) for pw, num, den in ELL_S[k] if pw) for k in range(1, 8)]
+            sp, cp = mp.sin(psi), mp.cos(psi)
+
+        def derivs(t):
+            M = om * t + al
+            if not elliptical:
+                X, XM = mp.sin(M), mp.cos(M)
+                return [k2 * (t + tau * X), k2 * f0 * X, k2 * f0 * tau * t * XM, k2 * f0 * tau * XM]
+            co = [mp.cos(k * M) for k in range(8)]
+            si = [mp.sin(k * M) for k in range(8)]
+            cc = sum(C[k] * co[k] for k in range(8))
+            ss = sum(S[k] * si[k] for k in range(1, 8))
+            X, XM = sp * cc + cp * ss, sp * sum(-k * C[k] * si[k] for k in range(8)) + cp * sum(k * S[k] * co[k] for k in range(1, 8))
+            Xp = cp * cc - sp * ss
+            Xe = sp * sum(dC[k] * co[k] for k in range(8)) + cp * sum(dS[k] * si[k] for k in range(1, 8))
+            return [k2 * (t + tau * X), k2 * f0 * X, k2 * f0 * tau * t * XM, k2 * f0 * tau * XM, k2 * f0 * tau * Xp, k2 * f0 * tau * Xe]
+
+        nodes = mp.calculus.quadrature.GaussLegendre(mp.mp).calc_nodes(6, mp.mp.prec)      # 96 nodes on (-1, 1)
+        panels = max(1, -(-int(n_quad) // 96))
+        n = 6 if elliptical else 4
+        mean = [mp.mpf(0)] * n
+        mom = [[mp.mpf(0)] * n for _ in range(n)]
+        for p in range(panels):
+            a, b = t_obs * p / panels, t_obs * (p + 1) / panels
+            for x, w in nodes:
+                d = derivs((a + b) / 2 + (b - a) / 2 * x)
+                ww = w / (2 * panels)
+                for i in range(n):
+                    mean[i] += ww * d[i]
+                    for j in range(i, n):
+                        mom[i][j] += ww * d[i] * d[j]
+        g = mp.matrix(n, n)
+        for i in range(n):
+            for j in range(n):
+                g[i, j] = mom[min(i, j)][max(i, j)] - mean[i] * mean[j]                      # eq 13
+        gam = mp.matrix(n - 1, n - 1)
+        for i in range(n - 1):
+            for j in range(n - 1):
+                gam[i, j] = g[i + 1, j + 1] - g[0, i + 1] * g[0, j + 1] / g[0, 0]              # eq 22
+        return float(mp.sqrt(abs(mp.det(gam))))
 
 
 def mismatch_direct(t_obs, phase_a, phase_b, n_quad=N_QUAD):
@@ -243,7 +310,7 @@ def template_of(lam, elliptical):
 # ----------------------------------------------------------------------------------------------
 # section 2.3 / 2.7: placement, volume, number of templates
 # ----------------------------------------------------------------------------------------------
-def generate(uniforms, space, rho_max, n_quad=N_QUAD):
+def generate(uniforms, space, rho_max, n_quad=N_QUAD, digits=None):
     """Rejection placement (G28): proposal i is accepted iff u_i5 * rho_max < rho(lam_i).
     uniforms: [n, 6].  Returns (accepted templates [k, 5], rho [n], accepted mask [n], volume estimate),
     the proper volume V = int rho d lam (eq 17) estimated as mean(rho_i / q(lam_i))."""
@@ -253,7 +320,7 @@ def generate(uniforms, space, rho_max, n_quad=N_QUAD):
     out, mask = [], np.zeros(len(uniforms), bool)
     for i, u in enumerate(uniforms):
         lam = proposal(u, space)
-        rho[i] = density(space["f_max"], lam, space["t_obs"], ell, n_quad)
+        rho[i] = density(space["f_max"], lam, space["t_obs"], ell, n_quad, digits)
         vol += rho[i] / proposal_pdf(lam, space)
         if float(u[5]) * rho_max < rho[i]:
             mask[i] = True

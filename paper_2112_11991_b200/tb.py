@@ -39,6 +39,13 @@ class PlanOpts(C.Structure):
                 ("delay_model", C.c_int32)]
 
 
+class BankSpace(C.Structure):
+    _fields_ = [("struct_size", C.c_uint32), ("device", C.c_int32), ("t_obs_s", C.c_double), ("f_max_hz", C.c_double),
+                ("p_orb_min_s", C.c_double), ("p_orb_max_s", C.c_double), ("m_pulsar_min", C.c_double),
+                ("m_comp_max", C.c_double), ("theta", C.c_double), ("e_max", C.c_double), ("elliptical", C.c_int32),
+                ("pad", C.c_int32)]
+
+
 class Timings(C.Structure):
     _fields_ = [("ms_resample", C.c_double), ("ms_fft", C.c_double), ("ms_spectrum", C.c_double),
                 ("ms_normalise", C.c_double), ("ms_hsum", C.c_double), ("ms_total", C.c_double),
@@ -54,7 +61,8 @@ class Timings(C.Structure):
 EXPORTS = ["tb_plan_create", "tb_plan_set_series", "tb_search_templates", "tb_get_candidates", "tb_clear_candidates", "tb_plan_destroy",
            "tb_reduce_candidates", "tb_debug_set_candidates",
            "tb_strerror", "tb_last_error", "tb_get_timings", "tb_debug_resample_indices", "tb_debug_spectrum",
-           "tb_debug_resampled", "tb_debug_hsums", "tb_debug_series", "tb_sigma_to_power", "tb_plan_info", "tb_template_knot_log2"]
+           "tb_debug_resampled", "tb_debug_hsums", "tb_debug_series", "tb_sigma_to_power", "tb_plan_info", "tb_template_knot_log2",
+           "tb_bank_density", "tb_bank_generate", "tb_bank_n_templates"]
 
 _vp, _u64, _u32 = C.c_void_p, C.c_uint64, C.c_uint32
 lib.tb_plan_create.argtypes = [C.POINTER(_vp), _vp, _u64, C.c_double, C.POINTER(PlanOpts)]
@@ -78,6 +86,9 @@ lib.tb_debug_series.argtypes = [_vp, _vp, C.POINTER(C.c_double)]
 lib.tb_sigma_to_power.argtypes = [_u32, C.c_double, C.POINTER(C.c_double)]
 lib.tb_plan_info.argtypes = [_vp, C.POINTER(C.c_float), C.POINTER(_u32), C.POINTER(_u32)]
 lib.tb_template_knot_log2.argtypes = [_vp, _vp, C.POINTER(C.c_int32)]
+lib.tb_bank_density.argtypes = [C.POINTER(BankSpace), _vp, _u64, _vp]
+lib.tb_bank_generate.argtypes = [C.POINTER(BankSpace), _vp, _u64, C.c_double, _vp, _u64, C.POINTER(_u64), _vp, C.POINTER(C.c_double)]
+lib.tb_bank_n_templates.argtypes = [C.c_double, C.c_double, _u32, C.c_double, C.c_int32, C.POINTER(C.c_double)]
 for _name in EXPORTS:
     if _name not in ("tb_strerror", "tb_last_error"):
         getattr(lib, _name).restype = C.c_int
@@ -332,3 +343,46 @@ class Plan:
             self.close()
         except Exception:
             pass
+
+
+# ---------------------------------------------------------------------------------- template bank (f3)
+def bank_space(t_obs_s, f_max_hz, p_orb_min_s, p_orb_max_s, m_pulsar_min=1.4, m_comp_max=8.0, theta=1.0, e_max=0.1,
+               elliptical=False, device=0) -> BankSpace:
+    s = BankSpace()
+    s.struct_size = C.sizeof(BankSpace)
+    s.device = int(device)
+    s.t_obs_s, s.f_max_hz, s.p_orb_min_s, s.p_orb_max_s = float(t_obs_s), float(f_max_hz), float(p_orb_min_s), float(p_orb_max_s)
+    s.m_pulsar_min, s.m_comp_max, s.theta, s.e_max = float(m_pulsar_min), float(m_comp_max), float(theta), float(e_max)
+    s.elliptical = int(bool(elliptical))
+    return s
+
+
+def tb_bank_density(space: BankSpace, lam) -> np.ndarray:
+    """lam: float64[n, 5] = (tau, Omega, alpha, psi, e) -> rho float64[n]."""
+    lam = np.ascontiguousarray(np.asarray(lam, dtype=np.float64).reshape(-1, 5))
+    rho = np.zeros(len(lam), dtype=np.float64)
+    _check(lib.tb_bank_density(C.byref(space), lam.ctypes.data, len(lam), rho.ctypes.data))
+    return rho
+
+
+def tb_bank_generate(space: BankSpace, uniforms, rho_max, capacity=None):
+    """uniforms: float64[n, 6] in [0, 1).  Returns (templates float64[k, 5], rho float64[n], volume estimate)."""
+    u = np.ascontiguousarray(np.asarray(uniforms, dtype=np.float64).reshape(-1, 6))
+    cap = len(u) if capacity is None else int(capacity)
+    out = np.zeros(max(cap, 1), dtype=TEMPLATE_DTYPE)
+    rho = np.zeros(len(u), dtype=np.float64)
+    n_acc, vol = _u64(0), C.c_double(0.0)
+    rc = lib.tb_bank_generate(C.byref(space), u.ctypes.data, len(u), float(rho_max), out.ctypes.data, cap, C.byref(n_acc),
+                              rho.ctypes.data, C.byref(vol))
+    if rc != TB_OK:
+        err = TbError(rc)
+        err.n_total = int(n_acc.value)
+        raise err
+    k = int(n_acc.value)
+    return out[:k].view(np.float64).reshape(k, 5).copy(), rho, float(vol.value)
+
+
+def tb_bank_n_templates(eta, m_star, n_dim, volume, exact=True) -> float:
+    out = C.c_double(0.0)
+    _check(lib.tb_bank_n_templates(float(eta), float(m_star), int(n_dim), float(volume), int(bool(exact)), C.byref(out)))
+    return float(out.value)

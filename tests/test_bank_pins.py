@@ -172,7 +172,15 @@ def test_density_against_50_digit_arithmetic():
 
     assert bank.density(F0, LAM_E, T_OBS, True, 512) == pytest.approx(float(density_mp(F0, LAM_E, T_OBS, 8)), rel=1e-10)
     slow = [3.0, 2 * math.pi / (8 * 3600.0), 1.0, 0.7, 0.05]
-    assert bank.density(66.67, slow, 4320.0, True, 128) == pytest.approx(float(density_mp(66.67, slow, 4320.0, 2)), rel=1e-5)
+    truth = float(density_mp(66.67, slow, 4320.0, 2))
+    assert bank.density(66.67, slow, 4320.0, True, 128) == pytest.approx(truth, rel=1e-5)                 # longdouble: cond 7e10
+    assert bank.density(66.67, slow, 4320.0, True, 192, digits=40) == pytest.approx(truth, rel=1e-13)     # the oracle's own mpmath path
+    degenerate = [6.86, 1.4637555785e-4, 1.3354, 1.3173, 0.0015]                # e -> 0: psi and alpha degenerate, cond 1e15
+    truth = float(density_mp(66.67, degenerate, 4320.0, 2))
+    assert bank.density(66.67, degenerate, 4320.0, True, 192, digits=40) == pytest.approx(truth, rel=1e-13)
+    assert abs(bank.density(66.67, degenerate, 4320.0, True, 128) / truth - 1) > 1e-3                    # why digits exists (G29)
+    circ = LAM_C
+    assert bank.density(F0, circ, T_OBS, False, 512, digits=40) == pytest.approx(bank.density(F0, circ, T_OBS, False, 512), rel=1e-12)
 
 
 def test_density_is_a_density_under_change_of_coordinates():

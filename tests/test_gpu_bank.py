@@ -1,0 +1,143 @@
+"""-m gpu: the device template-bank generator (tb_bank_density / tb_bank_generate)
+against oracle/tb_bank.py on the same seeded uniforms.
+
+Tolerances (reading G29).  The density is a determinant of a metric whose
+condition number is ~1e4 for the several-orbit banks of BASELINE.json's configs and ~1e11 for the
+paper's own box (P_orb = 6-12 h in a 1.2 h observation; 1e15 where e -> 0).  The oracle evaluates
+eq 13 -> eq 22 -> det literally: in x87 extended precision for the former (accurate to ~1e-12) and in
+40-digit mpmath arithmetic for the latter (longdouble is off by up to a factor 4 there); the device
+orthogonalises the sampled derivative columns in fp64, error ~ sqrt(cond) * 1e-16 * (a few hundred
+operations).  Hence REL_WELL = 1e-9 and REL_ILL = 1e-6.
+The accept decision u5 * rho_max < rho is an integer decided by floating point: both sides take it
+in fp64 on their own rho, and a disagreement is excused only inside the tolerance band of rho.
+"""
+import math
+import multiprocessing as mp
+
+import numpy as np
+import pytest
+
+from oracle import tb_bank as obank
+
+pytestmark = pytest.mark.gpu
+
+REL_WELL, REL_ILL = 1e-9, 1e-6
+
+T5, TS5 = 2 ** 23 * 64e-6, 64e-6                     # BASELINE configs[3]/[4]: 537 s
+SPACES = {
+    # several-orbit banks shaped like BASELINE configs 2 and 4 (P_orb = 0.1-0.35 T_obs; tau bounded by eq 31)
+    "c2-circular": dict(t_obs=2 ** 22 * 256e-6, f_max=50.0, p_orb_min=0.1 * 2 ** 22 * 256e-6, p_orb_max=0.35 * 2 ** 22 * 256e-6,
+                        m_pulsar_min=1.4, m_comp_max=8.0, theta=1.0, e_max=0.1, elliptical=False),
+    "c4-elliptical": dict(t_obs=T5, f_max=40.0, p_orb_min=0.1 * T5, p_orb_max=0.2 * T5, m_pulsar_min=1.4, m_comp_max=8.0,
+                          theta=1.0, e_max=0.1, elliptical=True),
+    # the paper's own box (Table 1)
+    "paper-circular": dict(t_obs=4320.0, f_max=66.67, p_orb_min=6 * 3600.0, p_orb_max=12 * 3600.0, m_pulsar_min=1.4, m_comp_max=8.0,
+                           theta=1.0, e_max=0.1, elliptical=False),
+    "paper-elliptical": dict(t_obs=4320.0, f_max=66.67, p_orb_min=6 * 3600.0, p_orb_max=12 * 3600.0, m_pulsar_min=1.4, m_comp_max=8.0,
+                             theta=1.0, e_max=0.1, elliptical=True),
+}
+
+
+@pytest.fixture(scope="module")
+def tb():
+    import torch
+    assert torch.cuda.is_available(), "these tests need a CUDA device"
+    from paper_2112_11991_b200 import build
+    build.build()
+    from paper_2112_11991_b200 import tb
+    return tb
+
+
+def c_space(tb, sp):
+    return tb.bank_space(sp["t_obs"], sp["f_max"], sp["p_orb_min"], sp["p_orb_max"], sp["m_pulsar_min"], sp["m_comp_max"],
+                         sp["theta"], sp["e_max"], sp["elliptical"])
+
+
+def _rho_job(args):
+    sp, u, digits = args
+    lam = obank.proposal(u, sp)
+    n_quad = 192 if digits else obank.N_QUAD          # the paper's box covers at most 0.2 revolutions
+    return obank.density(sp["f_max"], lam, sp["t_obs"], bool(sp["elliptical"]), n_quad, digits), obank.proposal_pdf(lam, sp), lam
+
+
+def oracle_points(sp, uniforms, digits=None):
+    obank.quadrature(sp["t_obs"])                    # fills the rule's cache before the workers fork
+    with mp.get_context("fork").Pool(min(16, mp.cpu_count())) as pool:
+        res = pool.map(_rho_job, [(sp, u, digits) for u in uniforms], chunksize=4)
+    return np.array([r[0] for r in res]), np.array([r[1] for r in res]), [r[2] for r in res]
+
+
+@pytest.mark.parametrize("name", list(SPACES))
+def test_density_and_placement_parity(tb, name):
+    sp = SPACES[name]
+    rel = REL_ILL if name.startswith("paper") else REL_WELL
+    rng = np.random.default_rng({"c2-circular": 1, "c4-elliptical": 2, "paper-circular": 3, "paper-elliptical": 4}[name])
+    u = rng.random((192, 6))
+    rho_o, q_o, lams = oracle_points(sp, u, 40 if name.startswith("paper") else None)
+    assert np.all(rho_o > 0)
+    # (1) density at given points
+    lam5 = np.array([list(l) + [0.0] * (5 - len(l)) for l in lams])
+    rho_g = tb.tb_bank_density(c_space(tb, sp), lam5)
+    err = np.abs(rho_g - rho_o) / rho_o
+    assert err.max() <= rel, f"{name}: density off by {err.max():.3g} at point {err.argmax()}"
+    # (2) placement from the same uniforms
+    rho_max = float(np.quantile(rho_o, 0.7))
+    out_g, rho_g2, vol_g = tb.tb_bank_generate(c_space(tb, sp), u, rho_max)
+    assert np.abs(rho_g2 - rho_o).max() <= rel * rho_o.max() and np.all(np.abs(rho_g2 - rho_o) <= rel * rho_o)
+    acc_o = u[:, 5] * rho_max < rho_o
+    acc_g = u[:, 5] * rho_max < rho_g2
+    differ = np.nonzero(acc_o != acc_g)[0]
+    assert all(abs(u[i, 5] * rho_max - rho_o[i]) <= rel * rho_o[i] for i in differ), "accept decision differs outside the band"
+    assert len(out_g) == acc_g.sum() and 20 < len(out_g) < 192
+    expect = np.array([obank.template_of(lams[i], bool(sp["elliptical"])) for i in np.nonzero(acc_g)[0]])
+    assert np.allclose(out_g, expect, rtol=1e-13, atol=0.0), "accepted templates differ / are out of order"
+    vol_o = float(np.mean(rho_o / q_o))
+    assert vol_g == pytest.approx(vol_o, rel=10 * rel)
+    # (3) N_R of eq 20 / eq 21 from that volume
+    n_dim = 5 if sp["elliptical"] else 3
+    for exact in (True, False):
+        assert tb.tb_bank_n_templates(0.9, 0.2, n_dim, vol_g, exact) == pytest.approx(obank.n_templates(0.9, 0.2, n_dim, vol_o, exact), rel=20 * rel)
+    print(f"{name}: worst density error {err.max():.2e}, accepted {len(out_g)}/192, V = {vol_g:.4g}, "
+          f"N_R(0.9, 0.2) = {tb.tb_bank_n_templates(0.9, 0.2, n_dim, vol_g, False):.4g}")
+
+
+def test_edge_cases(tb):
+    sp = SPACES["c2-circular"]
+    cs = c_space(tb, sp)
+    out, rho, vol = tb.tb_bank_generate(cs, np.zeros((0, 6)), 1.0)
+    assert len(out) == 0 and len(rho) == 0 and vol == 0.0
+    assert len(tb.tb_bank_density(cs, np.zeros((0, 5)))) == 0
+    u = np.random.default_rng(0).random((64, 6))
+    with pytest.raises(tb.TbError) as ei:                          # capacity too small: count still reported
+        tb.tb_bank_generate(cs, u, 1e-30, capacity=10)
+    assert ei.value.code == tb.TB_ERR_CAPACITY and ei.value.n_total == 64
+    out, rho, _ = tb.tb_bank_generate(cs, u, 1e300)                # nothing accepted
+    assert len(out) == 0 and np.all(rho > 0)
+    u0 = u.copy()
+    u0[:, 1] = 0.0                                                 # tau = 0: no Doppler modulation, zero density (L257)
+    out, rho, _ = tb.tb_bank_generate(cs, u0, 1.0)
+    assert np.all(rho == 0.0) and len(out) == 0
+    for bad in [dict(sp, t_obs=-1.0), dict(sp, p_orb_min=0.0), dict(sp, theta=2.0), dict(sp, elliptical=True, e_max=0.5),
+                dict(sp, p_orb_min=sp["t_obs"] / 40.0)]:            # 40 revolutions: beyond the quadrature's range
+        with pytest.raises(tb.TbError) as ei:
+            tb.tb_bank_generate(c_space(tb, bad), u, 1.0)
+        assert ei.value.code == tb.TB_ERR_INVALID_ARG
+    with pytest.raises(tb.TbError):
+        tb.tb_bank_generate(cs, u + 1.0, 1.0)                      # uniforms outside [0, 1)
+
+
+def test_generated_bank_feeds_the_search(tb, c1):
+    """A bank drawn for C1's box goes straight into tb_search_templates; adding the true template
+    recovers the injected pulsar among them (the generator's templates are valid tb_template rows)."""
+    sp = dict(t_obs=c1.t_obs, f_max=50.0, p_orb_min=40.0, p_orb_max=90.0, m_pulsar_min=1.4, m_comp_max=8.0, theta=0.02,
+              e_max=0.1, elliptical=False)
+    u = np.random.default_rng(7).random((400, 6))
+    _, rho, _ = tb.tb_bank_generate(c_space(tb, sp), u, 1e300)
+    bank, _, _ = tb.tb_bank_generate(c_space(tb, sp), u, float(np.quantile(rho, 0.9)))
+    assert 40 < len(bank) < 400 and np.all(bank[:, 3:] == 0)
+    with tb.Plan(c1.series, c1.tsamp) as plan:
+        plan.search(np.vstack([c1.templates[:1], bank]), 0, c1.folds, 6.0)
+        cands, n = plan.candidates()
+    assert n > 0 and 0 in set(cands["template_id"])
+    best = cands[np.argmax(cands["sigma"])]
+    assert int(best["template_id"]) == 0 and (int(best["fold"]), int(best["bin"])) == (3, 52429)
