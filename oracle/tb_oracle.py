@@ -218,6 +218,25 @@ def interbin_power(X):
     return np.maximum(raw, 0.5 * (dif.real**2 + dif.imag**2))
 
 
+def interbin_power_oversampled(X):
+    """SURVEY 8(f) row f4, reading G12b: the 2x-oversampled ("Fourier interpolated") spectrum of
+    N = 2 Nb half bins,
+        P'_{2k}   = |X_k|^2,
+        P'_{2k+1} = (pi/4)^2 |X_k - X_{k+1}|^2,      k = 0..Nb-1,
+    with X_0 <- 0 first (G13) and X_Nb the Nyquist bin of the FFT.  (pi/4)(X_k - X_{k+1}) is the
+    two-bin estimate of the Fourier amplitude at k + 1/2 of Ransom et al. 2002, the paper's reference
+    for scalloping: a tone midway between two bins, which the raw bins see at
+    (2/pi)^2 = 0.405 of its power, comes back at 1.0.  Half bin q is the frequency q / (2 T_obs)."""
+    X = np.array(X, dtype=np.complex128)
+    nb = X.size - 1
+    X[0] = 0.0
+    out = np.empty(2 * nb, dtype=np.float64)
+    out[0::2] = X[:nb].real**2 + X[:nb].imag**2
+    dif = X[:nb] - X[1:nb + 1]
+    out[1::2] = (math.pi / 4.0) ** 2 * (dif.real**2 + dif.imag**2)
+    return out
+
+
 def block_medians(P, window):
     """m_b = median(P[bW:(b+1)W]) (mean of the two middle order statistics), reading G15 of
     "Fourier de-reddening" (PAPER.md:L660, L448)."""
@@ -289,6 +308,11 @@ def sigma_to_power(fold: int, sigma: float) -> float:
     return (mu + sigma * s) ** 2
 
 
+def lowest_bin_oversampled(n_samples, tsamp, f_min):
+    """k_lo in half bins (G12b): twice lowest_bin's, so that both modes cut at the same frequency."""
+    return 2 * lowest_bin(n_samples, tsamp, f_min)
+
+
 def lowest_bin(n_samples, tsamp, f_min):
     """k_lo = ceil(f_min * N * tsamp) (G20)."""
     return int(math.ceil(f_min * (float(n_samples) * float(tsamp))))
@@ -310,26 +334,28 @@ def candidates_from_sums(sums, template_id, sigma_threshold, k_lo):
 # ----------------------------------------------------------------------------------------------
 # whole path for one template / a bank
 # ----------------------------------------------------------------------------------------------
-def spectrum_of_template(series, tsamp, tmpl, window=1024, fill=None, idx=None):
+def spectrum_of_template(series, tsamp, tmpl, window=1024, fill=None, idx=None, oversample=False):
     """Steps O1-O6 for one template.  ``idx`` overrides the computed source indices (used by the
-    parity tests to re-run the oracle with an excused tie flipped).  Returns a dict."""
+    parity tests to re-run the oracle with an excused tie flipped).  ``oversample``: the 2x-oversampled
+    spectrum of reading G12b (N half bins instead of N/2 bins).  Returns a dict."""
     x = np.asarray(series, dtype=np.float32)
     if fill is None:
         fill = fill_value(x)
     if idx is None:
         idx = resample_indices(x.size, tsamp, tmpl)
     y = gather(x, idx, fill)
-    P = interbin_power(rfft_forward(y))
+    P = interbin_power_oversampled(rfft_forward(y)) if oversample else interbin_power(rfft_forward(y))
     m_b = block_medians(P, window)
     return {"idx": idx, "resampled": y, "power": P, "medians": m_b, "normalised": normalise(P, m_b, window)}
 
 
 def search_template(series, tsamp, tmpl, template_id=0, folds=(0, 1, 2, 3, 4), sigma_threshold=6.0,
-                    window=1024, f_min=0.1, fill=None, idx=None):
-    """Steps O1-O9 for one template: list of (template, L, k, S, sigma)."""
-    spec = spectrum_of_template(series, tsamp, tmpl, window, fill, idx)
+                    window=1024, f_min=0.1, fill=None, idx=None, oversample=False):
+    """Steps O1-O9 for one template: list of (template, L, k, S, sigma); with ``oversample`` k counts
+    half bins (fundamental frequency k / (2^(L+1) T_obs))."""
+    spec = spectrum_of_template(series, tsamp, tmpl, window, fill, idx, oversample)
     sums = harmonic_sums(spec["normalised"], folds)
-    k_lo = lowest_bin(len(series), tsamp, f_min)
+    k_lo = (lowest_bin_oversampled if oversample else lowest_bin)(len(series), tsamp, f_min)
     return candidates_from_sums(sums, template_id, sigma_threshold, k_lo)
 
 

@@ -205,8 +205,49 @@ def config5(log2n: int = 23, n_circ: int = 256, n_ell: int = 256, noise: bool = 
     return Workload(f"C5/2^{log2n}", n, tsamp, x, templates, (), ())
 
 
+# ------------------------------------------------------------------ paper-shaped workloads
+def config_paper(log2n: int = 24, n_templates: int = 1024) -> Workload:
+    """The paper's own simulation set-up (Table 2): 2^24 samples at 256 us
+    (72 min), a 15 ms pulsar in a P_orb = 8 h, e = 0.1 orbit around an 8 M_sun companion seen at 60 deg
+    (tau = 6.6 lt-s), i.e. P_orb = 6.7 T_obs; bank: template 0 = truth, the rest P_orb~U[6,12] h,
+    tau~U[0,7] lt-s, phi0, omega~U[0,2pi), e~U[0,0.1] (Table 1).  Duty cycle 10 % (Table 2)."""
+    n, tsamp = 1 << log2n, 256e-6
+    rng = _rng(6)
+    noise = rng.standard_normal(n)
+    phi0 = rng.uniform(0.0, 2.0 * np.pi)
+    psr = (0.015, 8.0 * 3600.0, 6.6, phi0, 0.1, 1.0, default_amplitude(n) * math.sqrt(DUTY / 0.10))
+    bank = _bank(rng, n_templates - 1, 6.0 * 3600.0, 12.0 * 3600.0, 0.0, 7.0, elliptical=True)
+    x = noise + pulse_train(n, tsamp, *psr, duty=0.10)
+    templates = np.vstack([np.array([[psr[1], psr[2], psr[3], psr[4], psr[5]]]), bank])
+    return Workload("paper/2^%d" % log2n, n, tsamp, x.astype(np.float32), templates, (0,), (psr,))
+
+
+def config_terzan(log2n: int = 28, n_templates: int = 8) -> Workload:
+    """A Terzan-5-length series (7.2 h downsampled to 81.9 us = 2^28.2 samples): 2^28
+    samples at 81.92 us (6.1 h), a 5 ms pulsar in a circular P_orb = 7 T_obs orbit, tau = 12 lt-s; bank:
+    template 0 = truth, the rest P_orb~U[5,10] T_obs, tau~U[0,20] lt-s, phi0~U[0,2pi) ("a circular-orbit
+    search between 5-10 T_obs ... up to a companion mass of 10 M_sun").  The series is built in float32
+    chunks: at 2^28 samples every float64 temporary is 2 GiB."""
+    n, tsamp = 1 << log2n, 81.92e-6
+    T = n * tsamp
+    rng = _rng(7)
+    x = rng.standard_normal(n, dtype=np.float32)
+    phi0 = rng.uniform(0.0, 2.0 * np.pi)
+    psr = (0.005, 7.0 * T, 12.0, phi0, 0.0, 0.0, default_amplitude(n))
+    bank = _bank(rng, n_templates - 1, 5.0 * T, 10.0 * T, 0.0, 20.0)
+    step = 1 << 22
+    sig = DUTY / (2.0 * math.sqrt(2.0 * math.log(2.0)))
+    for j0 in range(0, n, step):
+        s = (j0 + np.arange(min(step, n - j0), dtype=np.float64)) * tsamp
+        ph = emission_times(s, *psr[1:6]) / psr[0]
+        d = ph - np.rint(ph)
+        x[j0:j0 + len(s)] += (psr[6] * np.exp(-0.5 * (d / sig) ** 2)).astype(np.float32)
+    templates = np.vstack([np.array([[psr[1], psr[2], psr[3], 0.0, 0.0]]), bank])
+    return Workload("terzan/2^%d" % log2n, n, tsamp, x, templates, (0,), (psr,))
+
+
 def by_name(name: str, **kw) -> Workload:
-    return {"C1": config1, "C2": config2, "C3": config3, "C4": config4, "C5": config5}[name](**kw)
+    return {"C1": config1, "C2": config2, "C3": config3, "C4": config4, "C5": config5, "paper": config_paper, "terzan": config_terzan}[name](**kw)
 
 
 def shard_templates(n_templates: int, rank: int, world: int):

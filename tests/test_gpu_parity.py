@@ -236,11 +236,42 @@ def test_c4_full_size_elliptical(tb):
 
 def test_c3_full_size_quantised(tb):
     """2^25 samples: the oracle needs ~20 s and ~6 GB per template, so the default run compares the
-    true template, 31 of the ~890 templates with a (noise) candidate and 64 sampled others; with
-    TB_PARITY_FULL=1 all of them (955 templates: profiles/r02_parity_full.txt)."""
+    true template, 15 of the ~890 templates with a (noise) candidate and 32 sampled others; with
+    TB_PARITY_FULL=1 all of them and 64 sampled (955 templates: profiles/r02_parity_full.txt)."""
     w = wl_mod.config3()
-    cands, rep = full_bank_parity(tb, w, 6.0, [0], n_sampled=64, seed=33, max_hit_templates=31)
+    cands, rep = full_bank_parity(tb, w, 6.0, [0], n_sampled=64 if FULL else 32, seed=33, max_hit_templates=15)
     assert 0 in by_template(cands)
+
+
+def test_paper_shaped_bank_at_2p24(tb):
+    """the paper's own simulation shape (Table 2: 2^24 samples at 256 us, 15 ms
+    pulsar, e = 0.1, P_orb = 8 h = 6.7 T_obs) and a bank over Table 1's box (P_orb = 6-12 h, e <= 0.1)."""
+    w = wl_mod.config_paper()
+    cands, rep = full_bank_parity(tb, w, 6.0, [0], n_sampled=12, seed=66, max_hit_templates=12)
+    per = by_template(cands)
+    best = per[0][np.argmax(per[0]["sigma"])]
+    f = best["bin"] / ((1 << int(best["fold"])) * w.t_obs)
+    assert abs(f - 1 / 0.015) < 2.0 / w.t_obs and float(best["sigma"]) > 10
+
+
+@pytest.mark.skipif(not FULL, reason="2^28 samples: the oracle needs ~55 GB and minutes per template; run with TB_PARITY_FULL=1 "
+                                     "(recorded in profiles/r02_parity_full.txt)")
+def test_terzan_length_series_2p28(tb):
+    """a Terzan-5-length series (L489), N = 2^28 (the largest the plan accepts; library-FFT
+    path): the true template and one other compared in full with the oracle, one at a time."""
+    w = wl_mod.config_terzan()
+    with tb.Plan(w.series, w.tsamp, enable_timings=True) as plan:
+        plan.search(w.templates, 0, w.folds, 6.0)
+        assert plan.timings()["fft_path_used"] == 1
+        cands, n = plan.candidates()
+        per = by_template(cands)
+        assert 0 in per
+        best = per[0][np.argmax(per[0]["sigma"])]
+        assert abs(best["bin"] / ((1 << int(best["fold"])) * w.t_obs) - 200.0) < 2.0 / w.t_obs
+        rep = pooled_parity(plan, w, [0, 3], 6.0, w.folds, per, hsums_ids=[0], workers=1)
+    SUMMARY.append(f"{w.name} sigma 6: bank {len(w.templates)} searched on the GPU, {len(cands)} candidates; oracle compared on 2 templates "
+                   f"(1 with all 5 x Nb harmonic sums); index flips {sum(r['flips'] for r in rep.values())}, worst spectrum error "
+                   f"{max(r['err_norm'] for r in rep.values()):.2g}")
 
 
 @pytest.mark.parametrize("log2n,n_check", [(20, 64), (22, 64), (23, 64), (24, 16), (26, 4)])

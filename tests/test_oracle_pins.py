@@ -524,3 +524,54 @@ def test_ell_delay_against_the_kepler_solve_and_closed_forms():
     a = orc.resample_indices(1 << 18, tsamp, tm, model="ell")
     b = orc.resample_indices(1 << 18, tsamp, tm)
     assert np.count_nonzero(a != b) > 1000 and 2 <= np.max(np.abs(a - b)) <= 8
+
+
+# ------------------------------------------------------------------ G12b: 2x-oversampled interbinning
+def test_oversampled_interbinning_closed_forms():
+    """Tone at an integer bin: P'_{2k0} = (A N / 2)^2 and both neighbouring half bins (pi/4)^2 of it; tone
+    midway between bins: the raw bins see (2/pi)^2 = 0.405, the half bin between them 1.0 (N -> infinity);
+    even entries are the raw powers; X_0 is removed before differencing; the last half bin uses the Nyquist bin."""
+    n, A = 4096, 0.7
+    j = np.arange(n)
+    full = (A * n / 2) ** 2
+    X = orc.rfft_forward(A * np.cos(2 * np.pi * 200 * j / n + 0.4) + 5.0)            # + DC
+    P = orc.interbin_power_oversampled(X)
+    assert P.size == n and P[0] == 0.0
+    assert P[400] == pytest.approx(full, rel=1e-12)
+    assert P[399] == pytest.approx((math.pi / 4) ** 2 * full, rel=1e-9) and P[401] == pytest.approx((math.pi / 4) ** 2 * full, rel=1e-9)
+    assert P[1] == pytest.approx((math.pi / 4) ** 2 * abs(X[1]) ** 2, rel=1e-12, abs=1e-18)      # DC did not leak in
+    raw = np.abs(X[: n // 2]) ** 2
+    raw[0] = 0.0
+    assert np.allclose(P[0::2], raw, rtol=1e-13, atol=1e-12)
+    Xh = orc.rfft_forward(A * np.cos(2 * np.pi * 200.5 * j / n + 0.4))
+    Ph = orc.interbin_power_oversampled(Xh)
+    assert Ph[400] / full == pytest.approx((2 / math.pi) ** 2, rel=5e-3) and Ph[402] / full == pytest.approx((2 / math.pi) ** 2, rel=5e-3)
+    assert Ph[401] / full == pytest.approx(1.0, rel=5e-3)
+    assert np.argmax(Ph) == 401
+    Xn = orc.rfft_forward(np.cos(np.pi * j))                                          # Nyquist tone
+    assert orc.interbin_power_oversampled(Xn)[-1] == pytest.approx((math.pi / 4) ** 2 * n * n, rel=1e-12)
+    # white noise: even half bins have unit mean (in units of N sigma^2), odd ones pi^2/8
+    rng = np.random.default_rng(4)
+    Pn = orc.interbin_power_oversampled(orc.rfft_forward(rng.standard_normal(1 << 16))) / (1 << 16)
+    assert Pn[0::2].mean() == pytest.approx(1.0, rel=0.02) and Pn[1::2].mean() == pytest.approx(math.pi ** 2 / 8, rel=0.02)
+
+
+def test_oversampled_search_recovers_a_half_bin_pulsar():
+    """End to end on a scalloped signal: a sinusoid midway between two bins in noise.  The oversampled
+    search finds it in the odd half bin with ~pi^2/4 more power than the plain spectrum's raw bins; its
+    candidate frequencies are k / (2^(L+1) T_obs); k_lo doubles."""
+    n, tsamp = 1 << 14, 1e-3
+    rng = np.random.default_rng(8)
+    j = np.arange(n)
+    x = (rng.standard_normal(n) + 0.12 * np.cos(2 * np.pi * 1000.5 * j / n)).astype(np.float32)
+    tmpl = (50.0, 0.0, 0.0, 0.0, 0.0)                                                 # tau = 0: no resampling
+    over = orc.search_template(x, tsamp, tmpl, 0, (0,), 5.0, window=1024, oversample=True)
+    assert orc.lowest_bin_oversampled(n, tsamp, 0.1) == 2 * orc.lowest_bin(n, tsamp, 0.1)
+    best = max(over, key=lambda c: c[4])
+    assert best[2] == 2001                                                            # half bin 2 * 1000.5
+    spec = orc.spectrum_of_template(x, tsamp, tmpl, 1024, oversample=True)
+    plain = orc.spectrum_of_template(x, tsamp, tmpl, 1024)
+    assert spec["power"].size == n and spec["medians"].size == n // 1024 and plain["power"].size == n // 2
+    raw_best = max(spec["power"][2000], spec["power"][2002])                          # even half bins are the raw |X_k|^2
+    assert spec["power"][2001] > 1.8 * raw_best                                       # (pi/2)^2 = 2.47 without noise
+    assert plain["power"][1001] == pytest.approx(0.5 * (4 / math.pi) ** 2 * spec["power"][2001], rel=1e-12)   # G12's 1/2 |dX|^2

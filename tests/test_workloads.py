@@ -30,6 +30,23 @@ def test_small_variants_of_c2_c3_c4_c5():
     assert beta.min() >= 0.001 and beta.max() <= 0.1
 
 
+def test_paper_shaped_workloads_small():
+    """the paper's own simulation shape (Table 2) and a Terzan-5-length series, scaled down."""
+    p = wl.config_paper(log2n=16, n_templates=8)
+    assert p.tsamp == 256e-6 and p.templates.shape == (8, 5) and p.true_ids == (0,)
+    assert p.templates[0, 0] == 8 * 3600.0 and p.templates[0, 3] == 0.1
+    t = p.templates[1:]
+    assert t[:, 0].min() >= 6 * 3600 and t[:, 0].max() <= 12 * 3600 and t[:, 1].max() <= 7 and t[:, 3].max() <= 0.1
+    z = wl.config_terzan(log2n=16, n_templates=4)
+    assert z.tsamp == 81.92e-6 and z.series.dtype == np.float32 and np.all(z.templates[:, 3:] == 0)
+    assert 5 * z.t_obs <= z.templates[1:, 0].min() and z.templates[1:, 0].max() <= 10 * z.t_obs
+    assert np.array_equal(z.series, wl.config_terzan(log2n=16, n_templates=4).series)
+    # chunked injection = one-shot injection
+    ref = wl.pulse_train(z.n_samples, z.tsamp, *z.pulsars[0][:7])
+    noise = wl._rng(7).standard_normal(z.n_samples, dtype=np.float32)
+    assert np.allclose(z.series - noise, ref.astype(np.float32), atol=1e-6)
+
+
 def test_injection_is_inverse_of_the_gather_map():
     """s = t' - (Delta(t') - Delta(0)) solved for t': residual check (reading G3)."""
     s = np.linspace(0, 100, 1001)
