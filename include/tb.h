@@ -122,6 +122,13 @@ typedef struct {
                                      G26): cos E and sqrt(1-e^2) sin E from the printed series through e^6, no Kepler
                                      solve; differs from 0 by about 1.2 e^7 tau (0.015 samples at e = 0.1, tau/tsamp =
                                      1.25e5), so a mode of its own with its own oracle, not bit-compatible with 0 */
+    int32_t  interbin_oversample; /* 0: the interbinned spectrum of N/2 bins (G12); 1: the 2x-oversampled spectrum of
+                                     N HALF bins (reading G12b; Ransom et al. 2002, the paper's reference for scalloping,
+                                     L289): P'_2k = |X_k|^2, P'_2k+1 = (pi/4)^2 |X_k - X_k+1|^2.  Everything downstream
+                                     counts half bins: W of them per median block, candidate.bin = half bin of the highest
+                                     summed harmonic (fundamental frequency bin / (2^(fold+1) N tsamp) Hz), k_lo doubled,
+                                     tb_debug_spectrum / tb_debug_hsums return N (5 N) values.  Library-FFT path only
+                                     (fft_path 2 -> TB_ERR_INVALID_ARG), not with whiten, N <= 2^27 */
 } tb_plan_opts;
 
 /* Per-stage device time of the last tb_search_templates call (CUDA events on the plan's stream,

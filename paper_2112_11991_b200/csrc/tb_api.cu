@@ -40,7 +40,9 @@ struct tb_plan {
     int device = 0;
     cudaStream_t stream = nullptr;
     bool own_stream = false;
-    uint64_t n = 0, nb = 0;
+    uint64_t n = 0, nb = 0;                         // samples, FFT bins N/2
+    uint64_t nsp = 0;                                // spectrum bins: nb, or 2 nb half bins with interbin_oversample (G12b)
+    bool over = false;
     double tsamp = 0.0;
     uint32_t window = 1024, log2w = 10, nblk = 0;
     double f_min = 0.1;
@@ -434,6 +436,11 @@ void launch_spectrum(tb_plan* p, uint32_t nt, float* d_raw)
     const unsigned grid = (unsigned)(cta_per_row * nt), threads = (SP_WARPS + 1) * 32;
     unsigned long long* fb = p->d_cursor + 1;
     const int nb = (int)p->nb, nblk = (int)p->nblk;
+    if (p->over) {                                       // 2x-oversampled spectrum (G12b): nsp = 2 nb half bins
+        if (d_raw) k_spectrum_median<W, false, true, false, true><<<grid, threads, 0, p->stream>>>(p->d_fft, p->ld, p->d_power, p->d_med, (int)p->nsp, nblk, cta_per_row, nullptr, nullptr, fb, d_raw, 0.f);
+        else       k_spectrum_median<W, false, false, false, true><<<grid, threads, 0, p->stream>>>(p->d_fft, p->ld, p->d_power, p->d_med, (int)p->nsp, nblk, cta_per_row, nullptr, nullptr, fb, nullptr, 0.f);
+        return;
+    }
     const bool white = p->whiten && !p->whitening_now;   // the whitening procedure itself needs the medians
     if (white) {
         if (d_raw) k_spectrum_median<W, false, true, true><<<grid, threads, 0, p->stream>>>(p->d_fft, p->ld, p->d_power, p->d_med, nb, nblk, cta_per_row, nullptr, nullptr, fb, d_raw, p->kappa);
@@ -673,27 +680,27 @@ int run_spectrum(tb_plan* p, uint32_t nt, float* d_raw)
 int run_hsum(tb_plan* p, size_t off, uint32_t nt, const FoldParams& fp, float* tap = nullptr)
 {
     const TmplDev* tm = p->d_tmpl + off;
-    if (p->nb >= (uint64_t)HS_T) {
-        const int tiles = (int)(p->nb / HS_T);
+    if (p->nsp >= (uint64_t)HS_T) {
+        const int tiles = (int)(p->nsp / HS_T);
         const int tpc = std::min(tiles, HS_TPC);                                     // tiles walked by one CTA (double-buffered)
         const size_t smem = HS_BUFS * HS_SMEM_FLOATS * sizeof(float);
         const unsigned grid = (unsigned)((tiles / tpc) * nt);
         if (tap) {
             if (int rc_ = allow_smem(p, reinterpret_cast<const void*>(k_hsum_tile<true>), smem)) return rc_;
-            k_hsum_tile<true><<<grid, HS_THREADS, smem, p->stream>>>(p->d_power, (int)p->nb, tiles / tpc, tpc, fp, tm, p->d_cand, p->d_cursor,
+            k_hsum_tile<true><<<grid, HS_THREADS, smem, p->stream>>>(p->d_power, (int)p->nsp, tiles / tpc, tpc, fp, tm, p->d_cand, p->d_cursor,
                                                                     (unsigned long long)p->max_cand, tap);
         } else {
             if (int rc_ = allow_smem(p, reinterpret_cast<const void*>(k_hsum_tile<false>), smem)) return rc_;
-            k_hsum_tile<false><<<grid, HS_THREADS, smem, p->stream>>>(p->d_power, (int)p->nb, tiles / tpc, tpc, fp, tm, p->d_cand, p->d_cursor,
+            k_hsum_tile<false><<<grid, HS_THREADS, smem, p->stream>>>(p->d_power, (int)p->nsp, tiles / tpc, tpc, fp, tm, p->d_cand, p->d_cursor,
                                                                      (unsigned long long)p->max_cand, nullptr);
         }
         TB_CUDA(p, cudaGetLastError());
         return TB_OK;
     }
-    const int cta_per_row = (int)((p->nb + 255) / 256);
-    if (tap) k_hsum_threshold<true><<<(unsigned)(cta_per_row * nt), 256, 0, p->stream>>>(p->d_power, (int)p->nb, cta_per_row, fp, tm, p->d_cand,
+    const int cta_per_row = (int)((p->nsp + 255) / 256);
+    if (tap) k_hsum_threshold<true><<<(unsigned)(cta_per_row * nt), 256, 0, p->stream>>>(p->d_power, (int)p->nsp, cta_per_row, fp, tm, p->d_cand,
                                                                                      p->d_cursor, (unsigned long long)p->max_cand, tap);
-    else     k_hsum_threshold<false><<<(unsigned)(cta_per_row * nt), 256, 0, p->stream>>>(p->d_power, (int)p->nb, cta_per_row, fp, tm, p->d_cand,
+    else     k_hsum_threshold<false><<<(unsigned)(cta_per_row * nt), 256, 0, p->stream>>>(p->d_power, (int)p->nsp, cta_per_row, fp, tm, p->d_cand,
                                                                                       p->d_cursor, (unsigned long long)p->max_cand, nullptr);
     TB_CUDA(p, cudaGetLastError());
     return TB_OK;
@@ -804,7 +811,7 @@ int make_fold_params(tb_plan* p, const uint32_t* folds, uint32_t n_folds, double
         const double root = mu + sigma * s;
         fp->thr[L] = seen[L] ? (root <= 0 ? 0.f : (float)(root * root)) : std::numeric_limits<float>::infinity();
     }
-    for (uint32_t L = 0; L < 5; ++L) fp->lo[L] = (uint32_t)std::min<uint64_t>((uint64_t)p->k_lo << L, p->nb);
+    for (uint32_t L = 0; L < 5; ++L) fp->lo[L] = (uint32_t)std::min<uint64_t>((uint64_t)p->k_lo << L, p->nsp);
     return TB_OK;
 }
 
@@ -894,9 +901,13 @@ int tb_plan_create(tb_plan** out, const float* series, uint64_t n_samples, doubl
     p->tsamp = tsamp_s;
     p->window = W;
     p->log2w = ilog2(W);
-    p->nblk = (uint32_t)(p->nb / W);
+    p->over = o.interbin_oversample != 0;
+    if (o.interbin_oversample != 0 && o.interbin_oversample != 1) { delete p; return TB_ERR_INVALID_ARG; }
+    if (p->over && (o.whiten || n_samples > (1ull << 27))) { delete p; return TB_ERR_INVALID_ARG; }   // no whitened variant; 2 nb must fit the 32-bit bin index
+    p->nsp = p->over ? 2 * p->nb : p->nb;
+    p->nblk = (uint32_t)(p->nsp / W);
     p->f_min = (o.f_min_hz == 0.0) ? 0.1 : (o.f_min_hz < 0 ? 0.0 : o.f_min_hz);
-    p->k_lo = (uint32_t)std::min<double>(std::ceil(p->f_min * ((double)n_samples * tsamp_s)), 4294967295.0);
+    p->k_lo = (uint32_t)std::min<double>(std::ceil(p->f_min * ((double)n_samples * tsamp_s)) * (p->over ? 2.0 : 1.0), 4294967295.0);   // half bins when oversampled
     p->max_cand = o.max_candidates ? o.max_candidates : (1ull << 22);
     p->timings = o.enable_timings != 0;
     p->whiten = o.whiten != 0;
@@ -926,7 +937,7 @@ int tb_plan_create(tb_plan** out, const float* series, uint64_t n_samples, doubl
     TB_TRY(cudaEventCreateWithFlags(&p->ev_staged, cudaEventDisableTiming));
 
     // chunk size B
-    const size_t per_t = (size_t)p->n * 4 + p->ld * 8 + (size_t)p->nb * 4 + (size_t)p->nblk * 4 + (size_t)p->n * 8;
+    const size_t per_t = (size_t)p->n * 4 + p->ld * 8 + (size_t)p->nsp * 4 + (size_t)p->nblk * 4 + (size_t)p->n * 8;
     uint32_t B = o.chunk_templates;
     if (B == 0) {
         size_t free_b = 0, total_b = 0;
@@ -948,8 +959,8 @@ int tb_plan_create(tb_plan** out, const float* series, uint64_t n_samples, doubl
         p->log2m1 = lm == 25 ? 9 : lm == 24 ? 8 : lm == 23 ? 10 : lm >= 17 ? 9 : 8;   // 2^25, 2^26: three passes, M2 = 2^16
         p->log2m2 = lm - p->log2m1;
         const bool fits = ((p->log2m2 >= 8 && p->log2m2 <= 13) || (p->log2m2 == 16 && lm >= 24)) && spectrum_t_supported(W, p->log2m1) && p->nblk >= 16 && p->nblk % 16 == 0;
-        if (o.fft_path >= 2 && !fits) { destroy(p); return TB_ERR_INVALID_ARG; }
-        p->own_fft = fits && o.fft_path != 1;
+        if (o.fft_path >= 2 && (!fits || p->over)) { destroy(p); return TB_ERR_INVALID_ARG; }
+        p->own_fft = fits && o.fft_path != 1 && !p->over;         // the oversampled spectrum is formed from the library R2C output
     }
     if (p->own_fft) {
         cudaDeviceGetAttribute(&p->n_sm, cudaDevAttrMultiProcessorCount, p->device);
@@ -959,7 +970,7 @@ int tb_plan_create(tb_plan** out, const float* series, uint64_t n_samples, doubl
     }
     TB_TRY(cudaMalloc(&p->d_resampled, (size_t)B * p->n * sizeof(float)));
     TB_TRY(cudaMalloc(&p->d_fft, (size_t)B * p->ld * sizeof(float2)));
-    TB_TRY(cudaMalloc(&p->d_power, (size_t)B * p->nb * sizeof(float)));
+    TB_TRY(cudaMalloc(&p->d_power, (size_t)B * p->nsp * sizeof(float)));
     TB_TRY(cudaMalloc(&p->d_med, (size_t)B * p->nblk * sizeof(float)));
     TB_TRY(cudaMalloc(&p->d_cand, p->max_cand * sizeof(Candidate)));
     TB_TRY(cudaMalloc(&p->d_cursor, 2 * sizeof(unsigned long long)));   // [0] candidate cursor, [1] median fallbacks
@@ -1204,14 +1215,14 @@ int tb_debug_spectrum(tb_plan* p, const tb_template* tmpl, float* p_interbinned,
         if ((rc = run_fft(p, 1))) return rc;
     }
     float* d_raw = nullptr;
-    TB_CUDA(p, cudaMalloc(&d_raw, p->nb * sizeof(float)));
+    TB_CUDA(p, cudaMalloc(&d_raw, p->nsp * sizeof(float)));
     rc = own ? run_spectrum_t(p, 1, d_raw) : run_spectrum(p, 1, d_raw);
     cudaError_t e = cudaSuccess;
-    if (!rc && p_interbinned) e = cudaMemcpyAsync(p_interbinned, d_raw, p->nb * sizeof(float), cudaMemcpyDeviceToHost, p->stream);
+    if (!rc && p_interbinned) e = cudaMemcpyAsync(p_interbinned, d_raw, p->nsp * sizeof(float), cudaMemcpyDeviceToHost, p->stream);
     if (!rc && e == cudaSuccess && medians)
         e = cudaMemcpyAsync(medians, p->d_med, p->nblk * sizeof(float), cudaMemcpyDeviceToHost, p->stream);
     if (!rc && e == cudaSuccess && p_normalised)
-        e = cudaMemcpyAsync(p_normalised, p->d_power, p->nb * sizeof(float), cudaMemcpyDeviceToHost, p->stream);
+        e = cudaMemcpyAsync(p_normalised, p->d_power, p->nsp * sizeof(float), cudaMemcpyDeviceToHost, p->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(p->stream);
     cudaFree(d_raw);
     if (rc) return rc;
@@ -1247,10 +1258,10 @@ int tb_debug_hsums(tb_plan* p, const tb_template* tmpl, float* sums_out)
     FoldParams fp;
     for (int L = 0; L < 5; ++L) { fp.thr[L] = std::numeric_limits<float>::infinity(); fp.mu[L] = 0.f; fp.inv_s[L] = 0.f; fp.lo[L] = 0; }
     float* d_tap = nullptr;
-    TB_CUDA(p, cudaMalloc(&d_tap, 5 * p->nb * sizeof(float)));
+    TB_CUDA(p, cudaMalloc(&d_tap, 5 * p->nsp * sizeof(float)));
     rc = run_hsum(p, 0, 1, fp, d_tap);
     cudaError_t e = cudaSuccess;
-    if (!rc) e = cudaMemcpyAsync(sums_out, d_tap, 5 * p->nb * sizeof(float), cudaMemcpyDeviceToHost, p->stream);
+    if (!rc) e = cudaMemcpyAsync(sums_out, d_tap, 5 * p->nsp * sizeof(float), cudaMemcpyDeviceToHost, p->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(p->stream);
     cudaFree(d_tap);
     if (rc) return rc;
@@ -1294,7 +1305,7 @@ int tb_debug_set_candidates(tb_plan* p, const tb_candidate* cands, uint64_t n)
     if (!p || (n && !cands)) return fail(p, TB_ERR_INVALID_ARG, "null argument");
     if (n > p->max_cand) return fail(p, TB_ERR_CAPACITY, "more rows than max_candidates");
     for (uint64_t i = 0; i < n; ++i)
-        if (cands[i].fold > TB_MAX_FOLD || cands[i].bin >= p->nb) return fail(p, TB_ERR_INVALID_ARG, "row " + std::to_string(i) + ": fold or bin out of range");
+        if (cands[i].fold > TB_MAX_FOLD || cands[i].bin >= p->nsp) return fail(p, TB_ERR_INVALID_ARG, "row " + std::to_string(i) + ": fold or bin out of range");
     TB_CUDA(p, cudaSetDevice(p->device));
     const unsigned long long count = n;
     if (n) TB_CUDA(p, cudaMemcpyAsync(p->d_cand, cands, n * sizeof(Candidate), cudaMemcpyHostToDevice, p->stream));

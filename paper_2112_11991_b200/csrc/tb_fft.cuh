@@ -472,6 +472,69 @@ k_fft_cols(const float* __restrict__ x, const SegRec* __restrict__ seg, size_t s
 constexpr int C32_PK = 16, C32_LP = 32 * C32_PK + 1;
 constexpr size_t C32_SMEM = (size_t)16 * C32_LP * sizeof(float2);
 
+// ---------------------------------------------------------------------------------------------
+// index phase of k_fft_cols32.  Work item = 4 consecutive output samples (columns 2q, 2q + 1 of row
+// r): thread (q, r0) = (tid & 7, tid >> 3) takes rows r0 + 32 i, i < 16.  One segment record (two
+// loads), one row address and one tie limit now serve four samples instead of two, the cubic's
+// arguments t_k are the same for every row of the thread, and every h >= 4 goes through the same
+// code (a group of 4 aligned samples never straddles a segment).  The indices are parked as int2 in
+// the points' own slots, slot(col, r) = fsm[col LP + r]; a barrier separates this from the gather,
+// which reads them with the (col, c) mapping of the FFT.
+// ---------------------------------------------------------------------------------------------
+template <bool CLAMP>
+__device__ __forceinline__ void cols32_park_indices(const SegRec* __restrict__ segs, int log2h, float inv_h,
+                                                    float2* __restrict__ fsm, int c0, int row_shift, int n)
+{
+    constexpr int LP = C32_LP;
+    constexpr float MAGIC = 12582912.0f;                                       // 1.5 * 2^23: round to nearest integer
+    const int q = threadIdx.x & 7, r0 = threadIdx.x >> 3;
+    const int nnq = (c0 + 2 * q) << 1;                                         // first sample of the group in row 0
+    const int o = nnq & ((1 << log2h) - 1);
+    float t[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) t[k] = (float)(o + k) * inv_h;
+    const int rec_shift = row_shift - log2h + 6;                               // log2 bytes between the records of rows r, r + 1
+    const char* __restrict__ rec = reinterpret_cast<const char*>(segs + (nnq >> log2h)) + ((size_t)r0 << rec_shift);
+    const unsigned rec_step = 32u << rec_shift;                                // rows r, r + 32; 15 rec_step < 2^27
+    const int nn0 = nnq + (r0 << row_shift), nn_step = 32 << row_shift;
+    int2* __restrict__ slot = reinterpret_cast<int2*>(fsm + (2 * q) * LP + r0);
+    unsigned ties = 0;                                                         // items with a sample too close to a rounding tie for fp32
+#pragma unroll 8
+    for (int i = 0; i < 16; ++i) {
+        const char* r = rec + (size_t)((unsigned)i * rec_step);
+        const float4 f = __ldg(reinterpret_cast<const float4*>(r));
+        const int2 ie = __ldg(reinterpret_cast<const int2*>(r) + 2);
+        float y[4], z[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            y[k] = fmaf(fmaf(fmaf(f.w, t[k], f.z), t[k], f.y), t[k], f.x);
+            z[k] = y[k] + MAGIC;
+        }
+        const float res = fmaxf(fmaxf(fabsf(y[0] - (z[0] - MAGIC)), fabsf(y[1] - (z[1] - MAGIC))),
+                                fmaxf(fabsf(y[2] - (z[2] - MAGIC)), fabsf(y[3] - (z[3] - MAGIC))));
+        ties |= (res > 0.5f - __int_as_float(ie.y) ? 1u : 0u) << i;
+        const int base = nn0 + i * nn_step - ie.x + 0x4B400000;
+        slot[i * 32]      = clamp_pair<CLAMP>(make_int2(base - __float_as_int(z[0]), base + 1 - __float_as_int(z[1])), n);
+        slot[i * 32 + LP] = clamp_pair<CLAMP>(make_int2(base + 2 - __float_as_int(z[2]), base + 3 - __float_as_int(z[3])), n);
+    }
+    while (ties) {                                                             // rare (about 4 eps per item): decide in fp64
+        const int i = __ffs(ties) - 1;
+        ties &= ties - 1;
+        const char* r = rec + (size_t)((unsigned)i * rec_step);
+        const double2 c01 = __ldg(reinterpret_cast<const double2*>(r) + 2);
+        const double2 c23 = __ldg(reinterpret_cast<const double2*>(r) + 3);
+        const int nn = nn0 + i * nn_step;
+        int s[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            const double tk = (double)(o + k) * (double)inv_h;
+            s[k] = nn + k - floor_to_int(fma(fma(fma(c23.y, tk, c23.x), tk, c01.y), tk, c01.x));
+        }
+        slot[i * 32]      = clamp_pair<CLAMP>(make_int2(s[0], s[1]), n);
+        slot[i * 32 + LP] = clamp_pair<CLAMP>(make_int2(s[2], s[3]), n);
+    }
+}
+
 template <bool DEBUG>
 __global__ void __launch_bounds__(FFT_THREADS, COLS_MINB)
 k_fft_cols32(const float* __restrict__ x, const SegRec* __restrict__ seg, size_t seg_stride,
@@ -502,7 +565,8 @@ k_fft_cols32(const float* __restrict__ x, const SegRec* __restrict__ seg, size_t
     float2* __restrict__ myslot = fsm + col * LP + c;                          // + a' PK, a' = 16 a + it
     const int nn0 = (int)((((size_t)c << log2m2) + c0 + col) << 1);
     const int row_shift = log2m2 + 1;
-    cols_park_indices<2, C, 16 * PK, PK, !DEBUG>(segs, log2h, inv_h, myslot, nn0, row_shift, n);
+    cols32_park_indices<!DEBUG>(segs, log2h, inv_h, fsm, c0, row_shift, n);
+    __syncthreads();                                                           // the indices were parked by other threads
     {   // gather (64 independent loads), radix 32 over a', twiddle, back to the same slots
         float2 v[32];
 #pragma unroll

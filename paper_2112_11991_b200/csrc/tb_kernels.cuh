@@ -397,7 +397,11 @@ __device__ __forceinline__ float warp_median(const float (&p)[W / 32], float* ca
 
 //   WHITE = true (plan option whiten, reading G25): the series was whitened once, the block medians
 //   are skipped and P^_k = kappa P_k with the plan's constant kappa (med[] receives ln2 / kappa).
-template <int W, bool UNPACK, bool RAW, bool WHITE = false>
+//   OVER = true (plan option interbin_oversample, reading G12b): the output is the 2x-oversampled
+//   spectrum of 2 nb_in half bins, P'_2k = |X_k|^2, P'_2k+1 = (pi/4)^2 |X_k - X_k+1|^2 (X_nb = the
+//   Nyquist bin of the R2C output); `nb` is then the number of half bins and a block of W half bins
+//   covers W/2 input bins.
+template <int W, bool UNPACK, bool RAW, bool WHITE = false, bool OVER = false>
 __global__ void __launch_bounds__((SP_WARPS + 1) * 32)
 k_spectrum_median(const float2* __restrict__ X, size_t ld, float* __restrict__ P, float* __restrict__ med,
                   int nb, int nblk_per_row, int cta_per_row, const float2* __restrict__ twn,
@@ -433,6 +437,26 @@ k_spectrum_median(const float2* __restrict__ X, size_t ld, float* __restrict__ P
                                     make_float2(wp.x * wl.x - wp.y * wl.y, wp.x * wl.y + wp.y * wl.x));
             }
         } else if (base > 0 && lane == 0) carry = __ldg(Xr + base - 1);
+        if constexpr (OVER) {
+            static_assert(!UNPACK && !WHITE, "the oversampled spectrum is formed from the library R2C output");
+            constexpr float C = 0.61685027506808491368f;     // (pi/4)^2
+#pragma unroll
+            for (int i = 0; i < ITER; ++i) {
+                const int q0 = base + i * 128 + lane * 4;    // first of the lane's 4 half bins; input bins k0, k0+1 (+ k0+2)
+                const int k0 = q0 >> 1;
+                float4 a = __ldg(reinterpret_cast<const float4*>(Xr + k0));
+                const float2 nx = __ldg(Xr + k0 + 2);
+                if (k0 == 0) { a.x = 0.f; a.y = 0.f; }       // X_0 <- 0 before differencing (G13)
+                float dx, dy;
+                float4 o;
+                o.x = a.x * a.x + a.y * a.y;
+                dx = a.x - a.z;  dy = a.y - a.w;  o.y = C * (dx * dx + dy * dy);
+                o.z = a.z * a.z + a.w * a.w;
+                dx = a.z - nx.x; dy = a.w - nx.y; o.w = C * (dx * dx + dy * dy);
+                if (RAW && owner) *reinterpret_cast<float4*>(Praw + (size_t)row * (size_t)nb + q0) = o;
+                p[4 * i + 0] = o.x; p[4 * i + 1] = o.y; p[4 * i + 2] = o.z; p[4 * i + 3] = o.w;
+            }
+        } else
 #pragma unroll
         for (int i = 0; i < ITER; ++i) {
             const int k0 = base + i * 128 + lane * 4;

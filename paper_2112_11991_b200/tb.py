@@ -36,7 +36,7 @@ class PlanOpts(C.Structure):
                 ("chunk_templates", C.c_uint32), ("series_is_device_ptr", C.c_int32), ("has_fill", C.c_int32),
                 ("fill_value", C.c_float), ("enable_timings", C.c_int32), ("fft_path", C.c_int32),
                 ("whiten", C.c_int32), ("n_zap_ranges", C.c_uint32), ("zap_ranges", C.c_void_p),
-                ("delay_model", C.c_int32)]
+                ("delay_model", C.c_int32), ("interbin_oversample", C.c_int32)]
 
 
 class BankSpace(C.Structure):
@@ -117,7 +117,7 @@ def as_templates(templates) -> np.ndarray:
 
 def tb_plan_create(series, n_samples, tsamp_s, *, device=0, stream=None, median_window=0, f_min_hz=0.0,
                    max_candidates=0, chunk_templates=0, series_is_device_ptr=False, fill_value=None,
-                   enable_timings=False, fft_path=0, whiten=False, zap_ranges=(), delay_model=0):
+                   enable_timings=False, fft_path=0, whiten=False, zap_ranges=(), delay_model=0, interbin_oversample=False):
     """series: numpy float32[N] (host) or an integer device address when series_is_device_ptr."""
     o = PlanOpts()
     o.struct_size = C.sizeof(PlanOpts)
@@ -129,6 +129,7 @@ def tb_plan_create(series, n_samples, tsamp_s, *, device=0, stream=None, median_
     o.fft_path = int(fft_path)
     o.whiten = int(bool(whiten))
     o.delay_model = int(delay_model)
+    o.interbin_oversample = int(bool(interbin_oversample))
     zap = np.ascontiguousarray(np.asarray(zap_ranges, dtype=np.uint32).reshape(-1, 2))
     o.n_zap_ranges, o.zap_ranges = len(zap), (zap.ctypes.data if len(zap) else None)
     if series_is_device_ptr:
@@ -250,17 +251,17 @@ def tb_debug_series(plan, n_samples):
     return x, k.value
 
 
-def tb_debug_hsums(plan, template, n_samples) -> np.ndarray:
-    """float32[5, N/2]: S_L[k] of every fold and bin through the production harmonic summer."""
+def tb_debug_hsums(plan, template, n_samples, oversample=False) -> np.ndarray:
+    """float32[5, N/2] (N half bins with interbin_oversample): S_L[k] of every fold and bin through the production harmonic summer."""
     t = as_templates(template)
-    out = np.empty((5, int(n_samples) // 2), dtype=np.float32)
+    out = np.empty((5, int(n_samples) // (1 if oversample else 2)), dtype=np.float32)
     _check(lib.tb_debug_hsums(plan, t.ctypes.data, out.ctypes.data), plan)
     return out
 
 
-def tb_debug_spectrum(plan, template, n_samples, median_window=1024):
+def tb_debug_spectrum(plan, template, n_samples, median_window=1024, oversample=False):
     t = as_templates(template)
-    nb = int(n_samples) // 2
+    nb = int(n_samples) // (1 if oversample else 2)
     p = np.empty(nb, dtype=np.float32)
     ph = np.empty(nb, dtype=np.float32)
     m = np.empty(nb // int(median_window), dtype=np.float32)
@@ -281,6 +282,7 @@ class Plan:
         self.n_samples = int(n_samples if n_samples is not None else len(series))
         self.tsamp = float(tsamp_s)
         self.median_window = int(opts.get("median_window", 0) or 1024)
+        self.oversample = bool(opts.get("interbin_oversample", False))
         self._series = series                        # keep host/device memory alive
         self.handle = tb_plan_create(series, self.n_samples, tsamp_s, **opts)
 
@@ -322,10 +324,10 @@ class Plan:
         return tb_debug_series(self.handle, self.n_samples)
 
     def debug_hsums(self, template):
-        return tb_debug_hsums(self.handle, template, self.n_samples)
+        return tb_debug_hsums(self.handle, template, self.n_samples, self.oversample)
 
     def debug_spectrum(self, template):
-        return tb_debug_spectrum(self.handle, template, self.n_samples, self.median_window)
+        return tb_debug_spectrum(self.handle, template, self.n_samples, self.median_window, self.oversample)
 
     def close(self):
         if self.handle is not None:

@@ -50,7 +50,7 @@ def check_indices(plan, wl, tmpl, model="bt"):
 WHITE_ATOL = 3e-5                           # |x'_gpu - x'_oracle| of a whitened (unit-variance) series: two fp32 FFTs of length N
 
 
-def compare_template(series, tsamp, tmpl, tid, W, fill, k_lo, f_min, gpu, sigma_threshold, folds, gpu_cands, kappa=None, model="bt"):
+def compare_template(series, tsamp, tmpl, tid, W, fill, k_lo, f_min, gpu, sigma_threshold, folds, gpu_cands, kappa=None, model="bt", oversample=False):
     """All comparisons for one template.  gpu: dict with idx, y, P, Ph, med and optionally S
     (float32[5, Nb]).  Returns a small report dict; raises AssertionError on a parity failure.
     kappa: None for the default path (per-template block medians, G15); for a whitened plan (reading
@@ -58,9 +58,9 @@ def compare_template(series, tsamp, tmpl, tid, W, fill, k_lo, f_min, gpu, sigma_
     series may then differ from the GPU's by the rounding of the whitening FFTs (WHITE_ATOL)."""
     n = len(series)
     n_flips = compare_indices(gpu["idx"], n, tsamp, tmpl, model)           # model: "bt" (Kepler solve) or "ell" (plan delay_model=1)
-    nb = n // 2
+    nb = n if oversample else n // 2                     # spectrum bins (half bins in the oversampled variant G12b)
     if kappa is None:
-        spec = orc.spectrum_of_template(series, tsamp, tmpl, W, fill, idx=gpu["idx"])
+        spec = orc.spectrum_of_template(series, tsamp, tmpl, W, fill, idx=gpu["idx"], oversample=oversample)
         assert np.array_equal(gpu["y"], spec["resampled"]), "resampled series differs"
         base = orc.median_baseline(spec["medians"], nb, W)
         eM = np.abs(gpu["med"].astype(np.float64) - spec["medians"]) / spec["medians"]
@@ -89,7 +89,7 @@ def compare_template(series, tsamp, tmpl, tid, W, fill, k_lo, f_min, gpu, sigma_
     if gpu_cands is not None:
         if sums is None or any(L not in sums for L in folds):
             sums = orc.harmonic_sums(spec["normalised"], folds)
-        assert k_lo == orc.lowest_bin(n, tsamp, f_min)
+        assert k_lo == (orc.lowest_bin_oversampled if oversample else orc.lowest_bin)(n, tsamp, f_min)
         ocand = orc.candidates_from_sums({L: sums[L] for L in folds}, tid, sigma_threshold, k_lo)
         report.update(compare_candidates(gpu_cands, ocand, sums, sigma_threshold))
     return report
@@ -103,7 +103,7 @@ def gpu_outputs(plan, tmpl, hsums=False):
     return out
 
 
-def check_template(plan, wl, tid, sigma_threshold=None, folds=None, gpu_cands=None, hsums=False, white=None, model="bt"):
+def check_template(plan, wl, tid, sigma_threshold=None, folds=None, gpu_cands=None, hsums=False, white=None, model="bt", oversample=False):
     """Full per-template parity in this process; returns a small report dict.
     white: (oracle's whitened series, oracle's kappa) for a plan created with whiten=True."""
     tmpl = wl.templates[tid]
@@ -113,7 +113,7 @@ def check_template(plan, wl, tid, sigma_threshold=None, folds=None, gpu_cands=No
     series, kappa = (wl.series, None) if white is None else white
     fill = info["fill_value"] if white is None else orc.fill_value(series)
     return compare_template(series, wl.tsamp, tmpl, tid, plan.median_window, fill, info["k_lo"], wl.f_min,
-                            gpu_outputs(plan, tmpl, hsums), sigma_threshold, folds, gpu_cands, kappa, model)
+                            gpu_outputs(plan, tmpl, hsums), sigma_threshold, folds, gpu_cands, kappa, model, oversample)
 
 
 def compare_candidates(gpu_cands, ocand, sums, sigma_threshold):
