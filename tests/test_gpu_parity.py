@@ -247,7 +247,7 @@ def test_paper_shaped_bank_at_2p24(tb):
     """the paper's own simulation shape (Table 2: 2^24 samples at 256 us, 15 ms
     pulsar, e = 0.1, P_orb = 8 h = 6.7 T_obs) and a bank over Table 1's box (P_orb = 6-12 h, e <= 0.1)."""
     w = wl_mod.config_paper()
-    cands, rep = full_bank_parity(tb, w, 6.0, [0], n_sampled=12 if FULL else 6, seed=66, max_hit_templates=6)
+    cands, rep = full_bank_parity(tb, w, 6.0, [0], n_sampled=12 if FULL else 4, seed=66, max_hit_templates=4)
     per = by_template(cands)
     best = per[0][np.argmax(per[0]["sigma"])]
     f = best["bin"] / ((1 << int(best["fold"])) * w.t_obs)
