@@ -20,6 +20,7 @@ constexpr int HS_TPC = 16;             // tiles walked by one CTA of the harmoni
 #include <new>
 #include <set>
 #include <string>
+#include <deque>
 #include <vector>
 
 using namespace tb;
@@ -32,7 +33,8 @@ namespace {
 
 constexpr int N_STAGE_EVENTS = 6;   // start, delay model (K0), resample / P1, fft / P2, spectrum+median+normalise, hsum
 
-struct EventSet { cudaEvent_t e[N_STAGE_EVENTS]; };
+// e[0..5] on the plan's stream; k[0], k[1] around K0 on the side stream it runs on (fused path)
+struct EventSet { cudaEvent_t e[N_STAGE_EVENTS]; cudaEvent_t k[2]; bool k_used; };
 
 }  // namespace
 
@@ -72,6 +74,9 @@ struct tb_plan {
     EllCoef* d_ell = nullptr;                        // [tmpl_cap], staged with the templates
     EllCoef* h_ell = nullptr;
     cudaEvent_t ev_staged = nullptr;                 // the last template upload has been consumed
+    // K0 of chunk i+1 (fp64-bound, 3 % of the step) runs on a side stream under P2 / spectrum / hsum of chunk i
+    cudaStream_t s_k0 = nullptr;
+    cudaEvent_t ev_main = nullptr, ev_p1 = nullptr, ev_k0 = nullptr;
     bool staged_pending = false;
 
     // hand-written FFT path (tb_fft.cuh): M = N/2 = M1 * M2
@@ -105,7 +110,7 @@ struct tb_plan {
     double* d_acc = nullptr;
     size_t work_bytes = 0;
 
-    std::vector<EventSet> events;
+    std::deque<EventSet> events;                   // deque: references stay valid when sets are appended
     size_t events_used = 0;
     tb_timings last = {};
 
@@ -495,13 +500,25 @@ int launch_cols32(tb_plan* p, size_t off, uint32_t nt, long long* d_idx, float* 
 }
 
 // K0 + P1: delay segments, then gather + column FFTs into T (the buffer the legacy path uses for y)
-int run_own_pass1(tb_plan* p, size_t off, uint32_t nt, long long* d_idx, float* d_y, cudaEvent_t after_k0 = nullptr)
+int run_k0(tb_plan* p, size_t off, uint32_t nt, cudaStream_t st)
 {
     const int cta_per_tmpl = (int)(((p->n >> p->chunk_log2h) + 255) / 256);   // chunk_log2h: smallest knot spacing in this chunk
-    k_delay_segments<<<(unsigned)(cta_per_tmpl * nt), K0_THREADS, 0, p->stream>>>(p->d_tmpl + off, (int)nt, (int)p->n, p->d_seg,
-                                                                           p->seg_stride, cta_per_tmpl, p->ell ? p->d_ell + off : nullptr);
+    k_delay_segments<<<(unsigned)(cta_per_tmpl * nt), K0_THREADS, 0, st>>>(p->d_tmpl + off, (int)nt, (int)p->n, p->d_seg,
+                                                                    p->seg_stride, cta_per_tmpl, p->ell ? p->d_ell + off : nullptr);
     TB_CUDA(p, cudaGetLastError());
-    if (after_k0) TB_CUDA(p, cudaEventRecord(after_k0, p->stream));
+    return TB_OK;
+}
+
+int run_p1(tb_plan* p, size_t off, uint32_t nt, long long* d_idx, float* d_y);
+
+int run_own_pass1(tb_plan* p, size_t off, uint32_t nt, long long* d_idx, float* d_y)
+{
+    if (int rc = run_k0(p, off, nt, p->stream)) return rc;
+    return run_p1(p, off, nt, d_idx, d_y);
+}
+
+int run_p1(tb_plan* p, size_t off, uint32_t nt, long long* d_idx, float* d_y)
+{
     const bool dbg = d_idx != nullptr;
     if (p->cols32) return dbg ? launch_cols32<true>(p, off, nt, d_idx, d_y) : launch_cols32<false>(p, off, nt, nullptr, nullptr);
     switch (p->log2m1 - 8) {
@@ -774,7 +791,7 @@ int upload_templates(tb_plan* p, const tb_template* tmpl, uint64_t k)
 }
 
 // constants of the templates staged at positions [off, off + nt), uploaded on the plan's stream
-int stage_chunk(tb_plan* p, const tb_template* tmpl, uint64_t off, uint64_t nt, uint32_t first_id)
+int stage_chunk(tb_plan* p, const tb_template* tmpl, uint64_t off, uint64_t nt, uint32_t first_id, cudaStream_t st)
 {
     int lmin = 7;
     for (uint64_t i = off; i < off + nt; ++i) {
@@ -784,11 +801,11 @@ int stage_chunk(tb_plan* p, const tb_template* tmpl, uint64_t off, uint64_t nt, 
         lmin = std::min(lmin, p->h_tmpl[i].log2h);
     }
     p->chunk_log2h = lmin;
-    TB_CUDA(p, cudaMemcpyAsync(p->d_tmpl + off, p->h_tmpl + off, nt * sizeof(TmplDev), cudaMemcpyHostToDevice, p->stream));
-    if (p->ell) TB_CUDA(p, cudaMemcpyAsync(p->d_ell + off, p->h_ell + off, nt * sizeof(EllCoef), cudaMemcpyHostToDevice, p->stream));
+    TB_CUDA(p, cudaMemcpyAsync(p->d_tmpl + off, p->h_tmpl + off, nt * sizeof(TmplDev), cudaMemcpyHostToDevice, st));
+    if (p->ell) TB_CUDA(p, cudaMemcpyAsync(p->d_ell + off, p->h_ell + off, nt * sizeof(EllCoef), cudaMemcpyHostToDevice, st));
     // recorded after EVERY chunk: whatever way the call ends, the next one waits for the last copy
     // out of the pinned staging buffer before it rewrites it
-    TB_CUDA(p, cudaEventRecord(p->ev_staged, p->stream));
+    TB_CUDA(p, cudaEventRecord(p->ev_staged, st));
     p->staged_pending = true;
     return TB_OK;
 }
@@ -826,7 +843,12 @@ void destroy(tb_plan* p)
     if (p->have_c2r) { cufftDestroy(p->c2r_plan); cufftDestroy(p->d2z_plan); }
     cudaFree(p->d_zap);
     for (auto& es : p->events) for (auto& e : es.e) cudaEventDestroy(e);
+    if (p->s_k0) { cudaStreamSynchronize(p->s_k0); cudaStreamDestroy(p->s_k0); }
+    for (auto& es : p->events) for (auto& e : es.k) cudaEventDestroy(e);
     if (p->ev_staged) cudaEventDestroy(p->ev_staged);
+    if (p->ev_main) cudaEventDestroy(p->ev_main);
+    if (p->ev_p1) cudaEventDestroy(p->ev_p1);
+    if (p->ev_k0) cudaEventDestroy(p->ev_k0);
     cudaFree(p->d_seg); cudaFree(p->d_tw1a); cudaFree(p->d_tw1b); cudaFree(p->d_tw2); cudaFree(p->d_twn); cudaFree(p->d_twb); cudaFree(p->d_twc);
     cudaFree(p->d_work); cudaFree(p->d_acc); cudaFree(p->d_series_owned); cudaFree(p->d_resampled); cudaFree(p->d_fft);
     cudaFree(p->d_power); cudaFree(p->d_med); cudaFree(p->d_cand); cudaFree(p->d_cursor); cudaFree(p->d_tmpl);
@@ -842,7 +864,7 @@ int single_template_stage(tb_plan* p, const tb_template* tmpl)
     if (!p || !tmpl) return fail(p, TB_ERR_INVALID_ARG, "null argument");
     TB_CUDA(p, cudaSetDevice(p->device));
     const int rc = upload_templates(p, tmpl, 1);
-    return rc ? rc : stage_chunk(p, tmpl, 0, 1, 0);
+    return rc ? rc : stage_chunk(p, tmpl, 0, 1, 0, p->stream);
 }
 
 }  // namespace
@@ -935,6 +957,10 @@ int tb_plan_create(tb_plan** out, const float* series, uint64_t n_samples, doubl
     if (o.stream) p->stream = (cudaStream_t)o.stream;
     else { TB_TRY(cudaStreamCreateWithFlags(&p->stream, cudaStreamNonBlocking)); p->own_stream = true; }
     TB_TRY(cudaEventCreateWithFlags(&p->ev_staged, cudaEventDisableTiming));
+    TB_TRY(cudaStreamCreateWithFlags(&p->s_k0, cudaStreamNonBlocking));
+    TB_TRY(cudaEventCreateWithFlags(&p->ev_main, cudaEventDisableTiming));
+    TB_TRY(cudaEventCreateWithFlags(&p->ev_p1, cudaEventDisableTiming));
+    TB_TRY(cudaEventCreateWithFlags(&p->ev_k0, cudaEventDisableTiming));
 
     // chunk size B
     const size_t per_t = (size_t)p->n * 4 + p->ld * 8 + (size_t)p->nsp * 4 + (size_t)p->nblk * 4 + (size_t)p->n * 8;
@@ -1051,42 +1077,77 @@ int tb_search_templates(tb_plan* p, const tb_template* tmpl, uint64_t n_template
     // two runs of chunks: the templates the fused path takes (positions [0, n_own) of the staging
     // order), then the rest through k_resample + cuFFT; fft_path_used is the OR of the two
     p->last.fft_path_used = (p->n_own ? 2u : 0u) | (p->n_own < n_templates ? 1u : 0u);
+    auto next_events = [&](EventSet** es) -> int {
+        *es = nullptr;
+        if (!p->timings) return TB_OK;
+        if (p->events_used == p->events.size()) {
+            EventSet ne;
+            for (auto& e : ne.e) TB_CUDA(p, cudaEventCreate(&e));
+            for (auto& e : ne.k) TB_CUDA(p, cudaEventCreate(&e));
+            p->events.push_back(ne);
+        }
+        *es = &p->events[p->events_used++];
+        (*es)->k_used = false;
+        return TB_OK;
+    };
+    // K0 (+ the upload of the chunk's constants) on the side stream: queue it for chunk [off, off + nt)
+    auto queue_k0 = [&](uint64_t off, uint32_t nt, EventSet* es, bool after_p1) -> int {
+        if (int r = stage_chunk(p, tmpl, off, nt, first_template_id, p->s_k0)) return r;
+        if (after_p1) TB_CUDA(p, cudaStreamWaitEvent(p->s_k0, p->ev_p1, 0));          // the segment table is free again
+        if (es) { TB_CUDA(p, cudaEventRecord(es->k[0], p->s_k0)); es->k_used = true; }
+        if (int r = run_k0(p, off, nt, p->s_k0)) return r;
+        if (es) TB_CUDA(p, cudaEventRecord(es->k[1], p->s_k0));
+        TB_CUDA(p, cudaEventRecord(p->ev_k0, p->s_k0));
+        p->last.n_kernel_launches += 1;
+        return TB_OK;
+    };
     for (int part = 0; part < 2; ++part) {
         const bool own = part == 0;
         const uint64_t lo = own ? 0 : p->n_own, hi = own ? p->n_own : n_templates;
+        EventSet *es = nullptr, *es_next = nullptr;
+        if (own && lo < hi) {                            // everything queued so far (earlier calls read d_tmpl / d_seg) first
+            TB_CUDA(p, cudaEventRecord(p->ev_main, p->stream));
+            TB_CUDA(p, cudaStreamWaitEvent(p->s_k0, p->ev_main, 0));
+            if ((rc = next_events(&es_next))) return rc;
+            if ((rc = queue_k0(lo, (uint32_t)std::min<uint64_t>(p->chunk, hi - lo), es_next, false))) return rc;
+        }
         for (uint64_t off = lo; off < hi; off += p->chunk) {
             const uint32_t nt = (uint32_t)std::min<uint64_t>(p->chunk, hi - off);
-            if ((rc = stage_chunk(p, tmpl, off, nt, first_template_id))) return rc;
-            EventSet* es = nullptr;
-            if (p->timings) {
-                if (p->events_used == p->events.size()) {
-                    EventSet ne;
-                    for (auto& e : ne.e) TB_CUDA(p, cudaEventCreate(&e));
-                    p->events.push_back(ne);
-                }
-                es = &p->events[p->events_used++];
-                TB_CUDA(p, cudaEventRecord(es->e[0], p->stream));
-            }
-            if (own) {                                   // K0 | P1 | P2 | transpose + unpack + spectrum + median + normalise
-                if ((rc = run_own_pass1(p, off, nt, nullptr, nullptr, es ? es->e[1] : nullptr))) return rc;
+            if (own) {                                   // K0 (side stream) | P1 | P2 | transpose + unpack + spectrum + median + normalise
+                es = es_next;
+                es_next = nullptr;
+                if (es) TB_CUDA(p, cudaEventRecord(es->e[0], p->stream));
+                TB_CUDA(p, cudaStreamWaitEvent(p->stream, p->ev_k0, 0));
+                if (es) TB_CUDA(p, cudaEventRecord(es->e[1], p->stream));
+                if ((rc = run_p1(p, off, nt, nullptr, nullptr))) return rc;
                 if (es) TB_CUDA(p, cudaEventRecord(es->e[2], p->stream));
+                TB_CUDA(p, cudaEventRecord(p->ev_p1, p->stream));
+                if (off + p->chunk < hi) {               // the next chunk's knots run under the rest of this chunk (measured: they
+                                                         // fit beside the spectrum former's CTAs, not beside the harmonic summer's)
+                    if ((rc = next_events(&es_next))) return rc;
+                    if ((rc = queue_k0(off + p->chunk, (uint32_t)std::min<uint64_t>(p->chunk, hi - off - p->chunk), es_next, true))) return rc;
+                }
                 if ((rc = run_own_pass2(p, nt))) return rc;
                 if (es) TB_CUDA(p, cudaEventRecord(es->e[3], p->stream));
                 if ((rc = run_spectrum_t(p, nt))) return rc;
                 p->last.n_kernel_launches += (p->log2m2 == 16) ? 3 : 2;
             } else {
+                if ((rc = stage_chunk(p, tmpl, off, nt, first_template_id, p->stream))) return rc;
+                if ((rc = next_events(&es))) return rc;
+                if (es) TB_CUDA(p, cudaEventRecord(es->e[0], p->stream));
                 if (es) TB_CUDA(p, cudaEventRecord(es->e[1], p->stream));
                 if ((rc = run_resample(p, off, nt, nullptr))) return rc;
                 if (es) TB_CUDA(p, cudaEventRecord(es->e[2], p->stream));
                 if ((rc = run_fft(p, nt))) return rc;
                 if (es) TB_CUDA(p, cudaEventRecord(es->e[3], p->stream));
                 if ((rc = run_spectrum(p, nt, nullptr))) return rc;
+                p->last.n_kernel_launches += 1;
             }
             if (es) TB_CUDA(p, cudaEventRecord(es->e[4], p->stream));
             if ((rc = run_hsum(p, off, nt, fp))) return rc;
             if (es) TB_CUDA(p, cudaEventRecord(es->e[5], p->stream));
             p->last.n_chunks++;
-            p->last.n_kernel_launches += 3;
+            p->last.n_kernel_launches += 2;
         }
     }
     return TB_OK;
@@ -1107,6 +1168,7 @@ int tb_get_timings(tb_plan* p, tb_timings* out)
     for (size_t i = 0; i < p->events_used; ++i) {
         float ms[5];
         for (int s = 0; s < 5; ++s) TB_CUDA(p, cudaEventElapsedTime(&ms[s], p->events[i].e[s], p->events[i].e[s + 1]));
+        if (p->events[i].k_used) TB_CUDA(p, cudaEventElapsedTime(&ms[0], p->events[i].k[0], p->events[i].k[1]));   // K0 ran on the side stream
         t.ms_delay += ms[0]; t.ms_resample += ms[1]; t.ms_fft += ms[2]; t.ms_spectrum += ms[3]; t.ms_hsum += ms[4];
     }
     if (p->events_used) {
