@@ -658,7 +658,66 @@ k_spectrum_t(const float2* __restrict__ Zt, float* __restrict__ P, float* __rest
         }
     }
 
-    {   // ---- phase 1: unpack + interbin, powers to shared memory in bin order ----
+    if constexpr (Q % 2 == 0) {
+        // ---- phase 1, two columns per thread: 128-bit loads (half as many entries in the load queue the
+        // kernel throttles on for the same bytes in flight).  Thread (column pair cp, row group) walks LR rows of
+        // the columns k2, k2 + 1 (k2 even); their mirrors are the columns m2 - 1 - k2, m2 - 2 - k2: one aligned
+        // 128-bit load too.  Two chains X_{k-1} -> X_k per thread instead of one.
+        constexpr int NP = NK2 / 2, NRG = ST_THREADS / NP, LR = M1 / NRG, UN = 4;
+        static_assert(NP * NRG == ST_THREADS && LR * NRG == M1 && LR % UN == 0, "pair mapping of the spectrum former");
+        const int k2off = 2 * (threadIdx.x % NP), k1s = (threadIdx.x / NP) * LR;
+        const int k2 = a + k2off;
+        const size_t m2 = (size_t)1 << log2m2;
+        const float2 wb[2] = {__ldg(twb + k2), __ldg(twb + k2 + 1)};
+        float2 pl[2], ph[2];                             // 2 X_{k-1}, 2 X_{M-k+1} of the step before the run, per column
+#pragma unroll
+        for (int j = 0; j < 2; ++j) {
+            const int kk2 = k2 + j;
+            const bool first = (k1s | kk2) == 0;
+            const int pk1 = k1s > 0 ? k1s - 1 : M1 - 1;
+            const int pk2 = k1s > 0 ? kk2 : (first ? 0 : kk2 - 1);
+            st_unpack_at<LOG2M1>(Zr, pk1, pk2, log2m2, twa, k1s > 0 ? wb[j] : __ldg(twb + pk2), pl[j], ph[j]);
+            if (first) { pl[j] = make_float2(0.f, 0.f); ph[j] = make_float2(0.f, 0.f); }
+        }
+        float* __restrict__ lo = s_lo + k1s + k2off * (M1 + 1);                           // column j: + j (M1 + 1)
+        float* __restrict__ hi = s_hi + (M1 - 1 - k1s) + (9 * Q - 1 - k2off) * (M1 + 1);  // column j: - j (M1 + 1)
+        const float4* zkp = reinterpret_cast<const float4*>(Zr + (size_t)k1s * m2 + k2);                      // walks down the rows
+        const float4* zmp = reinterpret_cast<const float4*>(Zr + (size_t)(M1 - k1s) * m2 + (m2 - 2 - k2));   // walks up; .xy mirrors column k2 + 1, .zw column k2
+        const size_t step4 = m2 >> 1;
+        const float2* __restrict__ wap = twa + k1s;
+#pragma unroll 1
+        for (int i0 = 0; i0 < LR; i0 += UN) {
+            float4 zk[UN], zm[UN];
+#pragma unroll
+            for (int u = 0; u < UN; ++u) {
+                zk[u] = __ldg(zkp);
+                if (i0 + u == 0 && k1s == 0) {           // k1 = 0 mirrors inside row 0: columns (m2 - k2) mod m2 and m2 - k2 - 1
+                    const float2 m0 = __ldg(Zr + ((m2 - k2) & (m2 - 1))), m1 = __ldg(Zr + (m2 - k2 - 1));
+                    zm[u] = make_float4(m1.x, m1.y, m0.x, m0.y);
+                } else zm[u] = __ldg(zmp);
+                zkp += step4; zmp -= step4;
+            }
+            const float2 wa = __ldg(wap + i0);
+            float2 w0 = make_float2(wa.x * wb[0].x - wa.y * wb[0].y, wa.x * wb[0].y + wa.y * wb[0].x);
+            float2 w1 = make_float2(wa.x * wb[1].x - wa.y * wb[1].y, wa.x * wb[1].y + wa.y * wb[1].x);
+#pragma unroll
+            for (int u = 0; u < UN; ++u) {
+                const int it = i0 + u;
+                float2 xk, xm;
+                st_unpack2(make_float2(zk[u].x, zk[u].y), make_float2(zm[u].z, zm[u].w), w0, xk, xm);
+                if (it == 0 && (k1s | k2) == 0) xk = make_float2(0.f, 0.f);                   // X_0 <- 0 (G13)
+                lo[it] = st_interbin(xk, pl[0]);
+                hi[-it] = st_interbin(ph[0], xm);
+                pl[0] = xk; ph[0] = xm;
+                st_unpack2(make_float2(zk[u].z, zk[u].w), make_float2(zm[u].x, zm[u].y), w1, xk, xm);
+                lo[it + (M1 + 1)] = st_interbin(xk, pl[1]);
+                hi[-it - (M1 + 1)] = st_interbin(ph[1], xm);
+                pl[1] = xk; ph[1] = xm;
+                w0 = make_float2(w0.x * rot.x - w0.y * rot.y, w0.x * rot.y + w0.y * rot.x);
+                w1 = make_float2(w1.x * rot.x - w1.y * rot.y, w1.x * rot.y + w1.y * rot.x);
+            }
+        }
+    } else {   // ---- phase 1: unpack + interbin, powers to shared memory in bin order ----
         const int k2off = threadIdx.x % NK2, k1s = (threadIdx.x / NK2) * LC;
         const int k2 = a + k2off;
         const size_t m2 = (size_t)1 << log2m2;
@@ -707,15 +766,15 @@ k_spectrum_t(const float2* __restrict__ Zt, float* __restrict__ P, float* __rest
                 w = make_float2(w.x * rot.x - w.y * rot.y, w.x * rot.y + w.y * rot.x);
             }
         }
-        if (threadIdx.x < 2) {                           // the two steps above the low tile: high bins hH0 + 1, hH0
-            const int kc2 = a + NK2;                     // k = kL0 + 9W + t = (k1 = t, k2 = a + 9Q)
-            const float2 wc = __ldg(twb + kc2);
-            float2 x0, h0, x1, h1;
-            if (threadIdx.x == 0) st_unpack_at<LOG2M1>(Zr, M1 - 1, kc2 - 1, log2m2, twa, __ldg(twb + kc2 - 1), x0, h0);
-            else                  st_unpack_at<LOG2M1>(Zr, 0, kc2, log2m2, twa, wc, x0, h0);
-            st_unpack_at<LOG2M1>(Zr, (int)threadIdx.x, kc2, log2m2, twa, wc, x1, h1);
-            s_hi[-2 - (int)threadIdx.x] = st_interbin(h0, h1);           // eh = 1 - t: (eh - 2) + ((eh - 2) >> LOG2M1)
-        }
+    }
+    if (threadIdx.x < 2) {                               // the two steps above the low tile: high bins hH0 + 1, hH0
+        const int kc2 = a + NK2;                         // k = kL0 + 9W + t = (k1 = t, k2 = a + 9Q)
+        const float2 wc = __ldg(twb + kc2);
+        float2 x0, h0, x1, h1;
+        if (threadIdx.x == 0) st_unpack_at<LOG2M1>(Zr, M1 - 1, kc2 - 1, log2m2, twa, __ldg(twb + kc2 - 1), x0, h0);
+        else                  st_unpack_at<LOG2M1>(Zr, 0, kc2, log2m2, twa, wc, x0, h0);
+        st_unpack_at<LOG2M1>(Zr, (int)threadIdx.x, kc2, log2m2, twa, wc, x1, h1);
+        s_hi[-2 - (int)threadIdx.x] = st_interbin(h0, h1);               // eh = 1 - t: (eh - 2) + ((eh - 2) >> LOG2M1)
     }
     __syncthreads();
 
