@@ -305,7 +305,9 @@ def run_ours(args, wl):
     if os.path.exists(tpath):
         with open(tpath) as f:
             tj = json.load(f)
-        if tj.get("_csrc_sha256_16") == source_digest():
+        if N != 1 << 23 or chunk != 64:
+            traffic_note = "the capture is of the N = 2^23, 64-template launch only"
+        elif tj.get("_csrc_sha256_16") == source_digest():
             traffic = tj.get(names[dom].split(" (")[0])
             traffic_note = tj.get("_source", "")
         else:
