@@ -523,7 +523,6 @@ int run_p1(tb_plan* p, size_t off, uint32_t nt, long long* d_idx, float* d_y)
     if (p->cols32) return dbg ? launch_cols32<true>(p, off, nt, d_idx, d_y) : launch_cols32<false>(p, off, nt, nullptr, nullptr);
     switch (p->log2m1 - 8) {
         case 0: return dbg ? launch_cols<1, 16, true>(p, off, nt, d_idx, d_y) : launch_cols<1, 16, false>(p, off, nt, nullptr, nullptr);
-        case 1: return dbg ? launch_cols<2, 16, true>(p, off, nt, d_idx, d_y) : launch_cols<2, 16, false>(p, off, nt, nullptr, nullptr);
         case 2: return dbg ? launch_cols<4, 8, true>(p, off, nt, d_idx, d_y) : launch_cols<4, 8, false>(p, off, nt, nullptr, nullptr);
     }
     return fail(p, TB_ERR_INVALID_ARG, "unsupported M1");
