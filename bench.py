@@ -276,8 +276,8 @@ def run_ours(args, wl):
     if path_used == 2:
         model = {"ms_delay": 0, "ms_resample": 4 * N + 4 * N // chunk, "ms_fft": 8 * N, "ms_spectrum": 6 * N, "ms_hsum": 2 * N}
         log2n = int(np.log2(N))
-        p1 = "P1 k_fft_cols32" if 18 <= log2n <= 23 or log2n == 26 else "P1 k_fft_cols"
-        p2 = "P2 k_fft_rows_t" if log2n <= 24 else "P2 k_fft_cols<DIRECT> + k_fft_rows_scatter"
+        p1 = "P1 k_fft_cols32" if 18 <= log2n <= 24 or log2n == 26 else "P1 k_fft_cols"
+        p2 = "P2 k_fft_rows_t" if log2n <= 23 else "P2 k_fft_rows_wide" if log2n <= 25 else "P2 k_fft_cols<DIRECT> + k_fft_rows_scatter"
         names = {"ms_delay": "K0 k_delay_segments (a2 knots)", "ms_resample": p1 + " (a2+a3, a4 pass 1)",
                  "ms_fft": p2 + " (a4 pass 2)", "ms_spectrum": "k_spectrum_t (a4 unpack, a5+a6+a7)",
                  "ms_hsum": "k_hsum_tile (a8+a9)"}

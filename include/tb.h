@@ -104,9 +104,9 @@ typedef struct {
     float    fill_value;
     int32_t  enable_timings;      /* 1: record CUDA events around every stage of every chunk */
     int32_t  fft_path;            /* 0: automatic (hand-written FFT with fused gather where it applies:
-                                     2^17 <= N <= 2^26 (two passes up to 2^24, three above), W in
-                                     {512, 1024, 2048} (256 or 1024 at 2^17 and 2^25; 1024 or 2048 at
-                                     2^24) and knot spacing >= 8; batched cuFFT otherwise); 1: always
+                                     2^17 <= N <= 2^26 (two passes up to 2^25, three at 2^26), W in
+                                     {512, 1024, 2048} (256 or 1024 at 2^17; 1024 or 2048 at 2^25) and
+                                     knot spacing >= 8; batched cuFFT otherwise); 1: always
                                      cuFFT; 2: hand-written or TB_ERR_INVALID_ARG */
     int32_t  whiten;              /* 1: front-end whitening once per series ("Fourier
                                      de-reddening", "birdie zapping"; reading G25): tb_plan_create and

@@ -84,7 +84,7 @@ struct tb_plan {
     int log2m1 = 0, log2m2 = 0;
     SegRec* d_seg = nullptr;                         // [chunk][seg_stride], grown on demand (seg_stride = n >> smallest knot spacing staged)
     size_t seg_stride = 0, seg_cap = 0;              // records per template, records allocated
-    float2 *d_tw1a = nullptr, *d_tw1b = nullptr, *d_tw2 = nullptr, *d_twn = nullptr, *d_twb = nullptr, *d_twc = nullptr;
+    float2 *d_tw1a = nullptr, *d_tw1b = nullptr, *d_tw2 = nullptr, *d_twn = nullptr, *d_twb = nullptr, *d_twc = nullptr, *d_tw512 = nullptr;
     bool cols32 = false;                             // pass 1 as 32 x 16 (M1 = 512)
     float2 rot = {1.f, 0.f};                         // W_N^1
     int chunk_log2h = 0;                             // smallest knot spacing among the templates of the chunk being launched
@@ -457,7 +457,7 @@ void launch_spectrum(tb_plan* p, uint32_t nt, float* d_raw)
 }
 
 // ---- hand-written FFT path -------------------------------------------------------------------
-// columns per CTA of pass 1: 16 (runs of 32 samples / 128 bytes), 8 at M1 = 1024 where 16 would not fit in shared memory
+// columns per CTA of pass 1: 16 (runs of 32 samples / 128 bytes); M1 = 1024 has its own kernel (k_fft_cols1k, 8 columns)
 template <int R1, int C> constexpr size_t cols_smem() { return (size_t)(C * (R1 * FFT_PA + 16 / C) + 256) * sizeof(float2); }
 
 template <int R1, int FFT_C, bool DEBUG>
@@ -499,6 +499,19 @@ int launch_cols32(tb_plan* p, size_t off, uint32_t nt, long long* d_idx, float* 
     return TB_OK;
 }
 
+template <bool DEBUG>
+int launch_cols1k(tb_plan* p, size_t off, uint32_t nt, long long* d_idx, float* d_y)
+{
+    auto kern = k_fft_cols1k<DEBUG>;
+    if (int rc_ = allow_smem(p, reinterpret_cast<const void*>(kern), (size_t)(C1K_SMEM))) return rc_;
+    const unsigned grid = (unsigned)(((1u << p->log2m2) / 8) * nt);
+    kern<<<grid, FFT_THREADS, C1K_SMEM, p->stream>>>(p->d_series, p->d_seg, p->seg_stride, p->d_tmpl + off, (int)nt, (int)p->n,
+                                                    p->log2m2, p->fill, p->d_twc, reinterpret_cast<float2*>(p->d_resampled),
+                                                    d_idx, d_y, p->pf_cols);
+    TB_CUDA(p, cudaGetLastError());
+    return TB_OK;
+}
+
 // K0 + P1: delay segments, then gather + column FFTs into T (the buffer the legacy path uses for y)
 int run_k0(tb_plan* p, size_t off, uint32_t nt, cudaStream_t st)
 {
@@ -523,7 +536,7 @@ int run_p1(tb_plan* p, size_t off, uint32_t nt, long long* d_idx, float* d_y)
     if (p->cols32) return dbg ? launch_cols32<true>(p, off, nt, d_idx, d_y) : launch_cols32<false>(p, off, nt, nullptr, nullptr);
     switch (p->log2m1 - 8) {
         case 0: return dbg ? launch_cols<1, 16, true>(p, off, nt, d_idx, d_y) : launch_cols<1, 16, false>(p, off, nt, nullptr, nullptr);
-        case 2: return dbg ? launch_cols<4, 8, true>(p, off, nt, d_idx, d_y) : launch_cols<4, 8, false>(p, off, nt, nullptr, nullptr);
+        case 2: return dbg ? launch_cols1k<true>(p, off, nt, d_idx, d_y) : launch_cols1k<false>(p, off, nt, nullptr, nullptr);
     }
     return fail(p, TB_ERR_INVALID_ARG, "unsupported M1");
 }
@@ -547,9 +560,21 @@ int run_own_pass23(tb_plan* p, uint32_t nt)
     return TB_OK;
 }
 
+// rows of 16384 points (N = 2^24): one CTA of 512 threads per row
+int launch_rows_wide(tb_plan* p, uint32_t nt)
+{
+    if (int rc_ = allow_smem(p, reinterpret_cast<const void*>(k_fft_rows_wide), RW_SMEM)) return rc_;
+    const unsigned grid = (unsigned)(nt << p->log2m1);
+    k_fft_rows_wide<<<grid, RW_THREADS, RW_SMEM, p->stream>>>(reinterpret_cast<const float2*>(p->d_resampled), p->d_fft, p->d_tw1b,
+                                                              p->d_tw512, p->n_sm);
+    TB_CUDA(p, cudaGetLastError());
+    return TB_OK;
+}
+
 int run_own_pass2(tb_plan* p, uint32_t nt)
 {
     if (p->log2m2 == 16) return run_own_pass23(p, nt);
+    if (p->log2m2 == 14) return launch_rows_wide(p, nt);
     switch (p->log2m2 - 8) {
         case 0: return launch_rows<1>(p, nt);
         case 1: return launch_rows<2>(p, nt);
@@ -623,7 +648,21 @@ int make_twiddles(tb_plan* p)
     };
     int rc;
     if ((rc = tw1(p->log2m1, &p->d_tw1a))) return rc;
-    if ((rc = tw1(p->log2m2 == 16 ? 8 : p->log2m2, &p->d_tw1b))) return rc;
+    if (p->log2m2 == 14) {                               // k_fft_rows_wide: W_L^w, W_L^{8w} (L = 16384, w < 512) and W_512^{c kb}
+        std::vector<float2> h(1024), h5(512);
+        for (int w = 0; w < 512; ++w) {
+            const long double a1 = -two_pi * (long double)w / 16384.0L, a8 = -two_pi * (long double)(8 * w) / 16384.0L;
+            h[w] = make_float2((float)cosl(a1), (float)sinl(a1));
+            h[512 + w] = make_float2((float)cosl(a8), (float)sinl(a8));
+        }
+        for (int kb = 0; kb < 16; ++kb)
+            for (int c = 0; c < 32; ++c) {
+                const long double a = -two_pi * (long double)(kb * c) / 512.0L;
+                h5[kb * 32 + c] = make_float2((float)cosl(a), (float)sinl(a));
+            }
+        if ((rc = upload(h, &p->d_tw1b))) return rc;
+        if ((rc = upload(h5, &p->d_tw512))) return rc;
+    } else if ((rc = tw1(p->log2m2 == 16 ? 8 : p->log2m2, &p->d_tw1b))) return rc;
     std::vector<float2> h2(256), hn((size_t)1 << p->log2m1), hb((size_t)1 << p->log2m2);
     for (int kb = 0; kb < 16; ++kb)
         for (int c = 0; c < 16; ++c) {
@@ -637,6 +676,15 @@ int make_twiddles(tb_plan* p)
     for (size_t b = 0; b < hb.size(); ++b) {
         const long double a = -two_pi * (long double)((uint64_t)b << p->log2m1) / (long double)p->n;
         hb[b] = make_float2((float)cosl(a), (float)sinl(a));
+    }
+    if (p->log2m1 == 10) {                               // W_1024^{c ka} of the 32 x 32 first pass
+        std::vector<float2> hc(1024);
+        for (int ka = 0; ka < 32; ++ka)
+            for (int c = 0; c < 32; ++c) {
+                const long double a = -two_pi * (long double)(ka * c) / 1024.0L;
+                hc[ka * 32 + c] = make_float2((float)cosl(a), (float)sinl(a));
+            }
+        if ((rc = upload(hc, &p->d_twc))) return rc;
     }
     if (p->log2m1 == 9) {                                // W_512^{c ka} of the 32 x 16 first pass
         std::vector<float2> hc(512);
@@ -848,7 +896,7 @@ void destroy(tb_plan* p)
     if (p->ev_main) cudaEventDestroy(p->ev_main);
     if (p->ev_p1) cudaEventDestroy(p->ev_p1);
     if (p->ev_k0) cudaEventDestroy(p->ev_k0);
-    cudaFree(p->d_seg); cudaFree(p->d_tw1a); cudaFree(p->d_tw1b); cudaFree(p->d_tw2); cudaFree(p->d_twn); cudaFree(p->d_twb); cudaFree(p->d_twc);
+    cudaFree(p->d_seg); cudaFree(p->d_tw512); cudaFree(p->d_tw1a); cudaFree(p->d_tw1b); cudaFree(p->d_tw2); cudaFree(p->d_twn); cudaFree(p->d_twb); cudaFree(p->d_twc);
     cudaFree(p->d_work); cudaFree(p->d_acc); cudaFree(p->d_series_owned); cudaFree(p->d_resampled); cudaFree(p->d_fft);
     cudaFree(p->d_power); cudaFree(p->d_med); cudaFree(p->d_cand); cudaFree(p->d_cursor); cudaFree(p->d_tmpl);
     if (p->h_tmpl) cudaFreeHost(p->h_tmpl);
@@ -977,13 +1025,13 @@ int tb_plan_create(tb_plan** out, const float* series, uint64_t n_samples, doubl
     p->user_fill = o.has_fill != 0;
     p->fill = o.fill_value;
 
-    // FFT path: hand-written two-pass FFT (M = N/2 = M1 * M2, M1 = 512, 256 at 2^17, 1024 at 2^24) when
-    // 2^17 <= N <= 2^26 (three passes with M2 = 256 x 256 at 2^25 and 2^26), W >= M1 and the median blocks pair up in groups of 16; batched cuFFT otherwise
+    // FFT path: hand-written two-pass FFT (M = N/2 = M1 * M2, M1 = 512, 256 at 2^17, 1024 at 2^25) when
+    // 2^17 <= N <= 2^26 (three passes with M2 = 256 x 256 at 2^26), W >= M1 and the median blocks pair up in groups of 16; batched cuFFT otherwise
     {
         const int lm = (int)ilog2(p->nb);
-        p->log2m1 = lm == 25 ? 9 : lm == 24 ? 8 : lm == 23 ? 10 : lm >= 17 ? 9 : 8;   // 2^25, 2^26: three passes, M2 = 2^16
+        p->log2m1 = lm == 24 ? 10 : lm >= 17 ? 9 : 8;   // 2^24, 2^25: rows of 16384 (k_fft_rows_wide) with M1 = 512, 1024; 2^26: three passes, M2 = 2^16
         p->log2m2 = lm - p->log2m1;
-        const bool fits = ((p->log2m2 >= 8 && p->log2m2 <= 13) || (p->log2m2 == 16 && lm >= 24)) && spectrum_t_supported(W, p->log2m1) && p->nblk >= 16 && p->nblk % 16 == 0;
+        const bool fits = ((p->log2m2 >= 8 && p->log2m2 <= 14) || (p->log2m2 == 16 && lm >= 24)) && spectrum_t_supported(W, p->log2m1) && p->nblk >= 16 && p->nblk % 16 == 0;
         if (o.fft_path >= 2 && (!fits || p->over)) { destroy(p); return TB_ERR_INVALID_ARG; }
         p->own_fft = fits && o.fft_path != 1 && !p->over;         // the oversampled spectrum is formed from the library R2C output
     }

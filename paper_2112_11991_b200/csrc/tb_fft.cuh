@@ -636,6 +636,160 @@ k_fft_cols32(const float* __restrict__ x, const SegRec* __restrict__ seg, size_t
 }
 
 // ---------------------------------------------------------------------------------------------
+// P1 for M1 = 1024 = 32 x 32 (N = 2^25): bundles of C = 8 columns (64 KB of shared memory), two radix-32
+// steps in registers with one barrier between them, the index phase per 4-sample work item as in
+// k_fft_cols32.  Row j1 = 32 a + c, output k1 = ka + 32 kc.  slot(col, r) = fsm[col LP + 33 (r / 32) +
+// r % 32], LP = 32 * 33 + 2: the index phase, the gather (thread (col, c): rows c + 32 a), the
+// write-back (ka in place of a) and the second step (thread (col, ka): 32 consecutive c) are all
+// conflict free for 64-bit elements.  twc: [ka 32 + c] = W_1024^{c ka}.
+// ---------------------------------------------------------------------------------------------
+constexpr int C1K_LP = 32 * 33 + 2;
+constexpr size_t C1K_SMEM = (size_t)8 * C1K_LP * sizeof(float2);
+
+template <bool DEBUG>
+__global__ void __launch_bounds__(FFT_THREADS, 2)        // measured: 2 CTAs/SM (128 registers) 151 us per template at 2^25, 3 CTAs (80) 174
+k_fft_cols1k(const float* __restrict__ x, const SegRec* __restrict__ seg, size_t seg_stride,
+             const TmplDev* __restrict__ tmpl, int n_tmpl, int n, int log2m2, float fill,
+             const float2* __restrict__ twc, float2* __restrict__ T,
+             long long* __restrict__ idx_out, float* __restrict__ y_out, int pf_dist)
+{
+    constexpr int C = 8, LP = C1K_LP, L = 1024;
+    constexpr float MAGIC = 12582912.0f;
+    extern __shared__ __align__(16) float2 fsm[];
+    const int b  = blockIdx.x % n_tmpl;
+    const int c0 = (blockIdx.x / n_tmpl) * C;
+    const size_t m = (size_t)L << log2m2;          // M
+    const int log2h = tmpl[b].log2h;
+    const float inv_h = 1.0f / (float)(1 << log2h);
+    const SegRec* __restrict__ segs = seg + (size_t)b * seg_stride;
+    float2* __restrict__ Tb = T + (size_t)b * m;
+    const int row_shift = log2m2 + 1;
+
+    if (!DEBUG && pf_dist > 0 && blockIdx.x + pf_dist < gridDim.x) {           // segment records of a later CTA -> L2
+        const unsigned nb = blockIdx.x + pf_dist;
+        const int bn = nb % n_tmpl, cn = (nb / n_tmpl) * C;
+        const int lh = __ldg(&tmpl[bn].log2h);
+        const SegRec* __restrict__ sn = seg + (size_t)bn * seg_stride;
+        for (int j1 = threadIdx.x; j1 < L; j1 += FFT_THREADS)
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(sn + ((int)((((size_t)j1 << log2m2) + cn) << 1) >> lh)));
+    }
+    {   // index phase: item = 4 consecutive samples (columns 2q, 2q + 1) of row r0 + 64 i
+        const int q = threadIdx.x & 3, r0 = threadIdx.x >> 2;
+        const int nnq = (c0 + 2 * q) << 1;
+        const int o = nnq & ((1 << log2h) - 1);
+        float t[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) t[k] = (float)(o + k) * inv_h;
+        const int rec_shift = row_shift - log2h + 6;
+        const char* __restrict__ rec = reinterpret_cast<const char*>(segs + (nnq >> log2h)) + ((size_t)r0 << rec_shift);
+        const size_t rec_step = (size_t)64 << rec_shift;
+        const int nnr = nnq + (r0 << row_shift), nn_step = 64 << row_shift;
+        int2* __restrict__ slot = reinterpret_cast<int2*>(fsm + (2 * q) * LP + 33 * (r0 >> 5) + (r0 & 31));   // + 66 i
+        unsigned ties = 0;
+#pragma unroll 8
+        for (int i = 0; i < 16; ++i) {
+            const char* r = rec + (size_t)i * rec_step;
+            const float4 f = __ldg(reinterpret_cast<const float4*>(r));
+            const int2 ie = __ldg(reinterpret_cast<const int2*>(r) + 2);
+            float y[4], z[4];
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                y[k] = fmaf(fmaf(fmaf(f.w, t[k], f.z), t[k], f.y), t[k], f.x);
+                z[k] = y[k] + MAGIC;
+            }
+            const float res = fmaxf(fmaxf(fabsf(y[0] - (z[0] - MAGIC)), fabsf(y[1] - (z[1] - MAGIC))),
+                                    fmaxf(fabsf(y[2] - (z[2] - MAGIC)), fabsf(y[3] - (z[3] - MAGIC))));
+            ties |= (res > 0.5f - __int_as_float(ie.y) ? 1u : 0u) << i;
+            const int base = nnr + i * nn_step - ie.x + 0x4B400000;
+            slot[i * 66]      = clamp_pair<!DEBUG>(make_int2(base - __float_as_int(z[0]), base + 1 - __float_as_int(z[1])), n);
+            slot[i * 66 + LP] = clamp_pair<!DEBUG>(make_int2(base + 2 - __float_as_int(z[2]), base + 3 - __float_as_int(z[3])), n);
+        }
+        while (ties) {                                                         // rare: decide in fp64
+            const int i = __ffs(ties) - 1;
+            ties &= ties - 1;
+            const char* r = rec + (size_t)i * rec_step;
+            const double2 c01 = __ldg(reinterpret_cast<const double2*>(r) + 2);
+            const double2 c23 = __ldg(reinterpret_cast<const double2*>(r) + 3);
+            const int nn = nnr + i * nn_step;
+            int sidx[4];
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                const double tk = (double)(o + k) * (double)inv_h;
+                sidx[k] = nn + k - floor_to_int(fma(fma(fma(c23.y, tk, c23.x), tk, c01.y), tk, c01.x));
+            }
+            slot[i * 66]      = clamp_pair<!DEBUG>(make_int2(sidx[0], sidx[1]), n);
+            slot[i * 66 + LP] = clamp_pair<!DEBUG>(make_int2(sidx[2], sidx[3]), n);
+        }
+    }
+    __syncthreads();
+    const int col = threadIdx.x & 7, c = threadIdx.x >> 3;
+    {   // gather (64 independent loads), radix 32 over a, twiddle W_1024^{c ka}, back to the same slots
+        float2* __restrict__ myslot = fsm + col * LP + c;                      // + 33 a
+        const int nn0 = (int)((((size_t)c << log2m2) + c0 + col) << 1);
+        float2 v[32];
+#pragma unroll
+        for (int a = 0; a < 32; ++a) {
+            const int2 sp = *reinterpret_cast<const int2*>(myslot + 33 * a);
+            if (DEBUG) {
+                v[a].x = ((unsigned)sp.x < (unsigned)n) ? __ldg(x + sp.x) : fill;
+                v[a].y = ((unsigned)sp.y < (unsigned)n) ? __ldg(x + sp.y) : fill;
+                const size_t nn = (size_t)b * n + (size_t)(nn0 + ((32 * a) << row_shift));
+                idx_out[nn] = sp.x; idx_out[nn + 1] = sp.y;
+                y_out[nn] = v[a].x; y_out[nn + 1] = v[a].y;
+            } else {
+                v[a].x = __ldg(x + sp.x);
+                v[a].y = __ldg(x + sp.y);
+            }
+        }
+        fft_reg<32>(v);
+        myslot[0] = v[0];
+        float2 t[8], q[4];
+        t[1] = __ldg(twc + 32 + c);
+        q[1] = __ldg(twc + 8 * 32 + c);
+        t[2] = cmul(t[1], t[1]); t[3] = cmul(t[2], t[1]); t[4] = cmul(t[2], t[2]);
+        t[5] = cmul(t[4], t[1]); t[6] = cmul(t[4], t[2]); t[7] = cmul(t[4], t[3]);
+        q[2] = cmul(q[1], q[1]); q[3] = cmul(q[2], q[1]);
+#pragma unroll
+        for (int ka = 1; ka < 8; ++ka) myslot[33 * ka] = cmul(v[ka], t[ka]);
+#pragma unroll
+        for (int h = 1; h < 4; ++h) {
+            myslot[33 * 8 * h] = cmul(v[8 * h], q[h]);
+#pragma unroll
+            for (int l = 1; l < 8; ++l) myslot[33 * (8 * h + l)] = cmul(v[8 * h + l], cmul(q[h], t[l]));
+        }
+    }
+    __syncthreads();
+    {   // item (col, ka): radix 32 over c, four-step twiddle W_M^{j2 k1}, k1 = ka + 32 kc, streaming stores of T[k1][j2]
+        const int ka = c;
+        const float2* p = fsm + col * LP + 33 * ka;
+        float2 v[32];
+#pragma unroll
+        for (int cc = 0; cc < 32; ++cc) v[cc] = p[cc];
+        fft_reg<32>(v);
+        const int j2 = c0 + col;
+        const float inv_m = 1.0f / (float)m;
+        float sb, cb, sg, cg;
+        sincospif(-2.0f * (float)(j2 * ka) * inv_m, &sb, &cb);                 // both arguments are exact in fp32
+        sincospif(-2.0f * (float)(j2 * 32) * inv_m, &sg, &cg);
+        float2 t[8], bq[4];                                                    // g^l, base g^{8h}
+        t[1] = make_float2(cg, sg);
+        t[2] = cmul(t[1], t[1]); t[3] = cmul(t[2], t[1]); t[4] = cmul(t[2], t[2]);
+        t[5] = cmul(t[4], t[1]); t[6] = cmul(t[4], t[2]); t[7] = cmul(t[4], t[3]);
+        const float2 g8 = cmul(t[4], t[4]);
+        bq[0] = make_float2(cb, sb);
+        bq[1] = cmul(bq[0], g8); bq[2] = cmul(bq[1], g8); bq[3] = cmul(bq[2], g8);
+        float2* out = Tb + ((size_t)ka << log2m2) + j2;
+        const size_t kstep = (size_t)32 << log2m2;
+#pragma unroll
+        for (int h = 0; h < 4; ++h) {
+            __stcs(out + (size_t)(8 * h) * kstep, cmul(v[8 * h], bq[h]));
+#pragma unroll
+            for (int l = 1; l < 8; ++l) __stcs(out + (size_t)(8 * h + l) * kstep, cmul(v[8 * h + l], cmul(bq[h], t[l])));
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
 // P2  row FFTs, transposed output.  CTA = R rows [k1, k1+R) of template b, row length
 //   M2 = R1*256 (R1 up to 32: 8192 points, 32 values per thread in the first radix step).
 //   Output Zt[k1][k2], k2 = ka + R1 kb + 16 R1 kc: the last step's work items run ka-fastest so
@@ -729,6 +883,86 @@ k_fft_rows_t(const float2* __restrict__ T, float2* __restrict__ Zt, int log2m1, 
         float2* out = Zb + (size_t)r * L + wp;     // k2 = wp + 16 R1 kc
 #pragma unroll
         for (int kc = 0; kc < 16; ++kc) __stcs(out + kc * (16 * R1), v[kc]);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// P2 for rows of M2 = 16384 points (N = 2^24 with M1 = 512): one row per CTA of 512 threads,
+//   L = 32 x 512 = 32 x (16 x 32).  Thread w loads T[a 512 + w], a < 32 (all loads before the first
+//   butterfly), radix 32 in registers over a, twiddle W_L^{w ka} (product tree from the table
+//   values ka = 1 and 8); then per ka a 512-point FFT over w = 32 b + c in shared memory: radix 16
+//   over b (items (ka, c), two per thread), twiddle W_512^{c kb}, radix 32 over c (item (ka, kb),
+//   one per thread, ka fastest).  Output Zt[k1][k2], k2 = ka + 32 (kb + 16 kc): a warp stores 32
+//   consecutive k2.  Element (ka, b, c) at ka PA + b PB + c with PB = 33, PA = 16 PB + 1 (odd):
+//   all three access patterns are conflict free for 64-bit elements.  128 KB of shared memory:
+//   one CTA per SM, so the next row is pulled into L2 while this one is transformed.
+//   tw1: [w] = W_L^w, [512 + w] = W_L^{8 w};  tw512: [kb 32 + c] = W_512^{c kb}.
+// ---------------------------------------------------------------------------------------------
+constexpr int RW_THREADS = 512, RW_PB = 33, RW_PA = 16 * RW_PB + 1, RW_L = 16384;
+constexpr size_t RW_SMEM = (size_t)(32 * RW_PA + 512) * sizeof(float2);
+
+__global__ void __launch_bounds__(RW_THREADS, 1)
+k_fft_rows_wide(const float2* __restrict__ T, float2* __restrict__ Zt, const float2* __restrict__ tw1,
+                const float2* __restrict__ tw512g, int pf_dist)
+{
+    constexpr int PA = RW_PA, PB = RW_PB, L = RW_L;
+    extern __shared__ __align__(16) float2 fsm[];
+    float2* tw512 = fsm + 32 * PA;
+    const float2* __restrict__ Tb = T + (size_t)blockIdx.x * L;
+    float2* __restrict__ Zb = Zt + (size_t)blockIdx.x * L;
+    const int w = threadIdx.x;
+    tw512[w] = __ldg(tw512g + w);
+    if (w == 0 && pf_dist > 0 && blockIdx.x + pf_dist < gridDim.x) {           // a later CTA's row -> L2
+        const float2* nxt = T + (size_t)(blockIdx.x + pf_dist) * L;
+        asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(nxt), "r"((unsigned)(L * sizeof(float2))) : "memory");
+    }
+    {
+        float2 v[32];
+#pragma unroll
+        for (int a = 0; a < 32; ++a) v[a] = __ldcs(Tb + a * 512 + w);
+        fft_reg<32>(v);
+        float2* p = fsm + (w >> 5) * PB + (w & 31);                            // (b, c) = (w / 32, w % 32); + ka PA
+        p[0] = v[0];
+        float2 t[8], q[4];
+        t[1] = __ldg(tw1 + w);
+        q[1] = __ldg(tw1 + 512 + w);
+        t[2] = cmul(t[1], t[1]); t[3] = cmul(t[2], t[1]); t[4] = cmul(t[2], t[2]);
+        t[5] = cmul(t[4], t[1]); t[6] = cmul(t[4], t[2]); t[7] = cmul(t[4], t[3]);
+        q[2] = cmul(q[1], q[1]); q[3] = cmul(q[2], q[1]);
+#pragma unroll
+        for (int ka = 1; ka < 8; ++ka) p[ka * PA] = cmul(v[ka], t[ka]);
+#pragma unroll
+        for (int h = 1; h < 4; ++h) {
+            p[8 * h * PA] = cmul(v[8 * h], q[h]);
+#pragma unroll
+            for (int l = 1; l < 8; ++l) p[(8 * h + l) * PA] = cmul(v[8 * h + l], cmul(q[h], t[l]));
+        }
+    }
+    __syncthreads();
+#pragma unroll 1
+    for (int i = threadIdx.x; i < 32 * 32; i += RW_THREADS) {                  // item (ka, c): radix 16 over b
+        const int c = i & 31, ka = i >> 5;
+        float2* p = fsm + ka * PA + c;
+        float2 v[16];
+#pragma unroll
+        for (int b = 0; b < 16; ++b) v[b] = p[b * PB];
+        fft_reg<16>(v);
+#pragma unroll
+        for (int kb = 1; kb < 16; ++kb) v[kb] = cmul(v[kb], tw512[kb * 32 + c]);
+#pragma unroll
+        for (int kb = 0; kb < 16; ++kb) p[kb * PB] = v[kb];
+    }
+    __syncthreads();
+    {                                                                          // item (ka, kb), ka fastest: radix 32 over c
+        const int ka = threadIdx.x & 31, kb = threadIdx.x >> 5;
+        const float2* p = fsm + ka * PA + kb * PB;
+        float2 v[32];
+#pragma unroll
+        for (int c = 0; c < 32; ++c) v[c] = p[c];
+        fft_reg<32>(v);
+        float2* out = Zb + ka + 32 * kb;                                       // k2 = ka + 32 (kb + 16 kc)
+#pragma unroll
+        for (int kc = 0; kc < 32; ++kc) __stcs(out + kc * 512, v[kc]);
     }
 }
 

@@ -296,13 +296,14 @@ def test_c5_bench_config_at_4_sigma(tb):
 
 # ------------------------------------------------------------------ hand-written FFT path: every instantiation
 @pytest.mark.parametrize("log2n,window", [(17, 256), (17, 1024), (18, 512), (19, 1024), (19, 2048), (20, 512),
-                                          (21, 1024), (21, 2048), (22, 2048), (23, 1024), (24, 1024), (24, 2048),
+                                          (21, 1024), (21, 2048), (22, 2048), (23, 1024), (24, 512), (24, 2048),
                                           (25, 1024), (26, 1024)])
 def test_own_fft_every_radix_and_window(tb, log2n, window):
     """One circular and one elliptical template per (row-FFT length, median window) pair the
     hand-written path is instantiated for: M2 = 256..8192 (R1 = 1..32; 2^23 is the bench
-    instantiation) x W = 256..2048, M1 = 1024 (2^24, 8-column bundles) and the three-pass variant
-    (2^25, 2^26), at 5 sigma (dozens of candidates per template), every harmonic sum compared.
+    instantiation) x W = 256..2048, the 16384-point rows of k_fft_rows_wide with M1 = 512 (2^24) and
+    M1 = 1024 (2^25, 8-column bundles in pass 1) and the three-pass variant (2^26), at 5 sigma (dozens
+    of candidates per template), every harmonic sum compared.
     fft_path=2 fails the plan if the pair is unsupported."""
     # C5's orbits at 2^17 samples of 64 us are too fast for 8-sample knots (exact fallback, cuFFT path): use C1 there
     w = wl_mod.config1() if log2n == 17 else wl_mod.config5(log2n=log2n)
