@@ -44,14 +44,25 @@ class Workload:
 
 
 # ------------------------------------------------------------------ signal model (injection only)
+def _settle(step_fn, x, max_iter, tol):
+    """x <- x - step_fn(x) up to max_iter times or until max|step| < tol.  When the last digit
+    flickers between two values (x_k == x_{k-2}) the remaining iterations are skipped and the value
+    the full loop would have ended on is returned, bit for bit: the tolerances below are tighter
+    than one ulp of the larger arguments, so without this every call ran all max_iter iterations."""
+    prev = None                                     # iterate before the last one
+    for k in range(max_iter):
+        step = step_fn(x)
+        new = x - step
+        if np.max(np.abs(step)) < tol:
+            return new
+        if prev is not None and np.array_equal(new, prev):          # period 2: new, x, new, x, ...
+            return new if (max_iter - 1 - k) % 2 == 0 else x
+        prev, x = x, new
+    return x
+
+
 def _ecc_anomaly(M, e):
-    E = M + e * np.sin(M)
-    for _ in range(60):
-        step = (E - e * np.sin(E) - M) / (1.0 - e * np.cos(E))
-        E -= step
-        if np.max(np.abs(step)) < 1e-15:
-            break
-    return E
+    return _settle(lambda E: (E - e * np.sin(E) - M) / (1.0 - e * np.cos(E)), M + e * np.sin(M), 60, 1e-15)
 
 
 def _delay_and_rate(t, p_orb, tau, phi0, e, om):
@@ -70,14 +81,12 @@ def emission_times(s, p_orb, tau, phi0, e, om):
     (eq A2 with the zero offset of L675), Newton in t'.  This is the exact inverse of the
     search's gather map (reading G3)."""
     d0, _ = _delay_and_rate(np.zeros(1), p_orb, tau, phi0, e, om)
-    t = np.array(s, dtype=np.float64)
-    for _ in range(60):
+
+    def step(t):
         d, dd = _delay_and_rate(t, p_orb, tau, phi0, e, om)
-        step = (t - (d - d0[0]) - s) / (1.0 - dd)
-        t -= step
-        if np.max(np.abs(step)) < 1e-13:
-            break
-    return t
+        return (t - (d - d0[0]) - s) / (1.0 - dd)
+
+    return _settle(step, np.array(s, dtype=np.float64), 60, 1e-13)
 
 
 def pulse_train(n, tsamp, p_spin, p_orb, tau, phi0, e, om, amp, duty=DUTY):
