@@ -473,11 +473,11 @@ int launch_cols(tb_plan* p, size_t off, uint32_t nt, long long* d_idx, float* d_
     return TB_OK;
 }
 
-template <int R1>
+template <int R1, bool TWIN = false>
 int launch_rows(tb_plan* p, uint32_t nt)
 {
     using Cfg = RowsCfg<R1>;
-    auto kern = k_fft_rows_t<R1>;
+    auto kern = k_fft_rows_t<R1, TWIN>;
     if (int rc_ = allow_smem(p, reinterpret_cast<const void*>(kern), (size_t)(Cfg::SMEM))) return rc_;
     const unsigned grid = (unsigned)(((1u << p->log2m1) / Cfg::R) * nt);
     kern<<<grid, FFT_THREADS, Cfg::SMEM, p->stream>>>(reinterpret_cast<const float2*>(p->d_resampled), p->d_fft, p->log2m1,
@@ -486,10 +486,13 @@ int launch_rows(tb_plan* p, uint32_t nt)
     return TB_OK;
 }
 
+// N = 2^23 (rows of 8192 points): the four-step twiddle is applied by pass 2 on load instead of pass 1 on store
+bool twiddle_in_pass2(const tb_plan* p) { return p->cols32 && p->log2m2 == 13; }
+
 template <bool DEBUG>
 int launch_cols32(tb_plan* p, size_t off, uint32_t nt, long long* d_idx, float* d_y)
 {
-    auto kern = k_fft_cols32<DEBUG>;
+    auto kern = twiddle_in_pass2(p) ? k_fft_cols32<DEBUG, false> : k_fft_cols32<DEBUG, true>;
     if (int rc_ = allow_smem(p, reinterpret_cast<const void*>(kern), (size_t)(C32_SMEM))) return rc_;
     const unsigned grid = (unsigned)(((1u << p->log2m2) / 16) * nt);
     kern<<<grid, FFT_THREADS, C32_SMEM, p->stream>>>(p->d_series, p->d_seg, p->seg_stride, p->d_tmpl + off, (int)nt, (int)p->n,
@@ -581,7 +584,7 @@ int run_own_pass2(tb_plan* p, uint32_t nt)
         case 2: return launch_rows<4>(p, nt);
         case 3: return launch_rows<8>(p, nt);
         case 4: return launch_rows<16>(p, nt);
-        case 5: return launch_rows<32>(p, nt);
+        case 5: return twiddle_in_pass2(p) ? launch_rows<32, true>(p, nt) : launch_rows<32>(p, nt);
     }
     return fail(p, TB_ERR_INVALID_ARG, "unsupported M2");
 }

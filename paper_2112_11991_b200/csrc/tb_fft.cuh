@@ -535,7 +535,9 @@ __device__ __forceinline__ void cols32_park_indices(const SegRec* __restrict__ s
     }
 }
 
-template <bool DEBUG>
+//   TW = false: the four-step twiddle W_M^{j2 k1} is left to pass 2 (k_fft_rows_t<32, true>, N = 2^23): pass 1 is
+//   bound by instruction issue, pass 2 by HBM with issue slots to spare.
+template <bool DEBUG, bool TW = true>
 __global__ void __launch_bounds__(FFT_THREADS, COLS_MINB)
 k_fft_cols32(const float* __restrict__ x, const SegRec* __restrict__ seg, size_t seg_stride,
              const TmplDev* __restrict__ tmpl, int n_tmpl, int n, int log2m2, float fill,
@@ -613,6 +615,13 @@ k_fft_cols32(const float* __restrict__ x, const SegRec* __restrict__ seg, size_t
         for (int cc = 0; cc < 16; ++cc) v[cc] = p[cc];
         fft_reg<16>(v);
         const int j2 = c0 + cl;
+        if constexpr (!TW) {
+            float2* out = Tb + ((size_t)ka << log2m2) + j2;
+            const unsigned kstep = 32u << log2m2;
+#pragma unroll
+            for (int kc = 0; kc < 16; ++kc) __stcs(out + (unsigned)kc * kstep, v[kc]);
+            continue;
+        }
         // W_M^{j2 k1} = W_M^{j2 ka} * g^kc, g = W_M^{32 j2}; both arguments are exact in fp32
         const float inv_m = 1.0f / (float)m;
         float sb, cb, sg, cg;
@@ -806,11 +815,15 @@ template <int R1> struct RowsCfg {
     static constexpr size_t SMEM = (size_t)(R * LP + 256) * sizeof(float2);
 };
 
-template <int R1>
+//   TWIN = true (R1 = 32 only): the input has not been multiplied by the four-step twiddle yet; element
+//   j2 = a 256 + w of row k1 takes W_M^{j2 k1} = W_M^{k1 w} (W_M^{256 k1})^a here, from two sincospif with
+//   exact arguments and a power tree, computed while the loads are in flight.
+template <int R1, bool TWIN = false>
 __global__ void __launch_bounds__(FFT_THREADS, RowsCfg<R1>::MINB)
 k_fft_rows_t(const float2* __restrict__ T, float2* __restrict__ Zt, int log2m1, const float2* __restrict__ tw1,
              const float2* __restrict__ tw2g, int pf_dist)
 {
+    static_assert(!TWIN || R1 == 32, "the twiddle-on-load variant is instantiated for 8192-point rows only");
     using Cfg = RowsCfg<R1>;
     constexpr int PA = Cfg::PA, PB = Cfg::PB, R = Cfg::R, LP = Cfg::LP;
     constexpr int L = R1 * 256;                    // M2
@@ -841,6 +854,25 @@ k_fft_rows_t(const float2* __restrict__ T, float2* __restrict__ Zt, int log2m1, 
         for (int r = 0; r < R; ++r)
 #pragma unroll
             for (int a = 0; a < R1; ++a) v[r][a] = __ldcs(Tb + (size_t)r * L + a * 256 + w);
+        if constexpr (TWIN) {
+            const float inv_m = 1.0f / (float)((size_t)L << log2m1);
+            float sb, cb, sg, cg;
+            sincospif(-2.0f * (float)(k1 * w) * inv_m, &sb, &cb);              // k1 w, 256 k1 < 2^17: exact in fp32
+            sincospif(-2.0f * (float)(k1 * 256) * inv_m, &sg, &cg);
+            float2 t[8], bq[4];                                                 // g^l, base g^{8h}
+            t[1] = make_float2(cg, sg);
+            t[2] = cmul(t[1], t[1]); t[3] = cmul(t[2], t[1]); t[4] = cmul(t[2], t[2]);
+            t[5] = cmul(t[4], t[1]); t[6] = cmul(t[4], t[2]); t[7] = cmul(t[4], t[3]);
+            const float2 g8 = cmul(t[4], t[4]);
+            bq[0] = make_float2(cb, sb);
+            bq[1] = cmul(bq[0], g8); bq[2] = cmul(bq[1], g8); bq[3] = cmul(bq[2], g8);
+#pragma unroll
+            for (int h = 0; h < 4; ++h) {
+                v[0][8 * h] = cmul(v[0][8 * h], bq[h]);
+#pragma unroll
+                for (int l = 1; l < 8; ++l) v[0][8 * h + l] = cmul(v[0][8 * h + l], cmul(bq[h], t[l]));
+            }
+        }
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             fft_reg<R1>(v[r]);
