@@ -134,11 +134,15 @@ typedef struct {
 /* Per-stage device time of the last tb_search_templates call (CUDA events on the plan's stream,
  * summed over chunks; zero unless opts.enable_timings), and the byte model of DESIGN.md section 7.
  *   hand-written FFT path (fft_path_used = 2)        cuFFT path (fft_path_used = 1)
- *   ms_delay     K0 k_delay_segments (a2 knots)      0
+ *   ms_delay     K0 k_delay_segments (a2 knots);     0
+ *                from the second chunk on it runs on a
+ *                side stream beside P2 / the spectrum
+ *                former of the previous chunk: the span
+ *                it was resident for, NOT additive
  *   ms_resample  P1 k_fft_cols32 / k_fft_cols        k_resample (a2+a3)
  *                (a2+a3 + a4 pass 1)
- *   ms_fft       P2 k_fft_rows_t (a4 pass 2; two     batched cuFFT R2C (a4)
- *                kernels at N >= 2^25)
+ *   ms_fft       P2 k_fft_rows_t / k_fft_rows_wide   batched cuFFT R2C (a4)
+ *                (a4 pass 2; two kernels at N = 2^26)
  *   ms_spectrum  k_spectrum_t (a4 unpack, a5-a7)     k_spectrum_median (a5-a7)
  *   ms_hsum      k_hsum_tile (a8+a9)                 same
  * ms_normalise is always 0 (a7 is fused into the spectrum kernels); kept for layout stability. */
