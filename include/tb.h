@@ -26,7 +26,8 @@
  *   - Work is queued on the plan's stream (opts.stream, or a stream the plan creates).
  *     tb_search_templates returns once the work is queued (host template staging is complete);
  *     tb_get_candidates / tb_get_timings / tb_debug_* synchronise that stream.
- *   - No global state in the library and no environment variables; plans are independent; one
+ *   - No global state in the library (one exception: the static scratch array of
+ *     tb_series_mean_noalloc, see there) and no environment variables; plans are independent; one
  *     plan must not be used from two threads at once.  Two device-wide side effects, both of
  *     performance only: tb_plan_create RAISES cudaLimitPersistingL2CacheSize to the size of the
  *     series if it is smaller (it is never lowered or reset, so other plans keep their L2 set-aside),
@@ -315,6 +316,41 @@ TB_API int tb_bank_generate(const tb_bank_space* space, const double* uniforms, 
 /* Host fp64: number of random templates for coverage eta at nominal mismatch m_star in n_dim
  * dimensions and proper volume `volume`: eq 20 (L131; exact != 0) or eq 21 (L136), C_n of eq 18 (L123). */
 TB_API int tb_bank_n_templates(double eta, double m_star, uint32_t n_dim, double volume, int32_t exact, double* n_out);
+
+/* ---- one entry point that allocates nothing ----
+ * tb_series_mean_noalloc: the fp64 mean of a float32 series that is already on the GPU, i.e. the value a
+ * plan uses to fill resampled samples whose source falls outside the series (reading G8; the resampling
+ * step is Alg. 1).  Every other GPU entry point of this library calls cudaMalloc, directly or through a plan.
+ * Some callers cannot afford that: a real-time acquisition loop, where cudaMalloc / cudaFree would take
+ * the driver's lock and make the device drain while copies and searches are in flight on other streams;
+ * and a process that handed the whole GPU to its own memory pool at start-up, where cudaMalloc simply
+ * fails.  This call makes no cudaMalloc, no cudaFree and no allocating library call.  Its only scratch
+ * memory (one partial sum per 65 536 samples and an arrival counter) is a static device array of
+ * TB_NOALLOC_SCRATCH_BYTES that every GPU on which the library's kernels get loaded holds until the
+ * process exits.
+ *
+ *   d_series     device float32[n_samples], on the device that is current on the calling thread
+ *   n_samples    1 .. TB_NOALLOC_MAX_SAMPLES (2^28); need not be a power of two.  More -> TB_ERR_CAPACITY
+ *                (the static array has no room for the partial sums), nothing is queued.  0 -> TB_ERR_INVALID_ARG
+ *   d_mean_out   device double[1], same device; written by the kernel: read it after the stream has
+ *                reached this point.  (float)*d_mean_out is the fill value a plan would derive
+ *   stream       a cudaStream_t of that device (NULL = the default stream).  The call only queues a
+ *                256-byte clear and one kernel on it and returns; it never synchronises
+ *   errbuf       optional (NULL): receives a one-line description when the call fails; errbuf_len bytes
+ *
+ * First call on each device: it also looks up the device address of the static array (cudaGetSymbolAddress,
+ * which makes the runtime load this library's kernels on that device if nothing did yet).  Make that
+ * first call during start-up, before any stream capture.  Later calls only queue work.
+ * Shared state: all calls in the process, from any thread, on any stream, use the same array on a given
+ * device, and it keeps what the last call left (the counter is cleared at the start of every call).  Two
+ * calls whose kernels may overlap on the GPU (different streams without an event between them) race on it
+ * and both results are garbage: order them, e.g. by using one stream.  Calls on different devices are
+ * independent.  The result is deterministic (fixed summation order, independent of the SM count) and
+ * agrees with the plan's fill value to fp64 rounding (a few 1e-16 relative). */
+#define TB_NOALLOC_MAX_SAMPLES   (1ull << 28)
+#define TB_NOALLOC_SCRATCH_BYTES 33024   /* (32 + 4096) doubles */
+TB_API int tb_series_mean_noalloc(const float* d_series, uint64_t n_samples, double* d_mean_out, void* stream,
+                           char* errbuf, uint64_t errbuf_len);
 
 #ifdef __cplusplus
 }

@@ -13,8 +13,8 @@ CSRC = os.path.join(HERE, "csrc")
 LIB_DIR = os.path.join(HERE, "lib")
 LIB_PATH = os.path.join(LIB_DIR, "libtb.so")
 CUDA_HOME = os.environ.get("CUDA_HOME", "/usr/local/cuda")
-SOURCES = ["tb_api.cu", "tb_bank.cu"]
-DEPS = ["tb_api.cu", "tb_bank.cu", "tb_kernels.cuh", "tb_fft.cuh", "tb_reduce.cuh", "tb_whiten.cuh", os.path.join("..", "..", "include", "tb.h")]
+SOURCES = ["tb_api.cu", "tb_bank.cu", "tb_noalloc.cu"]
+DEPS = ["tb_api.cu", "tb_bank.cu", "tb_noalloc.cu", "tb_kernels.cuh", "tb_fft.cuh", "tb_reduce.cuh", "tb_whiten.cuh", os.path.join("..", "..", "include", "tb.h")]
 
 
 def needs_build() -> bool:

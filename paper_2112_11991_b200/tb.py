@@ -21,6 +21,8 @@ lib = C.CDLL(_LIB_PATH)
 
 TB_OK, TB_ERR_INVALID_ARG, TB_ERR_CUDA, TB_ERR_CUFFT, TB_ERR_NOMEM, TB_ERR_OVERFLOW, TB_ERR_CAPACITY = 0, -1, -2, -3, -4, -5, -6
 
+TB_NOALLOC_MAX_SAMPLES, TB_NOALLOC_SCRATCH_BYTES = 1 << 28, 33024
+
 TEMPLATE_DTYPE = np.dtype([("p_orb_s", "<f8"), ("tau_lts", "<f8"), ("phi0_rad", "<f8"), ("ecc", "<f8"),
                            ("omega_rad", "<f8")])
 CANDIDATE_DTYPE = np.dtype([("template_id", "<u4"), ("fold", "<u4"), ("bin", "<u4"), ("power", "<f4"),
@@ -62,7 +64,7 @@ EXPORTS = ["tb_plan_create", "tb_plan_set_series", "tb_search_templates", "tb_ge
            "tb_reduce_candidates", "tb_debug_set_candidates",
            "tb_strerror", "tb_last_error", "tb_get_timings", "tb_debug_resample_indices", "tb_debug_spectrum",
            "tb_debug_resampled", "tb_debug_hsums", "tb_debug_series", "tb_sigma_to_power", "tb_plan_info", "tb_template_knot_log2",
-           "tb_bank_density", "tb_bank_generate", "tb_bank_n_templates"]
+           "tb_bank_density", "tb_bank_generate", "tb_bank_n_templates", "tb_series_mean_noalloc"]
 
 _vp, _u64, _u32 = C.c_void_p, C.c_uint64, C.c_uint32
 lib.tb_plan_create.argtypes = [C.POINTER(_vp), _vp, _u64, C.c_double, C.POINTER(PlanOpts)]
@@ -89,6 +91,7 @@ lib.tb_template_knot_log2.argtypes = [_vp, _vp, C.POINTER(C.c_int32)]
 lib.tb_bank_density.argtypes = [C.POINTER(BankSpace), _vp, _u64, _vp]
 lib.tb_bank_generate.argtypes = [C.POINTER(BankSpace), _vp, _u64, C.c_double, _vp, _u64, C.POINTER(_u64), _vp, C.POINTER(C.c_double)]
 lib.tb_bank_n_templates.argtypes = [C.c_double, C.c_double, _u32, C.c_double, C.c_int32, C.POINTER(C.c_double)]
+lib.tb_series_mean_noalloc.argtypes = [_vp, _u64, _vp, _vp, C.c_char_p, _u64]
 for _name in EXPORTS:
     if _name not in ("tb_strerror", "tb_last_error"):
         getattr(lib, _name).restype = C.c_int
@@ -388,3 +391,20 @@ def tb_bank_n_templates(eta, m_star, n_dim, volume, exact=True) -> float:
     out = C.c_double(0.0)
     _check(lib.tb_bank_n_templates(float(eta), float(m_star), int(n_dim), float(volume), int(bool(exact)), C.byref(out)))
     return float(out.value)
+
+
+def tb_series_mean_noalloc(d_series, n_samples, d_mean_out, stream=None) -> None:
+    """Queue the fp64 mean of a device-resident float32 series (the default fill value of a plan) on
+    `stream`, for callers that must not allocate device memory: a real-time loop that cannot take the
+    device-wide stall of cudaMalloc / cudaFree, or a process whose own pool already holds all GPU memory.
+
+    d_series, d_mean_out: integer device addresses (float32[n_samples] and float64[1]) on the current CUDA
+    device; stream: an integer cudaStream_t or None.  Nothing is allocated and nothing is synchronised:
+    read d_mean_out after the stream has got there.  n_samples <= TB_NOALLOC_MAX_SAMPLES, else TbError
+    (TB_ERR_CAPACITY).  All calls share one static scratch array per GPU: do not let two of them overlap
+    on the device.  See include/tb.h."""
+    err = C.create_string_buffer(384)
+    code = lib.tb_series_mean_noalloc(int(d_series) if d_series else None, int(n_samples),
+                                      int(d_mean_out) if d_mean_out else None, stream, err, len(err))
+    if code != TB_OK:
+        raise TbError(code, err.value.decode())
