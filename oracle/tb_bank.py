@@ -36,6 +36,16 @@ Readings:
        for the several-orbit banks of BASELINE.json's configs, cond ~ 1e4) or, with digits=D, in
        D-digit mpmath arithmetic (density_mp), which is what the paper's box is compared in.
 
+Against the paper's printed values (box of Table 1, eq 20 with eta = 0.9, m = 0.2):
+  circular    paper 10 128      here N_R = 9946 +- 174 (20 000 proposals): reproduced, and pinned by
+                                test_circular_template_count_of_the_papers_box
+  elliptical  paper 2 047 716   here N_R ~ 60 (V = 2.5 +- 0.6): NOT reproduced.  Dropping the tau X term of
+                                d Phi / d f (eq 28), the literal chain in float64 and the obvious omitted
+                                Jacobians of eq 29 were tried: none gives the printed
+                                count and the text does not say what was integrated.  The elliptical mode is
+                                therefore PARITY UNPINNED against the paper; its pins below fix the mathematics
+                                of reading G27, not the reading.
+
 Parity pins (tests/test_bank_pins.py, -m "not gpu"):
   phase_derivatives ... every column against central finite differences of the EXACT phase (Kepler
                         solve of oracle/tb_oracle.py, no series) at e = 0.05

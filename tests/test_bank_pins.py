@@ -286,3 +286,46 @@ def test_rejection_placement_by_brute_force():
     _, _, acc, _ = bank.generate(us, SPACE_C, top, n_quad=64)
     assert 400 < acc.sum() < 600                                # acceptance rate 1/3
     assert abs(us[acc, 1].mean() - 0.75) < 4 * math.sqrt(3.0 / 80.0 / acc.sum())
+
+
+# Table 1 of the paper: t_obs = 1.2 h, f_max = 66.67 Hz, P_orb ~ U(6, 12) h,
+# m_pulsar,min = 1.4, m_companion,max = 8.0 solar masses, tau ~ U(0, eq 31), eta = 0.9, m = 0.2
+PAPER_BOX = {"t_obs": 1.2 * 3600.0, "f_max": 66.67, "p_orb_min": 6 * 3600.0, "p_orb_max": 12 * 3600.0,
+             "m_pulsar_min": 1.4, "m_comp_max": 8.0, "theta": 1.0, "e_max": 0.1, "elliptical": False}
+
+
+def test_circular_template_count_of_the_papers_box():
+    """The only number the paper prints for anything this module computes: "we generated
+    10,128 orbital templates ... computed from equation 20 assuming a coverage eta = 0.9 and mismatch
+    m = 0.2" for the circular search over Table 1's box.  Metric (eq 13), projection (eq 22), density,
+    prior box (eq 31), proposal pdf and the Monte-Carlo volume (eq 17) all enter: a dropped factor of
+    2 pi, a wrong power of tau or Omega in the proposal pdf or a missing projection moves N_R by far more
+    than the Monte-Carlo error.  20 000 seeded proposals: V = 1618.5 +- 28.4, N_R = 9946 +- 174, i.e.
+    1.0 sigma below the printed value (whose own Monte-Carlo error the paper does not state)."""
+    n = 20000
+    u = np.random.default_rng(10128).random((n, 6))
+    _, rho, _, vol = bank.generate(u, PAPER_BOX, rho_max=1e30)
+    q = np.array([bank.proposal_pdf(bank.proposal(x, PAPER_BOX), PAPER_BOX) for x in u])
+    v = rho / q
+    assert vol == pytest.approx(float(v.mean()), rel=1e-12)
+    n_r = bank.n_templates(0.9, 0.2, 3, vol, exact=True)                 # eq 20 (L131)
+    sigma = n_r * float(v.std()) / math.sqrt(n) / vol
+    assert sigma < 250.0                                                 # the sample is large enough to mean something
+    assert abs(n_r - 10128.0) < 3.0 * sigma, (n_r, sigma)
+    # and the large-volume form eq 21 (L136) agrees with eq 20 here
+    assert bank.n_templates(0.9, 0.2, 3, vol, exact=False) == pytest.approx(n_r, rel=1e-3)
+
+
+def test_elliptical_count_of_the_papers_box_is_not_reproduced():
+    """PAPER.md:L316 also prints 2,04,7716 (2 047 716) templates for the five-parameter search of the same box
+    with e ~ U(0, 0.1).  Under reading G27 this oracle gives V ~ 2.5 and N_R ~ 60 (DESIGN.md section 13 lists
+    the alternative readings tried; none reproduces the printed count).  This test only records the order of
+    magnitude so that the disagreement stays visible: it is NOT a pin, the elliptical mode stays "parity
+    unpinned against the paper"."""
+    space = dict(PAPER_BOX, elliptical=True)
+    n = 300
+    u = np.random.default_rng(2047716).random((n, 6))
+    _, rho, _, vol = bank.generate(u, space, rho_max=1e30)
+    assert np.all(np.isfinite(rho)) and np.all(rho >= 0)
+    n_r = bank.n_templates(0.9, 0.2, 5, vol, exact=False)
+    assert 1.0 < n_r < 2.0e4, n_r                                        # four to five orders below 2 047 716

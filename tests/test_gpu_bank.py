@@ -141,3 +141,26 @@ def test_generated_bank_feeds_the_search(tb, c1):
     assert n > 0 and 0 in set(cands["template_id"])
     best = cands[np.argmax(cands["sigma"])]
     assert int(best["template_id"]) == 0 and (int(best["fold"]), int(best["bin"])) == (3, 52429)
+
+
+def test_papers_circular_template_count_on_the_device(tb):
+    """PAPER.md:L316 prints 10 128 circular templates for Table 1's box (eq 20, eta = 0.9, m = 0.2).  The device's
+    Monte-Carlo volume over the same 20 000 seeded proposals as the oracle's pin
+    (test_bank_pins.py::test_circular_template_count_of_the_papers_box) gives the same N_R, within 3 sigma of the
+    printed count.  The elliptical count (2 047 716) is not reproduced by either side: DESIGN.md section 13."""
+    from parity import SUMMARY
+    sp = SPACES["paper-circular"]
+    n = 20000
+    u = np.random.default_rng(10128).random((n, 6))
+    out, rho_g, vol_g = tb.tb_bank_generate(c_space(tb, sp), u, 1e300)
+    assert len(out) == 0
+    rho_o, q_o, _ = oracle_points(sp, u)                               # longdouble: cond ~ 1e4..1e8 in the circular box
+    v = rho_o / q_o
+    vol_o = float(v.mean())
+    assert np.abs(rho_g - rho_o).max() <= REL_ILL * rho_o.max()
+    assert vol_g == pytest.approx(vol_o, rel=10 * REL_ILL)
+    n_g = tb.tb_bank_n_templates(0.9, 0.2, 3, vol_g, True)
+    sigma = n_g * float(v.std()) / np.sqrt(n) / vol_o
+    assert abs(n_g - 10128.0) < 3.0 * sigma
+    SUMMARY.append(f"f3 paper box, circular: device V = {vol_g:.1f}, N_R(eq 20) = {n_g:.0f} +- {sigma:.0f} (oracle {obank.n_templates(0.9, 0.2, 3, vol_o, True):.0f}; "
+                   f"paper L316: 10 128); elliptical: not reproduced by either side (DESIGN.md section 13)")
