@@ -306,6 +306,10 @@ TB_API int tb_bank_density(const tb_bank_space* space, const double* lam, uint64
  * is P_orb = min + u0 (max - min), tau = u1 tau_max(Omega), alpha = 2 pi u2, psi = 2 pi u3, e = u4 e_max
  * and is accepted iff u5 * rho_max < rho.  Accepted proposals are written to `out` (host, capacity
  * entries) as templates (P_orb, tau, phi0 = alpha, e, omega = psi) IN PROPOSAL ORDER.
+ * rho_max must bound the density over the box for the accepted set to follow rho: a proposal with
+ * rho > rho_max is accepted with probability 1 (the sampled density is clipped at rho_max) and the call
+ * does not report it -- pass rho_out and check max(rho_out) <= rho_max (or draw a first batch with
+ * rho_max = +huge, which accepts nothing, to learn the maximum).  volume_out does not depend on rho_max.
  *   n_accepted   receives the number accepted (also when it exceeds capacity -> TB_ERR_CAPACITY)
  *   rho_out      optional (NULL), host double[n]: the density of every proposal
  *   volume_out   optional (NULL): Monte-Carlo estimate of the proper volume V = int rho d lambda

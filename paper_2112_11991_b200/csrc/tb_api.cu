@@ -383,13 +383,17 @@ void pin_series_in_l2(tb_plan* p)
     size_t have = 0;
     if (cudaDeviceGetLimit(&have, cudaLimitPersistingL2CacheSize) != cudaSuccess) have = 0;
     if (have < want) cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, want);
+    // the set-aside actually in force (the call above may have failed or been rounded): a window
+    // that asks for more persisting lines than there are only thrashes them
+    size_t limit = 0;
+    if (cudaDeviceGetLimit(&limit, cudaLimitPersistingL2CacheSize) != cudaSuccess || limit == 0) { cudaGetLastError(); return; }
     if (!p->own_stream && cudaStreamGetAttribute(p->stream, cudaStreamAttributeAccessPolicyWindow, &p->l2_prev) != cudaSuccess)
         std::memset(&p->l2_prev, 0, sizeof(p->l2_prev));
     cudaStreamAttrValue attr;
     std::memset(&attr, 0, sizeof(attr));
     attr.accessPolicyWindow.base_ptr = const_cast<float*>(p->d_series);
     attr.accessPolicyWindow.num_bytes = bytes;
-    attr.accessPolicyWindow.hitRatio = std::min(1.0f, (float)prop.persistingL2CacheMaxSize / (float)bytes);
+    attr.accessPolicyWindow.hitRatio = std::min(1.0f, (float)limit / (float)bytes);
     attr.accessPolicyWindow.hitProp = cudaAccessPropertyPersisting;
     attr.accessPolicyWindow.missProp = cudaAccessPropertyStreaming;
     if (cudaStreamSetAttribute(p->stream, cudaStreamAttributeAccessPolicyWindow, &attr) == cudaSuccess) p->l2_pinned = true;
@@ -1445,7 +1449,7 @@ int tb_reduce_candidates(tb_plan* p, double freq_tol_bins, tb_group* groups_out,
     DevBufs mem;
     SortRec *srt = nullptr, *rank = nullptr, *gt = nullptr;
     Peak* peaks = nullptr;
-    uint32_t *peak_of = nullptr, *F = nullptr, *rank_of_peak = nullptr, *gid = nullptr, *d_member = nullptr;
+    uint32_t *peak_of = nullptr, *F = nullptr, *Fs = nullptr, *rank_at = nullptr, *rank_of_peak = nullptr, *gid = nullptr, *d_member = nullptr;
     int* state = nullptr;
     unsigned int* ctr = nullptr;                     // [0] peaks, [1] undecided, [2] groups
     Group* groups = nullptr;
@@ -1469,6 +1473,8 @@ int tb_reduce_candidates(tb_plan* p, double freq_tol_bins, tb_group* groups_out,
     TB_CUDA(p, mem.get(&rank, ppad));
     TB_CUDA(p, mem.get(&gt, ppad));
     TB_CUDA(p, mem.get(&F, np));
+    TB_CUDA(p, mem.get(&Fs, np));
+    TB_CUDA(p, mem.get(&rank_at, np));
     TB_CUDA(p, mem.get(&state, np));
     TB_CUDA(p, mem.get(&rank_of_peak, np));
     TB_CUDA(p, mem.get(&gid, np));
@@ -1478,10 +1484,20 @@ int tb_reduce_candidates(tb_plan* p, double freq_tol_bins, tb_group* groups_out,
     if (int rc = device_sort(p, rank, ppad)) return rc;
     k_red_rank_init<<<blocks_for(np), 256, 0, p->stream>>>(peaks, rank, np, F, state, rank_of_peak);
 
-    // R3: rounds until every peak is a head or absorbed (each round decides at least the strongest open peak)
-    for (size_t round = 0; round <= np; ++round) {
+    // the same peaks sorted by F (gt is free until R4): the windows of R3 are binary searches in Fs
+    k_red_freq_keys<<<blocks_for(ppad), 256, 0, p->stream>>>(F, np, ppad, gt);
+    if (int rc = device_sort(p, gt, ppad)) return rc;
+    k_red_freq_split<<<blocks_for(np), 256, 0, p->stream>>>(gt, np, Fs, rank_at);
+
+    // R3: rounds until every peak is a head or absorbed (each round decides at least the strongest open peak).
+    // Four rounds are queued per look at the counter (most lists are done after two or three; a round
+    // with nothing left to decide costs one read per peak), so the host synchronises once per batch.
+    constexpr int ROUNDS_PER_CHECK = 4;
+    for (size_t round = 0; round <= np; round += ROUNDS_PER_CHECK) {
         TB_CUDA(p, cudaMemsetAsync(ctr + 1, 0, sizeof(unsigned int), p->stream));
-        k_red_distill_round<<<blocks_for(np), 256, 0, p->stream>>>(F, state, np, tol16, ctr + 1);
+        for (int k = 0; k < ROUNDS_PER_CHECK; ++k)
+            k_red_distill_round<<<blocks_for(np), 256, 0, p->stream>>>(F, Fs, rank_at, state, np, tol16,
+                                                                       k == ROUNDS_PER_CHECK - 1 ? ctr + 1 : nullptr);
         unsigned int open = 0;
         TB_CUDA(p, cudaMemcpyAsync(&open, ctr + 1, sizeof(open), cudaMemcpyDeviceToHost, p->stream));
         TB_CUDA(p, cudaStreamSynchronize(p->stream));

@@ -339,7 +339,7 @@ int tb_bank_density(const tb_bank_space* space, const double* lam, uint64_t n, d
     for (uint64_t i = 0; i < n; ++i) {
         const double* l = lam + 5 * i;
         for (int k = 0; k < 5; ++k) if (!std::isfinite(l[k])) return TB_ERR_INVALID_ARG;
-        if (l[0] < 0 || !(l[1] > 0) || l[4] < 0 || l[4] > 0.3) return TB_ERR_INVALID_ARG;
+        if (l[0] < 0 || !(l[1] > 0) || (sp.elliptical && (l[4] < 0 || l[4] > 0.3))) return TB_ERR_INVALID_ARG;   // psi, e are ignored when circular
         orbits = std::max(orbits, l[1] * sp.t_obs / TWO_PI);
     }
     const int threads = threads_for(orbits);

@@ -436,7 +436,9 @@ k_spectrum_median(const float2* __restrict__ X, size_t ld, float* __restrict__ P
                 carry = r2c_unpack2(__ldg(Xr + base - 1), __ldg(Xr + (nb - base + 1)),
                                     make_float2(wp.x * wl.x - wp.y * wl.y, wp.x * wl.y + wp.y * wl.x));
             }
-        } else if (base > 0 && lane == 0) carry = __ldg(Xr + base - 1);
+        } else if constexpr (!OVER) {                    // OVER counts `base` in half bins: Xr + base - 1 would lie past the row
+            if (base > 0 && lane == 0) carry = __ldg(Xr + base - 1);
+        }
         if constexpr (OVER) {
             static_assert(!UNPACK && !WHITE, "the oversampled spectrum is formed from the library R2C output");
             constexpr float C = 0.61685027506808491368f;     // (pi/4)^2

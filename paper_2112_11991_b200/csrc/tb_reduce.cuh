@@ -12,8 +12,13 @@
 //
 // The list is small next to the search (10^2..10^6 rows of 24 bytes), so the kernels are simple:
 // a bitonic sort (shared-memory tiles + global merge steps), a run scan, and R3 as rounds of a
-// data-parallel rule that reaches the sequential greedy result: a peak is decided once every
-// stronger related peak is decided (the first one that is a head absorbs it; none -> it is a head).
+// data-parallel rule that reaches the sequential greedy result: a peak is decided once its
+// strongest related peak that has not been absorbed is decided (a head absorbs it; none -> it is a
+// head itself).  The related peaks of a peak b are found, not scanned for: |q F_b - p F_a| <= tol
+// means F_a lies in [(q F_b - tol)/p, (q F_b + tol)/p], so with the peaks also sorted by F each of
+// the 159 coprime (p, q) pairs (a pair with a common factor g asks for tol/g: a subset) is one
+// binary search plus a walk over the window: O(159 log np + matches) per peak and round instead of
+// a walk over every stronger peak (O(np) each, O(np^2) per round, minutes at 10^5 peaks).
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -162,36 +167,68 @@ k_red_rank_init(const Peak* __restrict__ p, const SortRec* __restrict__ rank, si
     rank_of_peak[id] = (uint32_t)r;
 }
 
-// |q Fb - p Fa| <= tol for some 1 <= p, q <= 16: walk the two sorted sequences of multiples together
-__device__ __forceinline__ bool red_related(uint32_t Fa, uint32_t Fb, int64_t tol)
+// sort keys of the F-sorted view: (F, rank); padding sorts last
+__global__ void __launch_bounds__(256) k_red_freq_keys(const uint32_t* __restrict__ F, size_t n, size_t npad, SortRec* __restrict__ r)
 {
-    int64_t a = Fa, b = Fb;                          // current multiples p Fa, q Fb
-    int p = 1, q = 1;
-    while (true) {
-        const int64_t d = b - a;
-        if ((d < 0 ? -d : d) <= tol) return true;
-        if (d > 0) { if (++p > 16) return false; a += Fa; }
-        else       { if (++q > 16) return false; b += Fb; }
-    }
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= npad) return;
+    SortRec o;
+    if (i < n) { o.hi = F[i]; o.lo = (uint32_t)i; o.val = (uint32_t)i; }
+    else       { o.hi = ~0ull; o.lo = ~0u; o.val = ~0u; }
+    r[i] = o;
+}
+
+// the F-sorted view as two plain arrays (4-byte strides for the binary searches)
+__global__ void __launch_bounds__(256)
+k_red_freq_split(const SortRec* __restrict__ fs, size_t n, uint32_t* __restrict__ Fs, uint32_t* __restrict__ rank_at)
+{
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    Fs[i] = (uint32_t)fs[i].hi;
+    rank_at[i] = fs[i].val;
+}
+
+__device__ __forceinline__ bool red_coprime(int p, int q)
+{
+    while (q) { const int t = p % q; p = q; q = t; }
+    return p == 1;
 }
 
 // R3, one round.  state[r]: -1 undecided, r = head, h != r = absorbed by head h.  Decisions are final
 // and depend only on final decisions of stronger peaks, so concurrent rounds reach the greedy result.
+// Peak r looks up, window by window, the strongest (lowest-rank) related peak that is not absorbed:
+// none -> r is a head; a head -> it absorbs r; still undecided -> r waits for the next round.
 __global__ void __launch_bounds__(256)
-k_red_distill_round(const uint32_t* __restrict__ F, volatile int* state, size_t n, int64_t tol, unsigned int* __restrict__ undecided)
+k_red_distill_round(const uint32_t* __restrict__ F, const uint32_t* __restrict__ Fs, const uint32_t* __restrict__ rank_at,
+                    volatile int* state, size_t n, int64_t tol, unsigned int* __restrict__ undecided)
 {
     const size_t r = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (r >= n || state[r] >= 0) return;
-    const uint32_t Fb = F[r];
-    for (size_t a = 0; a < r; ++a) {
-        const int sa = state[a];
-        if (sa >= 0 && (size_t)sa != a) continue;                                    // absorbed peaks absorb nothing
-        if (!red_related(F[a], Fb, tol)) continue;
-        if (sa < 0) { atomicAdd(undecided, 1u); return; }                            // a stronger related peak is still open
-        state[r] = (int)a;
-        return;
+    const int64_t Fb = F[r];
+    uint32_t best = 0xffffffffu;
+    int best_state = 0;
+    for (int q = 1; q <= 16; ++q) {
+        const int64_t c = q * Fb;
+        for (int p = 1; p <= 16; ++p) {
+            if (!red_coprime(p, q)) continue;
+            int64_t lo = c - tol;                                                    // p Fa in [c - tol, c + tol]
+            lo = lo <= 0 ? 0 : (lo + p - 1) / p;
+            const int64_t hi = (c + tol) / p;
+            if (hi < lo) continue;
+            size_t a0 = 0, a1 = n;                                                   // first i with Fs[i] >= lo
+            while (a0 < a1) { const size_t m = (a0 + a1) >> 1; if ((int64_t)Fs[m] < lo) a0 = m + 1; else a1 = m; }
+            for (size_t i = a0; i < n && (int64_t)Fs[i] <= hi; ++i) {
+                const uint32_t a = rank_at[i];
+                if (a >= r || a >= best) continue;                                   // weaker than r, or no better than what we have
+                const int sa = state[a];
+                if (sa >= 0 && (uint32_t)sa != a) continue;                          // absorbed peaks absorb nothing
+                best = a; best_state = sa;
+            }
+        }
     }
-    state[r] = (int)r;
+    if (best == 0xffffffffu) { state[r] = (int)r; return; }
+    if (best_state < 0) { if (undecided) atomicAdd(undecided, 1u); return; }         // a stronger related peak is still open
+    state[r] = (int)best;
 }
 
 // R4a: heads numbered in rank order (single CTA, chunked scan)

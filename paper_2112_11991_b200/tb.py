@@ -186,18 +186,21 @@ def tb_get_candidates(plan, capacity=None):
 
 def tb_reduce_candidates(plan, freq_tol_bins=0.0, with_members=False, n_detections=0):
     """Returns (groups structured array in head order, member_of or None).  member_of (uint32 per
-    detection, in tb_get_candidates order) needs n_detections = the current candidate count."""
+    detection, in tb_get_candidates order) needs n_detections = the current candidate count.
+    One reduction per call: there are never more groups than detections, so groups_out is sized by the
+    detection count (n_detections, or the count tb_get_candidates reports) instead of by a first pass."""
     n = _u64(0)
-    code = lib.tb_reduce_candidates(plan, float(freq_tol_bins), None, 0, C.byref(n), None, 0)
-    if code == TB_OK:
-        return np.zeros(0, dtype=GROUP_DTYPE), (np.zeros(0, dtype=np.uint32) if with_members else None)
-    if code != TB_ERR_CAPACITY:
-        _check(code, plan)
-    out = np.zeros(int(n.value), dtype=GROUP_DTYPE)
+    n_det = int(n_detections)
+    if n_det == 0:
+        code = lib.tb_get_candidates(plan, None, 0, C.byref(n))            # count only
+        if code not in (TB_OK, TB_ERR_CAPACITY):
+            _check(code, plan)
+        n_det = int(n.value)
+    out = np.zeros(max(n_det, 1), dtype=GROUP_DTYPE)
     members = np.zeros(int(n_detections), dtype=np.uint32) if with_members else None
     _check(lib.tb_reduce_candidates(plan, float(freq_tol_bins), out.ctypes.data, out.size, C.byref(n),
                                     members.ctypes.data if with_members else None, int(n_detections)), plan)
-    return out[: n.value], members
+    return out[: n.value].copy(), members
 
 
 def tb_debug_set_candidates(plan, cands):
