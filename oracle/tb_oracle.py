@@ -79,8 +79,10 @@ def kepler_solve(M, e, tol=KEPLER_TOL, max_iter=KEPLER_MAX_ITER):
 
 
 def is_circular(tmpl) -> bool:
-    """A template with e == 0 and omega == 0 uses the circular closed form (boundary rule,
-    include/tb.h; eq 4 and eq A1 L666 at e = 0)."""
+    """A template with e == 0 and omega == 0 uses the circular closed form (eq 4 = eq A1
+    L666 at e = 0, omega = 0).  The library's own selector is e == 0 alone (include/tb.h: E = M, Delta =
+    tau sin(Omega t + phi0 + omega)); at e = 0 and omega != 0 this oracle goes through eq A1 with the Newton
+    solve, which returns E = M exactly there, so the two agree (reading G6)."""
     return float(tmpl[3]) == 0.0 and float(tmpl[4]) == 0.0
 
 

@@ -189,6 +189,24 @@ def test_t8_exponential_noise_normalises_to_unit_mean():
     assert abs(np.mean(ph[1:]) - 1.0) < 0.01
 
 
+def test_normalise_where_the_baseline_is_not_positive():
+    """"ours" (G15): a bin whose interpolated median is <= 0 normalises to 0, not to inf or NaN.  Blocks 1 and 2
+    are all zero, so m(k) = 0 between their centres; towards blocks 0 and 3 the baseline is interpolated and
+    positive, and the ordinary formula applies there (values by hand)."""
+    W = 4
+    P = np.array([2, 2, 2, 2, 0, 0, 0, 0, 0, 0, 0, 0, 6, 6, 6, 6], dtype=np.float64)
+    mb = orc.block_medians(P, W)
+    assert mb.tolist() == [2.0, 0.0, 0.0, 6.0]
+    out = orc.normalise(P, mb, W)
+    assert np.all(np.isfinite(out)) and out[0] == 0.0
+    assert np.all(out[4:12] == 0.0)                                  # numerator 0 or baseline 0: both give 0
+    assert out[1] == pytest.approx(2 * math.log(2) / 2.0)            # k = 1 < centre 1.5: flat baseline m = 2
+    assert out[3] == pytest.approx(2 * math.log(2) / (2.0 * (1 - 1.5 / 4)))      # k = 3: m = 2 (1 - (3 - 1.5)/4)
+    assert out[15] == pytest.approx(math.log(2))                     # flat beyond the last centre: m = 6
+    Pz = np.zeros(16)
+    assert np.all(orc.normalise(Pz + 1.0, np.zeros(4), W) == 0.0)    # a positive power over a zero baseline -> 0
+
+
 # ------------------------------------------------------------------ harmonic sums
 def _round_half_up(fr: Fraction) -> int:
     return math.floor(fr + Fraction(1, 2))
