@@ -255,7 +255,7 @@ def test_paper_shaped_bank_at_2p24(tb):
 
 
 @pytest.mark.skipif(not FULL, reason="2^28 samples: the oracle needs ~55 GB and minutes per template; run with TB_PARITY_FULL=1 "
-                                     "(recorded in profiles/r02_parity_full.txt)")
+                                     "(result table in profiles/r02_v1.md)")
 def test_terzan_length_series_2p28(tb):
     """a Terzan-5-length series (L489), N = 2^28 (the largest the plan accepts; library-FFT
     path): the true template and one other compared in full with the oracle, one at a time."""
