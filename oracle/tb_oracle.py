@@ -405,12 +405,22 @@ def whiten_series(series, window=1024, zap_bins=()):
     return (np.fft.irfft(Xw, n) * math.sqrt(float(n))).astype(np.float32)
 
 
-def whitened_level(series_white, window=1024):
+def whitened_level(series_white, window=1024, zap_bins=()):
     """kappa: the ONE normalisation constant of a whitened series, replacing the per-template block
     medians of O6: kappa = ln2 / mean_b(m_b), m_b = block medians of the interbinned spectrum of
-    the un-resampled whitened series.  P^_k = kappa * P_k for every template."""
+    the un-resampled whitened series.  P^_k = kappa * P_k for every template.
+    Blocks touched by a zapped range are left out of the mean (reading G25): a range [lo, hi) zeroes
+    X'_lo..X'_{hi-1}, which lowers the interbinned powers P_lo..P_hi and with them the medians of the blocks
+    lo // W .. hi // W -- to 0 once half a block is zapped -- and kappa would grow by about 1 / (1 - zapped
+    fraction of the band), raising every sigma.  If every block is touched, all blocks are used."""
     P = interbin_power(rfft_forward(series_white))
-    return LN2 / float(np.mean(block_medians(P, window)))
+    m_b = block_medians(P, window)
+    keep = np.ones(m_b.size, dtype=bool)
+    for lo, hi in zap_bins:
+        keep[int(lo) // window: int(hi) // window + 1] = False
+    if not keep.any():
+        keep[:] = True
+    return LN2 / float(np.mean(m_b[keep]))
 
 
 def spectrum_of_template_whitened(series_white, kappa, tsamp, tmpl, fill=None, idx=None):

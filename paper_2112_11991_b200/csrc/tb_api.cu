@@ -338,9 +338,25 @@ int whiten_series(tb_plan* p)
     std::vector<float> med(p->nblk);
     TB_CUDA(p, cudaMemcpyAsync(med.data(), p->d_med, p->nblk * sizeof(float), cudaMemcpyDeviceToHost, p->stream));
     TB_CUDA(p, cudaStreamSynchronize(p->stream));                // also fences the scratch freed by ~DevBufs
+    // blocks touched by a zapped range [lo, hi) (interbinned bins lo..hi) have depressed medians: leave
+    // them out of the mean, or kappa grows by 1 / (1 - zapped fraction) (reading G25)
+    std::vector<char> keep(p->nblk, 1);
+    for (const uint2& z : p->zap)
+        for (size_t b = z.x / p->window; b <= z.y / p->window && b < p->nblk; ++b) keep[b] = 0;
+    size_t n_keep = 0;
+    for (char k : keep) n_keep += k;
+    if (n_keep == 0) { std::fill(keep.begin(), keep.end(), 1); n_keep = p->nblk; }
     double acc = 0.0;
-    for (float m : med) acc += (double)m;
-    p->kappa = (float)(0.69314718055994530942 * (double)p->nblk / acc);
+    for (size_t b = 0; b < p->nblk; ++b) if (keep[b]) acc += (double)med[b];
+    p->kappa = (float)(0.69314718055994530942 * (double)n_keep / acc);
+    // the fp64 plans' work areas are several GB from 2^26 samples on and the chunk size B was chosen from
+    // the memory free before they existed: give them back (the stream was synchronised above; the next
+    // tb_plan_set_series builds them again, milliseconds against the seconds such a series takes to load)
+    if (p->n >= (1ull << 26)) {
+        cufftDestroy(p->c2r_plan); cufftDestroy(p->d2z_plan);
+        p->c2r_plan = p->d2z_plan = 0;
+        p->have_c2r = false;
+    }
     return TB_OK;
 }
 

@@ -25,7 +25,7 @@ def tb():
 
 def _whitened_oracle(series, window=1024, zap=()):
     xw = orc.whiten_series(series, window, zap)
-    return xw, orc.whitened_level(xw, window)
+    return xw, orc.whitened_level(xw, window, zap)
 
 
 def _check_series(plan, xw, kappa):
@@ -95,6 +95,26 @@ def test_whitened_both_paths_and_windows(tb, log2n, window, fft_path):
         cands, n = plan.candidates()
         rep = pooled_parity(plan, w, ids, 5.0, w.folds, by_template(cands), hsums_ids=ids, slots=[0, 1], white=(xw, kappa))
     assert all("err_hsum" in r for r in rep.values())
+
+
+def test_wide_birdie_list_does_not_inflate_kappa(tb, c1):
+    """6 % of the band zapped (whole blocks, a straddle, a part of a block; reading G25): the device's kappa is the
+    oracle's -- both leave the touched blocks out of the mean -- and stays within 1.5 % of the unzapped series'
+    kappa instead of growing by 1 / (1 - 0.06); candidates equal the oracle's on the true template."""
+    W = 1024
+    zap = [(8 * W, 10 * W), (30 * W + 100, 31 * W + 900), (50 * W, 50 * W + 300)]
+    xw, kappa = _whitened_oracle(c1.series, W, zap)
+    with tb.Plan(c1.series, c1.tsamp, whiten=True, zap_ranges=zap) as plan:
+        _check_series(plan, xw, kappa)
+        kg = plan.debug_series()[1]
+        plan.search(c1.templates[:2], 0, c1.folds, 6.0)
+        cands, _ = plan.candidates()
+        for tid in (0, 1):
+            check_template(plan, c1, tid, 6.0, c1.folds, by_template(cands).get(tid, cands[:0]), hsums=True, white=(xw, kappa))
+    with tb.Plan(c1.series, c1.tsamp, whiten=True) as plan:
+        k0 = plan.debug_series()[1]
+    assert abs(kg / k0 - 1.0) < 0.015
+    assert orc.whitened_level(xw, W) / kappa > 1.04              # what the round-2 rule (every block) would give
 
 
 def test_set_series_rewhitens(tb, c1):

@@ -505,6 +505,31 @@ def test_t10_on_the_whitened_series(c1):
     assert orc.search_template_whitened(xw, kappa, c1.tsamp, c1.templates[5], 1) == []
 
 
+def test_whitened_level_ignores_zapped_blocks():
+    """A birdie list covering 6 % of the band (reading G25): the normalised powers of the UNzapped bins of a
+    whitened white series must still average 1 (median ln 2).  With the zapped blocks inside the mean of the
+    block medians, kappa -- and every normalised power -- comes out 1 / (1 - 0.06) too large."""
+    rng = np.random.default_rng(31)
+    n, W = 1 << 17, 1024
+    x = rng.standard_normal(n).astype(np.float32)
+    zap = [(8 * W, 10 * W), (30 * W + 100, 31 * W + 900), (50 * W, 50 * W + 300)]           # whole blocks, a straddle, a part
+    xw = orc.whiten_series(x, W, zap)
+    P = orc.interbin_power(orc.rfft_forward(xw))
+    clear = np.ones(n // 2, dtype=bool)
+    clear[0] = False
+    for lo, hi in zap:
+        clear[lo - 1: hi + 2] = False
+    kappa = orc.whitened_level(xw, W, zap)
+    assert abs(np.median(kappa * P[clear]) - math.log(2)) < 0.012
+    level_all = orc.whitened_level(xw, W)                                  # the round-2 rule: every block
+    touched = {b for lo, hi in zap for b in range(lo // W, hi // W + 1)}
+    assert touched == {8, 9, 10, 30, 31, 50}
+    assert level_all / kappa > 1.04                                        # what the zapped blocks would have cost
+    # no zap ranges: unchanged; every block zapped: falls back to all blocks instead of dividing by nothing
+    assert orc.whitened_level(xw, W, ()) == level_all
+    assert np.isfinite(orc.whitened_level(xw, W, [(0, n // 2)]))
+
+
 # ------------------------------------------------------------------ f4: the ELL7 approximate-orbit delay (reading G26)
 def test_ell_table_is_the_printed_appendix_b():
     """The oracle's coefficient table against the numbers typed independently into the golden file
